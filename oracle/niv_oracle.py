@@ -1,0 +1,177 @@
+"""ctypes wrapper around oracle/niv_oracle.c (TEST INFRASTRUCTURE -- see the C header).
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs may import this.  It neither imports nor is imported by the CUDA binding.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "niv_oracle.c")
+_LIB = os.path.join(_HERE, "libniv_oracle.so")
+
+
+class OracleConfig(C.Structure):
+    _fields_ = [
+        ("n_levels", C.c_uint32), ("n_features", C.c_uint32), ("log2_table_size", C.c_uint32),
+        ("base_resolution", C.c_uint32), ("per_level_scale", C.c_double),
+        ("resolutions", C.c_uint32 * 16),
+        ("aabb_min", C.c_float * 3), ("aabb_max", C.c_float * 3),
+        ("sh_degree", C.c_uint32), ("n_params", C.c_uint32), ("n_frequencies", C.c_uint32),
+        ("n_hidden_layers", C.c_uint32), ("hidden_width", C.c_uint32), ("out_activation", C.c_uint32),
+    ]
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 -ffp-contract=off -fopenmp (no -ffast-math): the fp32 index path must not be contracted."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-fPIC", "-shared",
+               "-Wall", "-Wextra", "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.niv_oracle_half_to_double.restype = C.c_double
+        _lib.niv_oracle_half_to_double.argtypes = [C.c_uint16]
+        _lib.niv_oracle_hash.restype = C.c_uint32
+        _lib.niv_oracle_hash.argtypes = [C.c_uint32] * 4
+        _lib.niv_oracle_in_dim.restype = C.c_uint32
+        _lib.niv_oracle_max_threads.restype = C.c_int
+    return _lib
+
+
+def make_config(spec) -> OracleConfig:
+    """spec: any object with the ModelSpec attribute names (paper_2602_12949_b200.inputs.ModelSpec)."""
+    cfg = OracleConfig()
+    cfg.n_levels = spec.n_levels
+    cfg.n_features = spec.n_features
+    cfg.log2_table_size = spec.log2_table_size
+    cfg.base_resolution = spec.base_resolution
+    cfg.per_level_scale = spec.per_level_scale
+    res = getattr(spec, "resolutions", None)
+    if res:
+        for i, r in enumerate(res):
+            cfg.resolutions[i] = int(r)
+    for d in range(3):
+        cfg.aabb_min[d] = spec.aabb_min[d]
+        cfg.aabb_max[d] = spec.aabb_max[d]
+    cfg.sh_degree = spec.sh_degree
+    cfg.n_params = spec.n_params
+    cfg.n_frequencies = spec.n_frequencies
+    cfg.n_hidden_layers = spec.n_hidden_layers
+    cfg.hidden_width = spec.hidden_width
+    cfg.out_activation = spec.out_activation
+    return cfg
+
+
+def _p(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _chk(a: np.ndarray, dtype, name: str) -> np.ndarray:
+    a = np.ascontiguousarray(a, dtype=dtype)
+    if not a.flags.c_contiguous:
+        raise ValueError(name)
+    return a
+
+
+def level_table(spec):
+    cfg = make_config(spec)
+    N = np.zeros(spec.n_levels, dtype=np.uint32)
+    dense = np.zeros(spec.n_levels, dtype=np.uint32)
+    rc = lib().niv_oracle_level_table(C.byref(cfg), _p(N), _p(dense))
+    if rc:
+        raise ValueError("niv_oracle_level_table failed")
+    return N, dense.astype(bool)
+
+
+def hash_index(vx: int, vy: int, vz: int, log2_T: int) -> int:
+    return int(lib().niv_oracle_hash(vx & 0xFFFFFFFF, vy & 0xFFFFFFFF, vz & 0xFFFFFFFF, log2_T))
+
+
+def half_to_double(bits: int) -> float:
+    return float(lib().niv_oracle_half_to_double(bits))
+
+
+def sh16(n) -> np.ndarray:
+    v = np.ascontiguousarray(n, dtype=np.float64)
+    out = np.zeros(16, dtype=np.float64)
+    lib().niv_oracle_sh16(_p(v), _p(out))
+    return out
+
+
+def param_encode(t: float, n_frequencies: int) -> np.ndarray:
+    out = np.zeros(2 * n_frequencies, dtype=np.float64)
+    lib().niv_oracle_param_encode(C.c_double(t), C.c_uint32(n_frequencies), _p(out))
+    return out
+
+
+def mlp(spec, weights_blob, biases_blob, x) -> np.ndarray:
+    cfg = make_config(spec)
+    w = _chk(weights_blob, np.float16, "weights")
+    b = None if biases_blob is None else _chk(biases_blob, np.float32, "biases")
+    xx = _chk(x, np.float64, "x")
+    y = np.zeros(3, dtype=np.float64)
+    lib().niv_oracle_mlp(C.byref(cfg), _p(w), _p(b), _p(xx), _p(y))
+    return y
+
+
+def encode(spec, table, pos, nrm, param=None, want_features=True, n_threads: int = 0):
+    """-> dict(idx [n][L][8] u32, cell [n][L][3] i32, frac [n][L][3] f32, features [n][in_dim] f64)."""
+    cfg = make_config(spec)
+    table = _chk(table, np.float16, "table")
+    pos = _chk(pos, np.float32, "pos")
+    nrm = _chk(nrm, np.float32, "nrm")
+    n = pos.shape[0]
+    L = spec.n_levels
+    prm = None if param is None else _chk(param, np.float32, "param")
+    if spec.n_params and prm is None:
+        raise ValueError("param required")
+    idx = np.zeros((n, L, 8), dtype=np.uint32)
+    cell = np.zeros((n, L, 3), dtype=np.int32)
+    frac = np.zeros((n, L, 3), dtype=np.float32)
+    feat = np.zeros((n, spec.in_dim), dtype=np.float64) if want_features else None
+    rc = lib().niv_oracle_encode(C.byref(cfg), _p(table), _p(pos), _p(nrm), _p(prm), C.c_size_t(n),
+                                 _p(idx), _p(cell), _p(frac), _p(feat), C.c_int(n_threads))
+    if rc:
+        raise ValueError("niv_oracle_encode failed")
+    return {"idx": idx, "cell": cell, "frac": frac, "features": feat}
+
+
+def infer(spec, table, weights_blob, biases_blob, pos, nrm, param=None, n_threads: int = 0,
+          want_f64: bool = False):
+    """Full path O0..O9 -> out [n][3] fp32 (and fp64 if want_f64)."""
+    cfg = make_config(spec)
+    table = _chk(table, np.float16, "table")
+    w = _chk(weights_blob, np.float16, "weights")
+    b = None if biases_blob is None else _chk(biases_blob, np.float32, "biases")
+    pos = _chk(pos, np.float32, "pos")
+    nrm = _chk(nrm, np.float32, "nrm")
+    prm = None if param is None else _chk(param, np.float32, "param")
+    if spec.n_params and prm is None:
+        raise ValueError("param required")
+    n = pos.shape[0]
+    out32 = np.zeros((n, 3), dtype=np.float32)
+    out64 = np.zeros((n, 3), dtype=np.float64) if want_f64 else None
+    rc = lib().niv_oracle_infer(C.byref(cfg), _p(table), _p(w), _p(b), _p(pos), _p(nrm), _p(prm),
+                                _p(out32), _p(out64), C.c_size_t(n), C.c_int(n_threads))
+    if rc:
+        raise ValueError("niv_oracle_infer failed")
+    return (out32, out64) if want_f64 else out32
+
+
+def max_threads() -> int:
+    return int(lib().niv_oracle_max_threads())
