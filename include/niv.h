@@ -1,0 +1,148 @@
+/*
+ * niv.h -- C ABI of libniv: B200 (sm_100a) per-texel inference of the Neural Irradiance Volume.
+ *
+ * The operation (arxiv 2602.12949; line numbers refer to /root/reference/PAPER.md and SPEC.md):
+ *   "Starting from the G-buffer of the rendered scene, the position and normal buffers are input to the
+ *    neural model, which infers pixel-wise E(x, n) in a single batch"            (sec. 4.4)
+ *   E_theta = small ReLU MLP over [multi-level hash-grid encoding of x | encoding of n | encoding of the
+ *   scene parameter]                                               (sec. 4.1; 666-671 sec. 6)
+ * The exact arithmetic (op order of the fp32 index path, hash, corner order, SH convention, ...) is the
+ * list O0..O9 in DESIGN.md section 3.1; the readings taken where the paper is silent are DESIGN.md 3.2.
+ *
+ * Conventions
+ *   - every function returns an int status (NIV_OK or a negative NIV_ERR_*), never throws, never aborts;
+ *   - "device" pointers are CUDA device pointers on the model's device, "host" pointers are ordinary memory;
+ *   - the caller owns every buffer it passes; the model owns its own device copies of all parameters, so
+ *     parameter blobs may be freed as soon as niv_load_params returns;
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream);
+ *   - niv_infer / niv_encode / niv_debug_encode are asynchronous on `stream`, allocate nothing, never
+ *     synchronise (CUDA-graph capturable), are read-only on the model and safe for concurrent callers on
+ *     different streams;
+ *   - there is no CPU fallback: without a CUDA device every entry point that needs one returns NIV_ERR_CUDA.
+ */
+#ifndef NIV_H_
+#define NIV_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NIV_API_VERSION 1u
+#define NIV_MAX_LEVELS 16
+
+typedef struct niv_model niv_model;   /* opaque */
+
+enum {
+    NIV_OK = 0,
+    NIV_ERR_INVALID_ARG = -1,   /* NULL / mis-sized / mis-aligned argument                        */
+    NIV_ERR_UNSUPPORTED = -2,   /* a valid configuration this build has no kernel for             */
+    NIV_ERR_NOT_LOADED  = -3,   /* niv_infer before niv_load_params                               */
+    NIV_ERR_CUDA        = -4,   /* a CUDA runtime call failed (niv_last_cuda_error has the code)  */
+    NIV_ERR_ALLOC       = -5    /* host or device allocation failed                               */
+};
+
+enum { NIV_OUT_LINEAR = 0,      /* the paper: no activation on the final layer     */
+       NIV_OUT_SIGMOID = 1 };   /* BASELINE.json configs[0]                                       */
+
+/* Model hyper-parameters (table size T, latent dimension, scaling factor between levels,
+ * coarsest side, number of levels; PAPER.md:296 network; PAPER.md:669-670 scene parameters). */
+typedef struct {
+    uint32_t struct_size;         /* = sizeof(niv_config)                                           */
+    uint32_t api_version;         /* = NIV_API_VERSION                                              */
+    uint32_t n_levels;            /* L: 4, 8, 12 or 16                                              */
+    uint32_t n_features;          /* F: fp16 latents per table entry; this build: 2                 */
+    uint32_t log2_table_size;     /* T = 2^k entries PER LEVEL, 4 <= k <= 24                        */
+    uint32_t base_resolution;     /* N0: cells per side on the coarsest level                       */
+    double   per_level_scale;     /* b: N_l = floor(N0 * b^l)  (reading #2)               */
+    uint32_t resolutions[NIV_MAX_LEVELS]; /* optional explicit N_l; all zero => derive from N0, b   */
+    float    aabb_min[3], aabb_max[3];    /* scene box mapped to the unit cube (reading #8)         */
+    uint32_t sh_degree;           /* 4 => 16 real-SH coefficients of the normal (reading #13)       */
+    uint32_t n_params;            /* 0..2 per-call scalar scene parameters                          */
+    uint32_t n_frequencies;       /* sin/cos bands per parameter (8)                                */
+    uint32_t n_hidden_layers;     /* 1..3 hidden layers, all `hidden_width` wide                    */
+    uint32_t hidden_width;        /* 32, 64 or 128                                                  */
+    uint32_t out_activation;      /* NIV_OUT_*                                                      */
+    int32_t  device;              /* CUDA device ordinal                                            */
+} niv_config;
+
+/* What niv_create derived from the configuration (for tests, benchmarks and roofline arithmetic). */
+typedef struct {
+    uint32_t struct_size;
+    uint32_t in_dim;                       /* L*F + 16 + 2*n_frequencies*n_params                   */
+    uint32_t resolution[NIV_MAX_LEVELS];   /* N_l                                                   */
+    uint32_t is_dense[NIV_MAX_LEVELS];     /* 1: dense index, 0: spatial hash (reading #4)          */
+    uint64_t table_bytes;                  /* L * T * F * 2                                         */
+    uint64_t weight_bytes;                 /* sum over layers of out*in*2                           */
+    uint64_t bias_bytes;                   /* sum over layers of out*4                              */
+    uint32_t num_sms;                      /* SM count of the device                                */
+    uint32_t ctas_per_sm;                  /* resident CTAs per SM of the fused kernel              */
+    uint32_t tile_texels;                  /* texels per CTA tile (128)                             */
+    uint32_t smem_bytes;                   /* dynamic shared memory per CTA of the fused kernel     */
+} niv_info;
+
+/* Validate `cfg` completely and allocate device storage for the parameters (uninitialised).
+ * Errors: NULL / wrong struct_size / api_version / degenerate AABB / zero resolution -> NIV_ERR_INVALID_ARG;
+ * a shape this build has no kernel for (F != 2, L not in {4,8,12,16}, width not in {32,64,128}, sh_degree
+ * != 4, n_frequencies != 8, n_params > 2, n_hidden_layers not in 1..3) -> NIV_ERR_UNSUPPORTED.
+ * Shape errors are raised here, never at inference. */
+int niv_create(const niv_config *cfg, niv_model **out);
+
+int niv_get_info(const niv_model *m, niv_info *info);
+
+/* Copy the parameters into the model (host or device source, `src_on_device` != 0 for device pointers);
+ * synchronises `stream` before returning, so the sources may be freed.
+ *   table_fp16   [L][T][F] fp16, level-major; dense levels use their first (N_l+1)^3 entries, x fastest
+ *   weights_fp16 W1|W2|...|Wk, each [out][in] row-major fp16, layer-major; Wk has 3 rows
+ *   biases_f32   b1|b2|...|bk fp32, or NULL for zeros
+ * Byte counts must equal niv_info.{table,weight,bias}_bytes, else NIV_ERR_INVALID_ARG.
+ * "All parameters in half-precision". */
+int niv_load_params(niv_model *m, const void *table_fp16, size_t table_bytes,
+                    const void *weights_fp16, size_t weight_bytes,
+                    const float *biases_f32, size_t bias_bytes,
+                    int src_on_device, void *stream);
+
+/* The hot path: one fused kernel, out[i] = E_theta(pos[i], nrm[i][, param]) for i < n.
+ *   pos, nrm  device, [n][3] fp32 packed, base address 4-byte aligned; world-space position, unit normal
+ *   param     HOST, n_params floats in [0,1] shared by the whole call (NULL iff n_params == 0)
+ *   out       device, [n][3] fp32 packed RGB irradiance
+ * A texel whose normal is exactly (0,0,0) or whose inputs are not all finite is background: out = (0,0,0),
+ * no table access (reading #9).  Positions outside the AABB are clamped (reading #7).  n == 0 is a no-op.
+ * Errors: NULL pointers -> NIV_ERR_INVALID_ARG; before niv_load_params -> NIV_ERR_NOT_LOADED;
+ * launch failure -> NIV_ERR_CUDA. */
+int niv_infer(niv_model *m, const float *pos, const float *nrm, const float *param,
+              float *out, size_t n, void *stream);
+
+/* Stand-alone encoding kernel (rows a1..a9 without the MLP): features_fp16 is device, [n][in_dim] fp16
+ * row-major = [latents | SH-16 | parameter encoding], zero rows for background texels. */
+int niv_encode(niv_model *m, const float *pos, const float *nrm, const float *param,
+               void *features_fp16, size_t n, void *stream);
+
+/* Debug dump through the SAME device functions the fused kernel uses for O0..O3 (bit-exact parity of the
+ * integer path is checked on these).  All outputs are device pointers; any may be NULL.
+ *   idx [n][L][8] uint32 (corner j: bit d of j selects +1 on axis d), cell [n][L][3] int32,
+ *   frac [n][L][3] fp32, features [n][in_dim] fp32 (before fp16 packing).  Background texels: zeros. */
+int niv_debug_encode(niv_model *m, const float *pos, const float *nrm, const float *param, size_t n,
+                     uint32_t *idx, int32_t *cell, float *frac, float *features, void *stream);
+
+int niv_destroy(niv_model *m);
+
+const char *niv_error_string(int code);
+
+/* cudaError_t of the last failing CUDA call made by this library on the calling thread (0 if none). */
+int niv_last_cuda_error(void);
+
+/* ---- measured rooflines: micro-benchmarks that run on the caller's stream ----
+ * niv_probe_gather: every lane of `n_warps_total` warps issues `loads_per_lane` independent 4-byte loads
+ * (pattern 0: one uniformly random 32-byte sector of `buf` per load; pattern 1: random sector per WARP, lanes
+ * consecutive -- the coalesced L2 rate; pattern 2: random aligned 8-byte pair read as one 64-bit load).
+ * buf is device memory of `buf_bytes` (power of two); sink is device, >= 4 bytes.  Asynchronous. */
+int niv_probe_gather(const void *buf, size_t buf_bytes, int pattern, uint32_t n_ctas, uint32_t loads_per_lane,
+                     uint32_t seed, void *sink, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NIV_H_ */

@@ -1,0 +1,673 @@
+// niv.cu -- libniv: kernels and the C ABI declared in include/niv.h.
+//
+// Kernels (all sm_100a, hand-written):
+//   niv_fused_kernel<WIDTH>  rows a0..a12 of DESIGN.md section 1: persistent CTAs of 128 threads, one texel
+//                            per thread and 128-texel tiles; weights staged once per CTA with a bulk async
+//                            copy; gathers from the L2-resident table; every layer is a tcgen05.mma
+//                            (M=128, kind::f16, fp32 accumulators in TMEM); activations never leave the SM.
+//   niv_encode_kernel        rows a1..a9 only (stand-alone encoding, fp16 features to global memory).
+//   niv_debug_kernel         index / cell / fraction / fp32 feature dump through the same device functions.
+//   niv_probe_gather_kernel  random-sector gather micro-benchmark (the measured L2-gather roofline).
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <cmath>
+#include <new>
+#include <vector>
+
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+
+#include "../../include/niv.h"
+#include "niv_device.cuh"
+#include "niv_tc.cuh"
+
+namespace niv {
+
+// =====================================================================================================
+// fused encode + MLP
+// =====================================================================================================
+template <int WIDTH>
+__global__ void __launch_bounds__(kTile) niv_fused_kernel(const __grid_constant__ KParams P,
+                                                          const float* __restrict__ pos,
+                                                          const float* __restrict__ nrm,
+                                                          float* __restrict__ out, size_t n, uint32_t n_tiles)
+{
+    constexpr uint32_t TMEM_COLS = WIDTH < 32 ? 32 : WIDTH;
+    extern __shared__ __align__(1024) uint8_t smem[];
+    uint8_t* sW = smem;                                              // packed weights + biases
+    uint8_t* sA = smem + P.a_off;                                    // A operand: [K/8][128 rows][16 B]
+    float* sBias1 = reinterpret_cast<float*>(smem + P.misc_off);     // layer-1 bias with the parameter fold
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + P.misc_off + WIDTH * 4);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2);
+
+    const uint32_t tid = threadIdx.x;
+    const uint32_t warp = tid >> 5;
+    const uint32_t bar_w = smem_u32(&bars[0]);
+    const uint32_t bar_mma = smem_u32(&bars[1]);
+    const uint32_t sA_u32 = smem_u32(sA);
+    const uint32_t sW_u32 = smem_u32(sW);
+
+    // ---- a0: one-time setup: barriers, TMEM columns, weights
+    if (tid == 0) {
+        mbar_init(bar_w, 1);
+        mbar_init(bar_mma, 1);
+        mbar_fence_init();
+    }
+    if (warp == 0) tmem_alloc(smem_u32(tmem_slot), TMEM_COLS);
+    tc_fence_before_sync();
+    __syncthreads();
+    tc_fence_after_sync();
+    const uint32_t tmem = *tmem_slot;
+    if (tid == 0) {
+        mbar_arrive_expect_tx(bar_w, P.wpack_bytes);
+        bulk_g2s(sW_u32, P.wpack, P.wpack_bytes, bar_w);
+    }
+    mbar_wait(bar_w, 0);
+
+    // ---- a8: the parameter encoding is constant over the call: fold W1[:, enc_dim:] * enc(t) into the bias
+    if (tid < WIDTH) {
+        float b = reinterpret_cast<const float*>(sW + P.b_off[0])[tid];
+        const uint32_t np16 = 16 * P.n_params;
+        for (uint32_t q = 0; q < P.n_params; ++q) {
+            float enc[16];
+            param_encode8(P.t[q], enc);
+            const float* wp = reinterpret_cast<const float*>(sW + P.wparam_off) + tid * np16 + 16 * q;
+#pragma unroll
+            for (int k = 0; k < 16; ++k) b = fmaf(wp[k], enc[k], b);
+        }
+        sBias1[tid] = b;
+    }
+    __syncthreads();
+
+    const uint32_t lane_taddr = tmem + ((warp * 32u) << 16);
+    const uint32_t n_groups = P.L >> 2;               // 4 levels (8 latents) per 16-byte chunk
+    const uint32_t k1_chunks = P.kdim[0] >> 3;
+    uint32_t phase = 0;
+
+    for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const size_t i = (size_t)tile * kTile + tid;
+        const bool valid = i < n;
+        float p[3] = {0.f, 0.f, 0.f}, nv[3] = {0.f, 0.f, 0.f};
+        if (valid) {
+            load3(pos, i, p);
+            load3(nrm, i, nv);
+        }
+        const bool masked = !valid || texel_masked(p, nv);
+
+        // ---- a2..a9: encode this thread's texel into row `tid` of the A tile
+        const uint32_t row_u32 = sA_u32 + tid * 16;
+        if (!masked) {
+            float u[3];
+            normalise(P, p, u);
+            for (uint32_t g = 0; g < n_groups; ++g) {
+                float2 f[4];
+                encode_group4(P, (int)(g * 4), u, f);
+                uint4 c = make_uint4(pack_half2(f[0].x, f[0].y), pack_half2(f[1].x, f[1].y),
+                                     pack_half2(f[2].x, f[2].y), pack_half2(f[3].x, f[3].y));
+                *reinterpret_cast<uint4*>(sA + g * 2048 + tid * 16) = c;
+            }
+            float sh[16];
+            sh16(nv, sh);
+            uint4 c0 = make_uint4(pack_half2(sh[0], sh[1]), pack_half2(sh[2], sh[3]),
+                                  pack_half2(sh[4], sh[5]), pack_half2(sh[6], sh[7]));
+            uint4 c1 = make_uint4(pack_half2(sh[8], sh[9]), pack_half2(sh[10], sh[11]),
+                                  pack_half2(sh[12], sh[13]), pack_half2(sh[14], sh[15]));
+            *reinterpret_cast<uint4*>(sA + (n_groups + 0) * 2048 + tid * 16) = c0;
+            *reinterpret_cast<uint4*>(sA + (n_groups + 1) * 2048 + tid * 16) = c1;
+            for (uint32_t kc = n_groups + 2; kc < k1_chunks; ++kc)       // K padding up to a multiple of 16
+                *reinterpret_cast<uint4*>(sA + kc * 2048 + tid * 16) = make_uint4(0, 0, 0, 0);
+        } else {
+            for (uint32_t kc = 0; kc < k1_chunks; ++kc)
+                *reinterpret_cast<uint4*>(sA + kc * 2048 + tid * 16) = make_uint4(0, 0, 0, 0);
+        }
+        (void)row_u32;
+        fence_proxy_async_smem();
+        tc_fence_before_sync();
+        __syncthreads();
+
+        // ---- a10..a11: layers on the tensor cores
+        for (uint32_t layer = 0; layer < P.n_layers; ++layer) {
+            const uint32_t K = P.kdim[layer], N = P.npad[layer];
+            if (tid == 0) {
+                tc_fence_after_sync();
+                const uint32_t idesc = make_idesc_f16(kTile, N);
+                const uint32_t b_base = sW_u32 + P.w_off[layer];
+                for (uint32_t ks = 0; ks < (K >> 4); ++ks) {
+                    const uint64_t da = make_smem_desc(sA_u32 + ks * 4096u, 2048u, 128u);
+                    const uint64_t db = make_smem_desc(b_base + ks * (N * 32u), N * 16u, 128u);
+                    umma_f16_ss(tmem, da, db, idesc, ks > 0 ? 1u : 0u);
+                }
+                umma_commit(bar_mma);
+            }
+            mbar_wait(bar_mma, phase);
+            phase ^= 1u;
+            tc_fence_after_sync();
+
+            if (layer + 1 < P.n_layers) {
+                // hidden epilogue: bias + ReLU -> fp16 -> next layer's A operand (same buffer; the MMA is done)
+                const float* bias = (layer == 0) ? sBias1 : reinterpret_cast<const float*>(sW + P.b_off[layer]);
+#pragma unroll
+                for (int cc = 0; cc < WIDTH / 32; ++cc) {
+                    uint32_t r[32];
+                    tmem_ld_x32(lane_taddr + cc * 32, r);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int g = 0; g < 4; ++g) {
+                        uint32_t pk[4];
+#pragma unroll
+                        for (int h = 0; h < 4; ++h) {
+                            const int j = g * 8 + h * 2;
+                            float a = __uint_as_float(r[j]) + bias[cc * 32 + j];
+                            float b = __uint_as_float(r[j + 1]) + bias[cc * 32 + j + 1];
+                            pk[h] = pack_half2(fmaxf(a, 0.0f), fmaxf(b, 0.0f));
+                        }
+                        *reinterpret_cast<uint4*>(sA + (cc * 4 + g) * 2048 + tid * 16) =
+                            make_uint4(pk[0], pk[1], pk[2], pk[3]);
+                    }
+                }
+                fence_proxy_async_smem();
+                tc_fence_before_sync();
+                __syncthreads();
+            } else {
+                // ---- a11..a12: output layer: 3 useful columns, bias, activation, store
+                uint32_t r[4];
+                tmem_ld_x4(lane_taddr, r);
+                tmem_ld_wait();
+                tc_fence_before_sync();
+                if (valid) {
+                    const float* bias = (layer == 0) ? sBias1 : reinterpret_cast<const float*>(sW + P.b_off[layer]);
+                    float y[3];
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        float v = __uint_as_float(r[c]) + bias[c];
+                        if (P.out_act == NIV_OUT_SIGMOID) v = 1.0f / (1.0f + __expf(-v));
+                        y[c] = masked ? 0.0f : v;
+                    }
+                    out[3 * i] = y[0];
+                    out[3 * i + 1] = y[1];
+                    out[3 * i + 2] = y[2];
+                }
+            }
+        }
+    }
+
+    __syncthreads();
+    if (warp == 0) tmem_dealloc(tmem, TMEM_COLS);
+}
+
+// =====================================================================================================
+// stand-alone encode (fp16 features to global) and debug dump
+// =====================================================================================================
+__global__ void __launch_bounds__(128) niv_encode_kernel(const __grid_constant__ KParams P,
+                                                         const float* __restrict__ pos,
+                                                         const float* __restrict__ nrm,
+                                                         uint4* __restrict__ feat, size_t n)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t chunks = P.in_dim >> 3;
+    uint4* row = feat + i * chunks;
+    float p[3], nv[3];
+    load3(pos, i, p);
+    load3(nrm, i, nv);
+    if (texel_masked(p, nv)) {
+        for (uint32_t c = 0; c < chunks; ++c) row[c] = make_uint4(0, 0, 0, 0);
+        return;
+    }
+    float u[3];
+    normalise(P, p, u);
+    const uint32_t n_groups = P.L >> 2;
+    for (uint32_t g = 0; g < n_groups; ++g) {
+        float2 f[4];
+        encode_group4(P, (int)(g * 4), u, f);
+        row[g] = make_uint4(pack_half2(f[0].x, f[0].y), pack_half2(f[1].x, f[1].y),
+                            pack_half2(f[2].x, f[2].y), pack_half2(f[3].x, f[3].y));
+    }
+    float sh[16];
+    sh16(nv, sh);
+    row[n_groups] = make_uint4(pack_half2(sh[0], sh[1]), pack_half2(sh[2], sh[3]),
+                               pack_half2(sh[4], sh[5]), pack_half2(sh[6], sh[7]));
+    row[n_groups + 1] = make_uint4(pack_half2(sh[8], sh[9]), pack_half2(sh[10], sh[11]),
+                                   pack_half2(sh[12], sh[13]), pack_half2(sh[14], sh[15]));
+    for (uint32_t q = 0; q < P.n_params; ++q) {
+        float e[16];
+        param_encode8(P.t[q], e);
+        row[n_groups + 2 + 2 * q] = make_uint4(pack_half2(e[0], e[1]), pack_half2(e[2], e[3]),
+                                               pack_half2(e[4], e[5]), pack_half2(e[6], e[7]));
+        row[n_groups + 3 + 2 * q] = make_uint4(pack_half2(e[8], e[9]), pack_half2(e[10], e[11]),
+                                               pack_half2(e[12], e[13]), pack_half2(e[14], e[15]));
+    }
+}
+
+__global__ void __launch_bounds__(128) niv_debug_kernel(const __grid_constant__ KParams P,
+                                                        const float* __restrict__ pos,
+                                                        const float* __restrict__ nrm, size_t n,
+                                                        uint32_t* __restrict__ idx, int32_t* __restrict__ cell,
+                                                        float* __restrict__ frac, float* __restrict__ feat)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const uint32_t L = P.L;
+    float p[3], nv[3];
+    load3(pos, i, p);
+    load3(nrm, i, nv);
+    const bool masked = texel_masked(p, nv);
+    float u[3] = {0.f, 0.f, 0.f};
+    if (!masked) normalise(P, p, u);
+    for (uint32_t l = 0; l < L; ++l) {
+        int c[3] = {0, 0, 0};
+        float w[3] = {0.f, 0.f, 0.f};
+        uint32_t e[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        float2 f = make_float2(0.f, 0.f);
+        if (!masked) {
+            locate(P.lv[l], u, c, w);
+            corner_entries(P.lv[l], P.tmask, c, e);
+            if (feat) {
+                uint32_t v[8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) v[j] = __ldg(P.table + e[j]);
+                f = blend8(v, w);
+            }
+#pragma unroll
+            for (int j = 0; j < 8; ++j) e[j] -= P.lv[l].base;
+        }
+        if (idx)
+            for (int j = 0; j < 8; ++j) idx[(i * L + l) * 8 + j] = e[j];
+        if (cell)
+            for (int d = 0; d < 3; ++d) cell[(i * L + l) * 3 + d] = c[d];
+        if (frac)
+            for (int d = 0; d < 3; ++d) frac[(i * L + l) * 3 + d] = w[d];
+        if (feat) {
+            feat[i * P.in_dim + 2 * l] = f.x;
+            feat[i * P.in_dim + 2 * l + 1] = f.y;
+        }
+    }
+    if (feat) {
+        float sh[16];
+        sh16(nv, sh);
+        for (int k = 0; k < 16; ++k) feat[i * P.in_dim + 2 * L + k] = masked ? 0.f : sh[k];
+        for (uint32_t q = 0; q < P.n_params; ++q) {
+            float e[16];
+            param_encode8(P.t[q], e);
+            for (int k = 0; k < 16; ++k) feat[i * P.in_dim + 2 * L + 16 + 16 * q + k] = masked ? 0.f : e[k];
+        }
+    }
+}
+
+// =====================================================================================================
+// gather micro-benchmark
+// =====================================================================================================
+__device__ __forceinline__ uint32_t mix32(uint32_t x) {
+    x ^= x >> 16; x *= 0x7feb352du; x ^= x >> 15; x *= 0x846ca68bu; x ^= x >> 16;
+    return x;
+}
+
+__global__ void __launch_bounds__(256) niv_probe_gather_kernel(const uint32_t* __restrict__ buf, uint32_t word_mask,
+                                                               int pattern, uint32_t loads_per_lane, uint32_t seed,
+                                                               uint32_t* __restrict__ sink)
+{
+    const uint32_t gid = blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t wid = gid >> 5;
+    uint32_t acc = 0;
+    for (uint32_t it = 0; it < loads_per_lane; it += 8) {
+        uint32_t v[8];
+        uint2 v2[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            if (pattern == 0) {                 // every lane: its own random 4-byte word (random 32 B sector)
+                uint32_t a = mix32((gid * 0x9E3779B9u) ^ ((it + k) * 0x85EBCA6Bu) ^ seed) & word_mask;
+                v[k] = __ldg(buf + a);
+            } else if (pattern == 1) {          // random 128 B line per warp, lanes consecutive (coalesced)
+                uint32_t a = (mix32((wid * 0x9E3779B9u) ^ ((it + k) * 0x85EBCA6Bu) ^ seed) & word_mask & ~31u) + lane;
+                v[k] = __ldg(buf + a);
+            } else if (pattern == 2) {          // every lane: random aligned 8-byte pair, one 64-bit load
+                uint32_t a = mix32((gid * 0x9E3779B9u) ^ ((it + k) * 0x85EBCA6Bu) ^ seed) & word_mask & ~1u;
+                v2[k] = __ldg(reinterpret_cast<const uint2*>(buf + a));
+                v[k] = v2[k].x ^ v2[k].y;
+            } else {                            // groups of 8 lanes share one random 32 B sector (one word each)
+                uint32_t a = (mix32(((gid >> 3) * 0x9E3779B9u) ^ ((it + k) * 0x85EBCA6Bu) ^ seed) & word_mask & ~7u) + (lane & 7u);
+                v[k] = __ldg(buf + a);
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < 8; ++k) acc ^= v[k];
+    }
+    if (acc == 0x12345678u) sink[0] = acc;      // keep the loads alive
+}
+
+}  // namespace niv
+
+// =====================================================================================================
+// host side: the C ABI
+// =====================================================================================================
+using namespace niv;
+
+struct niv_model {
+    niv_config cfg;
+    niv_info info;
+    KParams kp;
+    uint32_t* d_table = nullptr;
+    uint8_t* d_wpack = nullptr;
+    std::vector<uint32_t> layer_out, layer_in;     // true (unpadded) shapes
+    bool loaded = false;
+    uint32_t grid_fused = 0;
+    uint32_t smem_fused = 0;
+};
+
+static thread_local int g_last_cuda_error = 0;
+
+#define NIV_CUDA(call)                                   \
+    do {                                                 \
+        cudaError_t e__ = (call);                        \
+        if (e__ != cudaSuccess) {                        \
+            g_last_cuda_error = (int)e__;                \
+            (void)cudaGetLastError();                    \
+            return NIV_ERR_CUDA;                         \
+        }                                                \
+    } while (0)
+
+static uint32_t round_up(uint32_t v, uint32_t m) { return (v + m - 1) / m * m; }
+
+template <int W>
+static int setup_fused(niv_model* m) {
+    NIV_CUDA(cudaFuncSetAttribute(niv_fused_kernel<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m->smem_fused));
+    int blocks = 0;
+    NIV_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks, niv_fused_kernel<W>, kTile, m->smem_fused));
+    const int tmem_cols = W < 32 ? 32 : W;
+    if (blocks > 512 / tmem_cols) blocks = 512 / tmem_cols;     // TMEM: 512 columns per SM
+    if (blocks < 1) return NIV_ERR_UNSUPPORTED;
+    m->info.ctas_per_sm = (uint32_t)blocks;
+    m->grid_fused = (uint32_t)blocks * m->info.num_sms;
+    return NIV_OK;
+}
+
+extern "C" int niv_create(const niv_config* cfg, niv_model** out)
+{
+    if (!cfg || !out) return NIV_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (cfg->struct_size != sizeof(niv_config) || cfg->api_version != NIV_API_VERSION) return NIV_ERR_INVALID_ARG;
+    if (cfg->n_levels == 0 || cfg->n_levels > NIV_MAX_LEVELS || cfg->n_features == 0) return NIV_ERR_INVALID_ARG;
+    if (cfg->log2_table_size < 4 || cfg->log2_table_size > 24) return NIV_ERR_INVALID_ARG;
+    if (cfg->n_hidden_layers == 0 || cfg->hidden_width == 0) return NIV_ERR_INVALID_ARG;
+    if (cfg->out_activation > NIV_OUT_SIGMOID) return NIV_ERR_INVALID_ARG;
+    for (int d = 0; d < 3; ++d) {
+        if (!std::isfinite(cfg->aabb_min[d]) || !std::isfinite(cfg->aabb_max[d])) return NIV_ERR_INVALID_ARG;
+        if (!(cfg->aabb_max[d] > cfg->aabb_min[d])) return NIV_ERR_INVALID_ARG;
+    }
+    bool explicit_res = false;
+    for (uint32_t l = 0; l < cfg->n_levels; ++l) explicit_res |= cfg->resolutions[l] != 0;
+    if (!explicit_res && (cfg->base_resolution == 0 || !(cfg->per_level_scale >= 1.0) || !std::isfinite(cfg->per_level_scale)))
+        return NIV_ERR_INVALID_ARG;
+    // shapes this build has kernels for
+    if (cfg->n_features != 2) return NIV_ERR_UNSUPPORTED;
+    if (cfg->n_levels % 4 != 0) return NIV_ERR_UNSUPPORTED;
+    if (cfg->sh_degree != 4 || cfg->n_params > 2 || (cfg->n_params && cfg->n_frequencies != 8)) return NIV_ERR_UNSUPPORTED;
+    if (cfg->n_hidden_layers > 3) return NIV_ERR_UNSUPPORTED;
+    if (cfg->hidden_width != 32 && cfg->hidden_width != 64 && cfg->hidden_width != 128) return NIV_ERR_UNSUPPORTED;
+
+    niv_model* m = new (std::nothrow) niv_model();
+    if (!m) return NIV_ERR_ALLOC;
+    m->cfg = *cfg;
+    niv_info& I = m->info;
+    memset(&I, 0, sizeof(I));
+    I.struct_size = sizeof(niv_info);
+    KParams& P = m->kp;
+    memset(&P, 0, sizeof(P));
+
+    // level table (readings #2, #4)
+    const uint64_t T = (uint64_t)1 << cfg->log2_table_size;
+    for (uint32_t l = 0; l < cfg->n_levels; ++l) {
+        uint64_t N;
+        if (explicit_res) N = cfg->resolutions[l];
+        else N = (uint64_t)std::floor((double)cfg->base_resolution * std::pow(cfg->per_level_scale, (double)l));
+        if (N == 0 || N >= (1u << 24)) { delete m; return NIV_ERR_INVALID_ARG; }
+        const uint64_t R = N + 1;
+        const bool dense = R * R * R <= T;
+        I.resolution[l] = (uint32_t)N;
+        I.is_dense[l] = dense ? 1u : 0u;
+        P.lv[l].Nf = (float)N;
+        P.lv[l].Nm1 = (int32_t)N - 1;
+        P.lv[l].R = (uint32_t)R;
+        P.lv[l].R2 = dense ? (uint32_t)(R * R) : 0u;
+        P.lv[l].base = (uint32_t)(l * T);
+        P.lv[l].dense = dense ? 1u : 0u;
+    }
+    for (int d = 0; d < 3; ++d) {
+        P.amin[d] = cfg->aabb_min[d];
+        volatile float ext = cfg->aabb_max[d] - cfg->aabb_min[d];
+        volatile float inv = 1.0f / ext;
+        P.ainv[d] = inv;
+    }
+    P.L = cfg->n_levels;
+    P.tmask = (uint32_t)(T - 1);
+    P.enc_dim = cfg->n_levels * cfg->n_features + 16;
+    P.in_dim = P.enc_dim + 2 * cfg->n_frequencies * cfg->n_params;
+    P.n_params = cfg->n_params;
+    P.n_layers = cfg->n_hidden_layers + 1;
+    P.out_act = cfg->out_activation;
+    I.in_dim = P.in_dim;
+    I.table_bytes = (uint64_t)cfg->n_levels * T * cfg->n_features * 2;
+    I.tile_texels = kTile;
+
+    // layer shapes and the packed weight blob layout
+    const uint32_t W = cfg->hidden_width;
+    uint32_t off = 0;
+    uint32_t in = P.in_dim;
+    for (uint32_t k = 0; k < P.n_layers; ++k) {
+        const uint32_t o = (k + 1 == P.n_layers) ? 3u : W;
+        m->layer_out.push_back(o);
+        m->layer_in.push_back(in);
+        I.weight_bytes += (uint64_t)o * in * 2;
+        I.bias_bytes += (uint64_t)o * 4;
+        P.kdim[k] = (k == 0) ? round_up(P.enc_dim, 16) : in;      // layer 1 consumes the encoded part only
+        P.npad[k] = round_up(o, 16);
+        P.w_off[k] = off;
+        off += P.kdim[k] * P.npad[k] * 2;
+        in = o;
+    }
+    for (uint32_t k = 0; k < P.n_layers; ++k) { P.b_off[k] = off; off += P.npad[k] * 4; }
+    P.wparam_off = off;
+    off += W * 16 * cfg->n_params * 4;
+    P.wpack_bytes = round_up(off, 16);
+    uint32_t kmax = P.kdim[0];
+    for (uint32_t k = 1; k < P.n_layers; ++k) kmax = kmax > P.kdim[k] ? kmax : P.kdim[k];
+    P.a_off = round_up(P.wpack_bytes, 128);
+    P.misc_off = P.a_off + kTile * kmax * 2;
+    m->smem_fused = P.misc_off + W * 4 + 2 * 8 + 16;
+    I.smem_bytes = m->smem_fused;
+
+    // device side
+    g_last_cuda_error = 0;
+    int rc = NIV_OK;
+    cudaError_t e = cudaSetDevice(cfg->device);
+    cudaDeviceProp prop;
+    if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, cfg->device);
+    if (e != cudaSuccess) { g_last_cuda_error = (int)e; (void)cudaGetLastError(); delete m; return NIV_ERR_CUDA; }
+    if (prop.major != 10) { delete m; return NIV_ERR_UNSUPPORTED; }           // sm_100a only; no fallback
+    I.num_sms = (uint32_t)prop.multiProcessorCount;
+    if (W == 32) rc = setup_fused<32>(m);
+    else if (W == 64) rc = setup_fused<64>(m);
+    else rc = setup_fused<128>(m);
+    if (rc != NIV_OK) { delete m; return rc; }
+    e = cudaMalloc(&m->d_table, I.table_bytes);
+    if (e == cudaSuccess) e = cudaMalloc(&m->d_wpack, P.wpack_bytes);
+    if (e != cudaSuccess) {
+        g_last_cuda_error = (int)e; (void)cudaGetLastError();
+        cudaFree(m->d_table); cudaFree(m->d_wpack); delete m;
+        return NIV_ERR_ALLOC;
+    }
+    P.table = m->d_table;
+    P.wpack = m->d_wpack;
+    *out = m;
+    return NIV_OK;
+}
+
+extern "C" int niv_get_info(const niv_model* m, niv_info* info)
+{
+    if (!m || !info) return NIV_ERR_INVALID_ARG;
+    *info = m->info;
+    return NIV_OK;
+}
+
+extern "C" int niv_load_params(niv_model* m, const void* table_fp16, size_t table_bytes,
+                               const void* weights_fp16, size_t weight_bytes,
+                               const float* biases_f32, size_t bias_bytes, int src_on_device, void* stream)
+{
+    if (!m || !table_fp16 || !weights_fp16) return NIV_ERR_INVALID_ARG;
+    if (table_bytes != m->info.table_bytes || weight_bytes != m->info.weight_bytes) return NIV_ERR_INVALID_ARG;
+    if (biases_f32 ? bias_bytes != m->info.bias_bytes : bias_bytes != 0) return NIV_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    NIV_CUDA(cudaSetDevice(m->cfg.device));
+    const KParams& P = m->kp;
+
+    // host copies of the small blobs
+    std::vector<uint16_t> w(weight_bytes / 2);
+    std::vector<float> b(m->info.bias_bytes / 4, 0.0f);
+    if (src_on_device) {
+        NIV_CUDA(cudaMemcpyAsync(w.data(), weights_fp16, weight_bytes, cudaMemcpyDeviceToHost, st));
+        if (biases_f32) NIV_CUDA(cudaMemcpyAsync(b.data(), biases_f32, bias_bytes, cudaMemcpyDeviceToHost, st));
+        NIV_CUDA(cudaStreamSynchronize(st));
+    } else {
+        memcpy(w.data(), weights_fp16, weight_bytes);
+        if (biases_f32) memcpy(b.data(), biases_f32, bias_bytes);
+    }
+
+    // pack: per layer, the UMMA K-major no-swizzle layout of B = W[out][in]:
+    //   element (n, k) at  (k/8) * (Npad*16) + n*16 + (k%8)*2  bytes; rows n >= out and columns k >= in are zero.
+    std::vector<uint8_t> pack(P.wpack_bytes, 0);
+    size_t wsrc = 0, bsrc = 0;
+    for (uint32_t k = 0; k < P.n_layers; ++k) {
+        const uint32_t o = m->layer_out[k], in = m->layer_in[k];
+        const uint32_t kuse = (k == 0) ? P.enc_dim : in;
+        uint16_t* dst = reinterpret_cast<uint16_t*>(pack.data() + P.w_off[k]);
+        for (uint32_t r = 0; r < o; ++r)
+            for (uint32_t c = 0; c < kuse; ++c)
+                dst[(size_t)(c >> 3) * (P.npad[k] * 8) + r * 8 + (c & 7)] = w[wsrc + (size_t)r * in + c];
+        if (k == 0 && P.n_params) {
+            float* wp = reinterpret_cast<float*>(pack.data() + P.wparam_off);
+            const uint32_t np16 = 16 * P.n_params;
+            for (uint32_t r = 0; r < o; ++r)
+                for (uint32_t c = 0; c < np16; ++c) {
+                    __half_raw hr; hr.x = w[wsrc + (size_t)r * in + P.enc_dim + c];
+                    wp[r * np16 + c] = __half2float(__half(hr));
+                }
+        }
+        float* bd = reinterpret_cast<float*>(pack.data() + P.b_off[k]);
+        for (uint32_t r = 0; r < o; ++r) bd[r] = b[bsrc + r];
+        wsrc += (size_t)o * in;
+        bsrc += o;
+    }
+    NIV_CUDA(cudaMemcpyAsync(m->d_wpack, pack.data(), P.wpack_bytes, cudaMemcpyHostToDevice, st));
+    NIV_CUDA(cudaMemcpyAsync(m->d_table, table_fp16, table_bytes,
+                             src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+    NIV_CUDA(cudaStreamSynchronize(st));
+    m->loaded = true;
+    return NIV_OK;
+}
+
+static int fill_params(const niv_model* m, const float* param, KParams& P)
+{
+    P = m->kp;
+    if (m->cfg.n_params) {
+        if (!param) return NIV_ERR_INVALID_ARG;
+        for (uint32_t q = 0; q < m->cfg.n_params; ++q) P.t[q] = param[q];
+    } else if (param) {
+        return NIV_ERR_INVALID_ARG;
+    }
+    return NIV_OK;
+}
+
+extern "C" int niv_infer(niv_model* m, const float* pos, const float* nrm, const float* param,
+                         float* out, size_t n, void* stream)
+{
+    if (!m) return NIV_ERR_INVALID_ARG;
+    if (!m->loaded) return NIV_ERR_NOT_LOADED;
+    if (n == 0) return NIV_OK;
+    if (!pos || !nrm || !out) return NIV_ERR_INVALID_ARG;
+    if (n > ((size_t)1 << 31)) return NIV_ERR_INVALID_ARG;
+    KParams P;
+    int rc = fill_params(m, param, P);
+    if (rc != NIV_OK) return rc;
+    const uint32_t n_tiles = (uint32_t)((n + kTile - 1) / kTile);
+    const uint32_t grid = n_tiles < m->grid_fused ? n_tiles : m->grid_fused;
+    cudaStream_t st = (cudaStream_t)stream;
+    switch (m->cfg.hidden_width) {
+        case 32:  niv_fused_kernel<32><<<grid, kTile, m->smem_fused, st>>>(P, pos, nrm, out, n, n_tiles); break;
+        case 64:  niv_fused_kernel<64><<<grid, kTile, m->smem_fused, st>>>(P, pos, nrm, out, n, n_tiles); break;
+        default:  niv_fused_kernel<128><<<grid, kTile, m->smem_fused, st>>>(P, pos, nrm, out, n, n_tiles); break;
+    }
+    NIV_CUDA(cudaGetLastError());
+    return NIV_OK;
+}
+
+extern "C" int niv_encode(niv_model* m, const float* pos, const float* nrm, const float* param,
+                          void* features_fp16, size_t n, void* stream)
+{
+    if (!m) return NIV_ERR_INVALID_ARG;
+    if (!m->loaded) return NIV_ERR_NOT_LOADED;
+    if (n == 0) return NIV_OK;
+    if (!pos || !nrm || !features_fp16 || ((uintptr_t)features_fp16 & 15)) return NIV_ERR_INVALID_ARG;
+    KParams P;
+    int rc = fill_params(m, param, P);
+    if (rc != NIV_OK) return rc;
+    const unsigned grid = (unsigned)((n + 127) / 128);
+    niv_encode_kernel<<<grid, 128, 0, (cudaStream_t)stream>>>(P, pos, nrm, (uint4*)features_fp16, n);
+    NIV_CUDA(cudaGetLastError());
+    return NIV_OK;
+}
+
+extern "C" int niv_debug_encode(niv_model* m, const float* pos, const float* nrm, const float* param, size_t n,
+                                uint32_t* idx, int32_t* cell, float* frac, float* features, void* stream)
+{
+    if (!m) return NIV_ERR_INVALID_ARG;
+    if (!m->loaded) return NIV_ERR_NOT_LOADED;
+    if (n == 0) return NIV_OK;
+    if (!pos || !nrm) return NIV_ERR_INVALID_ARG;
+    KParams P;
+    int rc = fill_params(m, param, P);
+    if (rc != NIV_OK) return rc;
+    const unsigned grid = (unsigned)((n + 127) / 128);
+    niv_debug_kernel<<<grid, 128, 0, (cudaStream_t)stream>>>(P, pos, nrm, n, idx, cell, frac, features);
+    NIV_CUDA(cudaGetLastError());
+    return NIV_OK;
+}
+
+extern "C" int niv_destroy(niv_model* m)
+{
+    if (!m) return NIV_OK;
+    cudaSetDevice(m->cfg.device);
+    cudaFree(m->d_table);
+    cudaFree(m->d_wpack);
+    delete m;
+    return NIV_OK;
+}
+
+extern "C" const char* niv_error_string(int code)
+{
+    switch (code) {
+        case NIV_OK: return "ok";
+        case NIV_ERR_INVALID_ARG: return "invalid argument";
+        case NIV_ERR_UNSUPPORTED: return "configuration not supported by this build (sm_100a kernels only)";
+        case NIV_ERR_NOT_LOADED: return "parameters not loaded";
+        case NIV_ERR_CUDA: return "CUDA runtime error (see niv_last_cuda_error)";
+        case NIV_ERR_ALLOC: return "allocation failed";
+        default: return "unknown error code";
+    }
+}
+
+extern "C" int niv_last_cuda_error(void) { return g_last_cuda_error; }
+
+extern "C" int niv_probe_gather(const void* buf, size_t buf_bytes, int pattern, uint32_t n_ctas,
+                                uint32_t loads_per_lane, uint32_t seed, void* sink, void* stream)
+{
+    if (!buf || !sink || buf_bytes < 4096 || (buf_bytes & (buf_bytes - 1)) || buf_bytes > ((size_t)1 << 33))
+        return NIV_ERR_INVALID_ARG;
+    if (pattern < 0 || pattern > 3 || n_ctas == 0 || loads_per_lane == 0 || (loads_per_lane & 7)) return NIV_ERR_INVALID_ARG;
+    const uint32_t word_mask = (uint32_t)(buf_bytes / 4 - 1);
+    niv_probe_gather_kernel<<<n_ctas, 256, 0, (cudaStream_t)stream>>>((const uint32_t*)buf, word_mask, pattern,
+                                                                     loads_per_lane, seed, (uint32_t*)sink);
+    NIV_CUDA(cudaGetLastError());
+    return NIV_OK;
+}
