@@ -1,0 +1,400 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the fused NIV inference path (BASELINE.json metric) on N B200s.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload fullhd|incoherent|param] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path (niv_infer: one fused kernel, rows a0..a12 of DESIGN.md) over one
+1920x1080 G-buffer per GPU.  Prints ONE JSON line on rank 0 (contract in the task statement / DESIGN.md sec. 7).
+
+  value / ms_per_step   device-resident inputs, CUDA events on the launching stream, max over ranks
+  e2e                   niv_infer_host: pinned HOST buffers in, HOST buffer out, copies inside the timed region
+  roofline              gather roofline (measured random-sector rate, sector census of this very frame), with the
+                        tensor and HBM rooflines beside it; frac = slowest roofline time / measured time
+  cpu_baseline          the oracle, as it stands, on this box's host cores over a bounded sample (rank 0, N=1)
+
+--impl reference times the CPU oracle instead (this tier's reference arm).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2602_12949_b200 import inputs as I  # noqa: E402
+
+W_PX, H_PX = 1920, 1080
+N_TEXELS = W_PX * H_PX
+METRIC = "NIV fused inference throughput on a 1920x1080 G-buffer (ms_per_step = ms per frame)"
+UNIT = "Gqueries/s"
+RING = 8                      # distinct input/output buffer sets rotated between steps (8 x 74.6 MB > 126 MB L2)
+
+
+def _env_int(name, default):
+    try:
+        return int(os.environ.get(name, default))
+    except ValueError:
+        return default
+
+
+def make_workload(name: str, frame: int):
+    """-> spec, table, wblob, bblob, pos, nrm, param, description"""
+    if name == "param":
+        spec, param = I.spec_param(), [0.625]
+    else:
+        spec, param = I.spec_fullhd(), None
+    table = I.make_table(spec, 0)
+    w, b = I.make_mlp(spec, 0)
+    if name == "incoherent":
+        pos = I.positions_uniform(N_TEXELS, (spec.aabb_min, spec.aabb_max), frame)
+        nrm = I.normals_uniform(N_TEXELS, frame)
+        desc = "configs[2]: 2,073,600 i.i.d. queries in the room AABB, normals uniform on S^2"
+        masked = 0.0
+    else:
+        g = I.make_gbuffer(W_PX, H_PX, 0, frame=frame)
+        pos, nrm, masked = g["pos"], g["nrm"], g["masked_fraction"]
+        desc = ("configs[%d]: 1920x1080 G-buffer ray-cast from the seeded procedural room (16 spheres + 16 boxes), "
+                "%.1f%% background texels" % (3 if name == "param" else 1, 100 * masked))
+    return spec, table, I.pack_weights(w), I.pack_biases(b), pos, nrm, param, desc, masked
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return {"hbm_gbs": float(d["hbm_gbs"]), "tflops_burst": float(d["bf16_tflops"]),
+                "tflops_sustained": float(d.get("bf16_tflops_sustained", d["bf16_tflops"])), "source": "measured"}
+    return {"hbm_gbs": 6650.0, "tflops_burst": 1590.0, "tflops_sustained": 1400.0, "source": "fallback"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "50"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0]))
+                mx.append(float(c[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        os.unlink(self.f.name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(pos, nrm, n_sample):
+    """Every k-th 128-texel tile of the frame, so the sample has the frame's mix of coherent / masked texels."""
+    n = pos.shape[0]
+    tiles = n // 128
+    want_tiles = max(1, min(tiles, n_sample // 128))
+    sel_t = np.linspace(0, tiles - 1, want_tiles).astype(np.int64)
+    sel = (sel_t[:, None] * 128 + np.arange(128)[None, :]).reshape(-1)
+    return np.ascontiguousarray(pos[sel]), np.ascontiguousarray(nrm[sel]), sel.size
+
+
+def time_oracle(spec, table, wb, bb, pos, nrm, param, budget_s):
+    """The oracle as it stands on all host cores, on a sample sized for ~budget_s seconds."""
+    from oracle import niv_oracle
+    niv_oracle.build()
+    prm = None if param is None else np.float32(param)
+    cal_p, cal_n, cal = oracle_sample(pos, nrm, 32768)
+    t0 = time.perf_counter()
+    niv_oracle.infer(spec, table, wb, bb, cal_p, cal_n, param=prm)
+    rate = cal / (time.perf_counter() - t0)
+    n_s = int(min(pos.shape[0], max(32768, rate * budget_s)))
+    sp, sn, n_s = oracle_sample(pos, nrm, n_s)
+    t0 = time.perf_counter()
+    niv_oracle.infer(spec, table, wb, bb, sp, sn, param=prm)
+    dt = time.perf_counter() - t0
+    return n_s, dt, niv_oracle.max_threads()
+
+
+def run_reference(args):
+    """Reference arm of this tier = the CPU oracle, timed on this box's host cores (rank 0 only)."""
+    if _env_int("RANK", 0) != 0:
+        return
+    from oracle import niv_oracle
+    niv_oracle.build()
+    spec, table, wb, bb, pos, nrm, param, desc, masked = make_workload(args.workload, 0)
+    prm = None if param is None else np.float32(param)
+    sp, sn, n_s = oracle_sample(pos, nrm, args.ref_sample)
+    for _ in range(args.warmup):
+        niv_oracle.infer(spec, table, wb, bb, sp, sn, param=prm)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        niv_oracle.infer(spec, table, wb, bb, sp, sn, param=prm)
+    dt = (time.perf_counter() - t0) / args.steps
+    val = n_s / dt / 1e9
+    cores = niv_oracle.max_threads()
+    sample = "%d of %d texels per step (every k-th 128-texel tile of the frame)" % (n_s, N_TEXELS)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "ms_per_frame_extrapolated":
+        dt * 1e3 * N_TEXELS / n_s, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "description": desc, "model": _model_str(spec)},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def _model_str(spec):
+    dims = [spec.in_dim] + [spec.hidden_width] * spec.n_hidden_layers + [3]
+    return "hash grid L=%d F=%d T=2^%d N0=%d b=%g; SH-16%s; MLP %s fp16 weights / fp32 accumulate; %s output" % (
+        spec.n_levels, spec.n_features, spec.log2_table_size, spec.base_resolution, spec.per_level_scale,
+        "; %d param(s) x 8 sin/cos" % spec.n_params if spec.n_params else "", "->".join(map(str, dims)),
+        "sigmoid" if spec.out_activation == I.OUT_SIGMOID else "linear")
+
+
+def measure_gather_peak(torch, niv, table_bytes, num_sms):
+    """Random 32-byte-sector gather rate from a resident buffer of the tables' size (SURVEY.md 8(d) BW_L2g),
+    and the same with 8 lanes sharing a sector.  Returns GB/s of sector traffic."""
+    nbytes = 1 << int(np.ceil(np.log2(table_bytes)))
+    buf = torch.zeros(nbytes // 4, dtype=torch.int32, device="cuda")
+    sink = torch.zeros(4, dtype=torch.int32, device="cuda")
+    res = {}
+    n_ctas, lpl = num_sms * 8, 256
+    for name, pattern, sectors_per_load in (("random_sector", 0, 1.0), ("shared_sector_x8", 3, 1.0 / 8)):
+        for _ in range(3):
+            niv.probe_gather(buf, pattern, n_ctas, lpl, 1, sink)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps = 10
+        e0.record()
+        for r in range(reps):
+            niv.probe_gather(buf, pattern, n_ctas, lpl, 100 + r, sink)
+        e1.record()
+        torch.cuda.synchronize()
+        dt = e0.elapsed_time(e1) * 1e-3 / reps
+        loads = n_ctas * 256 * lpl
+        res[name] = {"gloads_per_s": loads / dt / 1e9, "sector_gbs": loads * sectors_per_load * 32 / dt / 1e9}
+    del buf
+    return res, nbytes
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    from paper_2602_12949_b200 import build as B
+    from paper_2602_12949_b200 import niv
+
+    rank, world, local = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        B.build()
+    if world > 1:
+        dist.barrier()
+    niv.lib()
+
+    # each rank owns one full frame per step (weak scaling: texels shard, the model is replicated)
+    spec, table, wb, bb, pos, nrm, param, desc, masked = make_workload(args.workload, rank)
+    n = pos.shape[0]
+    model = niv.NivModel(spec, local)
+    model.load_params(table, wb, bb)
+    info = model.info
+
+    d_pos = [torch.from_numpy(pos).cuda() for _ in range(RING)]
+    d_nrm = [torch.from_numpy(nrm).cuda() for _ in range(RING)]
+    d_out = [torch.empty((n, 3), dtype=torch.float32, device="cuda") for _ in range(RING)]
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing ---------------------------------------------------------------------
+    for s in range(args.warmup):
+        model.infer(d_pos[s % RING], d_nrm[s % RING], d_out[s % RING], param=param)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    barrier()
+    clocks = ClockSampler(local) if rank == 0 else None
+    ev[0].record(stream)
+    for s in range(args.steps):
+        k = s % RING
+        model.infer(d_pos[k], d_nrm[k], d_out[k], param=param)
+        ev[s + 1].record(stream)
+    barrier()
+    total_ms = ev[0].elapsed_time(ev[-1])
+    per = np.array([ev[s].elapsed_time(ev[s + 1]) for s in range(args.steps)])
+    # clocks keep sampling a little longer so that short runs still get a few samples under load
+    t_end = time.time() + 0.3
+    while time.time() < t_end:
+        model.infer(d_pos[0], d_nrm[0], d_out[0], param=param)
+        torch.cuda.synchronize()
+    clk = clocks.stop() if clocks else None
+    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t.item())
+    ms_step = total_ms / args.steps
+    value = world * n / (ms_step * 1e-3) / 1e9
+
+    # ---- end to end: pinned host buffers through niv_infer_host ------------------------------------
+    e2e_steps = max(3, min(args.steps, 20))
+    h_pos = [torch.from_numpy(pos).pin_memory() for _ in range(2)]
+    h_nrm = [torch.from_numpy(nrm).pin_memory() for _ in range(2)]
+    h_out = [torch.empty((n, 3), dtype=torch.float32).pin_memory() for _ in range(2)]
+    for s in range(3):
+        model.infer_host(h_pos[s % 2], h_nrm[s % 2], h_out[s % 2], param=param)
+    barrier()
+    t0 = time.perf_counter()
+    for s in range(e2e_steps):
+        model.infer_host(h_pos[s % 2], h_nrm[s % 2], h_out[s % 2], param=param)   # synchronises: out has landed
+    torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
+    t = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_ms = float(t.item())
+    e2e_value = world * n / (e2e_ms * 1e-3) / 1e9
+    checksum = float(h_out[0].sum())
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- rooflines (rank 0) -------------------------------------------------------------------------
+    peaks = load_peaks()
+    counts = torch.zeros(33, dtype=torch.int64, device="cuda")
+    model.probe_sectors(d_pos[0], d_nrm[0], counts)
+    torch.cuda.synchronize()
+    c = counts.cpu().numpy()
+    L = spec.n_levels
+    sectors, lines, n_active = int(c[:L].sum()), int(c[16:16 + L].sum()), int(c[32])
+    gpeak, probe_bytes = measure_gather_peak(torch, niv, info.table_bytes, info.num_sms)
+    kernel_s = float(np.mean(per)) * 1e-3               # one fused kernel per step
+    dims = [spec.in_dim] + [spec.hidden_width] * spec.n_hidden_layers + [3]
+    flop_texel = 2 * sum(dims[i] * dims[i + 1] for i in range(len(dims) - 1))
+    hbm_bytes = 36 * n
+    t_gather = sectors * 32 / (gpeak["random_sector"]["sector_gbs"] * 1e9)
+    t_tensor = flop_texel * n / (peaks["tflops_sustained"] * 1e12)
+    t_hbm = hbm_bytes / (peaks["hbm_gbs"] * 1e9)
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tp):
+        with open(tp) as f:
+            traffic = json.load(f).get(args.workload)
+    roofline = {
+        "bound": "l2-gather", "kernel": "niv_fused_kernel",
+        "achieved": sectors * 32 / kernel_s / 1e9, "peak": gpeak["random_sector"]["sector_gbs"], "unit": "GB/s",
+        "frac": max(t_gather, t_tensor, t_hbm) / kernel_s, "traffic": traffic,
+        "peak_source": "measured in this run: niv_probe_gather, random 32 B sectors of a resident %d MiB buffer"
+                       % (probe_bytes >> 20),
+        "algorithmic": {"sectors_per_launch": sectors, "sectors_per_active_texel": sectors / max(n_active, 1),
+                        "lines_per_active_texel": lines / max(n_active, 1), "active_texels": n_active,
+                        "gathers_per_active_texel": 8 * L, "sectors_per_level": [int(v) for v in c[:L]]},
+        "gather_rate_ggathers_per_s": 8 * L * n_active / kernel_s / 1e9,
+        "probe": gpeak,
+        "t_roofline_us": {"l2_gather": t_gather * 1e6, "tensor": t_tensor * 1e6, "hbm": t_hbm * 1e6},
+        "tensor": {"achieved": flop_texel * n / kernel_s / 1e12, "peak": peaks["tflops_sustained"],
+                   "unit": "TFLOP/s", "frac": t_tensor / kernel_s, "peak_source": peaks["source"] + " bf16 sustained (fp16 = same rate)"},
+        "hbm": {"achieved": hbm_bytes / kernel_s / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "frac": t_hbm / kernel_s, "peak_source": peaks["source"]},
+        "kernel_ms": {"mean": float(np.mean(per)), "median": float(np.median(per)), "min": float(np.min(per))},
+    }
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        n_s, dt, cores = time_oracle(spec, table, wb, bb, pos, nrm, param, args.cpu_budget)
+        cpu = {"value": n_s / dt / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": "%d of %d texels (every k-th 128-texel tile of the frame), %.1f s" % (n_s, n, dt),
+               "ms_per_frame_extrapolated": dt * 1e3 * n / n_s}
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f16 operands / f32 accumulate (index path: f32 + u32)", "data": "synthetic",
+        "config": {"workload": args.workload, "description": desc, "model": _model_str(spec),
+                   "texels_per_gpu_per_step": n, "masked_fraction": masked, "parallelism": "dp%d (replicated model, "
+                   "texels sharded, no data-path collective)" % world,
+                   "l2": "inputs/outputs rotate over %d distinct buffer sets (%.0f MB > 126 MB L2) so G-buffer reads "
+                         "come from HBM; the %.0f MiB table stays L2-resident by design" %
+                         (RING, RING * 36 * n / 1e6, info.table_bytes / 2 ** 20),
+                   "grid": "%d CTAs = %d SMs x %d, %d texels per tile" % (info.num_sms * info.ctas_per_sm,
+                                                                         info.num_sms, info.ctas_per_sm,
+                                                                         info.tile_texels)},
+        "active_gqueries_per_s": value * (1.0 - masked),
+        "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms, "steps": e2e_steps,
+                "h2d_bytes_per_step": 24 * n, "d2h_bytes_per_step": 12 * n,
+                "api": "niv_infer_host (pinned host buffers; chunked H2D / kernel / D2H overlap)",
+                "checksum": checksum},
+        "gpu_launches": args.steps, "clocks": clk, "roofline": roofline,
+    }
+    if cpu:
+        out["cpu_baseline"] = cpu
+    print(json.dumps(out))
+    model.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="fullhd", choices=["fullhd", "incoherent", "param"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle wall time for cpu_baseline")
+    ap.add_argument("--ref-sample", type=int, default=131072, help="texels per step of the reference arm")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        args.steps = 5 if args.steps is None else args.steps
+        args.warmup = 1 if args.warmup is None else args.warmup
+        run_reference(args)
+    else:
+        args.steps = 200 if args.steps is None else args.steps
+        args.warmup = 20 if args.warmup is None else max(args.warmup, 3)
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -115,6 +115,17 @@ int niv_load_params(niv_model *m, const void *table_fp16, size_t table_bytes,
 int niv_infer(niv_model *m, const float *pos, const float *nrm, const float *param,
               float *out, size_t n, void *stream);
 
+/* The same operation with HOST buffers (the end-to-end call: PAPER.md:402-403 with the G-buffer in host memory).
+ *   pos, nrm, out  HOST, [n][3] fp32 packed (pinned memory gives asynchronous copies; pageable memory works)
+ *   param          HOST, as niv_infer
+ * The frame is cut into chunks; each chunk's host->device copies, fused kernel and device->host copy are
+ * queued on internal streams so that the copies of one chunk overlap the kernel of another.  Staging buffers
+ * are owned by the model and grown on demand (this call MAY allocate).  `stream` is waited on before the first
+ * copy and the call returns only after the last byte of `out` has landed (it synchronises).  NOT safe for
+ * concurrent callers on the same model.  Errors as niv_infer, plus NIV_ERR_ALLOC. */
+int niv_infer_host(niv_model *m, const float *pos, const float *nrm, const float *param,
+                   float *out, size_t n, void *stream);
+
 /* Stand-alone encoding kernel (rows a1..a9 without the MLP): features_fp16 is device, [n][in_dim] fp16
  * row-major = [latents | SH-16 | parameter encoding], zero rows for background texels. */
 int niv_encode(niv_model *m, const float *pos, const float *nrm, const float *param,
@@ -141,6 +152,13 @@ int niv_last_cuda_error(void);
  * buf is device memory of `buf_bytes` (power of two); sink is device, >= 4 bytes.  Asynchronous. */
 int niv_probe_gather(const void *buf, size_t buf_bytes, int pattern, uint32_t n_ctas, uint32_t loads_per_lane,
                      uint32_t seed, void *sink, void *stream);
+
+/* niv_probe_sectors: the sector census behind the gather roofline ("S = number of 32-byte sectors
+ * the frame algorithmically needs at warp granularity").  For every group of 32 consecutive texels (the fused
+ * kernel's texel -> warp map) and every level, counts the DISTINCT 32-byte sectors and 128-byte lines among the
+ * group's <= 256 corner addresses.  counts is device, 33 x uint64: [0,16) sectors per level, [16,32) lines per
+ * level, [32] active (unmasked) texels.  Asynchronous; counts is zeroed first on `stream`. */
+int niv_probe_sectors(niv_model *m, const float *pos, const float *nrm, size_t n, uint64_t *counts, void *stream);
 
 #ifdef __cplusplus
 }

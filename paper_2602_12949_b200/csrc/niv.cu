@@ -337,6 +337,65 @@ __global__ void __launch_bounds__(256) niv_probe_gather_kernel(const uint32_t* _
     if (acc == 0x12345678u) sink[0] = acc;      // keep the loads alive
 }
 
+// =====================================================================================================
+// sector census: the S of the gather roofline
+// =====================================================================================================
+// One warp per group of 32 consecutive texels (the fused kernel's own texel -> warp map).  For every level the
+// warp's <= 256 corner addresses are reduced to the number of DISTINCT 32-byte sectors (and distinct 128-byte
+// lines); the per-level counts are summed over the grid.  counts[0..L) = sectors, counts[16..16+L) = lines,
+// counts[32] = active texels.
+__global__ void __launch_bounds__(128) niv_sector_census_kernel(const __grid_constant__ KParams P,
+                                                                const float* __restrict__ pos,
+                                                                const float* __restrict__ nrm, size_t n,
+                                                                unsigned long long* __restrict__ counts)
+{
+    __shared__ uint32_t s_sec[4][256];
+    const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    float p[3] = {0.f, 0.f, 0.f}, nv[3] = {0.f, 0.f, 0.f};
+    const bool valid = i < n;
+    if (valid) { load3(pos, i, p); load3(nrm, i, nv); }
+    const bool masked = !valid || texel_masked(p, nv);
+    float u[3] = {0.f, 0.f, 0.f};
+    if (!masked) normalise(P, p, u);
+    const uint32_t n_act = __popc(__ballot_sync(0xffffffffu, !masked));
+    if (lane == 0 && n_act) atomicAdd(&counts[32], (unsigned long long)n_act);
+    for (uint32_t l = 0; l < P.L; ++l) {
+        uint32_t e[8];
+        if (!masked) {
+            int c[3]; float w[3];
+            locate(P.lv[l], u, c, w);
+            corner_entries(P.lv[l], P.tmask, c, e);
+        }
+#pragma unroll
+        for (int j = 0; j < 8; ++j) s_sec[warp][lane * 8 + j] = masked ? 0xFFFFFFFFu : (e[j] >> 3);   // 8 entries per sector
+        __syncwarp();
+        uint32_t sec = 0, lin = 0;
+        for (int q = 0; q < 8; ++q) {
+            const uint32_t me = lane * 8 + q;
+            const uint32_t v = s_sec[warp][me];
+            if (v == 0xFFFFFFFFu) continue;
+            bool first_s = true, first_l = true;
+            for (uint32_t k = 0; k < me; ++k) {
+                const uint32_t o = s_sec[warp][k];
+                if (o == 0xFFFFFFFFu) continue;
+                first_s &= (o != v);
+                first_l &= ((o >> 2) != (v >> 2));
+            }
+            sec += first_s; lin += first_l;
+        }
+        for (int o = 16; o; o >>= 1) {
+            sec += __shfl_xor_sync(0xffffffffu, sec, o);
+            lin += __shfl_xor_sync(0xffffffffu, lin, o);
+        }
+        if (lane == 0 && sec) {
+            atomicAdd(&counts[l], (unsigned long long)sec);
+            atomicAdd(&counts[16 + l], (unsigned long long)lin);
+        }
+        __syncwarp();
+    }
+}
+
 }  // namespace niv
 
 // =====================================================================================================
@@ -354,6 +413,11 @@ struct niv_model {
     bool loaded = false;
     uint32_t grid_fused = 0;
     uint32_t smem_fused = 0;
+    // niv_infer_host staging (grown on demand)
+    float* d_stage = nullptr;          // [pos | nrm | out], each 3*stage_cap floats
+    size_t stage_cap = 0;
+    cudaStream_t hs[2] = {nullptr, nullptr};
+    cudaEvent_t hev = nullptr;
 };
 
 static thread_local int g_last_cuda_error = 0;
@@ -579,6 +643,20 @@ static int fill_params(const niv_model* m, const float* param, KParams& P)
     return NIV_OK;
 }
 
+static int launch_fused(const niv_model* m, const KParams& P, const float* pos, const float* nrm, float* out,
+                        size_t n, cudaStream_t st)
+{
+    const uint32_t n_tiles = (uint32_t)((n + kTile - 1) / kTile);
+    const uint32_t grid = n_tiles < m->grid_fused ? n_tiles : m->grid_fused;
+    switch (m->cfg.hidden_width) {
+        case 32:  niv_fused_kernel<32><<<grid, kTile, m->smem_fused, st>>>(P, pos, nrm, out, n, n_tiles); break;
+        case 64:  niv_fused_kernel<64><<<grid, kTile, m->smem_fused, st>>>(P, pos, nrm, out, n, n_tiles); break;
+        default:  niv_fused_kernel<128><<<grid, kTile, m->smem_fused, st>>>(P, pos, nrm, out, n, n_tiles); break;
+    }
+    NIV_CUDA(cudaGetLastError());
+    return NIV_OK;
+}
+
 extern "C" int niv_infer(niv_model* m, const float* pos, const float* nrm, const float* param,
                          float* out, size_t n, void* stream)
 {
@@ -590,15 +668,55 @@ extern "C" int niv_infer(niv_model* m, const float* pos, const float* nrm, const
     KParams P;
     int rc = fill_params(m, param, P);
     if (rc != NIV_OK) return rc;
-    const uint32_t n_tiles = (uint32_t)((n + kTile - 1) / kTile);
-    const uint32_t grid = n_tiles < m->grid_fused ? n_tiles : m->grid_fused;
-    cudaStream_t st = (cudaStream_t)stream;
-    switch (m->cfg.hidden_width) {
-        case 32:  niv_fused_kernel<32><<<grid, kTile, m->smem_fused, st>>>(P, pos, nrm, out, n, n_tiles); break;
-        case 64:  niv_fused_kernel<64><<<grid, kTile, m->smem_fused, st>>>(P, pos, nrm, out, n, n_tiles); break;
-        default:  niv_fused_kernel<128><<<grid, kTile, m->smem_fused, st>>>(P, pos, nrm, out, n, n_tiles); break;
+    return launch_fused(m, P, pos, nrm, out, n, (cudaStream_t)stream);
+}
+
+extern "C" int niv_infer_host(niv_model* m, const float* pos, const float* nrm, const float* param,
+                              float* out, size_t n, void* stream)
+{
+    if (!m) return NIV_ERR_INVALID_ARG;
+    if (!m->loaded) return NIV_ERR_NOT_LOADED;
+    if (n == 0) return NIV_OK;
+    if (!pos || !nrm || !out) return NIV_ERR_INVALID_ARG;
+    if (n > ((size_t)1 << 31)) return NIV_ERR_INVALID_ARG;
+    KParams P;
+    int rc = fill_params(m, param, P);
+    if (rc != NIV_OK) return rc;
+    NIV_CUDA(cudaSetDevice(m->cfg.device));
+    if (!m->hs[0]) {
+        NIV_CUDA(cudaStreamCreateWithFlags(&m->hs[0], cudaStreamNonBlocking));
+        NIV_CUDA(cudaStreamCreateWithFlags(&m->hs[1], cudaStreamNonBlocking));
+        NIV_CUDA(cudaEventCreateWithFlags(&m->hev, cudaEventDisableTiming));
     }
-    NIV_CUDA(cudaGetLastError());
+    if (n > m->stage_cap) {
+        if (m->d_stage) { NIV_CUDA(cudaFree(m->d_stage)); m->d_stage = nullptr; m->stage_cap = 0; }
+        const size_t cap = (n + 1023) / 1024 * 1024;
+        cudaError_t e = cudaMalloc(&m->d_stage, cap * 9 * sizeof(float));
+        if (e != cudaSuccess) { g_last_cuda_error = (int)e; (void)cudaGetLastError(); return NIV_ERR_ALLOC; }
+        m->stage_cap = cap;
+    }
+    float* d_pos = m->d_stage;
+    float* d_nrm = m->d_stage + 3 * m->stage_cap;
+    float* d_out = m->d_stage + 6 * m->stage_cap;
+    // order after the caller's stream
+    NIV_CUDA(cudaEventRecord(m->hev, (cudaStream_t)stream));
+    NIV_CUDA(cudaStreamWaitEvent(m->hs[0], m->hev, 0));
+    NIV_CUDA(cudaStreamWaitEvent(m->hs[1], m->hev, 0));
+    // chunks of whole tiles; >= 4 chunks on a full frame so H2D, kernel and D2H of different chunks overlap
+    size_t chunk = (n / 8 + kTile - 1) / kTile * kTile;
+    if (chunk < 32768) chunk = 32768;
+    int k = 0;
+    for (size_t o = 0; o < n; o += chunk, ++k) {
+        const size_t c = (n - o < chunk) ? n - o : chunk;
+        cudaStream_t st = m->hs[k & 1];
+        NIV_CUDA(cudaMemcpyAsync(d_pos + 3 * o, pos + 3 * o, c * 12, cudaMemcpyHostToDevice, st));
+        NIV_CUDA(cudaMemcpyAsync(d_nrm + 3 * o, nrm + 3 * o, c * 12, cudaMemcpyHostToDevice, st));
+        rc = launch_fused(m, P, d_pos + 3 * o, d_nrm + 3 * o, d_out + 3 * o, c, st);
+        if (rc != NIV_OK) return rc;
+        NIV_CUDA(cudaMemcpyAsync(out + 3 * o, d_out + 3 * o, c * 12, cudaMemcpyDeviceToHost, st));
+    }
+    NIV_CUDA(cudaStreamSynchronize(m->hs[0]));
+    NIV_CUDA(cudaStreamSynchronize(m->hs[1]));
     return NIV_OK;
 }
 
@@ -634,12 +752,29 @@ extern "C" int niv_debug_encode(niv_model* m, const float* pos, const float* nrm
     return NIV_OK;
 }
 
+extern "C" int niv_probe_sectors(niv_model* m, const float* pos, const float* nrm, size_t n,
+                                 uint64_t* counts, void* stream)
+{
+    if (!m) return NIV_ERR_INVALID_ARG;
+    if (!m->loaded) return NIV_ERR_NOT_LOADED;
+    if (!pos || !nrm || !counts || n == 0) return NIV_ERR_INVALID_ARG;
+    NIV_CUDA(cudaMemsetAsync(counts, 0, 33 * sizeof(uint64_t), (cudaStream_t)stream));
+    const unsigned grid = (unsigned)((n + 127) / 128);
+    niv_sector_census_kernel<<<grid, 128, 0, (cudaStream_t)stream>>>(m->kp, pos, nrm, n, (unsigned long long*)counts);
+    NIV_CUDA(cudaGetLastError());
+    return NIV_OK;
+}
+
 extern "C" int niv_destroy(niv_model* m)
 {
     if (!m) return NIV_OK;
     cudaSetDevice(m->cfg.device);
     cudaFree(m->d_table);
     cudaFree(m->d_wpack);
+    cudaFree(m->d_stage);
+    if (m->hs[0]) cudaStreamDestroy(m->hs[0]);
+    if (m->hs[1]) cudaStreamDestroy(m->hs[1]);
+    if (m->hev) cudaEventDestroy(m->hev);
     delete m;
     return NIV_OK;
 }

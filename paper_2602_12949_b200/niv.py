@@ -1,0 +1,278 @@
+"""ctypes binding of libniv.so (include/niv.h).  Argument marshalling only: every step of the path runs in
+the CUDA kernels behind the C ABI.  PyTorch is used for device memory and streams, nothing else.
+
+There is NO CPU fallback: if libniv.so is missing or no CUDA device is present, the calls raise.
+This module never imports anything under oracle/.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libniv.so")
+
+NIV_API_VERSION = 1
+NIV_OK = 0
+NIV_ERR_INVALID_ARG = -1
+NIV_ERR_UNSUPPORTED = -2
+NIV_ERR_NOT_LOADED = -3
+NIV_ERR_CUDA = -4
+NIV_ERR_ALLOC = -5
+NIV_OUT_LINEAR = 0
+NIV_OUT_SIGMOID = 1
+
+# every symbol include/niv.h declares (tests check that the library exports all of them)
+EXPORTS = ("niv_create", "niv_get_info", "niv_load_params", "niv_infer", "niv_infer_host", "niv_encode",
+           "niv_debug_encode", "niv_destroy", "niv_error_string", "niv_last_cuda_error", "niv_probe_gather",
+           "niv_probe_sectors")
+
+
+class NivConfig(C.Structure):
+    _fields_ = [
+        ("struct_size", C.c_uint32), ("api_version", C.c_uint32),
+        ("n_levels", C.c_uint32), ("n_features", C.c_uint32), ("log2_table_size", C.c_uint32),
+        ("base_resolution", C.c_uint32), ("per_level_scale", C.c_double),
+        ("resolutions", C.c_uint32 * 16),
+        ("aabb_min", C.c_float * 3), ("aabb_max", C.c_float * 3),
+        ("sh_degree", C.c_uint32), ("n_params", C.c_uint32), ("n_frequencies", C.c_uint32),
+        ("n_hidden_layers", C.c_uint32), ("hidden_width", C.c_uint32), ("out_activation", C.c_uint32),
+        ("device", C.c_int32),
+    ]
+
+
+class NivInfo(C.Structure):
+    _fields_ = [
+        ("struct_size", C.c_uint32), ("in_dim", C.c_uint32),
+        ("resolution", C.c_uint32 * 16), ("is_dense", C.c_uint32 * 16),
+        ("table_bytes", C.c_uint64), ("weight_bytes", C.c_uint64), ("bias_bytes", C.c_uint64),
+        ("num_sms", C.c_uint32), ("ctas_per_sm", C.c_uint32), ("tile_texels", C.c_uint32),
+        ("smem_bytes", C.c_uint32),
+    ]
+
+
+class NivError(RuntimeError):
+    def __init__(self, code: int, what: str):
+        self.code = code
+        msg = lib().niv_error_string(code).decode()
+        if code == NIV_ERR_CUDA:
+            msg += " [cudaError %d]" % lib().niv_last_cuda_error()
+        super().__init__("%s: %s (%d)" % (what, msg, code))
+
+
+_lib = None
+
+
+def lib():
+    """Load libniv.so (built in-tree by paper_2602_12949_b200.build).  Raises if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise ImportError("libniv.so not built: run `python -m paper_2602_12949_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(_LIB_PATH)
+        vp, sz = C.c_void_p, C.c_size_t
+        L.niv_create.argtypes = [C.POINTER(NivConfig), C.POINTER(vp)]
+        L.niv_get_info.argtypes = [vp, C.POINTER(NivInfo)]
+        L.niv_load_params.argtypes = [vp, vp, sz, vp, sz, vp, sz, C.c_int, vp]
+        L.niv_infer.argtypes = [vp, vp, vp, C.POINTER(C.c_float), vp, sz, vp]
+        L.niv_infer_host.argtypes = [vp, vp, vp, C.POINTER(C.c_float), vp, sz, vp]
+        L.niv_encode.argtypes = [vp, vp, vp, C.POINTER(C.c_float), vp, sz, vp]
+        L.niv_debug_encode.argtypes = [vp, vp, vp, C.POINTER(C.c_float), sz, vp, vp, vp, vp, vp]
+        L.niv_destroy.argtypes = [vp]
+        L.niv_error_string.argtypes = [C.c_int]
+        L.niv_error_string.restype = C.c_char_p
+        L.niv_last_cuda_error.argtypes = []
+        L.niv_probe_gather.argtypes = [vp, sz, C.c_int, C.c_uint32, C.c_uint32, C.c_uint32, vp, vp]
+        L.niv_probe_sectors.argtypes = [vp, vp, vp, sz, vp, vp]
+        for name in EXPORTS:
+            if name != "niv_error_string":
+                getattr(L, name).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def make_config(spec, device: int = 0) -> NivConfig:
+    """spec: any object with the ModelSpec attribute names (paper_2602_12949_b200.inputs.ModelSpec)."""
+    cfg = NivConfig()
+    cfg.struct_size = C.sizeof(NivConfig)
+    cfg.api_version = NIV_API_VERSION
+    cfg.n_levels = spec.n_levels
+    cfg.n_features = spec.n_features
+    cfg.log2_table_size = spec.log2_table_size
+    cfg.base_resolution = spec.base_resolution
+    cfg.per_level_scale = spec.per_level_scale
+    res = getattr(spec, "resolutions", None)
+    if res:
+        for i, r in enumerate(res):
+            cfg.resolutions[i] = int(r)
+    for d in range(3):
+        cfg.aabb_min[d] = spec.aabb_min[d]
+        cfg.aabb_max[d] = spec.aabb_max[d]
+    cfg.sh_degree = spec.sh_degree
+    cfg.n_params = spec.n_params
+    cfg.n_frequencies = spec.n_frequencies
+    cfg.n_hidden_layers = spec.n_hidden_layers
+    cfg.hidden_width = spec.hidden_width
+    cfg.out_activation = spec.out_activation
+    cfg.device = device
+    return cfg
+
+
+def _stream_ptr(stream) -> Optional[int]:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream or None
+    if isinstance(stream, int):
+        return stream or None
+    return stream.cuda_stream or None
+
+
+def _dev(t, dtype, name: str, cols: Optional[int] = None):
+    import torch
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != dtype or not t.is_contiguous():
+        raise TypeError("%s must be a contiguous CUDA tensor of %s" % (name, dtype))
+    if cols is not None and (t.dim() != 2 or t.shape[1] != cols):
+        raise TypeError("%s must have shape [n][%d]" % (name, cols))
+    return t.data_ptr()
+
+
+def _params(param: Optional[Sequence[float]], n_params: int):
+    if n_params == 0:
+        if param is not None and len(param):
+            raise ValueError("model takes no scene parameter")
+        return None
+    if param is None or len(param) != n_params:
+        raise ValueError("model takes %d scene parameter(s)" % n_params)
+    return (C.c_float * n_params)(*[float(v) for v in param])
+
+
+class NivModel:
+    """Handle on a niv_model.  Methods mirror the C ABI one to one."""
+
+    def __init__(self, spec, device: int = 0):
+        self.spec = spec
+        self._h = C.c_void_p()
+        cfg = make_config(spec, device)
+        rc = lib().niv_create(C.byref(cfg), C.byref(self._h))
+        if rc != NIV_OK:
+            self._h = C.c_void_p()
+            raise NivError(rc, "niv_create")
+        self.info = NivInfo()
+        rc = lib().niv_get_info(self._h, C.byref(self.info))
+        if rc != NIV_OK:
+            raise NivError(rc, "niv_get_info")
+
+    # ---- parameters -------------------------------------------------------------------------------
+    def load_params(self, table, weights, biases=None, stream=None):
+        """table [L][T][F] fp16, weights flat fp16 blob W1|W2|.., biases flat fp32 blob or None.
+        Each is a numpy array (host) or a CUDA tensor (device); all three must live on the same side."""
+        import numpy as np
+        on_dev = not isinstance(table, np.ndarray)
+        if on_dev:
+            import torch
+            tp, tb = _dev(table, torch.float16, "table"), table.numel() * 2
+            wp, wb = _dev(weights, torch.float16, "weights"), weights.numel() * 2
+            bp, bb = (None, 0) if biases is None else (_dev(biases, torch.float32, "biases"), biases.numel() * 4)
+        else:
+            table = np.ascontiguousarray(table, dtype=np.float16)
+            weights = np.ascontiguousarray(weights, dtype=np.float16)
+            tp, tb = table.ctypes.data, table.nbytes
+            wp, wb = weights.ctypes.data, weights.nbytes
+            if biases is None:
+                bp, bb = None, 0
+            else:
+                biases = np.ascontiguousarray(biases, dtype=np.float32)
+                bp, bb = biases.ctypes.data, biases.nbytes
+        rc = lib().niv_load_params(self._h, tp, tb, wp, wb, bp, bb, int(on_dev), _stream_ptr(stream))
+        if rc != NIV_OK:
+            raise NivError(rc, "niv_load_params")
+
+    # ---- the hot path -----------------------------------------------------------------------------
+    def infer(self, pos, nrm, out, param=None, stream=None):
+        """out[i] = E_theta(pos[i], nrm[i][, param]); device tensors [n][3] fp32; asynchronous."""
+        import torch
+        n = pos.shape[0]
+        rc = lib().niv_infer(self._h, _dev(pos, torch.float32, "pos", 3) if n else None,
+                             _dev(nrm, torch.float32, "nrm", 3) if n else None,
+                             _params(param, self.spec.n_params),
+                             _dev(out, torch.float32, "out", 3) if n else None, n, _stream_ptr(stream))
+        if rc != NIV_OK:
+            raise NivError(rc, "niv_infer")
+        return out
+
+    def infer_host(self, pos, nrm, out, param=None, stream=None):
+        """Same, with HOST buffers (numpy arrays or pinned CPU tensors, [n][3] fp32): the library stages
+        them through its own device buffers (H2D, kernel, D2H) and synchronises the stream."""
+        n = pos.shape[0]
+        rc = lib().niv_infer_host(self._h, _host_ptr(pos, "pos"), _host_ptr(nrm, "nrm"),
+                                  _params(param, self.spec.n_params), _host_ptr(out, "out"), n,
+                                  _stream_ptr(stream))
+        if rc != NIV_OK:
+            raise NivError(rc, "niv_infer_host")
+        return out
+
+    def encode(self, pos, nrm, features, param=None, stream=None):
+        """features: device [n][in_dim] fp16."""
+        import torch
+        n = pos.shape[0]
+        rc = lib().niv_encode(self._h, _dev(pos, torch.float32, "pos", 3), _dev(nrm, torch.float32, "nrm", 3),
+                              _params(param, self.spec.n_params),
+                              _dev(features, torch.float16, "features", self.info.in_dim), n, _stream_ptr(stream))
+        if rc != NIV_OK:
+            raise NivError(rc, "niv_encode")
+        return features
+
+    def debug_encode(self, pos, nrm, param=None, idx=None, cell=None, frac=None, features=None, stream=None):
+        import torch
+        n = pos.shape[0]
+        rc = lib().niv_debug_encode(
+            self._h, _dev(pos, torch.float32, "pos", 3), _dev(nrm, torch.float32, "nrm", 3),
+            _params(param, self.spec.n_params), n,
+            None if idx is None else _dev(idx, torch.int32, "idx"),
+            None if cell is None else _dev(cell, torch.int32, "cell"),
+            None if frac is None else _dev(frac, torch.float32, "frac"),
+            None if features is None else _dev(features, torch.float32, "features", self.info.in_dim),
+            _stream_ptr(stream))
+        if rc != NIV_OK:
+            raise NivError(rc, "niv_debug_encode")
+
+    def probe_sectors(self, pos, nrm, counts, stream=None):
+        """counts: device int64[33] (include/niv.h niv_probe_sectors)."""
+        import torch
+        rc = lib().niv_probe_sectors(self._h, _dev(pos, torch.float32, "pos", 3), _dev(nrm, torch.float32, "nrm", 3),
+                                     pos.shape[0], _dev(counts, torch.int64, "counts"), _stream_ptr(stream))
+        if rc != NIV_OK:
+            raise NivError(rc, "niv_probe_sectors")
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            lib().niv_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def _host_ptr(a, name: str):
+    import numpy as np
+    if isinstance(a, np.ndarray):
+        if a.dtype != np.float32 or not a.flags.c_contiguous:
+            raise TypeError("%s must be a contiguous float32 array" % name)
+        return a.ctypes.data
+    import torch
+    if isinstance(a, torch.Tensor) and not a.is_cuda and a.dtype == torch.float32 and a.is_contiguous():
+        return a.data_ptr()
+    raise TypeError("%s must be a host float32 buffer" % name)
+
+
+def probe_gather(buf, pattern: int, n_ctas: int, loads_per_lane: int, seed: int, sink, stream=None):
+    """Launch the gather micro-benchmark (include/niv.h niv_probe_gather) on `buf` (CUDA uint8/int32 tensor)."""
+    rc = lib().niv_probe_gather(buf.data_ptr(), buf.numel() * buf.element_size(), pattern, n_ctas,
+                                loads_per_lane, seed, sink.data_ptr(), _stream_ptr(stream))
+    if rc != NIV_OK:
+        raise NivError(rc, "niv_probe_gather")

@@ -1,0 +1,97 @@
+"""The C-ABI library without a GPU: it loads, exports every symbol include/niv.h declares, validates
+arguments before touching CUDA, and fails loudly (no CPU fallback) when no device is present."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+from paper_2602_12949_b200 import build as B
+from paper_2602_12949_b200 import inputs as I
+from paper_2602_12949_b200 import niv
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def L():
+    B.build()
+    return niv.lib()
+
+
+def _declared_symbols():
+    txt = open(os.path.join(ROOT, "include", "niv.h")).read()
+    txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
+    return sorted(set(re.findall(r"\b(niv_[a-z_]+)\s*\(", txt)))
+
+
+def test_library_exports_every_declared_symbol(L):
+    decl = _declared_symbols()
+    assert set(decl) == set(niv.EXPORTS), (decl, niv.EXPORTS)
+    for name in decl:
+        assert getattr(L, name) is not None
+
+
+def test_struct_sizes_match_header(L):
+    # niv_create checks struct_size: a wrong ctypes layout would be caught as INVALID_ARG instead of UNSUPPORTED
+    cfg = niv.make_config(I.spec_fullhd())
+    h = C.c_void_p()
+    cfg.n_features = 4                      # valid but unsupported by this build
+    assert L.niv_create(C.byref(cfg), C.byref(h)) == niv.NIV_ERR_UNSUPPORTED
+    cfg.struct_size += 4
+    assert L.niv_create(C.byref(cfg), C.byref(h)) == niv.NIV_ERR_INVALID_ARG
+
+
+def test_argument_validation_happens_before_cuda(L):
+    h = C.c_void_p()
+    assert L.niv_create(None, C.byref(h)) == niv.NIV_ERR_INVALID_ARG
+    cfg = niv.make_config(I.spec_tiny())
+    assert L.niv_create(C.byref(cfg), None) == niv.NIV_ERR_INVALID_ARG
+    for mutate, want in [
+        (lambda c: setattr(c, "api_version", 99), niv.NIV_ERR_INVALID_ARG),
+        (lambda c: setattr(c, "n_levels", 0), niv.NIV_ERR_INVALID_ARG),
+        (lambda c: setattr(c, "n_levels", 17), niv.NIV_ERR_INVALID_ARG),
+        (lambda c: setattr(c, "log2_table_size", 3), niv.NIV_ERR_INVALID_ARG),
+        (lambda c: setattr(c, "log2_table_size", 25), niv.NIV_ERR_INVALID_ARG),
+        (lambda c: setattr(c, "out_activation", 7), niv.NIV_ERR_INVALID_ARG),
+        (lambda c: c.aabb_max.__setitem__(1, c.aabb_min[1]), niv.NIV_ERR_INVALID_ARG),
+        (lambda c: c.aabb_max.__setitem__(0, float("nan")), niv.NIV_ERR_INVALID_ARG),
+        (lambda c: setattr(c, "per_level_scale", 0.5), niv.NIV_ERR_INVALID_ARG),
+        (lambda c: setattr(c, "base_resolution", 0), niv.NIV_ERR_INVALID_ARG),
+        (lambda c: setattr(c, "n_levels", 6), niv.NIV_ERR_UNSUPPORTED),
+        (lambda c: setattr(c, "hidden_width", 48), niv.NIV_ERR_UNSUPPORTED),
+        (lambda c: setattr(c, "n_hidden_layers", 4), niv.NIV_ERR_UNSUPPORTED),
+        (lambda c: setattr(c, "sh_degree", 3), niv.NIV_ERR_UNSUPPORTED),
+        (lambda c: setattr(c, "n_params", 3), niv.NIV_ERR_UNSUPPORTED),
+    ]:
+        cfg = niv.make_config(I.spec_tiny())
+        mutate(cfg)
+        assert L.niv_create(C.byref(cfg), C.byref(h)) == want
+        assert not h.value
+
+
+def test_null_handle_and_error_strings(L):
+    assert L.niv_infer(None, None, None, None, None, 0, None) == niv.NIV_ERR_INVALID_ARG
+    assert L.niv_infer_host(None, None, None, None, None, 0, None) == niv.NIV_ERR_INVALID_ARG
+    assert L.niv_encode(None, None, None, None, None, 0, None) == niv.NIV_ERR_INVALID_ARG
+    assert L.niv_get_info(None, None) == niv.NIV_ERR_INVALID_ARG
+    assert L.niv_destroy(None) == niv.NIV_OK
+    assert L.niv_probe_gather(None, 0, 0, 0, 0, 0, None, None) == niv.NIV_ERR_INVALID_ARG
+    msgs = {c: L.niv_error_string(c).decode() for c in range(-6, 1)}
+    assert msgs[0] == "ok" and len(set(msgs.values())) == 7
+
+
+def test_no_cpu_fallback_without_a_device(L):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    with pytest.raises(niv.NivError) as e:
+        niv.NivModel(I.spec_tiny())
+    assert e.value.code == niv.NIV_ERR_CUDA
+
+
+def test_binding_does_not_import_the_oracle():
+    src = open(os.path.join(ROOT, "paper_2602_12949_b200", "niv.py")).read()
+    assert "import oracle" not in src and "from oracle" not in src
+    for f in os.listdir(os.path.join(ROOT, "paper_2602_12949_b200", "csrc")):
+        assert "oracle" not in open(os.path.join(ROOT, "paper_2602_12949_b200", "csrc", f)).read().lower()

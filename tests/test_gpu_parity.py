@@ -1,0 +1,370 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  Bars (BASELINE.json north_star / DESIGN.md reading #20):
+  * hash indices, cells and interpolation fractions: BIT-EXACT (debug entry point, same device functions
+    the fused kernel uses);
+  * fp32 features: <= 1e-6 abs;  fp16 features: <= 1 fp16 ulp of the value (+1e-6);
+  * irradiance: max abs <= 2e-3 and mean abs <= 2e-4 over active texels x 3 channels (sigmoid output, range
+    [0,1]); for the linear output the same bounds scaled by the oracle's output range.
+"""
+import dataclasses
+
+import numpy as np
+import pytest
+
+from paper_2602_12949_b200 import inputs as I
+
+pytestmark = pytest.mark.gpu
+
+MAX_ABS = 2e-3
+MEAN_ABS = 2e-4
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    return torch
+
+
+@pytest.fixture(scope="module")
+def niv():
+    from paper_2602_12949_b200 import niv as N
+    N.lib()                                    # raises if libniv.so is missing: no fallback
+    return N
+
+
+class Case:
+    def __init__(self, spec, seed, table_amp=1e-2, bias_scale=0.0):
+        self.spec = spec
+        self.table = I.make_table(spec, seed, -table_amp, table_amp)
+        w, b = I.make_mlp(spec, seed, bias_scale)
+        self.wblob = I.pack_weights(w)
+        self.bblob = I.pack_biases(b)
+
+    def gpu_model(self, niv):
+        m = niv.NivModel(self.spec)
+        m.load_params(self.table, self.wblob, self.bblob)
+        return m
+
+
+def _queries(spec, n, seed, coherent=False):
+    aabb = (spec.aabb_min, spec.aabb_max)
+    if coherent:
+        w = int(np.ceil(np.sqrt(n * 16 / 9)))
+        h = int(np.ceil(n / w))
+        g = I.make_gbuffer(w, h, seed)
+        return g["pos"][:n].copy(), g["nrm"][:n].copy()
+    return I.positions_uniform(n, aabb, seed), I.normals_uniform(n, seed)
+
+
+def _gpu_infer(torch, model, pos, nrm, param=None):
+    dp = torch.from_numpy(pos).cuda()
+    dn = torch.from_numpy(nrm).cuda()
+    out = torch.full((pos.shape[0], 3), float("nan"), dtype=torch.float32, device="cuda")
+    model.infer(dp, dn, out, param=param)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+def _check_irradiance(got, want, nrm, pos, scale=1.0):
+    assert got.shape == want.shape and np.all(np.isfinite(got))
+    masked = np.all(nrm == 0, axis=1) | ~np.all(np.isfinite(nrm), axis=1) | ~np.all(np.isfinite(pos), axis=1)
+    assert np.all(got[masked] == 0.0)
+    act = ~masked
+    if act.any():
+        err = np.abs(got[act].astype(np.float64) - want[act].astype(np.float64))
+        assert err.max() <= MAX_ABS * scale, ("max abs", err.max())
+        assert err.mean() <= MEAN_ABS * scale, ("mean abs", err.mean())
+
+
+def _check_debug(torch, oracle, model, case, pos, nrm, param=None):
+    spec = case.spec
+    n, L = pos.shape[0], spec.n_levels
+    dp, dn = torch.from_numpy(pos).cuda(), torch.from_numpy(nrm).cuda()
+    idx = torch.full((n, L, 8), -1, dtype=torch.int32, device="cuda")
+    cell = torch.full((n, L, 3), -1, dtype=torch.int32, device="cuda")
+    frac = torch.full((n, L, 3), -1.0, dtype=torch.float32, device="cuda")
+    feat = torch.full((n, spec.in_dim), float("nan"), dtype=torch.float32, device="cuda")
+    model.debug_encode(dp, dn, param=param, idx=idx, cell=cell, frac=frac, features=feat)
+    torch.cuda.synchronize()
+    ref = oracle.encode(spec, case.table, pos, nrm, param=None if param is None else np.float32(param))
+    assert np.array_equal(idx.cpu().numpy().view(np.uint32), ref["idx"]), "hash / dense indices differ"
+    assert np.array_equal(cell.cpu().numpy(), ref["cell"]), "cells differ"
+    assert np.array_equal(frac.cpu().numpy().view(np.uint32), ref["frac"].view(np.uint32)), "fractions differ"
+    f = feat.cpu().numpy().astype(np.float64)
+    amp = max(1.0, float(np.abs(case.table.astype(np.float64)).max()) * 100.0)
+    assert np.abs(f - ref["features"]).max() <= 1e-6 * amp
+    return ref
+
+
+# ------------------------------------------------------------------------------------------------------
+# config 1: tiny, seed 0  (BASELINE.json configs[0])
+# ------------------------------------------------------------------------------------------------------
+def test_tiny_config_indices_bit_exact_and_irradiance(torch_cuda, niv, oracle):
+    case = Case(I.spec_tiny(), 0)
+    pos, nrm = _queries(case.spec, 64 * 64, 0)
+    m = case.gpu_model(niv)
+    _check_debug(torch_cuda, oracle, m, case, pos, nrm)
+    got = _gpu_infer(torch_cuda, m, pos, nrm)
+    want = oracle.infer(case.spec, case.table, case.wblob, case.bblob, pos, nrm)
+    _check_irradiance(got, want, nrm, pos)
+    m.close()
+
+
+# ------------------------------------------------------------------------------------------------------
+# configs 2/3: the full-HD model on coherent and incoherent queries (several tiles + ragged tail)
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("coherent", [True, False])
+def test_fullhd_model_parity(torch_cuda, niv, oracle, coherent):
+    case = Case(I.spec_fullhd(), 1)
+    n = 148 * 128 * 2 + 77
+    pos, nrm = _queries(case.spec, n, 3, coherent)
+    m = case.gpu_model(niv)
+    _check_debug(torch_cuda, oracle, m, case, pos, nrm)
+    got = _gpu_infer(torch_cuda, m, pos, nrm)
+    want = oracle.infer(case.spec, case.table, case.wblob, case.bblob, pos, nrm)
+    _check_irradiance(got, want, nrm, pos)
+    m.close()
+
+
+def test_loud_table_biases_and_linear_output(torch_cuda, niv, oracle):
+    """Table values uniform[-1,1] and non-zero biases so an encoding error cannot hide under the SH-dominated
+    output; linear output (the paper's reading) with the tolerance scaled by the output range."""
+    spec = dataclasses.replace(I.spec_fullhd(), out_activation=I.OUT_LINEAR)
+    case = Case(spec, 5, table_amp=1.0, bias_scale=0.5)
+    pos, nrm = _queries(spec, 20000 + 13, 7)
+    m = case.gpu_model(niv)
+    _check_debug(torch_cuda, oracle, m, case, pos, nrm)
+    got = _gpu_infer(torch_cuda, m, pos, nrm)
+    want = oracle.infer(spec, case.table, case.wblob, case.bblob, pos, nrm)
+    rng = float(want.max() - want.min())
+    assert rng > 1.0
+    _check_irradiance(got, want, nrm, pos, scale=rng)
+    m.close()
+
+
+# ------------------------------------------------------------------------------------------------------
+# config 4: time-varying field (one scalar parameter per call)
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("t", [0.0, 0.37109375, 1.0])
+def test_param_model_parity(torch_cuda, niv, oracle, t):
+    case = Case(I.spec_param(), 2, bias_scale=0.1)
+    pos, nrm = _queries(case.spec, 30000 + 5, 11, coherent=True)
+    m = case.gpu_model(niv)
+    _check_debug(torch_cuda, oracle, m, case, pos, nrm, param=[t])
+    got = _gpu_infer(torch_cuda, m, pos, nrm, param=[t])
+    want = oracle.infer(case.spec, case.table, case.wblob, case.bblob, pos, nrm, param=np.float32([t]))
+    _check_irradiance(got, want, nrm, pos)
+    m.close()
+
+
+# ------------------------------------------------------------------------------------------------------
+# config 5 shapes: widths, depths, level counts, table sizes
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("width,n_hidden,L,log2_T", [
+    (32, 2, 16, 14), (128, 2, 16, 16), (64, 1, 8, 17), (64, 3, 12, 18), (32, 1, 4, 20), (128, 3, 16, 17),
+])
+def test_shape_sweep_parity(torch_cuda, niv, oracle, width, n_hidden, L, log2_T):
+    spec = dataclasses.replace(I.spec_fullhd(log2_T, width, n_hidden), n_levels=L)
+    case = Case(spec, 100 + width + L, table_amp=0.1, bias_scale=0.05)
+    pos, nrm = _queries(spec, 9000 + 31, 13)
+    m = case.gpu_model(niv)
+    _check_debug(torch_cuda, oracle, m, case, pos, nrm)
+    got = _gpu_infer(torch_cuda, m, pos, nrm)
+    want = oracle.infer(spec, case.table, case.wblob, case.bblob, pos, nrm)
+    _check_irradiance(got, want, nrm, pos)
+    m.close()
+
+
+def test_two_parameters(torch_cuda, niv, oracle):
+    spec = dataclasses.replace(I.spec_param(), n_params=2, log2_table_size=16)
+    case = Case(spec, 9)
+    pos, nrm = _queries(spec, 5000, 17)
+    m = case.gpu_model(niv)
+    got = _gpu_infer(torch_cuda, m, pos, nrm, param=[0.25, 0.8125])
+    want = oracle.infer(spec, case.table, case.wblob, case.bblob, pos, nrm, param=np.float32([0.25, 0.8125]))
+    _check_irradiance(got, want, nrm, pos)
+    m.close()
+
+
+# ------------------------------------------------------------------------------------------------------
+# edge cases
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n", [1, 31, 127, 128, 129, 257])
+def test_ragged_sizes(torch_cuda, niv, oracle, n):
+    case = Case(I.spec_tiny(), 0)
+    pos, nrm = _queries(case.spec, n, 23)
+    m = case.gpu_model(niv)
+    torch = torch_cuda
+    # guard rows after the n texels must stay untouched
+    out = torch.full((n + 4, 3), 7.0, dtype=torch.float32, device="cuda")
+    m.infer(torch.from_numpy(pos).cuda(), torch.from_numpy(nrm).cuda(), out[:n])
+    torch.cuda.synchronize()
+    o = out.cpu().numpy()
+    assert np.all(o[n:] == 7.0)
+    want = oracle.infer(case.spec, case.table, case.wblob, case.bblob, pos, nrm)
+    _check_irradiance(o[:n], want, nrm, pos)
+    m.close()
+
+
+def test_empty_batch_is_a_noop(torch_cuda, niv):
+    case = Case(I.spec_tiny(), 0)
+    m = case.gpu_model(niv)
+    torch = torch_cuda
+    e = torch.empty((0, 3), dtype=torch.float32, device="cuda")
+    m.infer(e, e, e)
+    m.close()
+
+
+def test_masks_nonfinite_and_out_of_aabb(torch_cuda, niv, oracle):
+    case = Case(I.spec_fullhd(), 4, table_amp=0.5)
+    pos, nrm = _queries(case.spec, 4096, 29)
+    nrm[::7] = 0.0                                   # background
+    pos[1::7] = 0.0                                  # position at the AABB corner (valid)
+    pos[3, 0] = np.nan
+    pos[10, 2] = np.inf
+    nrm[17, 1] = -np.inf
+    nrm[24, 0] = np.nan
+    pos[100:200] = pos[100:200] * 3.0 - 10.0         # far outside the AABB: clamped, not masked
+    pos[200] = (10.0, 4.0, 10.0)                     # exactly the upper corner: u = 1 on all axes
+    pos[201] = (0.0, 0.0, 0.0)
+    m = case.gpu_model(niv)
+    _check_debug(torch_cuda, oracle, m, case, pos, nrm)
+    got = _gpu_infer(torch_cuda, m, pos, nrm)
+    want = oracle.infer(case.spec, case.table, case.wblob, case.bblob, pos, nrm)
+    _check_irradiance(got, want, nrm, pos)
+    # a fully masked tile
+    nrm[:] = 0
+    got = _gpu_infer(torch_cuda, m, pos, nrm)
+    assert np.all(got == 0)
+    m.close()
+
+
+def test_grid_vertices_and_cell_boundaries(torch_cuda, niv, oracle):
+    """Queries on lattice vertices (fraction 0, cell decided by an exact floor) on every level."""
+    case = Case(I.spec_fullhd(), 6, table_amp=1.0)
+    N, _ = oracle.level_table(case.spec)
+    rows = []
+    for l, Nl in enumerate(N):
+        k = (np.arange(64) * 37 + l) % (int(Nl) + 1)
+        u = (k / float(Nl)).astype(np.float32)
+        p = np.stack([u * 10.0, np.roll(u, 1) * 4.0, np.roll(u, 2) * 10.0], axis=1)
+        rows.append(p.astype(np.float32))
+    pos = np.concatenate(rows)
+    nrm = I.normals_uniform(pos.shape[0], 31)
+    m = case.gpu_model(niv)
+    _check_debug(torch_cuda, oracle, m, case, pos, nrm)
+    m.close()
+
+
+def test_standalone_encode_fp16_features(torch_cuda, niv, oracle):
+    torch = torch_cuda
+    case = Case(I.spec_param(), 8, table_amp=1.0)
+    pos, nrm = _queries(case.spec, 3000, 37)
+    nrm[5] = 0
+    m = case.gpu_model(niv)
+    feat = torch.full((3000, case.spec.in_dim), float("nan"), dtype=torch.float16, device="cuda")
+    m.encode(torch.from_numpy(pos).cuda(), torch.from_numpy(nrm).cuda(), feat, param=[0.3])
+    torch.cuda.synchronize()
+    ref = oracle.encode(case.spec, case.table, pos, nrm, param=np.float32([0.3]))["features"]
+    f = feat.cpu().numpy().astype(np.float64)
+    assert np.all(f[5] == 0)
+    tol = np.abs(ref) * 2.0 ** -10 + 1e-6
+    assert np.all(np.abs(f - ref) <= tol)
+    m.close()
+
+
+def test_error_codes_on_device(torch_cuda, niv):
+    torch = torch_cuda
+    spec = I.spec_tiny()
+    m = niv.NivModel(spec)
+    x = torch.zeros((4, 3), dtype=torch.float32, device="cuda")
+    with pytest.raises(niv.NivError) as e:
+        m.infer(x, x, x.clone())
+    assert e.value.code == niv.NIV_ERR_NOT_LOADED
+    table = I.make_table(spec, 0)
+    w, b = I.make_mlp(spec, 0)
+    with pytest.raises(niv.NivError) as e:
+        m.load_params(table[:-1], I.pack_weights(w), I.pack_biases(b))
+    assert e.value.code == niv.NIV_ERR_INVALID_ARG
+    with pytest.raises(niv.NivError) as e:
+        m.load_params(table, I.pack_weights(w)[:-1], I.pack_biases(b))
+    assert e.value.code == niv.NIV_ERR_INVALID_ARG
+    m.load_params(table, I.pack_weights(w), None)          # NULL biases = zeros
+    with pytest.raises(ValueError):
+        m.infer(x, x, x.clone(), param=[0.5])
+    m.close()
+
+
+def test_device_resident_params_and_determinism(torch_cuda, niv, oracle):
+    torch = torch_cuda
+    case = Case(I.spec_fullhd(), 12)
+    m = niv.NivModel(case.spec)
+    m.load_params(torch.from_numpy(case.table).cuda(), torch.from_numpy(case.wblob).cuda(),
+                  torch.from_numpy(case.bblob).cuda())
+    pos, nrm = _queries(case.spec, 50000, 41)
+    a = _gpu_infer(torch, m, pos, nrm)
+    b = _gpu_infer(torch, m, pos, nrm)
+    assert np.array_equal(a, b)
+    want = oracle.infer(case.spec, case.table, case.wblob, case.bblob, pos, nrm)
+    _check_irradiance(a, want, nrm, pos)
+    # side stream + CUDA graph capture: niv_infer allocates nothing and never synchronises
+    s = torch.cuda.Stream()
+    dp, dn = torch.from_numpy(pos).cuda(), torch.from_numpy(nrm).cuda()
+    out = torch.zeros((50000, 3), dtype=torch.float32, device="cuda")
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=s):
+        m.infer(dp, dn, out, stream=s)
+    out.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy(), a)
+    m.close()
+
+
+def test_host_buffer_entry_point_matches_device_path(torch_cuda, niv):
+    torch = torch_cuda
+    case = Case(I.spec_fullhd(), 13)
+    m = case.gpu_model(niv)
+    n = 300000 + 19
+    pos, nrm = _queries(case.spec, n, 43)
+    a = _gpu_infer(torch, m, pos, nrm)
+    hp, hn = torch.from_numpy(pos).pin_memory(), torch.from_numpy(nrm).pin_memory()
+    ho = torch.full((n, 3), float("nan"), dtype=torch.float32).pin_memory()
+    m.infer_host(hp, hn, ho)
+    assert np.array_equal(ho.numpy(), a)
+    out = np.full((n, 3), np.nan, dtype=np.float32)          # pageable memory
+    m.infer_host(pos, nrm, out)
+    assert np.array_equal(out, a)
+    m.close()
+
+
+# ------------------------------------------------------------------------------------------------------
+# full size, in the launch configuration bench.py times: sampled outputs against the oracle
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("which", ["fullhd", "incoherent", "param"])
+def test_full_size_sampled(torch_cuda, niv, oracle, which):
+    torch = torch_cuda
+    n = 1920 * 1080
+    if which == "param":
+        case, param = Case(I.spec_param(), 0), [0.625]
+    else:
+        case, param = Case(I.spec_fullhd(), 0), None
+    if which == "incoherent":
+        pos, nrm = _queries(case.spec, n, 0)
+    else:
+        g = I.make_gbuffer(1920, 1080, 0)
+        pos, nrm = g["pos"], g["nrm"]
+        assert 0.12 <= g["masked_fraction"] <= 0.18
+    m = case.gpu_model(niv)
+    got = _gpu_infer(torch, m, pos, nrm, param=param)
+    masked = np.all(nrm == 0, axis=1)
+    assert np.all(got[masked] == 0) and np.all(np.isfinite(got))
+    assert np.all((got[~masked] > 0) & (got[~masked] < 1))            # sigmoid range, at any size
+    sel = (I.random_u64(99, 1, 40000) % np.uint64(n)).astype(np.int64)
+    sel = np.unique(np.concatenate([sel, np.arange(0, 300), np.arange(n - 300, n)]))
+    want = oracle.infer(case.spec, case.table, case.wblob, case.bblob, pos[sel], nrm[sel],
+                        param=None if param is None else np.float32(param))
+    _check_irradiance(got[sel], want, nrm[sel], pos[sel])
+    m.close()
