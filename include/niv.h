@@ -146,10 +146,17 @@ const char *niv_error_string(int code);
 int niv_last_cuda_error(void);
 
 /* ---- measured rooflines: micro-benchmarks that run on the caller's stream ----
- * niv_probe_gather: every lane of `n_warps_total` warps issues `loads_per_lane` independent 4-byte loads
- * (pattern 0: one uniformly random 32-byte sector of `buf` per load; pattern 1: random sector per WARP, lanes
- * consecutive -- the coalesced L2 rate; pattern 2: random aligned 8-byte pair read as one 64-bit load).
- * buf is device memory of `buf_bytes` (power of two); sink is device, >= 4 bytes.  Asynchronous. */
+ * niv_probe_gather: every lane of n_ctas x 256 threads issues `loads_per_lane` independent loads (8 in flight)
+ * at pseudo-random addresses of `buf`.  pattern:
+ *   0  one 4-byte word in a uniformly random 32-byte sector per lane (the random-sector rate of the roofline)
+ *   1  one random 128-byte line per WARP, lanes consecutive (the coalesced rate)
+ *   2  one random aligned 8-byte pair per lane, one 64-bit load
+ *   3  groups of 8 lanes share one random sector
+ *   4  one random aligned 16-byte quad per lane, one 128-bit load
+ *   5  one whole random 32-byte sector per lane, one 256-bit load
+ *   6  two 4-byte loads (two instructions) from one random sector per lane
+ *   7  as 0 with L1::no_allocate
+ * buf is device memory of `buf_bytes` (power of two, 32-byte aligned); sink is device, >= 4 bytes.  Asynchronous. */
 int niv_probe_gather(const void *buf, size_t buf_bytes, int pattern, uint32_t n_ctas, uint32_t loads_per_lane,
                      uint32_t seed, void *sink, void *stream);
 

@@ -11,6 +11,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <algorithm>
 #include <cmath>
 #include <new>
 #include <vector>
@@ -303,8 +304,12 @@ __device__ __forceinline__ uint32_t mix32(uint32_t x) {
     return x;
 }
 
+// One random address stream per lane (patterns 0, 2, 4, 5, 6, 7), per warp (1) or per group of 8 lanes (3);
+// 8 independent loads are in flight per thread.  PATTERN is a template parameter so that every variant is a
+// tight loop of its own load instruction.
+template <int PATTERN>
 __global__ void __launch_bounds__(256) niv_probe_gather_kernel(const uint32_t* __restrict__ buf, uint32_t word_mask,
-                                                               int pattern, uint32_t loads_per_lane, uint32_t seed,
+                                                               uint32_t loads_per_lane, uint32_t seed,
                                                                uint32_t* __restrict__ sink)
 {
     const uint32_t gid = blockIdx.x * blockDim.x + threadIdx.x;
@@ -313,22 +318,39 @@ __global__ void __launch_bounds__(256) niv_probe_gather_kernel(const uint32_t* _
     uint32_t acc = 0;
     for (uint32_t it = 0; it < loads_per_lane; it += 8) {
         uint32_t v[8];
-        uint2 v2[8];
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
-            if (pattern == 0) {                 // every lane: its own random 4-byte word (random 32 B sector)
-                uint32_t a = mix32((gid * 0x9E3779B9u) ^ ((it + k) * 0x85EBCA6Bu) ^ seed) & word_mask;
+            const uint32_t salt = ((it + k) * 0x85EBCA6Bu) ^ seed;
+            if (PATTERN == 0) {                 // every lane: its own random 4-byte word (random 32 B sector)
+                const uint32_t a = mix32((gid * 0x9E3779B9u) ^ salt) & word_mask;
                 v[k] = __ldg(buf + a);
-            } else if (pattern == 1) {          // random 128 B line per warp, lanes consecutive (coalesced)
-                uint32_t a = (mix32((wid * 0x9E3779B9u) ^ ((it + k) * 0x85EBCA6Bu) ^ seed) & word_mask & ~31u) + lane;
+            } else if (PATTERN == 1) {          // random 128 B line per warp, lanes consecutive (coalesced)
+                const uint32_t a = (mix32((wid * 0x9E3779B9u) ^ salt) & word_mask & ~31u) + lane;
                 v[k] = __ldg(buf + a);
-            } else if (pattern == 2) {          // every lane: random aligned 8-byte pair, one 64-bit load
-                uint32_t a = mix32((gid * 0x9E3779B9u) ^ ((it + k) * 0x85EBCA6Bu) ^ seed) & word_mask & ~1u;
-                v2[k] = __ldg(reinterpret_cast<const uint2*>(buf + a));
-                v[k] = v2[k].x ^ v2[k].y;
-            } else {                            // groups of 8 lanes share one random 32 B sector (one word each)
-                uint32_t a = (mix32(((gid >> 3) * 0x9E3779B9u) ^ ((it + k) * 0x85EBCA6Bu) ^ seed) & word_mask & ~7u) + (lane & 7u);
+            } else if (PATTERN == 2) {          // every lane: random aligned 8-byte pair, one 64-bit load
+                const uint32_t a = mix32((gid * 0x9E3779B9u) ^ salt) & word_mask & ~1u;
+                const uint2 t = __ldg(reinterpret_cast<const uint2*>(buf + a));
+                v[k] = t.x ^ t.y;
+            } else if (PATTERN == 3) {          // groups of 8 lanes share one random 32 B sector (one word each)
+                const uint32_t a = (mix32(((gid >> 3) * 0x9E3779B9u) ^ salt) & word_mask & ~7u) + (lane & 7u);
                 v[k] = __ldg(buf + a);
+            } else if (PATTERN == 4) {          // every lane: random aligned 16-byte quad, one 128-bit load
+                const uint32_t a = mix32((gid * 0x9E3779B9u) ^ salt) & word_mask & ~3u;
+                const uint4 t = __ldg(reinterpret_cast<const uint4*>(buf + a));
+                v[k] = t.x ^ t.y ^ t.z ^ t.w;
+            } else if (PATTERN == 5) {          // every lane: one whole random 32 B sector, one 256-bit load
+                const uint32_t a = mix32((gid * 0x9E3779B9u) ^ salt) & word_mask & ~7u;
+                uint32_t r[8];
+                asm volatile("ld.global.nc.v8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+                             : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                             : "l"(buf + a));
+                v[k] = r[0] ^ r[1] ^ r[2] ^ r[3] ^ r[4] ^ r[5] ^ r[6] ^ r[7];
+            } else if (PATTERN == 6) {          // every lane: TWO 4-byte loads (two instructions) from one random sector
+                const uint32_t a = mix32((gid * 0x9E3779B9u) ^ salt) & word_mask;
+                v[k] = __ldg(buf + a) ^ __ldg(buf + (a ^ 1u));
+            } else {                            // 7: as 0 but L1 no-allocate
+                const uint32_t a = mix32((gid * 0x9E3779B9u) ^ salt) & word_mask;
+                asm volatile("ld.global.nc.L1::no_allocate.b32 %0, [%1];" : "=r"(v[k]) : "l"(buf + a));
             }
         }
 #pragma unroll
@@ -437,10 +459,24 @@ static uint32_t round_up(uint32_t v, uint32_t m) { return (v + m - 1) / m * m; }
 template <int W>
 static int setup_fused(niv_model* m) {
     NIV_CUDA(cudaFuncSetAttribute(niv_fused_kernel<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m->smem_fused));
-    int blocks = 0;
-    NIV_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks, niv_fused_kernel<W>, kTile, m->smem_fused));
+    // Resident CTAs per SM from the kernel's own resource use.  (cudaOccupancyMaxActiveBlocksPerMultiprocessor
+    // answers 1 for this kernel on sm_100a with driver 580 -- measured, see DESIGN.md section 6 -- so it is not used.)
+    cudaFuncAttributes fa;
+    NIV_CUDA(cudaFuncGetAttributes(&fa, niv_fused_kernel<W>));
+    cudaDeviceProp prop;
+    NIV_CUDA(cudaGetDeviceProperties(&prop, m->cfg.device));
+    const int regs_per_cta = ((fa.numRegs + 7) / 8 * 8) * kTile;
+    const int smem_per_cta = (int)round_up(m->smem_fused + (uint32_t)fa.sharedSizeBytes + (uint32_t)prop.reservedSharedMemPerBlock, 128);
     const int tmem_cols = W < 32 ? 32 : W;
-    if (blocks > 512 / tmem_cols) blocks = 512 / tmem_cols;     // TMEM: 512 columns per SM
+    int blocks = prop.regsPerMultiprocessor / regs_per_cta;
+    blocks = std::min(blocks, (int)prop.sharedMemPerMultiprocessor / smem_per_cta);
+    blocks = std::min(blocks, prop.maxThreadsPerMultiProcessor / kTile);
+    blocks = std::min(blocks, 512 / tmem_cols);                // TMEM: 512 columns per SM
+    blocks = std::min(blocks, 32);
+    if (const char* s = getenv("NIV_CTAS_PER_SM")) { int v = atoi(s); if (v > 0) blocks = v; }   // tuning knob
+    if (getenv("NIV_DEBUG"))
+        fprintf(stderr, "[niv] fused<%d>: %d regs, %d B smem/CTA, %d TMEM cols -> %d CTAs/SM\n", W, fa.numRegs,
+                smem_per_cta, tmem_cols, blocks);
     if (blocks < 1) return NIV_ERR_UNSUPPORTED;
     m->info.ctas_per_sm = (uint32_t)blocks;
     m->grid_fused = (uint32_t)blocks * m->info.num_sms;
@@ -799,10 +835,22 @@ extern "C" int niv_probe_gather(const void* buf, size_t buf_bytes, int pattern, 
 {
     if (!buf || !sink || buf_bytes < 4096 || (buf_bytes & (buf_bytes - 1)) || buf_bytes > ((size_t)1 << 33))
         return NIV_ERR_INVALID_ARG;
-    if (pattern < 0 || pattern > 3 || n_ctas == 0 || loads_per_lane == 0 || (loads_per_lane & 7)) return NIV_ERR_INVALID_ARG;
+    if (pattern < 0 || pattern > 7 || n_ctas == 0 || loads_per_lane == 0 || (loads_per_lane & 7)) return NIV_ERR_INVALID_ARG;
+    if (((uintptr_t)buf & 31) != 0) return NIV_ERR_INVALID_ARG;
     const uint32_t word_mask = (uint32_t)(buf_bytes / 4 - 1);
-    niv_probe_gather_kernel<<<n_ctas, 256, 0, (cudaStream_t)stream>>>((const uint32_t*)buf, word_mask, pattern,
-                                                                     loads_per_lane, seed, (uint32_t*)sink);
+    const uint32_t* b = (const uint32_t*)buf;
+    uint32_t* sk = (uint32_t*)sink;
+    cudaStream_t st = (cudaStream_t)stream;
+    switch (pattern) {
+        case 0: niv_probe_gather_kernel<0><<<n_ctas, 256, 0, st>>>(b, word_mask, loads_per_lane, seed, sk); break;
+        case 1: niv_probe_gather_kernel<1><<<n_ctas, 256, 0, st>>>(b, word_mask, loads_per_lane, seed, sk); break;
+        case 2: niv_probe_gather_kernel<2><<<n_ctas, 256, 0, st>>>(b, word_mask, loads_per_lane, seed, sk); break;
+        case 3: niv_probe_gather_kernel<3><<<n_ctas, 256, 0, st>>>(b, word_mask, loads_per_lane, seed, sk); break;
+        case 4: niv_probe_gather_kernel<4><<<n_ctas, 256, 0, st>>>(b, word_mask, loads_per_lane, seed, sk); break;
+        case 5: niv_probe_gather_kernel<5><<<n_ctas, 256, 0, st>>>(b, word_mask, loads_per_lane, seed, sk); break;
+        case 6: niv_probe_gather_kernel<6><<<n_ctas, 256, 0, st>>>(b, word_mask, loads_per_lane, seed, sk); break;
+        default: niv_probe_gather_kernel<7><<<n_ctas, 256, 0, st>>>(b, word_mask, loads_per_lane, seed, sk); break;
+    }
     NIV_CUDA(cudaGetLastError());
     return NIV_OK;
 }
