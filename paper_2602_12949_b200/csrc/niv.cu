@@ -29,10 +29,10 @@ namespace niv {
 // fused encode + MLP
 // =====================================================================================================
 template <int WIDTH>
-__global__ void __launch_bounds__(kTile) niv_fused_kernel(const __grid_constant__ KParams P,
-                                                          const float* __restrict__ pos,
-                                                          const float* __restrict__ nrm,
-                                                          float* __restrict__ out, size_t n, uint32_t n_tiles)
+__global__ void __launch_bounds__(kTile) niv_fused_v0_kernel(const __grid_constant__ KParams P,
+                                                             const float* __restrict__ pos,
+                                                             const float* __restrict__ nrm,
+                                                             float* __restrict__ out, size_t n, uint32_t n_tiles)
 {
     constexpr uint32_t TMEM_COLS = WIDTH < 32 ? 32 : WIDTH;
     extern __shared__ __align__(1024) uint8_t smem[];
@@ -101,13 +101,8 @@ __global__ void __launch_bounds__(kTile) niv_fused_kernel(const __grid_constant_
         if (!masked) {
             float u[3];
             normalise(P, p, u);
-            for (uint32_t g = 0; g < n_groups; ++g) {
-                float2 f[4];
-                encode_group4(P, (int)(g * 4), u, f);
-                uint4 c = make_uint4(pack_half2(f[0].x, f[0].y), pack_half2(f[1].x, f[1].y),
-                                     pack_half2(f[2].x, f[2].y), pack_half2(f[3].x, f[3].y));
-                *reinterpret_cast<uint4*>(sA + g * 2048 + tid * 16) = c;
-            }
+            for (uint32_t g = 0; g < n_groups; ++g)
+                *reinterpret_cast<uint4*>(sA + g * 2048 + tid * 16) = encode_group4(P, (int)(g * 4), u);
             float sh[16];
             sh16(nv, sh);
             uint4 c0 = make_uint4(pack_half2(sh[0], sh[1]), pack_half2(sh[2], sh[3]),
@@ -198,6 +193,371 @@ __global__ void __launch_bounds__(kTile) niv_fused_kernel(const __grid_constant_
 }
 
 // =====================================================================================================
+// fused encode + MLP, v1: specialised on <WIDTH, L>, level loop fully unrolled and software-pipelined
+// =====================================================================================================
+// Differences from v0 (profiles/r01_v0_baseline.md: 2435 instructions per texel, latency-bound on the gathers):
+//   * the level loop is unrolled (level constants become immediate constant-bank operands) and the gathers run
+//     NB levels ahead of the blend, two batches in flight per thread;
+//   * blend on packed half2 (blend8_h2): the result is directly the fp16 pair of the A operand;
+//   * biases ride in the MMA: every layer gets one extra K-step whose A operand is a constant "ones" chunk
+//     ([1, 1, 0, ...] per row, written once per CTA) and whose B rows are (bias_hi, bias_lo, 0, ...) in fp16,
+//     bias_hi + bias_lo = the fp32 bias to 2^-22 relative; the hidden epilogue is then one
+//     cvt.rn.relu.f16x2.f32 per two activations;
+//   * the per-call parameter fold (a8) is written into layer 1's bias row in shared memory.
+__device__ __forceinline__ uint32_t pack_relu_half2(float lo, float hi) {
+    uint32_t d;
+    asm("cvt.rn.relu.f16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
+    return d;
+}
+
+template <int WIDTH, int L, int NB>
+__global__ void __launch_bounds__(kTile) niv_fused_kernel(const __grid_constant__ KParams P,
+                                                          const float* __restrict__ pos,
+                                                          const float* __restrict__ nrm,
+                                                          float* __restrict__ out, size_t n, uint32_t n_tiles)
+{
+    constexpr uint32_t TMEM_COLS = WIDTH < 32 ? 32 : WIDTH;
+    constexpr int NG = L / NB;                        // gather batches per texel
+    constexpr int HC = L / 4;                         // 16-byte chunks of hash latents
+    extern __shared__ __align__(1024) uint8_t smem[];
+    uint8_t* sW = smem;                                              // packed weights (+ bias K-rows)
+    uint8_t* sA = smem + P.a_off;                                    // A operand: [K/8][128 rows][16 B]
+    uint8_t* sOnes = smem + P.ones_off;                              // [2][128 rows][16 B]: the bias K-step's A
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + P.misc_off);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2);
+
+    const uint32_t tid = threadIdx.x;
+    const uint32_t warp = tid >> 5;
+    const uint32_t bar_w = smem_u32(&bars[0]);
+    const uint32_t bar_mma = smem_u32(&bars[1]);
+    const uint32_t sA_u32 = smem_u32(sA);
+    const uint32_t sW_u32 = smem_u32(sW);
+    const uint32_t sOnes_u32 = smem_u32(sOnes);
+
+    // ---- a0: one-time setup: barriers, TMEM columns, weights, ones chunk
+    if (tid == 0) {
+        mbar_init(bar_w, 1);
+        mbar_init(bar_mma, 1);
+        mbar_fence_init();
+    }
+    if (warp == 0) tmem_alloc(smem_u32(tmem_slot), TMEM_COLS);
+    *reinterpret_cast<uint4*>(sOnes + tid * 16) = make_uint4(0x3C003C00u, 0u, 0u, 0u);      // fp16 (1, 1, 0, ...)
+    *reinterpret_cast<uint4*>(sOnes + 2048 + tid * 16) = make_uint4(0u, 0u, 0u, 0u);
+    tc_fence_before_sync();
+    __syncthreads();
+    tc_fence_after_sync();
+    const uint32_t tmem = *tmem_slot;
+    if (tid == 0) {
+        mbar_arrive_expect_tx(bar_w, P.wpack_bytes);
+        bulk_g2s(sW_u32, P.wpack, P.wpack_bytes, bar_w);
+    }
+    mbar_wait(bar_w, 0);
+
+    // ---- a8: the parameter encoding is constant over the call: b1' = b1 + W1[:, enc_dim:] * enc(t), written as
+    //      (hi, lo) fp16 into layer 1's bias K-row
+    if (P.n_params != 0 && tid < WIDTH) {
+        float b = reinterpret_cast<const float*>(sW + P.b_off[0])[tid];
+        const uint32_t np16 = 16 * P.n_params;
+        for (uint32_t q = 0; q < P.n_params; ++q) {
+            float enc[16];
+            param_encode8(P.t[q], enc);
+            const float* wp = reinterpret_cast<const float*>(sW + P.wparam_off) + tid * np16 + 16 * q;
+#pragma unroll
+            for (int k = 0; k < 16; ++k) b = fmaf(wp[k], enc[k], b);
+        }
+        const __half hi = __float2half_rn(b);
+        const __half lo = __float2half_rn(b - __half2float(hi));
+        const uint32_t word = (uint32_t)__half_as_ushort(hi) | ((uint32_t)__half_as_ushort(lo) << 16);
+        *reinterpret_cast<uint32_t*>(sW + P.w_off[0] + (P.kdim[0] >> 3) * (P.npad[0] * 16u) + tid * 16u) = word;
+    }
+    // (the first tile's fence + barrier below also publish the ones chunk and the bias row to the async proxy)
+
+    const uint32_t lane_taddr = tmem + ((warp * 32u) << 16);
+    const uint32_t k1_chunks = P.kdim[0] >> 3;
+    uint32_t phase = 0;
+
+    for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const size_t i = (size_t)tile * kTile + tid;
+        const bool valid = i < n;
+        float p[3] = {0.f, 0.f, 0.f}, nv[3] = {0.f, 0.f, 0.f};
+        if (valid) {
+            load3(pos, i, p);
+            load3(nrm, i, nv);
+        }
+        const bool masked = !valid || texel_masked(p, nv);
+
+        // ---- a2..a9: encode this thread's texel into row `tid` of the A tile
+        uint8_t* rowp = sA + tid * 16;
+        if (!masked) {
+            float u[3];
+            normalise(P, p, u);
+            uint32_t f[L];
+            Batch<NB> ba, bb;
+            batch_issue<NB>(P, 0, u, ba);
+#pragma unroll
+            for (int g = 0; g < NG; g += 2) {
+                if (g + 1 < NG) batch_issue<NB>(P, (g + 1) * NB, u, bb);
+                batch_blend<NB>(ba, f + g * NB);
+                if (g + 2 < NG) batch_issue<NB>(P, (g + 2) * NB, u, ba);
+                if (g + 1 < NG) batch_blend<NB>(bb, f + (g + 1) * NB);
+            }
+#pragma unroll
+            for (int c = 0; c < HC; ++c)
+                *reinterpret_cast<uint4*>(rowp + c * 2048) = make_uint4(f[4 * c], f[4 * c + 1], f[4 * c + 2], f[4 * c + 3]);
+            float sh[16];
+            sh16(nv, sh);
+            *reinterpret_cast<uint4*>(rowp + (HC + 0) * 2048) =
+                make_uint4(pack_half2(sh[0], sh[1]), pack_half2(sh[2], sh[3]), pack_half2(sh[4], sh[5]), pack_half2(sh[6], sh[7]));
+            *reinterpret_cast<uint4*>(rowp + (HC + 1) * 2048) =
+                make_uint4(pack_half2(sh[8], sh[9]), pack_half2(sh[10], sh[11]), pack_half2(sh[12], sh[13]), pack_half2(sh[14], sh[15]));
+            if ((HC + 2) & 1)                                            // K padding up to a multiple of 16
+                *reinterpret_cast<uint4*>(rowp + (HC + 2) * 2048) = make_uint4(0, 0, 0, 0);
+        } else {
+            for (uint32_t kc = 0; kc < k1_chunks; ++kc)
+                *reinterpret_cast<uint4*>(rowp + kc * 2048) = make_uint4(0, 0, 0, 0);
+        }
+        fence_proxy_async_smem();
+        tc_fence_before_sync();
+        __syncthreads();
+
+        // ---- a10..a11: layers on the tensor cores
+        for (uint32_t layer = 0; layer < P.n_layers; ++layer) {
+            const uint32_t K = P.kdim[layer], N = P.npad[layer];
+            if (tid == 0) {
+                tc_fence_after_sync();
+                const uint32_t idesc = make_idesc_f16(kTile, N);
+                const uint32_t b_base = sW_u32 + P.w_off[layer];
+                const uint32_t ksteps = K >> 4;
+                for (uint32_t ks = 0; ks < ksteps; ++ks) {
+                    const uint64_t da = make_smem_desc(sA_u32 + ks * 4096u, 2048u, 128u);
+                    const uint64_t db = make_smem_desc(b_base + ks * (N * 32u), N * 16u, 128u);
+                    umma_f16_ss(tmem, da, db, idesc, ks > 0 ? 1u : 0u);
+                }
+                {   // + bias: ones chunk x (bias_hi, bias_lo) rows
+                    const uint64_t da = make_smem_desc(sOnes_u32, 2048u, 128u);
+                    const uint64_t db = make_smem_desc(b_base + ksteps * (N * 32u), N * 16u, 128u);
+                    umma_f16_ss(tmem, da, db, idesc, 1u);
+                }
+                umma_commit(bar_mma);
+            }
+            mbar_wait(bar_mma, phase);
+            phase ^= 1u;
+            tc_fence_after_sync();
+
+            if (layer + 1 < P.n_layers) {
+                // hidden epilogue: ReLU + fp16 pack in one conversion -> next layer's A operand (same buffer)
+#pragma unroll
+                for (int cc = 0; cc < WIDTH / 32; ++cc) {
+                    uint32_t r[32];
+                    tmem_ld_x32(lane_taddr + cc * 32, r);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int g = 0; g < 4; ++g) {
+                        uint32_t pk[4];
+#pragma unroll
+                        for (int h = 0; h < 4; ++h)
+                            pk[h] = pack_relu_half2(__uint_as_float(r[g * 8 + h * 2]), __uint_as_float(r[g * 8 + h * 2 + 1]));
+                        *reinterpret_cast<uint4*>(rowp + (cc * 4 + g) * 2048) = make_uint4(pk[0], pk[1], pk[2], pk[3]);
+                    }
+                }
+                fence_proxy_async_smem();
+                tc_fence_before_sync();
+                __syncthreads();
+            } else {
+                // ---- a11..a12: output layer: 3 useful columns (bias already in), activation, store
+                uint32_t r[4];
+                tmem_ld_x4(lane_taddr, r);
+                tmem_ld_wait();
+                tc_fence_before_sync();
+                if (valid) {
+                    float y[3];
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        float v = __uint_as_float(r[c]);
+                        if (P.out_act == NIV_OUT_SIGMOID) v = __fdividef(1.0f, 1.0f + __expf(-v));
+                        y[c] = masked ? 0.0f : v;
+                    }
+                    out[3 * i] = y[0];
+                    out[3 * i + 1] = y[1];
+                    out[3 * i + 2] = y[2];
+                }
+            }
+        }
+    }
+
+    __syncthreads();
+    if (warp == 0) tmem_dealloc(tmem, TMEM_COLS);
+}
+
+// =====================================================================================================
+// fused encode + MLP, v2: as v1, with the A operand of every layer in TENSOR MEMORY (WIDTH <= 64)
+// =====================================================================================================
+// profiles/r01_v1_nb4.md: v1 is bound by the L1TEX data pipe (69 % busy: 220 K gather wavefronts, 46 K
+// shared-store wavefronts per SM) and its 43 KB of shared memory per CTA leave only ~50 KB of L1 per SM.
+// Here thread t keeps row t of the A operand in TMEM lane t: tcgen05.st instead of STS (no L1TEX wavefronts,
+// no generic->async proxy fence), tcgen05.mma reads A from TMEM, and shared memory holds the weights only.
+// TMEM columns per CTA (128 allocated): D [0, WIDTH) fp32 | A [64, 96) packed fp16 pairs | ones [96, 104).
+template <int WIDTH, int L, int NB>
+__global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(const __grid_constant__ KParams P,
+                                                               const float* __restrict__ pos,
+                                                               const float* __restrict__ nrm,
+                                                               float* __restrict__ out, size_t n, uint32_t n_tiles)
+{
+    static_assert(WIDTH <= 64, "A-in-TMEM kernel: D + A + ones must fit 128 columns");
+    constexpr uint32_t TMEM_COLS = 128, A_COL = 64, ONES_COL = 96;
+    constexpr int NG = L / NB;
+    constexpr int AW = (L + 8 + 7) / 8 * 8;          // 32-bit words of one layer-1 A row (K1 = 2 * AW)
+    extern __shared__ __align__(1024) uint8_t smem[];
+    uint8_t* sW = smem;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + P.misc_off);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2);
+
+    const uint32_t tid = threadIdx.x;
+    const uint32_t warp = tid >> 5;
+    const uint32_t bar_w = smem_u32(&bars[0]);
+    const uint32_t bar_mma = smem_u32(&bars[1]);
+    const uint32_t sW_u32 = smem_u32(sW);
+
+    if (tid == 0) {
+        mbar_init(bar_w, 1);
+        mbar_init(bar_mma, 1);
+        mbar_fence_init();
+    }
+    if (warp == 0) tmem_alloc(smem_u32(tmem_slot), TMEM_COLS);
+    tc_fence_before_sync();
+    __syncthreads();
+    tc_fence_after_sync();
+    const uint32_t tmem = *tmem_slot;
+    const uint32_t lane_taddr = tmem + ((warp * 32u) << 16);
+    if (tid == 0) {
+        mbar_arrive_expect_tx(bar_w, P.wpack_bytes);
+        bulk_g2s(sW_u32, P.wpack, P.wpack_bytes, bar_w);
+    }
+    {   // the bias K-step's A operand: (1, 1, 0, ..., 0) in every row, written once
+        uint32_t ones[8] = {0x3C003C00u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
+        tmem_st_x8(lane_taddr + ONES_COL, ones);
+    }
+    mbar_wait(bar_w, 0);
+
+    // ---- a8: fold the per-call parameter encoding into layer 1's bias K-row (hi, lo) in shared memory
+    if (P.n_params != 0 && tid < WIDTH) {
+        float b = reinterpret_cast<const float*>(sW + P.b_off[0])[tid];
+        const uint32_t np16 = 16 * P.n_params;
+        for (uint32_t q = 0; q < P.n_params; ++q) {
+            float enc[16];
+            param_encode8(P.t[q], enc);
+            const float* wp = reinterpret_cast<const float*>(sW + P.wparam_off) + tid * np16 + 16 * q;
+#pragma unroll
+            for (int k = 0; k < 16; ++k) b = fmaf(wp[k], enc[k], b);
+        }
+        const __half hi = __float2half_rn(b);
+        const __half lo = __float2half_rn(b - __half2float(hi));
+        const uint32_t word = (uint32_t)__half_as_ushort(hi) | ((uint32_t)__half_as_ushort(lo) << 16);
+        *reinterpret_cast<uint32_t*>(sW + P.w_off[0] + (P.kdim[0] >> 3) * (P.npad[0] * 16u) + tid * 16u) = word;
+    }
+    fence_proxy_async_smem();          // the bias row is read by the tensor core through the async proxy
+
+    uint32_t phase = 0;
+    for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        const size_t i = (size_t)tile * kTile + tid;
+        const bool valid = i < n;
+        float p[3] = {0.f, 0.f, 0.f}, nv[3] = {0.f, 0.f, 0.f};
+        if (valid) {
+            load3(pos, i, p);
+            load3(nrm, i, nv);
+        }
+        const bool masked = !valid || texel_masked(p, nv);
+
+        // ---- a2..a9: this thread's A row in registers.  Rows are independent in the GEMMs and masked rows are
+        //      overwritten with zeros at the store, so a masked thread just passes zeros.
+        uint32_t a[AW];
+#pragma unroll
+        for (int k = 0; k < AW; ++k) a[k] = 0u;
+        if (!masked) {
+            float u[3];
+            normalise(P, p, u);
+            Batch<NB> ba, bb;
+            batch_issue<NB>(P, 0, u, ba);
+            float sh[16];
+            sh16(nv, sh);
+#pragma unroll
+            for (int k = 0; k < 8; ++k) a[L + k] = pack_half2(sh[2 * k], sh[2 * k + 1]);
+#pragma unroll
+            for (int g = 0; g < NG; g += 2) {
+                if (g + 1 < NG) batch_issue<NB>(P, (g + 1) * NB, u, bb);
+                batch_blend<NB>(ba, a + g * NB);
+                if (g + 2 < NG) batch_issue<NB>(P, (g + 2) * NB, u, ba);
+                if (g + 1 < NG) batch_blend<NB>(bb, a + (g + 1) * NB);
+            }
+        }
+        __syncwarp();
+        tmem_st_x16(lane_taddr + A_COL, a);
+        if (AW > 16) tmem_st_x8(lane_taddr + A_COL + 16, a + 16);
+        tmem_st_wait();
+        tc_fence_before_sync();
+        __syncthreads();
+
+        for (uint32_t layer = 0; layer < P.n_layers; ++layer) {
+            const uint32_t K = P.kdim[layer], N = P.npad[layer];
+            if (tid == 0) {
+                tc_fence_after_sync();
+                const uint32_t idesc = make_idesc_f16(kTile, N);
+                const uint32_t b_base = sW_u32 + P.w_off[layer];
+                const uint32_t ksteps = K >> 4;
+                for (uint32_t ks = 0; ks < ksteps; ++ks) {
+                    const uint64_t db = make_smem_desc(b_base + ks * (N * 32u), N * 16u, 128u);
+                    umma_f16_ts(tmem, tmem + A_COL + ks * 8u, db, idesc, ks > 0 ? 1u : 0u);
+                }
+                const uint64_t db = make_smem_desc(b_base + ksteps * (N * 32u), N * 16u, 128u);
+                umma_f16_ts(tmem, tmem + ONES_COL, db, idesc, 1u);            // + bias
+                umma_commit(bar_mma);
+            }
+            mbar_wait(bar_mma, phase);
+            phase ^= 1u;
+            tc_fence_after_sync();
+
+            if (layer + 1 < P.n_layers) {
+                // hidden epilogue: D (fp32) -> ReLU + fp16 pack -> A columns of the next layer
+#pragma unroll
+                for (int cc = 0; cc < WIDTH / 32; ++cc) {
+                    uint32_t r[32];
+                    tmem_ld_x32(lane_taddr + cc * 32, r);
+                    tmem_ld_wait();
+                    uint32_t pk[16];
+#pragma unroll
+                    for (int h = 0; h < 16; ++h)
+                        pk[h] = pack_relu_half2(__uint_as_float(r[2 * h]), __uint_as_float(r[2 * h + 1]));
+                    tmem_st_x16(lane_taddr + A_COL + cc * 16, pk);
+                }
+                tmem_st_wait();
+                tc_fence_before_sync();
+                __syncthreads();
+            } else {
+                uint32_t r[4];
+                tmem_ld_x4(lane_taddr, r);
+                tmem_ld_wait();
+                tc_fence_before_sync();
+                if (valid) {
+                    float y[3];
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        float v = __uint_as_float(r[c]);
+                        if (P.out_act == NIV_OUT_SIGMOID) v = __fdividef(1.0f, 1.0f + __expf(-v));
+                        y[c] = masked ? 0.0f : v;
+                    }
+                    out[3 * i] = y[0];
+                    out[3 * i + 1] = y[1];
+                    out[3 * i + 2] = y[2];
+                }
+            }
+        }
+    }
+
+    __syncthreads();
+    if (warp == 0) tmem_dealloc(tmem, TMEM_COLS);
+}
+
+// =====================================================================================================
 // stand-alone encode (fp16 features to global) and debug dump
 // =====================================================================================================
 __global__ void __launch_bounds__(128) niv_encode_kernel(const __grid_constant__ KParams P,
@@ -219,12 +579,7 @@ __global__ void __launch_bounds__(128) niv_encode_kernel(const __grid_constant__
     float u[3];
     normalise(P, p, u);
     const uint32_t n_groups = P.L >> 2;
-    for (uint32_t g = 0; g < n_groups; ++g) {
-        float2 f[4];
-        encode_group4(P, (int)(g * 4), u, f);
-        row[g] = make_uint4(pack_half2(f[0].x, f[0].y), pack_half2(f[1].x, f[1].y),
-                            pack_half2(f[2].x, f[2].y), pack_half2(f[3].x, f[3].y));
-    }
+    for (uint32_t g = 0; g < n_groups; ++g) row[g] = encode_group4(P, (int)(g * 4), u);
     float sh[16];
     sh16(nv, sh);
     row[n_groups] = make_uint4(pack_half2(sh[0], sh[1]), pack_half2(sh[2], sh[3]),
@@ -267,11 +622,9 @@ __global__ void __launch_bounds__(128) niv_debug_kernel(const __grid_constant__ 
             if (feat) {
                 uint32_t v[8];
 #pragma unroll
-                for (int j = 0; j < 8; ++j) v[j] = __ldg(P.table + e[j]);
+                for (int j = 0; j < 8; ++j) v[j] = __ldg(P.lv[l].tb + e[j]);
                 f = blend8(v, w);
             }
-#pragma unroll
-            for (int j = 0; j < 8; ++j) e[j] -= P.lv[l].base;
         }
         if (idx)
             for (int j = 0; j < 8; ++j) idx[(i * L + l) * 8 + j] = e[j];
@@ -390,7 +743,8 @@ __global__ void __launch_bounds__(128) niv_sector_census_kernel(const __grid_con
             corner_entries(P.lv[l], P.tmask, c, e);
         }
 #pragma unroll
-        for (int j = 0; j < 8; ++j) s_sec[warp][lane * 8 + j] = masked ? 0xFFFFFFFFu : (e[j] >> 3);   // 8 entries per sector
+        for (int j = 0; j < 8; ++j)                                           // 8 entries per 32-byte sector
+            s_sec[warp][lane * 8 + j] = masked ? 0xFFFFFFFFu : ((P.lv[l].base + e[j]) >> 3);
         __syncwarp();
         uint32_t sec = 0, lin = 0;
         for (int q = 0; q < 8; ++q) {
@@ -435,6 +789,7 @@ struct niv_model {
     bool loaded = false;
     uint32_t grid_fused = 0;
     uint32_t smem_fused = 0;
+    void (*fused)(KParams, const float*, const float*, float*, size_t, uint32_t) = nullptr;
     // niv_infer_host staging (grown on demand)
     float* d_stage = nullptr;          // [pos | nrm | out], each 3*stage_cap floats
     size_t stage_cap = 0;
@@ -456,31 +811,72 @@ static thread_local int g_last_cuda_error = 0;
 
 static uint32_t round_up(uint32_t v, uint32_t m) { return (v + m - 1) / m * m; }
 
-template <int W>
-static int setup_fused(niv_model* m) {
-    NIV_CUDA(cudaFuncSetAttribute(niv_fused_kernel<W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m->smem_fused));
-    // Resident CTAs per SM from the kernel's own resource use.  (cudaOccupancyMaxActiveBlocksPerMultiprocessor
-    // answers 1 for this kernel on sm_100a with driver 580 -- measured, see DESIGN.md section 6 -- so it is not used.)
+// Resident CTAs per SM from the kernel's own resource use.  (cudaOccupancyMaxActiveBlocksPerMultiprocessor
+// answers 1 for these kernels on sm_100a with driver 580 -- measured, see DESIGN.md section 6 -- so it is not used.)
+template <typename K>
+static int setup_kernel(niv_model* m, K kernel, int tmem_cols, const char* name) {
+    NIV_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m->smem_fused));
     cudaFuncAttributes fa;
-    NIV_CUDA(cudaFuncGetAttributes(&fa, niv_fused_kernel<W>));
+    NIV_CUDA(cudaFuncGetAttributes(&fa, kernel));
     cudaDeviceProp prop;
     NIV_CUDA(cudaGetDeviceProperties(&prop, m->cfg.device));
     const int regs_per_cta = ((fa.numRegs + 7) / 8 * 8) * kTile;
     const int smem_per_cta = (int)round_up(m->smem_fused + (uint32_t)fa.sharedSizeBytes + (uint32_t)prop.reservedSharedMemPerBlock, 128);
-    const int tmem_cols = W < 32 ? 32 : W;
     int blocks = prop.regsPerMultiprocessor / regs_per_cta;
     blocks = std::min(blocks, (int)prop.sharedMemPerMultiprocessor / smem_per_cta);
     blocks = std::min(blocks, prop.maxThreadsPerMultiProcessor / kTile);
     blocks = std::min(blocks, 512 / tmem_cols);                // TMEM: 512 columns per SM
     blocks = std::min(blocks, 32);
-    if (const char* s = getenv("NIV_CTAS_PER_SM")) { int v = atoi(s); if (v > 0) blocks = v; }   // tuning knob
+    if (const char* s = getenv("NIV_CTAS_PER_SM")) { int v = atoi(s); if (v > 0) blocks = std::min(blocks, v); }   // tuning knob
     if (getenv("NIV_DEBUG"))
-        fprintf(stderr, "[niv] fused<%d>: %d regs, %d B smem/CTA, %d TMEM cols -> %d CTAs/SM\n", W, fa.numRegs,
+        fprintf(stderr, "[niv] %s: %d regs, %d B smem/CTA, %d TMEM cols -> %d CTAs/SM\n", name, fa.numRegs,
                 smem_per_cta, tmem_cols, blocks);
     if (blocks < 1) return NIV_ERR_UNSUPPORTED;
     m->info.ctas_per_sm = (uint32_t)blocks;
     m->grid_fused = (uint32_t)blocks * m->info.num_sms;
     return NIV_OK;
+}
+
+typedef void (*fused_fn)(KParams, const float*, const float*, float*, size_t, uint32_t);
+
+template <int W, int L>
+static fused_fn pick_nb(int nb) { return nb == 4 ? niv_fused_kernel<W, L, 4> : niv_fused_kernel<W, L, 2>; }
+template <int W>
+static fused_fn pick_l(uint32_t L, int nb) {
+    switch (L) {
+        case 4:  return niv_fused_kernel<W, 4, 4>;
+        case 8:  return pick_nb<W, 8>(nb);
+        case 12: return niv_fused_kernel<W, 12, 4>;
+        case 16: return pick_nb<W, 16>(nb);
+        default: return nullptr;
+    }
+}
+static fused_fn pick_fused(uint32_t W, uint32_t L, int nb) {
+    if (W == 32) return pick_l<32>(L, nb);
+    if (W == 64) return pick_l<64>(L, nb);
+    return pick_l<128>(L, nb);
+}
+template <int W, int L>
+static fused_fn pick_tmem_nb(int nb) { return nb == 4 ? niv_fused_tmem_kernel<W, L, 4> : niv_fused_tmem_kernel<W, L, 2>; }
+template <int W>
+static fused_fn pick_tmem_l(uint32_t L, int nb) {
+    switch (L) {
+        case 4:  return niv_fused_tmem_kernel<W, 4, 4>;
+        case 8:  return pick_tmem_nb<W, 8>(nb);
+        case 12: return niv_fused_tmem_kernel<W, 12, 4>;
+        case 16: return pick_tmem_nb<W, 16>(nb);
+        default: return nullptr;
+    }
+}
+static fused_fn pick_tmem(uint32_t W, uint32_t L, int nb) {
+    if (W == 32) return pick_tmem_l<32>(L, nb);
+    if (W == 64) return pick_tmem_l<64>(L, nb);
+    return nullptr;
+}
+static fused_fn pick_v0(uint32_t W) {
+    if (W == 32) return niv_fused_v0_kernel<32>;
+    if (W == 64) return niv_fused_v0_kernel<64>;
+    return niv_fused_v0_kernel<128>;
 }
 
 extern "C" int niv_create(const niv_config* cfg, niv_model** out)
@@ -502,7 +898,7 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
         return NIV_ERR_INVALID_ARG;
     // shapes this build has kernels for
     if (cfg->n_features != 2) return NIV_ERR_UNSUPPORTED;
-    if (cfg->n_levels % 4 != 0) return NIV_ERR_UNSUPPORTED;
+    if (cfg->n_levels % 4 != 0) return NIV_ERR_UNSUPPORTED;            // {4, 8, 12, 16}
     if (cfg->sh_degree != 4 || cfg->n_params > 2 || (cfg->n_params && cfg->n_frequencies != 8)) return NIV_ERR_UNSUPPORTED;
     if (cfg->n_hidden_layers > 3) return NIV_ERR_UNSUPPORTED;
     if (cfg->hidden_width != 32 && cfg->hidden_width != 64 && cfg->hidden_width != 128) return NIV_ERR_UNSUPPORTED;
@@ -564,7 +960,7 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
         P.kdim[k] = (k == 0) ? round_up(P.enc_dim, 16) : in;      // layer 1 consumes the encoded part only
         P.npad[k] = round_up(o, 16);
         P.w_off[k] = off;
-        off += P.kdim[k] * P.npad[k] * 2;
+        off += (P.kdim[k] + 16) * P.npad[k] * 2;                 // + the bias K-step: rows (bias_hi, bias_lo, 0, ..)
         in = o;
     }
     for (uint32_t k = 0; k < P.n_layers; ++k) { P.b_off[k] = off; off += P.npad[k] * 4; }
@@ -574,7 +970,8 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     uint32_t kmax = P.kdim[0];
     for (uint32_t k = 1; k < P.n_layers; ++k) kmax = kmax > P.kdim[k] ? kmax : P.kdim[k];
     P.a_off = round_up(P.wpack_bytes, 128);
-    P.misc_off = P.a_off + kTile * kmax * 2;
+    P.ones_off = P.a_off + kTile * kmax * 2;
+    P.misc_off = P.ones_off + 2 * kTile * 16;
     m->smem_fused = P.misc_off + W * 4 + 2 * 8 + 16;
     I.smem_bytes = m->smem_fused;
 
@@ -587,9 +984,25 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     if (e != cudaSuccess) { g_last_cuda_error = (int)e; (void)cudaGetLastError(); delete m; return NIV_ERR_CUDA; }
     if (prop.major != 10) { delete m; return NIV_ERR_UNSUPPORTED; }           // sm_100a only; no fallback
     I.num_sms = (uint32_t)prop.multiProcessorCount;
-    if (W == 32) rc = setup_fused<32>(m);
-    else if (W == 64) rc = setup_fused<64>(m);
-    else rc = setup_fused<128>(m);
+    {
+        const char* kv = getenv("NIV_KERNEL");          // A-B knob: 0 = v0 (generic), 1 = v1 (A in smem), 2 = v2 (A in TMEM)
+        const char* nbv = getenv("NIV_NB");             // gather batch: 2 or 4 levels
+        const int nb = nbv ? atoi(nbv) : 4;
+        int kind = kv ? atoi(kv) : 2;
+        if (kind == 2 && W > 64) kind = 1;
+        int tmem_cols = W < 32 ? 32 : (int)W;
+        if (kind == 0) m->fused = pick_v0(W);
+        else if (kind == 1) m->fused = pick_fused(W, cfg->n_levels, nb);
+        else {
+            m->fused = pick_tmem(W, cfg->n_levels, nb);
+            tmem_cols = 128;
+            m->smem_fused = P.a_off + 2 * 8 + 16;        // weights + barriers only
+            P.misc_off = P.a_off;
+            I.smem_bytes = m->smem_fused;
+        }
+        if (!m->fused) { delete m; return NIV_ERR_UNSUPPORTED; }
+        rc = setup_kernel(m, m->fused, tmem_cols, kind == 0 ? "fused_v0" : kind == 1 ? "fused_v1" : "fused_v2");
+    }
     if (rc != NIV_OK) { delete m; return rc; }
     e = cudaMalloc(&m->d_table, I.table_bytes);
     if (e == cudaSuccess) e = cudaMalloc(&m->d_wpack, P.wpack_bytes);
@@ -600,6 +1013,7 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     }
     P.table = m->d_table;
     P.wpack = m->d_wpack;
+    for (uint32_t l = 0; l < cfg->n_levels; ++l) P.lv[l].tb = m->d_table + P.lv[l].base;
     *out = m;
     return NIV_OK;
 }
@@ -655,7 +1069,15 @@ extern "C" int niv_load_params(niv_model* m, const void* table_fp16, size_t tabl
                 }
         }
         float* bd = reinterpret_cast<float*>(pack.data() + P.b_off[k]);
-        for (uint32_t r = 0; r < o; ++r) bd[r] = b[bsrc + r];
+        for (uint32_t r = 0; r < o; ++r) {
+            bd[r] = b[bsrc + r];
+            // bias K-step rows: K index kdim -> bias_hi, kdim + 1 -> bias_lo (hi + lo = bias to 2^-22 relative)
+            const __half hi = __float2half_rn(b[bsrc + r]);
+            const __half lo = __float2half_rn(b[bsrc + r] - __half2float(hi));
+            uint16_t* brow = dst + (size_t)(P.kdim[k] >> 3) * (P.npad[k] * 8) + r * 8;
+            brow[0] = __half_as_ushort(hi);
+            brow[1] = __half_as_ushort(lo);
+        }
         wsrc += (size_t)o * in;
         bsrc += o;
     }
@@ -684,11 +1106,7 @@ static int launch_fused(const niv_model* m, const KParams& P, const float* pos, 
 {
     const uint32_t n_tiles = (uint32_t)((n + kTile - 1) / kTile);
     const uint32_t grid = n_tiles < m->grid_fused ? n_tiles : m->grid_fused;
-    switch (m->cfg.hidden_width) {
-        case 32:  niv_fused_kernel<32><<<grid, kTile, m->smem_fused, st>>>(P, pos, nrm, out, n, n_tiles); break;
-        case 64:  niv_fused_kernel<64><<<grid, kTile, m->smem_fused, st>>>(P, pos, nrm, out, n, n_tiles); break;
-        default:  niv_fused_kernel<128><<<grid, kTile, m->smem_fused, st>>>(P, pos, nrm, out, n, n_tiles); break;
-    }
+    m->fused<<<grid, kTile, m->smem_fused, st>>>(P, pos, nrm, out, n, n_tiles);
     NIV_CUDA(cudaGetLastError());
     return NIV_OK;
 }

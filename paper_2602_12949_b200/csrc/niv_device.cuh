@@ -19,6 +19,7 @@ struct LevelP {
     uint32_t R2;        // R*R
     uint32_t base;      // first table entry of this level = l*T
     uint32_t dense;     // 1 dense, 0 hashed
+    const uint32_t* tb; // table + base: this level's first entry (so that a gather address is ONE IMAD.WIDE)
 };
 
 struct KParams {
@@ -42,6 +43,7 @@ struct KParams {
     uint32_t b_off[kMaxLayers];
     uint32_t wparam_off;        // fp32 [width][16*n_params] columns of W1 that multiply the parameter encoding
     uint32_t a_off;             // byte offset of the A tile in shared memory
+    uint32_t ones_off;          // byte offset of the constant "ones" A chunk of the bias K-step (v1 kernel)
     uint32_t misc_off;          // byte offset of folded bias / barriers
 };
 
@@ -72,11 +74,18 @@ __device__ __forceinline__ void locate(const LevelP& lv, const float u[3], int c
     }
 }
 
-// ---------------------------------------------------------------- O3: the 8 corner entries (level base added)
+// ---------------------------------------------------------------- O3: the 8 corner entries, relative to the level's first entry
 // corner j: bit 0 -> +1 in x, bit 1 -> +1 in y, bit 2 -> +1 in z.
+// (a ^ b) & c as ONE LOP3 (immLut 0x28); inline PTX so that the optimiser cannot re-associate the XORs into
+// a 3-input XOR followed by a separate AND (16 instead of 12 logic ops per level).
+__device__ __forceinline__ uint32_t xor_and(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t d;
+    asm("lop3.b32 %0, %1, %2, %3, 0x28;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+    return d;
+}
 __device__ __forceinline__ void corner_entries(const LevelP& lv, uint32_t tmask, const int c[3], uint32_t e[8]) {
     if (lv.dense) {
-        uint32_t b = lv.base + (uint32_t)c[0] + lv.R * (uint32_t)c[1] + lv.R2 * (uint32_t)c[2];
+        uint32_t b = (uint32_t)c[0] + lv.R * (uint32_t)c[1] + lv.R2 * (uint32_t)c[2];
 #pragma unroll
         for (int j = 0; j < 8; ++j)
             e[j] = b + (j & 1) + ((j >> 1) & 1) * lv.R + ((j >> 2) & 1) * lv.R2;
@@ -87,7 +96,7 @@ __device__ __forceinline__ void corner_entries(const LevelP& lv, uint32_t tmask,
         uint32_t yz[4] = { y0 ^ z0, y1 ^ z0, y0 ^ z1, y1 ^ z1 };
 #pragma unroll
         for (int j = 0; j < 8; ++j)
-            e[j] = lv.base + ((((j & 1) ? x1 : x0) ^ yz[j >> 1]) & tmask);
+            e[j] = xor_and((j & 1) ? x1 : x0, yz[j >> 1], tmask);
     }
 }
 
@@ -114,24 +123,58 @@ __device__ __forceinline__ uint32_t pack_half2(float a, float b) {
     return *reinterpret_cast<uint32_t*>(&h);
 }
 
-// One group of 4 levels (8 latents = one 16-byte fp16 chunk of the A operand): all 32 gathers are issued
-// before the first use so that they are in flight together.
-__device__ __forceinline__ void encode_group4(const KParams& P, int l0, const float u[3], float2 f[4]) {
-    uint32_t e[4][8];
-    float w[4][3];
+// ---------------------------------------------------------------- O4 on the fused path: half2 lerp tree
+// F = 2: one table entry IS one half2, so the blend runs on packed fp16 pairs: lerp in x (4), y (2), z (1),
+// each lerp = HADD2 (b - a) + HFMA2 (w * d + a) -> 14 instructions per level instead of 16 conversions +
+// 16 FFMA + 15 weight ops, and the result is already the packed fp16 pair the A operand wants.
+// Error: <= 15 * 2^-11 * max|table| worst case, ~2e-4 * max|table| rms.
+__device__ __forceinline__ __half2 u2h(uint32_t v) { return *reinterpret_cast<__half2*>(&v); }
+__device__ __forceinline__ uint32_t h2u(__half2 v) { return *reinterpret_cast<uint32_t*>(&v); }
+__device__ __forceinline__ __half2 lerp2(__half2 a, __half2 b, __half2 w) { return __hfma2(w, __hsub2(b, a), a); }
+__device__ __forceinline__ uint32_t blend8_h2(const uint32_t v[8], const uint32_t w2[3]) {
+    const __half2 wx = u2h(w2[0]), wy = u2h(w2[1]), wz = u2h(w2[2]);
+    const __half2 a0 = lerp2(u2h(v[0]), u2h(v[1]), wx), a1 = lerp2(u2h(v[2]), u2h(v[3]), wx);
+    const __half2 a2 = lerp2(u2h(v[4]), u2h(v[5]), wx), a3 = lerp2(u2h(v[6]), u2h(v[7]), wx);
+    const __half2 b0 = lerp2(a0, a1, wy), b1 = lerp2(a2, a3, wy);
+    return h2u(lerp2(b0, b1, wz));
+}
+
+// A batch of NB levels in flight: the 8*NB gathers are issued by batch_issue and consumed by batch_blend, so
+// the caller can issue the next batch before blending the current one (software pipelining inside a thread).
+template <int NB>
+struct Batch {
+    uint32_t v[NB][8];      // gathered entries (2 x fp16 each)
+    uint32_t w2[NB][3];     // interpolation fractions, each duplicated into a half2
+};
+template <int NB>
+__device__ __forceinline__ void batch_issue(const KParams& P, int l0, const float u[3], Batch<NB>& b) {
 #pragma unroll
-    for (int q = 0; q < 4; ++q) {
+    for (int q = 0; q < NB; ++q) {
+        const LevelP& lv = P.lv[l0 + q];
         int c[3];
-        locate(P.lv[l0 + q], u, c, w[q]);
-        corner_entries(P.lv[l0 + q], P.tmask, c, e[q]);
+        float w[3];
+        uint32_t e[8];
+        locate(lv, u, c, w);
+        corner_entries(lv, P.tmask, c, e);
+#pragma unroll
+        for (int j = 0; j < 8; ++j) b.v[q][j] = __ldg(lv.tb + e[j]);
+#pragma unroll
+        for (int d = 0; d < 3; ++d) b.w2[q][d] = pack_half2(w[d], w[d]);
     }
-    uint32_t v[4][8];
+}
+template <int NB>
+__device__ __forceinline__ void batch_blend(const Batch<NB>& b, uint32_t* f) {
 #pragma unroll
-    for (int q = 0; q < 4; ++q)
-#pragma unroll
-        for (int j = 0; j < 8; ++j) v[q][j] = __ldg(P.table + e[q][j]);
-#pragma unroll
-    for (int q = 0; q < 4; ++q) f[q] = blend8(v[q], w[q]);
+    for (int q = 0; q < NB; ++q) f[q] = blend8_h2(b.v[q], b.w2[q]);
+}
+
+// One group of 4 levels (8 latents = one 16-byte fp16 chunk of the A operand), gathers issued together.
+__device__ __forceinline__ uint4 encode_group4(const KParams& P, int l0, const float u[3]) {
+    Batch<4> b;
+    batch_issue<4>(P, l0, u, b);
+    uint32_t f[4];
+    batch_blend<4>(b, f);
+    return make_uint4(f[0], f[1], f[2], f[3]);
 }
 
 // ---------------------------------------------------------------- O5: real SH, bands 0..3 (reading #13)
