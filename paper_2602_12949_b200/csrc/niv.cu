@@ -1,10 +1,13 @@
 // niv.cu -- libniv: kernels and the C ABI declared in include/niv.h.
 //
 // Kernels (all sm_100a, hand-written):
-//   niv_fused_kernel<WIDTH>  rows a0..a12 of DESIGN.md section 1: persistent CTAs of 128 threads, one texel
-//                            per thread and 128-texel tiles; weights staged once per CTA with a bulk async
-//                            copy; gathers from the L2-resident table; every layer is a tcgen05.mma
-//                            (M=128, kind::f16, fp32 accumulators in TMEM); activations never leave the SM.
+//   niv_fused_tmem_kernel<WIDTH, L, NB>  rows a0..a12 of DESIGN.md section 1 (the default, WIDTH <= 64):
+//                            persistent CTAs of 128 threads, one texel per thread, 128-texel tiles; weights
+//                            staged once per CTA with a bulk async copy; gathers from the L2-resident table run
+//                            NB levels ahead of the packed-fp16 blend; every layer is a tcgen05.mma (M = 128,
+//                            kind::f16, fp32 accumulators AND the fp16 A operand in tensor memory, biases as
+//                            one extra K-step); activations never leave the SM.
+//   niv_fused_kernel<WIDTH, L, NB>       the same with the A operand in shared memory (WIDTH = 128, and A/B runs).
 //   niv_encode_kernel        rows a1..a9 only (stand-alone encoding, fp16 features to global memory).
 //   niv_debug_kernel         index / cell / fraction / fp32 feature dump through the same device functions.
 //   niv_probe_gather_kernel  random-sector gather micro-benchmark (the measured L2-gather roofline).
@@ -26,176 +29,10 @@
 namespace niv {
 
 // =====================================================================================================
-// fused encode + MLP
-// =====================================================================================================
-template <int WIDTH>
-__global__ void __launch_bounds__(kTile) niv_fused_v0_kernel(const __grid_constant__ KParams P,
-                                                             const float* __restrict__ pos,
-                                                             const float* __restrict__ nrm,
-                                                             float* __restrict__ out, size_t n, uint32_t n_tiles)
-{
-    constexpr uint32_t TMEM_COLS = WIDTH < 32 ? 32 : WIDTH;
-    extern __shared__ __align__(1024) uint8_t smem[];
-    uint8_t* sW = smem;                                              // packed weights + biases
-    uint8_t* sA = smem + P.a_off;                                    // A operand: [K/8][128 rows][16 B]
-    float* sBias1 = reinterpret_cast<float*>(smem + P.misc_off);     // layer-1 bias with the parameter fold
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + P.misc_off + WIDTH * 4);
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2);
-
-    const uint32_t tid = threadIdx.x;
-    const uint32_t warp = tid >> 5;
-    const uint32_t bar_w = smem_u32(&bars[0]);
-    const uint32_t bar_mma = smem_u32(&bars[1]);
-    const uint32_t sA_u32 = smem_u32(sA);
-    const uint32_t sW_u32 = smem_u32(sW);
-
-    // ---- a0: one-time setup: barriers, TMEM columns, weights
-    if (tid == 0) {
-        mbar_init(bar_w, 1);
-        mbar_init(bar_mma, 1);
-        mbar_fence_init();
-    }
-    if (warp == 0) tmem_alloc(smem_u32(tmem_slot), TMEM_COLS);
-    tc_fence_before_sync();
-    __syncthreads();
-    tc_fence_after_sync();
-    const uint32_t tmem = *tmem_slot;
-    if (tid == 0) {
-        mbar_arrive_expect_tx(bar_w, P.wpack_bytes);
-        bulk_g2s(sW_u32, P.wpack, P.wpack_bytes, bar_w);
-    }
-    mbar_wait(bar_w, 0);
-
-    // ---- a8: the parameter encoding is constant over the call: fold W1[:, enc_dim:] * enc(t) into the bias
-    if (tid < WIDTH) {
-        float b = reinterpret_cast<const float*>(sW + P.b_off[0])[tid];
-        const uint32_t np16 = 16 * P.n_params;
-        for (uint32_t q = 0; q < P.n_params; ++q) {
-            float enc[16];
-            param_encode8(P.t[q], enc);
-            const float* wp = reinterpret_cast<const float*>(sW + P.wparam_off) + tid * np16 + 16 * q;
-#pragma unroll
-            for (int k = 0; k < 16; ++k) b = fmaf(wp[k], enc[k], b);
-        }
-        sBias1[tid] = b;
-    }
-    __syncthreads();
-
-    const uint32_t lane_taddr = tmem + ((warp * 32u) << 16);
-    const uint32_t n_groups = P.L >> 2;               // 4 levels (8 latents) per 16-byte chunk
-    const uint32_t k1_chunks = P.kdim[0] >> 3;
-    uint32_t phase = 0;
-
-    for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-        const size_t i = (size_t)tile * kTile + tid;
-        const bool valid = i < n;
-        float p[3] = {0.f, 0.f, 0.f}, nv[3] = {0.f, 0.f, 0.f};
-        if (valid) {
-            load3(pos, i, p);
-            load3(nrm, i, nv);
-        }
-        const bool masked = !valid || texel_masked(p, nv);
-
-        // ---- a2..a9: encode this thread's texel into row `tid` of the A tile
-        const uint32_t row_u32 = sA_u32 + tid * 16;
-        if (!masked) {
-            float u[3];
-            normalise(P, p, u);
-            for (uint32_t g = 0; g < n_groups; ++g)
-                *reinterpret_cast<uint4*>(sA + g * 2048 + tid * 16) = encode_group4(P, (int)(g * 4), u);
-            float sh[16];
-            sh16(nv, sh);
-            uint4 c0 = make_uint4(pack_half2(sh[0], sh[1]), pack_half2(sh[2], sh[3]),
-                                  pack_half2(sh[4], sh[5]), pack_half2(sh[6], sh[7]));
-            uint4 c1 = make_uint4(pack_half2(sh[8], sh[9]), pack_half2(sh[10], sh[11]),
-                                  pack_half2(sh[12], sh[13]), pack_half2(sh[14], sh[15]));
-            *reinterpret_cast<uint4*>(sA + (n_groups + 0) * 2048 + tid * 16) = c0;
-            *reinterpret_cast<uint4*>(sA + (n_groups + 1) * 2048 + tid * 16) = c1;
-            for (uint32_t kc = n_groups + 2; kc < k1_chunks; ++kc)       // K padding up to a multiple of 16
-                *reinterpret_cast<uint4*>(sA + kc * 2048 + tid * 16) = make_uint4(0, 0, 0, 0);
-        } else {
-            for (uint32_t kc = 0; kc < k1_chunks; ++kc)
-                *reinterpret_cast<uint4*>(sA + kc * 2048 + tid * 16) = make_uint4(0, 0, 0, 0);
-        }
-        (void)row_u32;
-        fence_proxy_async_smem();
-        tc_fence_before_sync();
-        __syncthreads();
-
-        // ---- a10..a11: layers on the tensor cores
-        for (uint32_t layer = 0; layer < P.n_layers; ++layer) {
-            const uint32_t K = P.kdim[layer], N = P.npad[layer];
-            if (tid == 0) {
-                tc_fence_after_sync();
-                const uint32_t idesc = make_idesc_f16(kTile, N);
-                const uint32_t b_base = sW_u32 + P.w_off[layer];
-                for (uint32_t ks = 0; ks < (K >> 4); ++ks) {
-                    const uint64_t da = make_smem_desc(sA_u32 + ks * 4096u, 2048u, 128u);
-                    const uint64_t db = make_smem_desc(b_base + ks * (N * 32u), N * 16u, 128u);
-                    umma_f16_ss(tmem, da, db, idesc, ks > 0 ? 1u : 0u);
-                }
-                umma_commit(bar_mma);
-            }
-            mbar_wait(bar_mma, phase);
-            phase ^= 1u;
-            tc_fence_after_sync();
-
-            if (layer + 1 < P.n_layers) {
-                // hidden epilogue: bias + ReLU -> fp16 -> next layer's A operand (same buffer; the MMA is done)
-                const float* bias = (layer == 0) ? sBias1 : reinterpret_cast<const float*>(sW + P.b_off[layer]);
-#pragma unroll
-                for (int cc = 0; cc < WIDTH / 32; ++cc) {
-                    uint32_t r[32];
-                    tmem_ld_x32(lane_taddr + cc * 32, r);
-                    tmem_ld_wait();
-#pragma unroll
-                    for (int g = 0; g < 4; ++g) {
-                        uint32_t pk[4];
-#pragma unroll
-                        for (int h = 0; h < 4; ++h) {
-                            const int j = g * 8 + h * 2;
-                            float a = __uint_as_float(r[j]) + bias[cc * 32 + j];
-                            float b = __uint_as_float(r[j + 1]) + bias[cc * 32 + j + 1];
-                            pk[h] = pack_half2(fmaxf(a, 0.0f), fmaxf(b, 0.0f));
-                        }
-                        *reinterpret_cast<uint4*>(sA + (cc * 4 + g) * 2048 + tid * 16) =
-                            make_uint4(pk[0], pk[1], pk[2], pk[3]);
-                    }
-                }
-                fence_proxy_async_smem();
-                tc_fence_before_sync();
-                __syncthreads();
-            } else {
-                // ---- a11..a12: output layer: 3 useful columns, bias, activation, store
-                uint32_t r[4];
-                tmem_ld_x4(lane_taddr, r);
-                tmem_ld_wait();
-                tc_fence_before_sync();
-                if (valid) {
-                    const float* bias = (layer == 0) ? sBias1 : reinterpret_cast<const float*>(sW + P.b_off[layer]);
-                    float y[3];
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) {
-                        float v = __uint_as_float(r[c]) + bias[c];
-                        if (P.out_act == NIV_OUT_SIGMOID) v = 1.0f / (1.0f + __expf(-v));
-                        y[c] = masked ? 0.0f : v;
-                    }
-                    out[3 * i] = y[0];
-                    out[3 * i + 1] = y[1];
-                    out[3 * i + 2] = y[2];
-                }
-            }
-        }
-    }
-
-    __syncthreads();
-    if (warp == 0) tmem_dealloc(tmem, TMEM_COLS);
-}
-
-// =====================================================================================================
 // fused encode + MLP, v1: specialised on <WIDTH, L>, level loop fully unrolled and software-pipelined
 // =====================================================================================================
-// Differences from v0 (profiles/r01_v0_baseline.md: 2435 instructions per texel, latency-bound on the gathers):
+// Differences from the first kernel (v0, profiles/r01_v0_baseline.md: 2435 instructions per texel, a runtime
+// level loop, fp32 blend, fp32 bias + ReLU epilogue):
 //   * the level loop is unrolled (level constants become immediate constant-bank operands) and the gathers run
 //     NB levels ahead of the blend, two batches in flight per thread;
 //   * blend on packed half2 (blend8_h2): the result is directly the fp16 pair of the A operand;
@@ -458,13 +295,25 @@ __global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(const __grid_cons
     fence_proxy_async_smem();          // the bias row is read by the tensor core through the async proxy
 
     uint32_t phase = 0;
+    // G-buffer texel of the first tile; inside the loop the NEXT tile's texel is requested before the current
+    // one is encoded, so its HBM latency hides under a whole tile of work (a1 prefetch)
+    float pn[3] = {0.f, 0.f, 0.f}, nn[3] = {0.f, 0.f, 0.f};
+    if ((size_t)blockIdx.x * kTile + tid < n) {
+        load3(pos, (size_t)blockIdx.x * kTile + tid, pn);
+        load3(nrm, (size_t)blockIdx.x * kTile + tid, nn);
+    }
     for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         const size_t i = (size_t)tile * kTile + tid;
         const bool valid = i < n;
-        float p[3] = {0.f, 0.f, 0.f}, nv[3] = {0.f, 0.f, 0.f};
-        if (valid) {
-            load3(pos, i, p);
-            load3(nrm, i, nv);
+        const float p[3] = {pn[0], pn[1], pn[2]}, nv[3] = {nn[0], nn[1], nn[2]};
+        {
+            const size_t inext = i + (size_t)gridDim.x * kTile;
+#pragma unroll
+            for (int d = 0; d < 3; ++d) { pn[d] = 0.f; nn[d] = 0.f; }
+            if (inext < n) {
+                load3(pos, inext, pn);
+                load3(nrm, inext, nn);
+            }
         }
         const bool masked = !valid || texel_masked(p, nv);
 
@@ -490,6 +339,15 @@ __global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(const __grid_cons
                 if (g + 1 < NG) batch_blend<NB>(bb, a + (g + 1) * NB);
             }
         }
+#ifdef NIV_EXPERIMENT_NOMLP           // timing experiment only: encode, no layers
+        if (valid) {
+            uint32_t x = 0;
+#pragma unroll
+            for (int k = 0; k < AW; ++k) x ^= a[k];
+            out[3 * i] = __uint_as_float(x); out[3 * i + 1] = 0.f; out[3 * i + 2] = 0.f;
+        }
+        continue;
+#endif
         __syncwarp();
         tmem_st_x16(lane_taddr + A_COL, a);
         if (AW > 16) tmem_st_x8(lane_taddr + A_COL + 16, a + 16);
@@ -832,6 +690,14 @@ static int setup_kernel(niv_model* m, K kernel, int tmem_cols, const char* name)
         fprintf(stderr, "[niv] %s: %d regs, %d B smem/CTA, %d TMEM cols -> %d CTAs/SM\n", name, fa.numRegs,
                 smem_per_cta, tmem_cols, blocks);
     if (blocks < 1) return NIV_ERR_UNSUPPORTED;
+    {   // the gathers live on L1 hits: ask for the smallest shared-memory carve-out that still holds `blocks` CTAs,
+        // the rest of the 228 KB becomes L1
+        int pct = (blocks * smem_per_cta * 100 + (int)prop.sharedMemPerMultiprocessor - 1) / (int)prop.sharedMemPerMultiprocessor;
+        if (const char* s = getenv("NIV_CARVEOUT")) { int v = atoi(s); if (v >= 0) pct = v; }
+        pct = std::min(100, std::max(0, pct));
+        NIV_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, pct));
+        if (getenv("NIV_DEBUG")) fprintf(stderr, "[niv] %s: shared-memory carve-out %d %%\n", name, pct);
+    }
     m->info.ctas_per_sm = (uint32_t)blocks;
     m->grid_fused = (uint32_t)blocks * m->info.num_sms;
     return NIV_OK;
@@ -872,11 +738,6 @@ static fused_fn pick_tmem(uint32_t W, uint32_t L, int nb) {
     if (W == 32) return pick_tmem_l<32>(L, nb);
     if (W == 64) return pick_tmem_l<64>(L, nb);
     return nullptr;
-}
-static fused_fn pick_v0(uint32_t W) {
-    if (W == 32) return niv_fused_v0_kernel<32>;
-    if (W == 64) return niv_fused_v0_kernel<64>;
-    return niv_fused_v0_kernel<128>;
 }
 
 extern "C" int niv_create(const niv_config* cfg, niv_model** out)
@@ -985,14 +846,14 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     if (prop.major != 10) { delete m; return NIV_ERR_UNSUPPORTED; }           // sm_100a only; no fallback
     I.num_sms = (uint32_t)prop.multiProcessorCount;
     {
-        const char* kv = getenv("NIV_KERNEL");          // A-B knob: 0 = v0 (generic), 1 = v1 (A in smem), 2 = v2 (A in TMEM)
-        const char* nbv = getenv("NIV_NB");             // gather batch: 2 or 4 levels
+        const char* kv = getenv("NIV_KERNEL");          // A-B knob: 1 = v1 (A operand in shared memory), 2 = v2 (A in TMEM)
+        const char* nbv = getenv("NIV_NB");             // levels per gather batch: 2 or 4
         const int nb = nbv ? atoi(nbv) : 4;
         int kind = kv ? atoi(kv) : 2;
-        if (kind == 2 && W > 64) kind = 1;
+        if (kind != 1 && kind != 2) kind = 2;
+        if (W > 64) kind = 1;                           // width 128: D alone fills the CTA's TMEM budget
         int tmem_cols = W < 32 ? 32 : (int)W;
-        if (kind == 0) m->fused = pick_v0(W);
-        else if (kind == 1) m->fused = pick_fused(W, cfg->n_levels, nb);
+        if (kind == 1) m->fused = pick_fused(W, cfg->n_levels, nb);
         else {
             m->fused = pick_tmem(W, cfg->n_levels, nb);
             tmem_cols = 128;
@@ -1001,7 +862,7 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
             I.smem_bytes = m->smem_fused;
         }
         if (!m->fused) { delete m; return NIV_ERR_UNSUPPORTED; }
-        rc = setup_kernel(m, m->fused, tmem_cols, kind == 0 ? "fused_v0" : kind == 1 ? "fused_v1" : "fused_v2");
+        rc = setup_kernel(m, m->fused, tmem_cols, kind == 1 ? "fused_v1" : "fused_v2");
     }
     if (rc != NIV_OK) { delete m; return rc; }
     e = cudaMalloc(&m->d_table, I.table_bytes);

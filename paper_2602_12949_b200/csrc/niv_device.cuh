@@ -157,7 +157,16 @@ __device__ __forceinline__ void batch_issue(const KParams& P, int l0, const floa
         locate(lv, u, c, w);
         corner_entries(lv, P.tmask, c, e);
 #pragma unroll
-        for (int j = 0; j < 8; ++j) b.v[q][j] = __ldg(lv.tb + e[j]);
+        for (int j = 0; j < 8; ++j) {
+#ifdef NIV_EXPERIMENT_SKIPX1          // timing experiment only (wrong results): what the +x corner loads cost
+            if (j & 1) { b.v[q][j] = b.v[q][j - 1]; continue; }
+#endif
+#ifdef NIV_EXPERIMENT_NOGATHER        // timing experiment only: index arithmetic kept, no table access
+            b.v[q][j] = e[j];
+            continue;
+#endif
+            b.v[q][j] = __ldg(lv.tb + e[j]);
+        }
 #pragma unroll
         for (int d = 0; d < 3; ++d) b.w2[q][d] = pack_half2(w[d], w[d]);
     }

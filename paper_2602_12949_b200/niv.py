@@ -11,7 +11,7 @@ import os
 from typing import Optional, Sequence
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libniv.so")
+_LIB_PATH = os.environ.get("NIV_LIB") or os.path.join(_HERE, "libniv.so")   # NIV_LIB: an experimental build
 
 NIV_API_VERSION = 1
 NIV_OK = 0
