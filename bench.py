@@ -30,6 +30,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+from paper_2602_12949_b200 import dist as D  # noqa: E402
 from paper_2602_12949_b200 import inputs as I  # noqa: E402
 
 W_PX, H_PX = 1920, 1080
@@ -219,7 +220,7 @@ def run_ours(args):
     from paper_2602_12949_b200 import build as B
     from paper_2602_12949_b200 import niv
 
-    rank, world, local = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)
+    rank, world, local = D.env_rank_world()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
     torch.cuda.set_device(local)
@@ -232,7 +233,7 @@ def run_ours(args):
     niv.lib()
 
     # each rank owns one full frame per step (weak scaling: texels shard, the model is replicated)
-    spec, table, wb, bb, pos, nrm, param, desc, masked = make_workload(args.workload, rank)
+    spec, table, wb, bb, pos, nrm, param, desc, masked = make_workload(args.workload, D.frame_of_rank(rank, world)[0])
     n = pos.shape[0]
     model = niv.NivModel(spec, local)
     model.load_params(table, wb, bb)
@@ -268,12 +269,9 @@ def run_ours(args):
         model.infer(d_pos[0], d_nrm[0], d_out[0], param=param)
         torch.cuda.synchronize()
     clk = clocks.stop() if clocks else None
-    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
+    total_ms = D.reduce_max(total_ms, "cuda")
     ms_step = total_ms / args.steps
-    value = world * n / (ms_step * 1e-3) / 1e9
+    value = D.whole_job_gqps(n, world, ms_step)
 
     # ---- end to end: pinned host buffers through niv_infer_host ------------------------------------
     e2e_steps = max(3, min(args.steps, 20))
@@ -288,11 +286,8 @@ def run_ours(args):
         model.infer_host(h_pos[s % 2], h_nrm[s % 2], h_out[s % 2], param=param)   # synchronises: out has landed
     torch.cuda.synchronize()
     e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
-    t = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_ms = float(t.item())
-    e2e_value = world * n / (e2e_ms * 1e-3) / 1e9
+    e2e_ms = D.reduce_max(e2e_ms, "cuda")
+    e2e_value = D.whole_job_gqps(n, world, e2e_ms)
     checksum = float(h_out[0].sum())
 
     if rank != 0:
@@ -322,7 +317,7 @@ def run_ours(args):
         with open(tp) as f:
             traffic = json.load(f).get(args.workload)
     roofline = {
-        "bound": "l2-gather", "kernel": "niv_fused_kernel",
+        "bound": "l2-gather", "kernel": "niv_fused_tmem_kernel" if spec.hidden_width <= 64 else "niv_fused_kernel",
         "achieved": sectors * 32 / kernel_s / 1e9, "peak": gpeak["random_sector"]["sector_gbs"], "unit": "GB/s",
         "frac": max(t_gather, t_tensor, t_hbm) / kernel_s, "traffic": traffic,
         "peak_source": "measured in this run: niv_probe_gather, random 32 B sectors of a resident %d MiB buffer"
