@@ -370,6 +370,71 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_sweep(args):
+    """BASELINE.json configs[4]: table size x MLP width at full HD, and resolution x frames per call.  One JSON line
+    per case on stdout (NOT the contract line: a table for profiles/)."""
+    import torch
+
+    from paper_2602_12949_b200 import build as B
+    from paper_2602_12949_b200 import niv
+
+    B.build()
+    niv.lib()
+    torch.cuda.set_device(0)
+    gb_cache = {}
+
+    def gbuf(w, h, frames):
+        key = (w, h, frames)
+        if key not in gb_cache:
+            gs = [I.make_gbuffer(w, h, 0, frame=f) for f in range(frames)]
+            gb_cache[key] = (np.concatenate([g["pos"] for g in gs]), np.concatenate([g["nrm"] for g in gs]),
+                             float(np.mean([g["masked_fraction"] for g in gs])))
+        return gb_cache[key]
+
+    def one(log2_T, width, w, h, frames):
+        spec = I.spec_fullhd(log2_T, width, 2)
+        pos, nrm, masked = gbuf(w, h, frames)
+        n = pos.shape[0]
+        model = niv.NivModel(spec, 0)
+        wts, bs = I.make_mlp(spec, 0)
+        model.load_params(I.make_table(spec, 0), I.pack_weights(wts), I.pack_biases(bs))
+        ring = max(2, min(8, int(np.ceil(200e6 / (36.0 * n)))))
+        d_pos = [torch.from_numpy(pos).cuda() for _ in range(ring)]
+        d_nrm = [torch.from_numpy(nrm).cuda() for _ in range(ring)]
+        d_out = [torch.empty((n, 3), dtype=torch.float32, device="cuda") for _ in range(ring)]
+        for k in range(5):
+            model.infer(d_pos[k % ring], d_nrm[k % ring], d_out[k % ring])
+        steps = 30
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for k in range(steps):
+            model.infer(d_pos[k % ring], d_nrm[k % ring], d_out[k % ring])
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / steps
+        counts = torch.zeros(33, dtype=torch.int64, device="cuda")
+        model.probe_sectors(d_pos[0], d_nrm[0], counts)
+        torch.cuda.synchronize()
+        sectors = int(counts[:16].sum().item())
+        info = model.info
+        row = {"log2_T": log2_T, "table_MiB": info.table_bytes / 2 ** 20, "width": width, "res": "%dx%d" % (w, h),
+               "frames_per_call": frames, "texels": n, "masked": masked, "ms_per_call": ms, "ms_per_frame": ms / frames,
+               "gqueries_per_s": n / ms / 1e6, "gather_sector_GBs": sectors * 32 / ms / 1e6,
+               "hbm_io_GBs": 36.0 * n / ms / 1e6, "ctas_per_sm": info.ctas_per_sm, "smem_bytes": info.smem_bytes}
+        print(json.dumps(row), flush=True)
+        model.close()
+        del d_pos, d_nrm, d_out
+        torch.cuda.empty_cache()
+
+    for log2_T in (14, 16, 18, 20):
+        for width in (32, 64, 128):
+            one(log2_T, width, W_PX, H_PX, 1)
+    for (w, h) in ((1280, 720), (1920, 1080), (2560, 1440), (3840, 2160)):
+        for frames in (1, 2, 4):
+            one(17, 64, w, h, frames)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -378,9 +443,13 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="fullhd", choices=["fullhd", "incoherent", "param"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[4]: table-size / width / resolution sweep")
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle wall time for cpu_baseline")
     ap.add_argument("--ref-sample", type=int, default=131072, help="texels per step of the reference arm")
     args = ap.parse_args()
+    if args.sweep:
+        run_sweep(args)
+        return
     if args.impl == "reference":
         args.steps = 5 if args.steps is None else args.steps
         args.warmup = 1 if args.warmup is None else args.warmup

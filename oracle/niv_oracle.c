@@ -9,7 +9,8 @@
  *
  * What E_theta is (sec. 4.1; 402-403 sec. 4.4; 666-671 sec. 6):
  *   position x  --multi-level hash-grid encoding-->  L*F latents
- *   normal   n  --real spherical harmonics, bands 0..3--> 16 values  (BASELINE.json configs)
+ *   normal   n  --real spherical harmonics, bands 0..3--> 16 values  (BASELINE.json configs),
+ *                 or the direction itself, 3 values (the paper's own model)
  *   scalar   t  --sin/cos frequency encoding-->  2*B values per parameter
  *   concat --> fully connected ReLU network, no activation on the final layer
  *    --> optional output activation --> RGB irradiance.
@@ -212,9 +213,24 @@ void niv_oracle_param_encode(double t, uint32_t n_frequencies, double *out)
     }
 }
 
+/* ---- direction input (O5): sh_degree 4 -> the 16 real-SH values (BASELINE.json configs);
+ * sh_degree 0 -> the direction itself, (x, y, z) as given: the paper's own model feeds "the input
+ * position and direction" to the network and needs no basis functions (
+ * SPEC.md:306 "raw 3-vector"). ---- */
+static uint32_t dir_dim_of(const niv_oracle_config *cfg)
+{
+    return cfg->sh_degree == 0 ? 3u : cfg->sh_degree * cfg->sh_degree;
+}
+
+static void dir_encode(const niv_oracle_config *cfg, const double n[3], double *out)
+{
+    if (cfg->sh_degree == 0) { out[0] = n[0]; out[1] = n[1]; out[2] = n[2]; }
+    else niv_oracle_sh16(n, out);
+}
+
 static uint32_t in_dim_of(const niv_oracle_config *cfg)
 {
-    return cfg->n_levels * cfg->n_features + cfg->sh_degree * cfg->sh_degree
+    return cfg->n_levels * cfg->n_features + dir_dim_of(cfg)
          + 2 * cfg->n_frequencies * cfg->n_params;
 }
 
@@ -254,7 +270,7 @@ static int check_cfg(const niv_oracle_config *cfg)
     if (cfg->n_levels == 0 || cfg->n_levels > NIV_ORACLE_MAX_LEVELS) return -1;
     if (cfg->n_features == 0 || cfg->n_features > 16) return -1;
     if (cfg->log2_table_size == 0 || cfg->log2_table_size > 30) return -1;
-    if (cfg->sh_degree != 4) return -1;
+    if (cfg->sh_degree != 4 && cfg->sh_degree != 0) return -1;
     if (in_dim_of(cfg) > NIV_ORACLE_MAX_DIM || cfg->hidden_width > NIV_ORACLE_MAX_DIM) return -1;
     return 0;
 }
@@ -289,10 +305,10 @@ int niv_oracle_encode(const niv_oracle_config *cfg, const uint16_t *table,
         encode_one(cfg, N, dense, table, pos + 3 * i, ii, cc, ff, xx);
         if (xx) {
             double nn[3] = { (double)nrm[3 * i], (double)nrm[3 * i + 1], (double)nrm[3 * i + 2] };
-            niv_oracle_sh16(nn, xx + L * F);                         /* O5 */
+            dir_encode(cfg, nn, xx + L * F);                         /* O5 */
             for (uint32_t q = 0; q < cfg->n_params; ++q)             /* O6 */
                 niv_oracle_param_encode((double)param[q], cfg->n_frequencies,
-                                        xx + L * F + 16 + 2 * cfg->n_frequencies * q);
+                                        xx + L * F + dir_dim_of(cfg) + 2 * cfg->n_frequencies * q);
         }
     }
     return 0;
@@ -319,10 +335,10 @@ int niv_oracle_infer(const niv_oracle_config *cfg, const uint16_t *table,
             double x[NIV_ORACLE_MAX_DIM];
             encode_one(cfg, N, dense, table, pos + 3 * i, NULL, NULL, NULL, x);   /* O1-O4 */
             double nn[3] = { (double)nrm[3 * i], (double)nrm[3 * i + 1], (double)nrm[3 * i + 2] };
-            niv_oracle_sh16(nn, x + L * F);                          /* O5, O7 */
+            dir_encode(cfg, nn, x + L * F);                          /* O5, O7 */
             for (uint32_t q = 0; q < cfg->n_params; ++q)             /* O6, O7 */
                 niv_oracle_param_encode((double)param[q], cfg->n_frequencies,
-                                        x + L * F + 16 + 2 * cfg->n_frequencies * q);
+                                        x + L * F + dir_dim_of(cfg) + 2 * cfg->n_frequencies * q);
             niv_oracle_mlp(cfg, weights, biases, x, y);              /* O8 */
             if (cfg->out_activation == 1)                            /* O9 */
                 for (int c = 0; c < 3; ++c) y[c] = 1.0 / (1.0 + exp(-y[c]));

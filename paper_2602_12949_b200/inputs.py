@@ -80,7 +80,7 @@ class ModelSpec:
     out_activation: int = OUT_SIGMOID
     n_params: int = 0             # per-call scalar scene parameters
     n_frequencies: int = 8        # sin/cos bands per parameter
-    sh_degree: int = 4            # 4 => 16 coefficients (BASELINE.json)
+    sh_degree: int = 4            # 4 => 16 SH coefficients (BASELINE.json); 0 => the raw direction, 3 values (paper)
     resolutions: Optional[Tuple[int, ...]] = None   # explicit N_l override
 
     @property
@@ -88,8 +88,12 @@ class ModelSpec:
         return 1 << self.log2_table_size
 
     @property
+    def dir_dim(self) -> int:
+        return 3 if self.sh_degree == 0 else self.sh_degree ** 2
+
+    @property
     def in_dim(self) -> int:
-        return self.n_levels * self.n_features + self.sh_degree ** 2 + 2 * self.n_frequencies * self.n_params
+        return self.n_levels * self.n_features + self.dir_dim + 2 * self.n_frequencies * self.n_params
 
     @property
     def layer_shapes(self) -> List[Tuple[int, int]]:
@@ -115,6 +119,18 @@ def spec_fullhd(log2_T: int = 17, width: int = 64, n_hidden: int = 2) -> ModelSp
 def spec_param() -> ModelSpec:
     """BASELINE.json configs[3]: T=2^18, one scalar t (8 sin/cos bands), MLP 64->64->64->3."""
     return ModelSpec(16, 2, 18, 16, 1.5, *ROOM_AABB, hidden_width=64, n_hidden_layers=2, n_params=1)
+
+
+PAPER_RESOLUTIONS = (16, 22, 32, 45, 64, 90, 128, 181)     # floor(16 * sqrt(2)^l), l = 0..7 (exact: 16 * 2^(l/2))
+
+
+def spec_paper(n_levels: int = 8, width: int = 64) -> ModelSpec:
+    """The paper's own model family (Table 1 382-389): T = 2^17, latent dimension 4, scale
+    sqrt(2) between levels, coarsest side 16, 2..8 levels; "four-layer" ReLU MLP = 4 weight matrices (3 hidden
+    layers); position + direction in, no basis functions on the direction, no activation on the final layer.
+    Resolutions are passed explicitly so that no pow() rounding decides an integer."""
+    return ModelSpec(n_levels, 4, 17, 16, 2.0 ** 0.5, *ROOM_AABB, hidden_width=width, n_hidden_layers=3,
+                     out_activation=OUT_LINEAR, sh_degree=0, resolutions=PAPER_RESOLUTIONS[:n_levels])
 
 
 # ----------------------------------------------------------------------------

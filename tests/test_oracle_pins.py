@@ -252,7 +252,8 @@ def _brute_force_latents(spec, N, dense, table, u):
     1-|p_d-v_d|), no corner selection, separately coded index/hash (north_star: brute-force enumeration)."""
     T = spec.table_size
     tab = table.astype(np.float64)
-    feats = np.zeros((len(u), spec.n_levels * 2))
+    F = spec.n_features
+    feats = np.zeros((len(u), spec.n_levels * F))
     for l in range(spec.n_levels):
         n = int(N[l])
         R = n + 1
@@ -269,7 +270,7 @@ def _brute_force_latents(spec, N, dense, table, u):
             wx = np.maximum(0.0, 1.0 - np.abs(p[0] - vx))
             wy = np.maximum(0.0, 1.0 - np.abs(p[1] - vy))
             wz = np.maximum(0.0, 1.0 - np.abs(p[2] - vz))
-            feats[q, 2 * l:2 * l + 2] = ((wx * wy * wz)[:, None] * vals).sum(axis=0)
+            feats[q, F * l:F * l + F] = ((wx * wy * wz)[:, None] * vals).sum(axis=0)
     return feats
 
 
@@ -298,6 +299,59 @@ def test_brute_force_enumeration_4x4(oracle):
     # sees the direction only: hence 2e-7 here; test_sh16_matches_scipy holds 5e-15 on exactly-unit input
     np.testing.assert_allclose(out64, ref, rtol=0, atol=2e-7)
     assert np.array_equal(out32, out64.astype(np.float32))
+
+
+def test_paper_family_brute_force_4x4(oracle):
+    """The paper's own model family: latent dimension 4, scale sqrt(2), coarsest
+    side 16, position + RAW direction in, four weight matrices, no output activation -- a 4x4 G-buffer through the
+    whole path against the tent-sum over every lattice vertex and a numpy matmul chain.  T = 2^14 so that levels
+    2..3 are hashed and the enumeration stays small."""
+    spec = dataclasses.replace(I.spec_paper(4, 32), log2_table_size=14, aabb_min=I.UNIT_AABB[0], aabb_max=I.UNIT_AABB[1])
+    assert spec.in_dim == 4 * 4 + 3 and spec.layer_shapes == [(32, 19), (32, 32), (32, 32), (3, 32)]
+    table = I.make_table(spec, 3, -1.0, 1.0)
+    weights, biases = I.make_mlp(spec, 3, bias_scale=0.1)
+    N, dense = oracle.level_table(spec)
+    assert list(N) == [16, 22, 32, 45] and list(dense) == [True, True, False, False]
+    pos = I.positions_uniform(16, I.UNIT_AABB, 5)
+    nrm = I.normals_uniform(16, 5)
+    lat = _brute_force_latents(spec, N, dense, table, pos)
+    enc = oracle.encode(spec, table, pos, nrm)
+    np.testing.assert_allclose(enc["features"][:, :16], lat, rtol=0, atol=1e-13)
+    assert np.array_equal(enc["features"][:, 16:19], nrm.astype(np.float64))          # the direction as given
+    h = np.concatenate([lat, nrm.astype(np.float64)], axis=1)
+    for k, (w, b) in enumerate(zip(weights, biases)):
+        h = h @ w.astype(np.float64).T + b.astype(np.float64)
+        if k + 1 < len(weights):
+            h = np.maximum(h, 0.0)
+    out32, out64 = oracle.infer(spec, table, I.pack_weights(weights), I.pack_biases(biases), pos, nrm, want_f64=True)
+    np.testing.assert_allclose(out64, h, rtol=0, atol=1e-12)                            # linear output
+    assert np.array_equal(out32, out64.astype(np.float32))
+
+
+def test_paper_family_vertex_and_partition_of_unity(oracle):
+    """F = 4: a query on a lattice vertex returns that vertex's four latents; a per-level constant table gives
+    that constant for any position (dense and hashed levels of the full 8-level paper grid)."""
+    spec = dataclasses.replace(I.spec_paper(8, 64), aabb_min=I.UNIT_AABB[0], aabb_max=I.UNIT_AABB[1])
+    N, dense = oracle.level_table(spec)
+    assert list(N) == list(I.PAPER_RESOLUTIONS) and list(dense) == [True] * 4 + [False] * 4
+    table = I.make_table(spec, 7, -1.0, 1.0)
+    nrm = I.normals_uniform(8, 1)
+    for l in (0, 2, 4, 6):                    # power-of-two resolutions: k/N and (k/N)*N are exact in fp32
+        n = int(N[l])
+        k = np.array([[1, 2, 3], [n, n, n], [0, n // 2, n - 1], [5, 0, 7]], dtype=np.int64)
+        pos = (k / float(n)).astype(np.float32)
+        enc = oracle.encode(spec, table, pos, nrm[:4])
+        for q in range(4):
+            vx, vy, vz = (int(v) for v in k[q])
+            e = vx + (n + 1) * (vy + (n + 1) * vz) if dense[l] else _hash_py(vx, vy, vz, spec.table_size)
+            np.testing.assert_allclose(enc["features"][q, 4 * l:4 * l + 4], table[l][e].astype(np.float64), atol=1e-15)
+    const = np.zeros_like(table)
+    for l in range(8):
+        const[l, :, :] = np.float16(0.125 * (l + 1))
+    pos = I.positions_uniform(64, I.UNIT_AABB, 9)
+    enc = oracle.encode(spec, const, pos, I.normals_uniform(64, 9))
+    want = np.repeat(0.125 * (np.arange(8) + 1), 4)
+    np.testing.assert_allclose(enc["features"][:, :32], np.broadcast_to(want, (64, 32)), atol=1e-14)
 
 
 # ------------------------------------------------------------------ SH-16
