@@ -15,6 +15,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <new>
 #include <vector>
@@ -129,14 +130,14 @@ __global__ void __launch_bounds__(kTile) niv_fused_kernel(const __grid_constant_
             float u[3];
             normalise(P, p, u);
             uint32_t f[L];
-            Batch<NB> ba, bb;
-            batch_issue<NB>(P, 0, u, ba);
+            Batch<NB, 2> ba, bb;
+            batch_issue<NB, 2>(P, 0, u, ba);
 #pragma unroll
             for (int g = 0; g < NG; g += 2) {
-                if (g + 1 < NG) batch_issue<NB>(P, (g + 1) * NB, u, bb);
-                batch_blend<NB>(ba, f + g * NB);
-                if (g + 2 < NG) batch_issue<NB>(P, (g + 2) * NB, u, ba);
-                if (g + 1 < NG) batch_blend<NB>(bb, f + (g + 1) * NB);
+                if (g + 1 < NG) batch_issue<NB, 2>(P, (g + 1) * NB, u, bb);
+                batch_blend<NB, 2>(ba, f + g * NB);
+                if (g + 2 < NG) batch_issue<NB, 2>(P, (g + 2) * NB, u, ba);
+                if (g + 1 < NG) batch_blend<NB, 2>(bb, f + (g + 1) * NB);
             }
 #pragma unroll
             for (int c = 0; c < HC; ++c)
@@ -234,7 +235,7 @@ __global__ void __launch_bounds__(kTile) niv_fused_kernel(const __grid_constant_
 // Here thread t keeps row t of the A operand in TMEM lane t: tcgen05.st instead of STS (no L1TEX wavefronts,
 // no generic->async proxy fence), tcgen05.mma reads A from TMEM, and shared memory holds the weights only.
 // TMEM columns per CTA (128 allocated): D [0, WIDTH) fp32 | A [64, 96) packed fp16 pairs | ones [96, 104).
-template <int WIDTH, int L, int NB>
+template <int WIDTH, int L, int NB, int F, bool RAWDIR>
 __global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(const __grid_constant__ KParams P,
                                                                const float* __restrict__ pos,
                                                                const float* __restrict__ nrm,
@@ -243,11 +244,14 @@ __global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(const __grid_cons
     static_assert(WIDTH <= 64, "A-in-TMEM kernel: D + A + ones must fit 128 columns");
     constexpr uint32_t TMEM_COLS = 128, A_COL = 64, ONES_COL = 96;
     constexpr int NG = L / NB;
-    constexpr int AW = (L + 8 + 7) / 8 * 8;          // 32-bit words of one layer-1 A row (K1 = 2 * AW)
+    constexpr int HW = L * F / 2;                     // 32-bit words of hash latents in one A row
+    constexpr int DW = RAWDIR ? 2 : 8;                // ... of the direction input: (x, y | z, 0) or SH-16
+    constexpr int AW = (HW + DW + 7) / 8 * 8;         // ... of one layer-1 A row (K1 = 2 * AW)
     extern __shared__ __align__(1024) uint8_t smem[];
     uint8_t* sW = smem;
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + P.misc_off);
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2);
+    uint32_t* s_tile = tmem_slot + 1;                 // [2]: the tile after next, handed from thread 0 to the CTA
 
     const uint32_t tid = threadIdx.x;
     const uint32_t warp = tid >> 5;
@@ -261,6 +265,9 @@ __global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(const __grid_cons
         mbar_fence_init();
     }
     if (warp == 0) tmem_alloc(smem_u32(tmem_slot), TMEM_COLS);
+    // dynamic tile scheduling: tile blockIdx.x is static, every further tile comes from a global counter, so a CTA
+    // that drew cheap (background) tiles or a fast SM simply draws more of them and the grid drains together
+    if (tid == 0) s_tile[0] = gridDim.x + atomicAdd(P.tile_ctr, 1u);
     tc_fence_before_sync();
     __syncthreads();
     tc_fence_after_sync();
@@ -302,12 +309,15 @@ __global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(const __grid_cons
         load3(pos, (size_t)blockIdx.x * kTile + tid, pn);
         load3(nrm, (size_t)blockIdx.x * kTile + tid, nn);
     }
-    for (uint32_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    uint32_t tile = blockIdx.x, tnext = s_tile[0], it = 0;
+    while (tile < n_tiles) {
         const size_t i = (size_t)tile * kTile + tid;
         const bool valid = i < n;
         const float p[3] = {pn[0], pn[1], pn[2]}, nv[3] = {nn[0], nn[1], nn[2]};
+        uint32_t tnn_mine = 0;
+        if (tid == 0) tnn_mine = gridDim.x + atomicAdd(P.tile_ctr, 1u);       // the tile after next
         {
-            const size_t inext = i + (size_t)gridDim.x * kTile;
+            const size_t inext = (size_t)tnext * kTile + tid;
 #pragma unroll
             for (int d = 0; d < 3; ++d) { pn[d] = 0.f; nn[d] = 0.f; }
             if (inext < n) {
@@ -325,18 +335,23 @@ __global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(const __grid_cons
         if (!masked) {
             float u[3];
             normalise(P, p, u);
-            Batch<NB> ba, bb;
-            batch_issue<NB>(P, 0, u, ba);
-            float sh[16];
-            sh16(nv, sh);
+            Batch<NB, F> ba, bb;
+            batch_issue<NB, F>(P, 0, u, ba);
+            if (RAWDIR) {                             // the paper's model: the direction itself
+                a[HW] = pack_half2(nv[0], nv[1]);
+                a[HW + 1] = pack_half2(nv[2], 0.0f);
+            } else {
+                float sh[16];
+                sh16(nv, sh);
 #pragma unroll
-            for (int k = 0; k < 8; ++k) a[L + k] = pack_half2(sh[2 * k], sh[2 * k + 1]);
+                for (int k = 0; k < 8; ++k) a[HW + k] = pack_half2(sh[2 * k], sh[2 * k + 1]);
+            }
 #pragma unroll
             for (int g = 0; g < NG; g += 2) {
-                if (g + 1 < NG) batch_issue<NB>(P, (g + 1) * NB, u, bb);
-                batch_blend<NB>(ba, a + g * NB);
-                if (g + 2 < NG) batch_issue<NB>(P, (g + 2) * NB, u, ba);
-                if (g + 1 < NG) batch_blend<NB>(bb, a + (g + 1) * NB);
+                if (g + 1 < NG) batch_issue<NB, F>(P, (g + 1) * NB, u, bb);
+                batch_blend<NB, F>(ba, a + g * NB * (F / 2));
+                if (g + 2 < NG) batch_issue<NB, F>(P, (g + 2) * NB, u, ba);
+                if (g + 1 < NG) batch_blend<NB, F>(bb, a + (g + 1) * NB * (F / 2));
             }
         }
 #ifdef NIV_EXPERIMENT_NOMLP           // timing experiment only: encode, no layers
@@ -346,14 +361,20 @@ __global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(const __grid_cons
             for (int k = 0; k < AW; ++k) x ^= a[k];
             out[3 * i] = __uint_as_float(x); out[3 * i + 1] = 0.f; out[3 * i + 2] = 0.f;
         }
+        if (tid == 0) s_tile[(it + 1) & 1] = tnn_mine;
+        __syncthreads();
+        tile = tnext; tnext = s_tile[(it + 1) & 1]; ++it;
         continue;
 #endif
         __syncwarp();
-        tmem_st_x16(lane_taddr + A_COL, a);
-        if (AW > 16) tmem_st_x8(lane_taddr + A_COL + 16, a + 16);
+        if constexpr (AW == 8) tmem_st_x8(lane_taddr + A_COL, a);
+        else tmem_st_x16(lane_taddr + A_COL, a);
+        if constexpr (AW > 16) tmem_st_x8(lane_taddr + A_COL + 16, a + 16);
         tmem_st_wait();
+        if (tid == 0) s_tile[(it + 1) & 1] = tnn_mine;
         tc_fence_before_sync();
         __syncthreads();
+        const uint32_t tnn = s_tile[(it + 1) & 1];
 
         for (uint32_t layer = 0; layer < P.n_layers; ++layer) {
             const uint32_t K = P.kdim[layer], N = P.npad[layer];
@@ -409,6 +430,9 @@ __global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(const __grid_cons
                 }
             }
         }
+        tile = tnext;
+        tnext = tnn;
+        ++it;
     }
 
     __syncthreads();
@@ -473,15 +497,20 @@ __global__ void __launch_bounds__(128) niv_debug_kernel(const __grid_constant__ 
         int c[3] = {0, 0, 0};
         float w[3] = {0.f, 0.f, 0.f};
         uint32_t e[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-        float2 f = make_float2(0.f, 0.f);
+        float f[4] = {0.f, 0.f, 0.f, 0.f};
+        const uint32_t FW = P.n_features >> 1;               // 32-bit words per entry
         if (!masked) {
             locate(P.lv[l], u, c, w);
             corner_entries(P.lv[l], P.tmask, c, e);
             if (feat) {
-                uint32_t v[8];
+                for (uint32_t h = 0; h < FW; ++h) {
+                    uint32_t v[8];
 #pragma unroll
-                for (int j = 0; j < 8; ++j) v[j] = __ldg(P.lv[l].tb + e[j]);
-                f = blend8(v, w);
+                    for (int j = 0; j < 8; ++j) v[j] = __ldg(P.lv[l].tb + (size_t)e[j] * FW + h);
+                    const float2 t = blend8(v, w);
+                    f[2 * h] = t.x;
+                    f[2 * h + 1] = t.y;
+                }
             }
         }
         if (idx)
@@ -490,19 +519,25 @@ __global__ void __launch_bounds__(128) niv_debug_kernel(const __grid_constant__ 
             for (int d = 0; d < 3; ++d) cell[(i * L + l) * 3 + d] = c[d];
         if (frac)
             for (int d = 0; d < 3; ++d) frac[(i * L + l) * 3 + d] = w[d];
-        if (feat) {
-            feat[i * P.in_dim + 2 * l] = f.x;
-            feat[i * P.in_dim + 2 * l + 1] = f.y;
-        }
+        if (feat)
+            for (uint32_t k = 0; k < P.n_features; ++k) feat[i * P.in_dim + P.n_features * l + k] = f[k];
     }
     if (feat) {
-        float sh[16];
-        sh16(nv, sh);
-        for (int k = 0; k < 16; ++k) feat[i * P.in_dim + 2 * L + k] = masked ? 0.f : sh[k];
+        const uint32_t o = P.n_features * L;
+        uint32_t dd;
+        if (P.raw_dir) {
+            dd = 3;
+            for (int k = 0; k < 3; ++k) feat[i * P.in_dim + o + k] = masked ? 0.f : nv[k];
+        } else {
+            dd = 16;
+            float sh[16];
+            sh16(nv, sh);
+            for (int k = 0; k < 16; ++k) feat[i * P.in_dim + o + k] = masked ? 0.f : sh[k];
+        }
         for (uint32_t q = 0; q < P.n_params; ++q) {
             float e[16];
             param_encode8(P.t[q], e);
-            for (int k = 0; k < 16; ++k) feat[i * P.in_dim + 2 * L + 16 + 16 * q + k] = masked ? 0.f : e[k];
+            for (int k = 0; k < 16; ++k) feat[i * P.in_dim + o + dd + 16 * q + k] = masked ? 0.f : e[k];
         }
     }
 }
@@ -601,8 +636,8 @@ __global__ void __launch_bounds__(128) niv_sector_census_kernel(const __grid_con
             corner_entries(P.lv[l], P.tmask, c, e);
         }
 #pragma unroll
-        for (int j = 0; j < 8; ++j)                                           // 8 entries per 32-byte sector
-            s_sec[warp][lane * 8 + j] = masked ? 0xFFFFFFFFu : ((P.lv[l].base + e[j]) >> 3);
+        for (int j = 0; j < 8; ++j)                                           // 8 (F = 2) or 4 (F = 4) entries per 32-byte sector
+            s_sec[warp][lane * 8 + j] = masked ? 0xFFFFFFFFu : ((P.lv[l].base + e[j]) >> (P.n_features == 4 ? 2 : 3));
         __syncwarp();
         uint32_t sec = 0, lin = 0;
         for (int q = 0; q < 8; ++q) {
@@ -637,6 +672,8 @@ __global__ void __launch_bounds__(128) niv_sector_census_kernel(const __grid_con
 // =====================================================================================================
 using namespace niv;
 
+constexpr uint32_t kCtrSlots = 64;      // launches of one model that may be in flight at once (different streams)
+
 struct niv_model {
     niv_config cfg;
     niv_info info;
@@ -648,6 +685,8 @@ struct niv_model {
     uint32_t grid_fused = 0;
     uint32_t smem_fused = 0;
     void (*fused)(KParams, const float*, const float*, float*, size_t, uint32_t) = nullptr;
+    uint32_t* d_ctr = nullptr;                     // kCtrSlots tile counters, 128 B apart; one per launch in flight
+    mutable std::atomic<uint32_t> ctr_next{0};
     // niv_infer_host staging (grown on demand)
     float* d_stage = nullptr;          // [pos | nrm | out], each 3*stage_cap floats
     size_t stage_cap = 0;
@@ -723,18 +762,32 @@ static fused_fn pick_fused(uint32_t W, uint32_t L, int nb) {
     return pick_l<128>(L, nb);
 }
 template <int W, int L>
-static fused_fn pick_tmem_nb(int nb) { return nb == 4 ? niv_fused_tmem_kernel<W, L, 4> : niv_fused_tmem_kernel<W, L, 2>; }
+static fused_fn pick_tmem_nb(int nb) {
+    return nb == 4 ? niv_fused_tmem_kernel<W, L, 4, 2, false> : niv_fused_tmem_kernel<W, L, 2, 2, false>;
+}
 template <int W>
 static fused_fn pick_tmem_l(uint32_t L, int nb) {
     switch (L) {
-        case 4:  return niv_fused_tmem_kernel<W, 4, 4>;
+        case 4:  return niv_fused_tmem_kernel<W, 4, 4, 2, false>;
         case 8:  return pick_tmem_nb<W, 8>(nb);
-        case 12: return niv_fused_tmem_kernel<W, 12, 4>;
+        case 12: return niv_fused_tmem_kernel<W, 12, 4, 2, false>;
         case 16: return pick_tmem_nb<W, 16>(nb);
         default: return nullptr;
     }
 }
-static fused_fn pick_tmem(uint32_t W, uint32_t L, int nb) {
+// the paper's own family: F = 4, raw direction, 2..8 levels, 2 levels (16 x 8-byte gathers) per batch
+template <int W>
+static fused_fn pick_tmem_paper(uint32_t L) {
+    switch (L) {
+        case 2: return niv_fused_tmem_kernel<W, 2, 2, 4, true>;
+        case 4: return niv_fused_tmem_kernel<W, 4, 2, 4, true>;
+        case 6: return niv_fused_tmem_kernel<W, 6, 2, 4, true>;
+        case 8: return niv_fused_tmem_kernel<W, 8, 2, 4, true>;
+        default: return nullptr;
+    }
+}
+static fused_fn pick_tmem(uint32_t W, uint32_t L, int nb, uint32_t F) {
+    if (F == 4) return W == 32 ? pick_tmem_paper<32>(L) : W == 64 ? pick_tmem_paper<64>(L) : nullptr;
     if (W == 32) return pick_tmem_l<32>(L, nb);
     if (W == 64) return pick_tmem_l<64>(L, nb);
     return nullptr;
@@ -758,9 +811,14 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     if (!explicit_res && (cfg->base_resolution == 0 || !(cfg->per_level_scale >= 1.0) || !std::isfinite(cfg->per_level_scale)))
         return NIV_ERR_INVALID_ARG;
     // shapes this build has kernels for
-    if (cfg->n_features != 2) return NIV_ERR_UNSUPPORTED;
-    if (cfg->n_levels % 4 != 0) return NIV_ERR_UNSUPPORTED;            // {4, 8, 12, 16}
-    if (cfg->sh_degree != 4 || cfg->n_params > 2 || (cfg->n_params && cfg->n_frequencies != 8)) return NIV_ERR_UNSUPPORTED;
+    // two model families: BASELINE.json's (F = 2, SH-16 direction, L in {4, 8, 12, 16}) and the paper's own
+    // (F = 4, raw direction, L in {2, 4, 6, 8}, width <= 64)
+    if (cfg->n_features == 2) {
+        if (cfg->sh_degree != 4 || cfg->n_levels % 4 != 0) return NIV_ERR_UNSUPPORTED;
+    } else if (cfg->n_features == 4) {
+        if (cfg->sh_degree != 0 || cfg->n_levels % 2 != 0 || cfg->n_levels > 8 || cfg->hidden_width > 64) return NIV_ERR_UNSUPPORTED;
+    } else return NIV_ERR_UNSUPPORTED;
+    if (cfg->n_params > 2 || (cfg->n_params && cfg->n_frequencies != 8)) return NIV_ERR_UNSUPPORTED;
     if (cfg->n_hidden_layers > 3) return NIV_ERR_UNSUPPORTED;
     if (cfg->hidden_width != 32 && cfg->hidden_width != 64 && cfg->hidden_width != 128) return NIV_ERR_UNSUPPORTED;
 
@@ -799,7 +857,9 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     }
     P.L = cfg->n_levels;
     P.tmask = (uint32_t)(T - 1);
-    P.enc_dim = cfg->n_levels * cfg->n_features + 16;
+    P.n_features = cfg->n_features;
+    P.raw_dir = cfg->sh_degree == 0 ? 1u : 0u;
+    P.enc_dim = cfg->n_levels * cfg->n_features + (P.raw_dir ? 3u : 16u);
     P.in_dim = P.enc_dim + 2 * cfg->n_frequencies * cfg->n_params;
     P.n_params = cfg->n_params;
     P.n_layers = cfg->n_hidden_layers + 1;
@@ -855,7 +915,7 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
         int tmem_cols = W < 32 ? 32 : (int)W;
         if (kind == 1) m->fused = pick_fused(W, cfg->n_levels, nb);
         else {
-            m->fused = pick_tmem(W, cfg->n_levels, nb);
+            m->fused = pick_tmem(W, cfg->n_levels, nb, cfg->n_features);
             tmem_cols = 128;
             m->smem_fused = P.a_off + 2 * 8 + 16;        // weights + barriers only
             P.misc_off = P.a_off;
@@ -867,14 +927,15 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     if (rc != NIV_OK) { delete m; return rc; }
     e = cudaMalloc(&m->d_table, I.table_bytes);
     if (e == cudaSuccess) e = cudaMalloc(&m->d_wpack, P.wpack_bytes);
+    if (e == cudaSuccess) e = cudaMalloc(&m->d_ctr, kCtrSlots * 128);
     if (e != cudaSuccess) {
         g_last_cuda_error = (int)e; (void)cudaGetLastError();
-        cudaFree(m->d_table); cudaFree(m->d_wpack); delete m;
+        cudaFree(m->d_table); cudaFree(m->d_wpack); cudaFree(m->d_ctr); delete m;
         return NIV_ERR_ALLOC;
     }
     P.table = m->d_table;
     P.wpack = m->d_wpack;
-    for (uint32_t l = 0; l < cfg->n_levels; ++l) P.lv[l].tb = m->d_table + P.lv[l].base;
+    for (uint32_t l = 0; l < cfg->n_levels; ++l) P.lv[l].tb = m->d_table + (size_t)P.lv[l].base * (cfg->n_features / 2);
     *out = m;
     return NIV_OK;
 }
@@ -962,9 +1023,12 @@ static int fill_params(const niv_model* m, const float* param, KParams& P)
     return NIV_OK;
 }
 
-static int launch_fused(const niv_model* m, const KParams& P, const float* pos, const float* nrm, float* out,
+static int launch_fused(const niv_model* m, const KParams& Pin, const float* pos, const float* nrm, float* out,
                         size_t n, cudaStream_t st)
 {
+    KParams P = Pin;
+    P.tile_ctr = m->d_ctr + (size_t)(m->ctr_next.fetch_add(1u) % kCtrSlots) * 32;
+    NIV_CUDA(cudaMemsetAsync(P.tile_ctr, 0, sizeof(uint32_t), st));
     const uint32_t n_tiles = (uint32_t)((n + kTile - 1) / kTile);
     const uint32_t grid = n_tiles < m->grid_fused ? n_tiles : m->grid_fused;
     m->fused<<<grid, kTile, m->smem_fused, st>>>(P, pos, nrm, out, n, n_tiles);
@@ -1042,6 +1106,7 @@ extern "C" int niv_encode(niv_model* m, const float* pos, const float* nrm, cons
     if (!m->loaded) return NIV_ERR_NOT_LOADED;
     if (n == 0) return NIV_OK;
     if (!pos || !nrm || !features_fp16 || ((uintptr_t)features_fp16 & 15)) return NIV_ERR_INVALID_ARG;
+    if (m->cfg.n_features != 2) return NIV_ERR_UNSUPPORTED;      // the stand-alone kernel serves the F = 2 / SH-16 family
     KParams P;
     int rc = fill_params(m, param, P);
     if (rc != NIV_OK) return rc;
@@ -1086,6 +1151,7 @@ extern "C" int niv_destroy(niv_model* m)
     cudaSetDevice(m->cfg.device);
     cudaFree(m->d_table);
     cudaFree(m->d_wpack);
+    cudaFree(m->d_ctr);
     cudaFree(m->d_stage);
     if (m->hs[0]) cudaStreamDestroy(m->hs[0]);
     if (m->hs[1]) cudaStreamDestroy(m->hs[1]);

@@ -19,7 +19,7 @@ struct LevelP {
     uint32_t R2;        // R*R
     uint32_t base;      // first table entry of this level = l*T
     uint32_t dense;     // 1 dense, 0 hashed
-    const uint32_t* tb; // table + base: this level's first entry (so that a gather address is ONE IMAD.WIDE)
+    const uint32_t* tb; // this level's first entry = table + base * (F/2) words (a gather address is ONE IMAD.WIDE)
 };
 
 struct KParams {
@@ -27,13 +27,16 @@ struct KParams {
     float    ainv[3];           // fl32(1 / fl32(max - min))
     uint32_t L;
     uint32_t tmask;             // T - 1
-    uint32_t in_dim;            // L*F + 16 + 16*n_params
-    uint32_t enc_dim;           // L*F + 16     (what the layer-1 MMA consumes)
+    uint32_t in_dim;            // L*F + dir_dim + 16*n_params
+    uint32_t enc_dim;           // L*F + dir_dim  (what the layer-1 MMA consumes); dir_dim = 16 (SH) or 3 (raw)
+    uint32_t n_features;        // F
+    uint32_t raw_dir;           // 1: the direction itself is the input (paper), 0: SH-16
     uint32_t n_params;
     uint32_t n_layers;          // hidden + 1
     uint32_t out_act;
     float    t[2];              // per-call scene parameters
     LevelP   lv[kMaxLevels];
+    uint32_t* tile_ctr;         // per-launch tile counter (zeroed on the stream before the launch): dynamic tile scheduling
     const uint32_t* table;      // [L][T] entries of 2 x fp16
     const uint8_t*  wpack;      // packed weights + biases (see niv.cu pack_weights)
     uint32_t wpack_bytes;
@@ -141,13 +144,15 @@ __device__ __forceinline__ uint32_t blend8_h2(const uint32_t v[8], const uint32_
 
 // A batch of NB levels in flight: the 8*NB gathers are issued by batch_issue and consumed by batch_blend, so
 // the caller can issue the next batch before blending the current one (software pipelining inside a thread).
-template <int NB>
+// F = fp16 latents per entry: 2 (one 32-bit word per entry, BASELINE.json) or 4 (one 64-bit word, the paper).
+template <int NB, int F>
 struct Batch {
-    uint32_t v[NB][8];      // gathered entries (2 x fp16 each)
-    uint32_t w2[NB][3];     // interpolation fractions, each duplicated into a half2
+    uint32_t v[NB][8][F / 2];   // gathered entries (F/2 x half2 each)
+    uint32_t w2[NB][3];         // interpolation fractions, each duplicated into a half2
 };
-template <int NB>
-__device__ __forceinline__ void batch_issue(const KParams& P, int l0, const float u[3], Batch<NB>& b) {
+template <int NB, int F>
+__device__ __forceinline__ void batch_issue(const KParams& P, int l0, const float u[3], Batch<NB, F>& b) {
+    static_assert(F == 2 || F == 4, "F = 2 or 4");
 #pragma unroll
     for (int q = 0; q < NB; ++q) {
         const LevelP& lv = P.lv[l0 + q];
@@ -159,30 +164,43 @@ __device__ __forceinline__ void batch_issue(const KParams& P, int l0, const floa
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
 #ifdef NIV_EXPERIMENT_SKIPX1          // timing experiment only (wrong results): what the +x corner loads cost
-            if (j & 1) { b.v[q][j] = b.v[q][j - 1]; continue; }
+            if (j & 1) { for (int h = 0; h < F / 2; ++h) b.v[q][j][h] = b.v[q][j - 1][h]; continue; }
 #endif
 #ifdef NIV_EXPERIMENT_NOGATHER        // timing experiment only: index arithmetic kept, no table access
-            b.v[q][j] = e[j];
+            for (int h = 0; h < F / 2; ++h) b.v[q][j][h] = e[j];
             continue;
 #endif
-            b.v[q][j] = __ldg(lv.tb + e[j]);
+            if (F == 2) {
+                b.v[q][j][0] = __ldg(lv.tb + e[j]);
+            } else {
+                const uint2 t = __ldg(reinterpret_cast<const uint2*>(lv.tb) + e[j]);
+                b.v[q][j][0] = t.x;
+                b.v[q][j][F / 2 - 1] = t.y;
+            }
         }
 #pragma unroll
         for (int d = 0; d < 3; ++d) b.w2[q][d] = pack_half2(w[d], w[d]);
     }
 }
-template <int NB>
-__device__ __forceinline__ void batch_blend(const Batch<NB>& b, uint32_t* f) {
+template <int NB, int F>
+__device__ __forceinline__ void batch_blend(const Batch<NB, F>& b, uint32_t* f) {
 #pragma unroll
-    for (int q = 0; q < NB; ++q) f[q] = blend8_h2(b.v[q], b.w2[q]);
+    for (int q = 0; q < NB; ++q)
+#pragma unroll
+        for (int h = 0; h < F / 2; ++h) {
+            uint32_t v[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) v[j] = b.v[q][j][h];
+            f[q * (F / 2) + h] = blend8_h2(v, b.w2[q]);
+        }
 }
 
-// One group of 4 levels (8 latents = one 16-byte fp16 chunk of the A operand), gathers issued together.
+// One group of 4 levels (8 latents = one 16-byte fp16 chunk of the A operand), gathers issued together (F = 2).
 __device__ __forceinline__ uint4 encode_group4(const KParams& P, int l0, const float u[3]) {
-    Batch<4> b;
-    batch_issue<4>(P, l0, u, b);
+    Batch<4, 2> b;
+    batch_issue<4, 2>(P, l0, u, b);
     uint32_t f[4];
-    batch_blend<4>(b, f);
+    batch_blend<4, 2>(b, f);
     return make_uint4(f[0], f[1], f[2], f[3]);
 }
 

@@ -189,6 +189,40 @@ def test_two_parameters(torch_cuda, niv, oracle):
 
 
 # ------------------------------------------------------------------------------------------------------
+# the paper's own model family: F = 4, sqrt(2) levels, raw direction, four weight matrices, linear output
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("L,width", [(8, 64), (6, 64), (4, 32), (2, 64), (8, 32)])
+def test_paper_family_parity(torch_cuda, niv, oracle, L, width):
+    spec = I.spec_paper(L, width)
+    case = Case(spec, 200 + L + width, table_amp=0.1, bias_scale=0.05)
+    pos, nrm = _queries(spec, 148 * 128 + 45, 19, coherent=(L == 8))
+    nrm[3] = 0.0
+    m = case.gpu_model(niv)
+    ref = _check_debug(torch_cuda, oracle, m, case, pos, nrm)
+    assert ref["features"].shape[1] == 4 * L + 3
+    got = _gpu_infer(torch_cuda, m, pos, nrm)
+    want = oracle.infer(spec, case.table, case.wblob, case.bblob, pos, nrm)
+    rng = max(1.0, float(want.max() - want.min()))            # linear output: bounds relative to the output range
+    _check_irradiance(got, want, nrm, pos, scale=rng)
+    m.close()
+
+
+def test_paper_family_full_hd_sampled(torch_cuda, niv, oracle):
+    torch = torch_cuda
+    spec = I.spec_paper(8, 64)
+    case = Case(spec, 0)
+    g = I.make_gbuffer(1920, 1080, 0)
+    pos, nrm = g["pos"], g["nrm"]
+    m = case.gpu_model(niv)
+    got = _gpu_infer(torch, m, pos, nrm)
+    n = pos.shape[0]
+    sel = np.unique((I.random_u64(77, 1, 30000) % np.uint64(n)).astype(np.int64))
+    want = oracle.infer(spec, case.table, case.wblob, case.bblob, pos[sel], nrm[sel])
+    _check_irradiance(got[sel], want, nrm[sel], pos[sel], scale=max(1.0, float(want.max() - want.min())))
+    m.close()
+
+
+# ------------------------------------------------------------------------------------------------------
 # edge cases
 # ------------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("n", [1, 31, 127, 128, 129, 257])
