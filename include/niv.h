@@ -16,8 +16,9 @@
  *     parameter blobs may be freed as soon as niv_load_params returns;
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream);
  *   - niv_infer / niv_encode / niv_debug_encode are asynchronous on `stream`, allocate nothing, never
- *     synchronise (CUDA-graph capturable), are read-only on the model and safe for concurrent callers on
- *     different streams;
+ *     synchronise (CUDA-graph capturable), are read-only on the model's parameters and safe for concurrent callers
+ *     on different streams (niv_infer draws one of 64 per-launch tile counters round robin and zeroes it on
+ *     `stream`: up to 64 launches of one model may be in flight at once);
  *   - there is no CPU fallback: without a CUDA device every entry point that needs one returns NIV_ERR_CUDA.
  */
 #ifndef NIV_H_
@@ -52,18 +53,19 @@ enum { NIV_OUT_LINEAR = 0,      /* the paper: no activation on the final layer (
 typedef struct {
     uint32_t struct_size;         /* = sizeof(niv_config)                                           */
     uint32_t api_version;         /* = NIV_API_VERSION                                              */
-    uint32_t n_levels;            /* L: 4, 8, 12 or 16                                              */
-    uint32_t n_features;          /* F: fp16 latents per table entry; this build: 2                 */
+    uint32_t n_levels;            /* L: 4, 8, 12 or 16 (F = 2);  2, 4, 6 or 8 (F = 4)                 */
+    uint32_t n_features;          /* F: fp16 latents per table entry: 2 (BASELINE.json) or 4 (paper) */
     uint32_t log2_table_size;     /* T = 2^k entries PER LEVEL, 4 <= k <= 24                        */
     uint32_t base_resolution;     /* N0: cells per side on the coarsest level                       */
     double   per_level_scale;     /* b: N_l = floor(N0 * b^l)  (reading #2)               */
     uint32_t resolutions[NIV_MAX_LEVELS]; /* optional explicit N_l; all zero => derive from N0, b   */
     float    aabb_min[3], aabb_max[3];    /* scene box mapped to the unit cube (reading #8)         */
-    uint32_t sh_degree;           /* 4 => 16 real-SH coefficients of the normal (reading #13)       */
+    uint32_t sh_degree;           /* 4 => 16 real-SH coefficients of the normal (reading #13, F = 2);
+                                     0 => the direction itself, 3 inputs (F = 4)  */
     uint32_t n_params;            /* 0..2 per-call scalar scene parameters                          */
     uint32_t n_frequencies;       /* sin/cos bands per parameter (8)                                */
     uint32_t n_hidden_layers;     /* 1..3 hidden layers, all `hidden_width` wide                    */
-    uint32_t hidden_width;        /* 32, 64 or 128                                                  */
+    uint32_t hidden_width;        /* 32, 64 or 128 (F = 4: 32 or 64)                                */
     uint32_t out_activation;      /* NIV_OUT_*                                                      */
     int32_t  device;              /* CUDA device ordinal                                            */
 } niv_config;
@@ -71,7 +73,7 @@ typedef struct {
 /* What niv_create derived from the configuration (for tests, benchmarks and roofline arithmetic). */
 typedef struct {
     uint32_t struct_size;
-    uint32_t in_dim;                       /* L*F + 16 + 2*n_frequencies*n_params                   */
+    uint32_t in_dim;                       /* L*F + (16 | 3) + 2*n_frequencies*n_params             */
     uint32_t resolution[NIV_MAX_LEVELS];   /* N_l                                                   */
     uint32_t is_dense[NIV_MAX_LEVELS];     /* 1: dense index, 0: spatial hash (reading #4)          */
     uint64_t table_bytes;                  /* L * T * F * 2                                         */
@@ -85,8 +87,9 @@ typedef struct {
 
 /* Validate `cfg` completely and allocate device storage for the parameters (uninitialised).
  * Errors: NULL / wrong struct_size / api_version / degenerate AABB / zero resolution -> NIV_ERR_INVALID_ARG;
- * a shape this build has no kernel for (F != 2, L not in {4,8,12,16}, width not in {32,64,128}, sh_degree
- * != 4, n_frequencies != 8, n_params > 2, n_hidden_layers not in 1..3) -> NIV_ERR_UNSUPPORTED.
+ * a shape this build has no kernel for -> NIV_ERR_UNSUPPORTED.  Two model families have kernels: BASELINE.json's
+ * (F = 2, sh_degree 4, L in {4,8,12,16}, width 32/64/128) and the paper's own (F = 4, sh_degree 0,
+ * L in {2,4,6,8}, width 32/64); both with n_hidden_layers 1..3, n_params 0..2, n_frequencies 8.
  * Shape errors are raised here, never at inference. */
 int niv_create(const niv_config *cfg, niv_model **out);
 
@@ -127,14 +130,15 @@ int niv_infer_host(niv_model *m, const float *pos, const float *nrm, const float
                    float *out, size_t n, void *stream);
 
 /* Stand-alone encoding kernel (rows a1..a9 without the MLP): features_fp16 is device, [n][in_dim] fp16
- * row-major = [latents | SH-16 | parameter encoding], zero rows for background texels. */
+ * row-major = [latents | SH-16 | parameter encoding], zero rows for background texels.  F = 2 family only
+ * (NIV_ERR_UNSUPPORTED for F = 4, whose rows are not a multiple of 16 bytes). */
 int niv_encode(niv_model *m, const float *pos, const float *nrm, const float *param,
                void *features_fp16, size_t n, void *stream);
 
 /* Debug dump through the SAME device functions the fused kernel uses for O0..O3 (bit-exact parity of the
  * integer path is checked on these).  All outputs are device pointers; any may be NULL.
- *   idx [n][L][8] uint32 (corner j: bit d of j selects +1 on axis d), cell [n][L][3] int32,
- *   frac [n][L][3] fp32, features [n][in_dim] fp32 (before fp16 packing).  Background texels: zeros. */
+ *   idx [n][L][8] uint32 (corner j: bit d of j selects +1 on axis d; entry index inside the level), cell [n][L][3]
+ *   int32, frac [n][L][3] fp32, features [n][in_dim] fp32 (fp32 blend, before fp16 packing).  Background: zeros. */
 int niv_debug_encode(niv_model *m, const float *pos, const float *nrm, const float *param, size_t n,
                      uint32_t *idx, int32_t *cell, float *frac, float *features, void *stream);
 
