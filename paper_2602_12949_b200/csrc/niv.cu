@@ -301,6 +301,16 @@ __global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(const __grid_cons
     }
     fence_proxy_async_smem();          // the bias row is read by the tensor core through the async proxy
 
+    // shared-memory descriptor (low half) of every layer's B operand at K-step 0: (address >> 4) | (N * 16 >> 4) << 16,
+    // the high half is the constant 0x4008 = SBO 128 B >> 4 | descriptor version 1 << 14 (niv_tc.cuh make_smem_desc)
+    constexpr uint32_t K1 = 2 * AW;
+    const uint32_t n_layers = P.n_layers;
+    uint32_t desc_lo0[kMaxLayers];
+#pragma unroll
+    for (int l = 0; l < kMaxLayers; ++l) {
+        const uint32_t N = (l + 1 == (int)n_layers) ? 16u : (uint32_t)WIDTH;
+        desc_lo0[l] = (((sW_u32 + P.w_off[l]) & 0x3FFFFu) >> 4) | (N << 16);
+    }
     uint32_t phase = 0;
     // G-buffer texel of the first tile; inside the loop the NEXT tile's texel is requested before the current
     // one is encoded, so its HBM latency hides under a whole tile of work (a1 prefetch)
@@ -376,26 +386,30 @@ __global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(const __grid_cons
         __syncthreads();
         const uint32_t tnn = s_tile[(it + 1) & 1];
 
-        for (uint32_t layer = 0; layer < P.n_layers; ++layer) {
-            const uint32_t K = P.kdim[layer], N = P.npad[layer];
+        // ---- a10..a12: the layers.  K depends on the layer's position only (compile time), N on whether it is the
+        //      last one (run time, uniform); the descriptors are one add per K-step from values prepared before the
+        //      tile loop, so the issuing thread's critical path is ~6 instructions per MMA.
+#pragma unroll
+        for (int layer = 0; layer < kMaxLayers; ++layer) {
+            if (layer >= (int)n_layers) break;
+            const bool last_layer = layer + 1 == (int)n_layers;
+            const uint32_t ksteps_ct = layer == 0 ? K1 / 16 : WIDTH / 16;
             if (tid == 0) {
                 tc_fence_after_sync();
+                const uint32_t N = last_layer ? 16u : (uint32_t)WIDTH;
                 const uint32_t idesc = make_idesc_f16(kTile, N);
-                const uint32_t b_base = sW_u32 + P.w_off[layer];
-                const uint32_t ksteps = K >> 4;
-                for (uint32_t ks = 0; ks < ksteps; ++ks) {
-                    const uint64_t db = make_smem_desc(b_base + ks * (N * 32u), N * 16u, 128u);
-                    umma_f16_ts(tmem, tmem + A_COL + ks * 8u, db, idesc, ks > 0 ? 1u : 0u);
-                }
-                const uint64_t db = make_smem_desc(b_base + ksteps * (N * 32u), N * 16u, 128u);
-                umma_f16_ts(tmem, tmem + ONES_COL, db, idesc, 1u);            // + bias
+                const uint32_t lo = desc_lo0[layer], step = 2u * N;
+#pragma unroll
+                for (uint32_t ks = 0; ks < ksteps_ct; ++ks)
+                    umma_f16_ts2(tmem, tmem + A_COL + ks * 8u, lo + ks * step, 0x4008u, idesc, ks > 0 ? 1u : 0u);
+                umma_f16_ts2(tmem, tmem + ONES_COL, lo + ksteps_ct * step, 0x4008u, idesc, 1u);        // + bias
                 umma_commit(bar_mma);
             }
             mbar_wait(bar_mma, phase);
             phase ^= 1u;
             tc_fence_after_sync();
 
-            if (layer + 1 < P.n_layers) {
+            if (!last_layer) {
                 // hidden epilogue: D (fp32) -> ReLU + fp16 pack -> A columns of the next layer
 #pragma unroll
                 for (int cc = 0; cc < WIDTH / 32; ++cc) {
