@@ -76,7 +76,7 @@ double niv_oracle_half_to_double(uint16_t h)
  * stored in a hash table"). */
 int niv_oracle_level_table(const niv_oracle_config *cfg, uint32_t *N, uint32_t *is_dense)
 {
-    if (!cfg || cfg->n_levels == 0 || cfg->n_levels > NIV_ORACLE_MAX_LEVELS) return -1;
+    if (!cfg || cfg->n_levels > NIV_ORACLE_MAX_LEVELS) return -1;
     int explicit_res = 0;
     for (uint32_t l = 0; l < cfg->n_levels; ++l) if (cfg->resolutions[l]) explicit_res = 1;
     uint64_t T = (uint64_t)1 << cfg->log2_table_size;
@@ -98,6 +98,8 @@ uint32_t niv_oracle_hash(uint32_t vx, uint32_t vy, uint32_t vz, uint32_t log2_T)
     uint32_t h = (vx * 1u) ^ (vy * 2654435761u) ^ (vz * 805459861u);
     return h & (uint32_t)(((uint64_t)1 << log2_T) - 1);
 }
+
+void niv_oracle_param_encode(double t, uint32_t n_frequencies, double *out);
 
 static int texel_masked(const float *p, const float *n)
 {
@@ -123,6 +125,10 @@ static void encode_one(const niv_oracle_config *cfg, const uint32_t *N, const ui
         v = fmaxf(v, 0.0f);
         v = fminf(v, 1.0f);
         u[d] = v;
+    }
+    if (L == 0 && feat) {                                          /* grid-less: positional encoding of u */
+        for (int d = 0; d < 3; ++d)
+            niv_oracle_param_encode((double)u[d], cfg->n_frequencies, feat + 2 * cfg->n_frequencies * d);
     }
     for (uint32_t l = 0; l < L; ++l) {
         int32_t c[3];
@@ -228,10 +234,18 @@ static void dir_encode(const niv_oracle_config *cfg, const double n[3], double *
     else niv_oracle_sh16(n, out);
 }
 
+/* ---- position input: L > 0 -> the L*F grid latents (O1-O4); L == 0 -> the grid-less models of Table 1
+ * ("Networks without grid encoding use eight-band positional encoding"): the normalised
+ * position u (O1) is frequency-encoded per axis, x then y then z, each [sin(2^0 pi u), cos(2^0 pi u), ...,
+ * sin(2^(B-1) pi u), cos(2^(B-1) pi u)] with B = n_frequencies. ---- */
+static uint32_t pos_dim_of(const niv_oracle_config *cfg)
+{
+    return cfg->n_levels ? cfg->n_levels * cfg->n_features : 6 * cfg->n_frequencies;
+}
+
 static uint32_t in_dim_of(const niv_oracle_config *cfg)
 {
-    return cfg->n_levels * cfg->n_features + dir_dim_of(cfg)
-         + 2 * cfg->n_frequencies * cfg->n_params;
+    return pos_dim_of(cfg) + dir_dim_of(cfg) + 2 * cfg->n_frequencies * cfg->n_params;
 }
 
 uint32_t niv_oracle_in_dim(const niv_oracle_config *cfg) { return in_dim_of(cfg); }
@@ -267,7 +281,8 @@ void niv_oracle_mlp(const niv_oracle_config *cfg, const uint16_t *weights, const
 static int check_cfg(const niv_oracle_config *cfg)
 {
     if (!cfg) return -1;
-    if (cfg->n_levels == 0 || cfg->n_levels > NIV_ORACLE_MAX_LEVELS) return -1;
+    if (cfg->n_levels > NIV_ORACLE_MAX_LEVELS) return -1;
+    if (cfg->n_levels == 0 && cfg->n_frequencies == 0) return -1;
     if (cfg->n_features == 0 || cfg->n_features > 16) return -1;
     if (cfg->log2_table_size == 0 || cfg->log2_table_size > 30) return -1;
     if (cfg->sh_degree != 4 && cfg->sh_degree != 0) return -1;
@@ -305,10 +320,10 @@ int niv_oracle_encode(const niv_oracle_config *cfg, const uint16_t *table,
         encode_one(cfg, N, dense, table, pos + 3 * i, ii, cc, ff, xx);
         if (xx) {
             double nn[3] = { (double)nrm[3 * i], (double)nrm[3 * i + 1], (double)nrm[3 * i + 2] };
-            dir_encode(cfg, nn, xx + L * F);                         /* O5 */
+            dir_encode(cfg, nn, xx + pos_dim_of(cfg));                         /* O5 */
             for (uint32_t q = 0; q < cfg->n_params; ++q)             /* O6 */
                 niv_oracle_param_encode((double)param[q], cfg->n_frequencies,
-                                        xx + L * F + dir_dim_of(cfg) + 2 * cfg->n_frequencies * q);
+                                        xx + pos_dim_of(cfg) + dir_dim_of(cfg) + 2 * cfg->n_frequencies * q);
         }
     }
     return 0;
@@ -335,10 +350,10 @@ int niv_oracle_infer(const niv_oracle_config *cfg, const uint16_t *table,
             double x[NIV_ORACLE_MAX_DIM];
             encode_one(cfg, N, dense, table, pos + 3 * i, NULL, NULL, NULL, x);   /* O1-O4 */
             double nn[3] = { (double)nrm[3 * i], (double)nrm[3 * i + 1], (double)nrm[3 * i + 2] };
-            dir_encode(cfg, nn, x + L * F);                          /* O5, O7 */
+            dir_encode(cfg, nn, x + pos_dim_of(cfg));                          /* O5, O7 */
             for (uint32_t q = 0; q < cfg->n_params; ++q)             /* O6, O7 */
                 niv_oracle_param_encode((double)param[q], cfg->n_frequencies,
-                                        x + L * F + dir_dim_of(cfg) + 2 * cfg->n_frequencies * q);
+                                        x + pos_dim_of(cfg) + dir_dim_of(cfg) + 2 * cfg->n_frequencies * q);
             niv_oracle_mlp(cfg, weights, biases, x, y);              /* O8 */
             if (cfg->out_activation == 1)                            /* O9 */
                 for (int c = 0; c < 3; ++c) y[c] = 1.0 / (1.0 + exp(-y[c]));

@@ -92,8 +92,13 @@ class ModelSpec:
         return 3 if self.sh_degree == 0 else self.sh_degree ** 2
 
     @property
+    def pos_dim(self) -> int:
+        """Grid latents, or (n_levels == 0) the 8-band positional encoding of the position."""
+        return self.n_levels * self.n_features if self.n_levels else 6 * self.n_frequencies
+
+    @property
     def in_dim(self) -> int:
-        return self.n_levels * self.n_features + self.dir_dim + 2 * self.n_frequencies * self.n_params
+        return self.pos_dim + self.dir_dim + 2 * self.n_frequencies * self.n_params
 
     @property
     def layer_shapes(self) -> List[Tuple[int, int]]:
@@ -131,6 +136,13 @@ def spec_paper(n_levels: int = 8, width: int = 64) -> ModelSpec:
     Resolutions are passed explicitly so that no pow() rounding decides an integer."""
     return ModelSpec(n_levels, 4, 17, 16, 2.0 ** 0.5, *ROOM_AABB, hidden_width=width, n_hidden_layers=3,
                      out_activation=OUT_LINEAR, sh_degree=0, resolutions=PAPER_RESOLUTIONS[:n_levels])
+
+
+def spec_paper_pe(width: int = 64) -> ModelSpec:
+    """The paper's grid-less models (Table 1 rows "-": widths 16 / 32 / 64): eight-band positional encoding of the
+    position (48 values) + the direction (3), four weight matrices, linear output; no table."""
+    return ModelSpec(0, 4, 17, 16, 2.0 ** 0.5, *ROOM_AABB, hidden_width=width, n_hidden_layers=3,
+                     out_activation=OUT_LINEAR, sh_degree=0)
 
 
 # ----------------------------------------------------------------------------

@@ -354,6 +354,45 @@ def test_paper_family_vertex_and_partition_of_unity(oracle):
     np.testing.assert_allclose(enc["features"][:, :32], np.broadcast_to(want, (64, 32)), atol=1e-14)
 
 
+def test_paper_gridless_models_brute_force_4x4(oracle):
+    """Table 1 rows without a grid: eight-band positional encoding of the position,
+    raw direction, four matrices.  SPEC.md:216-219 examples pin the band order; the whole path is checked against
+    numpy on a 4x4 G-buffer; the memory column of Table 1 (0.003 / 0.01 / 0.03 MB) is consistent with the input width
+    48 + 3 to one unit of its last printed digit (a weak pin: the column has one significant digit)."""
+    for width, mb in ((16, 0.003), (32, 0.01), (64, 0.03)):
+        spec = I.spec_paper_pe(width)
+        assert spec.in_dim == 51
+        n_par = sum(o * i for o, i in spec.layer_shapes)
+        assert abs(n_par * 2 / 1e6 - mb) <= 10 ** (-3 if mb < 0.005 else -2)     # one unit of the last printed digit
+    spec = dataclasses.replace(I.spec_paper_pe(32), aabb_min=(-1.0, 0.0, 2.0), aabb_max=(3.0, 2.0, 4.0))
+    weights, biases = I.make_mlp(spec, 4, bias_scale=0.1)
+    table = I.make_table(spec, 0)
+    assert table.size == 0
+    pos = I.positions_uniform(16, (spec.aabb_min, spec.aabb_max), 6)
+    nrm = I.normals_uniform(16, 6)
+    enc = oracle.encode(spec, table, pos, nrm)["features"]
+    ext = np.float32(spec.aabb_max) - np.float32(spec.aabb_min)
+    u = ((pos - np.float32(spec.aabb_min)) * (np.float32(1.0) / ext)).astype(np.float32).astype(np.float64)
+    k = 2.0 ** np.arange(8)
+    want = np.empty((16, 48))
+    for d in range(3):
+        want[:, 16 * d:16 * d + 16:2] = np.sin(np.pi * u[:, d:d + 1] * k)
+        want[:, 16 * d + 1:16 * d + 16:2] = np.cos(np.pi * u[:, d:d + 1] * k)
+    np.testing.assert_allclose(enc[:, :48], want, atol=1e-12)
+    assert np.array_equal(enc[:, 48:51], nrm.astype(np.float64))
+    # SPEC.md:217-218 on the position path: u = 0 -> (0, 1) pairs; u = 0.5 -> first band (1, 0)
+    e0 = oracle.encode(spec, table, np.float32([[-1.0, 1.0, 2.0]]), nrm[:1])["features"][0]
+    np.testing.assert_allclose(e0[0:16], np.tile([0.0, 1.0], 8), atol=1e-15)
+    np.testing.assert_allclose(e0[16:18], [1.0, 0.0], atol=1e-15)
+    h = np.concatenate([want, nrm.astype(np.float64)], axis=1)
+    for j, (w, b) in enumerate(zip(weights, biases)):
+        h = h @ w.astype(np.float64).T + b.astype(np.float64)
+        if j + 1 < len(weights):
+            h = np.maximum(h, 0.0)
+    out32, out64 = oracle.infer(spec, table, I.pack_weights(weights), I.pack_biases(biases), pos, nrm, want_f64=True)
+    np.testing.assert_allclose(out64, h, rtol=0, atol=1e-11)
+
+
 # ------------------------------------------------------------------ SH-16
 def _sh16_scipy(n):
     """Real orthonormal SH, bands 0..3, index l(l+1)+m, no Condon-Shortley sign, from scipy's complex Y_l^m."""
