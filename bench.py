@@ -47,12 +47,19 @@ def _env_int(name, default):
         return default
 
 
+PAPER_LEVELS, PAPER_WIDTH = 8, 64        # --paper-levels / --paper-width (workload "paper")
+# PAPER.md:383-389 (Table 1, RTX 4090, full HD): ms per frame by (grid levels, width)
+PAPER_TABLE1_MS = {(0, 16): 0.19, (0, 32): 0.20, (0, 64): 0.25, (2, 64): 0.31, (4, 64): 0.67, (6, 64): 1.06, (8, 64): 1.35}
+
+
 def make_workload(name: str, frame: int):
     """-> spec, table, wblob, bblob, pos, nrm, param, description"""
+    paper_levels, paper_width = PAPER_LEVELS, PAPER_WIDTH
     if name == "param":
         spec, param = I.spec_param(), [0.625]
     elif name == "paper":
-        spec, param = I.spec_paper(8, 64), None
+        spec = I.spec_paper(paper_levels, paper_width) if paper_levels else I.spec_paper_pe(paper_width)
+        param = None
     else:
         spec, param = I.spec_fullhd(), None
     table = I.make_table(spec, 0)
@@ -68,8 +75,10 @@ def make_workload(name: str, frame: int):
         desc = ("configs[%d]: 1920x1080 G-buffer ray-cast from the seeded procedural room (16 spheres + 16 boxes), "
                 "%.1f%% background texels" % (3 if name == "param" else 1, 100 * masked))
         if name == "paper":
-            desc = ("the paper's own largest model (PAPER.md Table 1 row 'width 64, 8 grid levels': F=4, scale sqrt 2, "
-                    "T=2^17, four weight matrices) on the configs[1] G-buffer, %.1f%% background texels" % (100 * masked))
+            desc = ("the paper's own model (PAPER.md Table 1 row 'width %d, %s grid levels': %s, four weight matrices) on "
+                    "the configs[1] G-buffer, %.1f%% background texels"
+                    % (paper_width, paper_levels or "-", "F=4, scale sqrt 2, T=2^17" if paper_levels else
+                       "eight-band positional encoding", 100 * masked))
     return spec, table, I.pack_weights(w), I.pack_biases(b), pos, nrm, param, desc, masked
 
 
@@ -187,8 +196,11 @@ def run_reference(args):
 
 def _model_str(spec):
     dims = [spec.in_dim] + [spec.hidden_width] * spec.n_hidden_layers + [3]
-    return "hash grid L=%d F=%d T=2^%d N0=%d b=%g; %s%s; MLP %s fp16 weights / fp32 accumulate; %s output" % (
-        spec.n_levels, spec.n_features, spec.log2_table_size, spec.base_resolution, spec.per_level_scale,
+    grid = ("hash grid L=%d F=%d T=2^%d N0=%d b=%g" % (spec.n_levels, spec.n_features, spec.log2_table_size,
+                                                        spec.base_resolution, spec.per_level_scale)
+            if spec.n_levels else "no grid: 8-band positional encoding")
+    return "%s; %s%s; MLP %s fp16 weights / fp32 accumulate; %s output" % (
+        grid,
         "raw direction" if spec.sh_degree == 0 else "SH-16",
         "; %d param(s) x 8 sin/cos" % spec.n_params if spec.n_params else "", "->".join(map(str, dims)),
         "sigmoid" if spec.out_activation == I.OUT_SIGMOID else "linear")
@@ -197,7 +209,7 @@ def _model_str(spec):
 def measure_gather_peak(torch, niv, table_bytes, num_sms):
     """Random 32-byte-sector gather rate from a resident buffer of the tables' size (SURVEY.md 8(d) BW_L2g),
     and the same with 8 lanes sharing a sector.  Returns GB/s of sector traffic."""
-    nbytes = 1 << int(np.ceil(np.log2(table_bytes)))
+    nbytes = 1 << int(np.ceil(np.log2(max(table_bytes, 8 << 20))))
     buf = torch.zeros(nbytes // 4, dtype=torch.int32, device="cuda")
     sink = torch.zeros(4, dtype=torch.int32, device="cuda")
     res = {}
@@ -361,7 +373,8 @@ def run_ours(args):
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
         # BASELINE.md holds a paper number only for the paper's own model: 1.35 ms per full-HD frame on an RTX 4090
         # = 1.536 Gqueries/s -- another machine's, context not target
-        "vs_baseline": (value / (N_TEXELS / 1.35e-3 / 1e9)) if (args.workload == "paper" and world == 1) else None,
+        "vs_baseline": (value / (N_TEXELS / (PAPER_TABLE1_MS[(PAPER_LEVELS, PAPER_WIDTH)] * 1e-3) / 1e9))
+        if (args.workload == "paper" and world == 1 and (PAPER_LEVELS, PAPER_WIDTH) in PAPER_TABLE1_MS) else None,
         "dtype": "f16 operands / f32 accumulate (index path: f32 + u32)", "data": "synthetic",
         "config": {"workload": args.workload, "description": desc, "model": _model_str(spec),
                    "texels_per_gpu_per_step": n, "masked_fraction": masked, "parallelism": "dp%d (replicated model, "
@@ -459,11 +472,15 @@ def main():
     ap.add_argument("--warmup", type=int, default=None)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="fullhd", choices=["fullhd", "incoherent", "param", "paper"])
+    ap.add_argument("--paper-levels", type=int, default=8, choices=[0, 2, 4, 6, 8], help="workload paper: grid levels (0 = none)")
+    ap.add_argument("--paper-width", type=int, default=64, choices=[16, 32, 64])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[4]: table-size / width / resolution sweep")
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle wall time for cpu_baseline")
     ap.add_argument("--ref-sample", type=int, default=131072, help="texels per step of the reference arm")
     args = ap.parse_args()
+    global PAPER_LEVELS, PAPER_WIDTH
+    PAPER_LEVELS, PAPER_WIDTH = args.paper_levels, args.paper_width
     if args.sweep:
         run_sweep(args)
         return

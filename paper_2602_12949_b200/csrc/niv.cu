@@ -244,7 +244,8 @@ __global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(const __grid_cons
     static_assert(WIDTH <= 64, "A-in-TMEM kernel: D + A + ones must fit 128 columns");
     constexpr uint32_t TMEM_COLS = 128, A_COL = 64, ONES_COL = 96;
     constexpr int NG = L / NB;
-    constexpr int HW = L * F / 2;                     // 32-bit words of hash latents in one A row
+    constexpr int HW = L ? L * F / 2 : 24;            // 32-bit words of hash latents in one A row (L = 0: the
+                                                      // 3 x 8 (sin, cos) pairs of the positional encoding)
     constexpr int DW = RAWDIR ? 2 : 8;                // ... of the direction input: (x, y | z, 0) or SH-16
     constexpr int AW = (HW + DW + 7) / 8 * 8;         // ... of one layer-1 A row (K1 = 2 * AW)
     extern __shared__ __align__(1024) uint8_t smem[];
@@ -345,41 +346,39 @@ __global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(const __grid_cons
         if (!masked) {
             float u[3];
             normalise(P, p, u);
-            Batch<NB, F> ba, bb;
-            batch_issue<NB, F>(P, 0, u, ba);
-            if (RAWDIR) {                             // the paper's model: the direction itself
-                a[HW] = pack_half2(nv[0], nv[1]);
-                a[HW + 1] = pack_half2(nv[2], 0.0f);
+            auto encode_direction = [&]() {
+                if (RAWDIR) {                         // the paper's model: the direction itself
+                    a[HW] = pack_half2(nv[0], nv[1]);
+                    a[HW + 1] = pack_half2(nv[2], 0.0f);
+                } else {
+                    float sh[16];
+                    sh16(nv, sh);
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) a[HW + k] = pack_half2(sh[2 * k], sh[2 * k + 1]);
+                }
+            };
+            if constexpr (L == 0) {                   // grid-less models: eight-band positional encoding
+                encode_direction();
+#pragma unroll
+                for (int d = 0; d < 3; ++d) posenc8_packed(u[d], a + 8 * d);
             } else {
-                float sh[16];
-                sh16(nv, sh);
+                Batch<NB, F> ba, bb;
+                batch_issue<NB, F>(P, 0, u, ba);
+                encode_direction();                   // arithmetic under the first batch's latency
 #pragma unroll
-                for (int k = 0; k < 8; ++k) a[HW + k] = pack_half2(sh[2 * k], sh[2 * k + 1]);
-            }
-#pragma unroll
-            for (int g = 0; g < NG; g += 2) {
-                if (g + 1 < NG) batch_issue<NB, F>(P, (g + 1) * NB, u, bb);
-                batch_blend<NB, F>(ba, a + g * NB * (F / 2));
-                if (g + 2 < NG) batch_issue<NB, F>(P, (g + 2) * NB, u, ba);
-                if (g + 1 < NG) batch_blend<NB, F>(bb, a + (g + 1) * NB * (F / 2));
+                for (int g = 0; g < NG; g += 2) {
+                    if (g + 1 < NG) batch_issue<NB, F>(P, (g + 1) * NB, u, bb);
+                    batch_blend<NB, F>(ba, a + g * NB * (F / 2));
+                    if (g + 2 < NG) batch_issue<NB, F>(P, (g + 2) * NB, u, ba);
+                    if (g + 1 < NG) batch_blend<NB, F>(bb, a + (g + 1) * NB * (F / 2));
+                }
             }
         }
-#ifdef NIV_EXPERIMENT_NOMLP           // timing experiment only: encode, no layers
-        if (valid) {
-            uint32_t x = 0;
-#pragma unroll
-            for (int k = 0; k < AW; ++k) x ^= a[k];
-            out[3 * i] = __uint_as_float(x); out[3 * i + 1] = 0.f; out[3 * i + 2] = 0.f;
-        }
-        if (tid == 0) s_tile[(it + 1) & 1] = tnn_mine;
-        __syncthreads();
-        tile = tnext; tnext = s_tile[(it + 1) & 1]; ++it;
-        continue;
-#endif
         __syncwarp();
         if constexpr (AW == 8) tmem_st_x8(lane_taddr + A_COL, a);
         else tmem_st_x16(lane_taddr + A_COL, a);
-        if constexpr (AW > 16) tmem_st_x8(lane_taddr + A_COL + 16, a + 16);
+        if constexpr (AW == 24) tmem_st_x8(lane_taddr + A_COL + 16, a + 16);
+        if constexpr (AW == 32) tmem_st_x16(lane_taddr + A_COL + 16, a + 16);
         tmem_st_wait();
         if (tid == 0) s_tile[(it + 1) & 1] = tnn_mine;
         tc_fence_before_sync();
@@ -411,16 +410,27 @@ __global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(const __grid_cons
 
             if (!last_layer) {
                 // hidden epilogue: D (fp32) -> ReLU + fp16 pack -> A columns of the next layer
+                if constexpr (WIDTH % 32 == 0) {
 #pragma unroll
-                for (int cc = 0; cc < WIDTH / 32; ++cc) {
-                    uint32_t r[32];
-                    tmem_ld_x32(lane_taddr + cc * 32, r);
+                    for (int cc = 0; cc < WIDTH / 32; ++cc) {
+                        uint32_t r[32];
+                        tmem_ld_x32(lane_taddr + cc * 32, r);
+                        tmem_ld_wait();
+                        uint32_t pk[16];
+#pragma unroll
+                        for (int h = 0; h < 16; ++h)
+                            pk[h] = pack_relu_half2(__uint_as_float(r[2 * h]), __uint_as_float(r[2 * h + 1]));
+                        tmem_st_x16(lane_taddr + A_COL + cc * 16, pk);
+                    }
+                } else {                              // width 16
+                    uint32_t r[16];
+                    tmem_ld_x16(lane_taddr, r);
                     tmem_ld_wait();
-                    uint32_t pk[16];
+                    uint32_t pk[8];
 #pragma unroll
-                    for (int h = 0; h < 16; ++h)
+                    for (int h = 0; h < 8; ++h)
                         pk[h] = pack_relu_half2(__uint_as_float(r[2 * h]), __uint_as_float(r[2 * h + 1]));
-                    tmem_st_x16(lane_taddr + A_COL + cc * 16, pk);
+                    tmem_st_x8(lane_taddr + A_COL, pk);
                 }
                 tmem_st_wait();
                 tc_fence_before_sync();
@@ -536,8 +546,15 @@ __global__ void __launch_bounds__(128) niv_debug_kernel(const __grid_constant__ 
         if (feat)
             for (uint32_t k = 0; k < P.n_features; ++k) feat[i * P.in_dim + P.n_features * l + k] = f[k];
     }
+    if (feat && L == 0) {                            // grid-less: accurate per-band sincospi (the fused path doubles angles)
+        for (int d = 0; d < 3; ++d) {
+            float e[16];
+            param_encode8(u[d], e);
+            for (int k = 0; k < 16; ++k) feat[i * P.in_dim + 16 * d + k] = masked ? 0.f : e[k];
+        }
+    }
     if (feat) {
-        const uint32_t o = P.n_features * L;
+        const uint32_t o = L ? P.n_features * L : 48u;
         uint32_t dd;
         if (P.raw_dir) {
             dd = 3;
@@ -801,6 +818,9 @@ static fused_fn pick_tmem_paper(uint32_t L) {
     }
 }
 static fused_fn pick_tmem(uint32_t W, uint32_t L, int nb, uint32_t F) {
+    if (L == 0)                                     // grid-less: positional encoding, no gathers
+        return W == 16 ? niv_fused_tmem_kernel<16, 0, 1, 2, true> : W == 32 ? niv_fused_tmem_kernel<32, 0, 1, 2, true>
+             : W == 64 ? niv_fused_tmem_kernel<64, 0, 1, 2, true> : nullptr;
     if (F == 4) return W == 32 ? pick_tmem_paper<32>(L) : W == 64 ? pick_tmem_paper<64>(L) : nullptr;
     if (W == 32) return pick_tmem_l<32>(L, nb);
     if (W == 64) return pick_tmem_l<64>(L, nb);
@@ -812,7 +832,7 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     if (!cfg || !out) return NIV_ERR_INVALID_ARG;
     *out = nullptr;
     if (cfg->struct_size != sizeof(niv_config) || cfg->api_version != NIV_API_VERSION) return NIV_ERR_INVALID_ARG;
-    if (cfg->n_levels == 0 || cfg->n_levels > NIV_MAX_LEVELS || cfg->n_features == 0) return NIV_ERR_INVALID_ARG;
+    if (cfg->n_levels > NIV_MAX_LEVELS || cfg->n_features == 0) return NIV_ERR_INVALID_ARG;
     if (cfg->log2_table_size < 4 || cfg->log2_table_size > 24) return NIV_ERR_INVALID_ARG;
     if (cfg->n_hidden_layers == 0 || cfg->hidden_width == 0) return NIV_ERR_INVALID_ARG;
     if (cfg->out_activation > NIV_OUT_SIGMOID) return NIV_ERR_INVALID_ARG;
@@ -822,19 +842,24 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     }
     bool explicit_res = false;
     for (uint32_t l = 0; l < cfg->n_levels; ++l) explicit_res |= cfg->resolutions[l] != 0;
-    if (!explicit_res && (cfg->base_resolution == 0 || !(cfg->per_level_scale >= 1.0) || !std::isfinite(cfg->per_level_scale)))
+    if (cfg->n_levels && !explicit_res && (cfg->base_resolution == 0 || !(cfg->per_level_scale >= 1.0) || !std::isfinite(cfg->per_level_scale)))
         return NIV_ERR_INVALID_ARG;
     // shapes this build has kernels for
     // two model families: BASELINE.json's (F = 2, SH-16 direction, L in {4, 8, 12, 16}) and the paper's own
     // (F = 4, raw direction, L in {2, 4, 6, 8}, width <= 64)
-    if (cfg->n_features == 2) {
+    // and the paper's grid-less models (n_levels = 0: eight-band positional encoding, raw direction, width 16/32/64)
+    if (cfg->n_levels == 0) {
+        if (cfg->sh_degree != 0 || cfg->n_frequencies != 8) return NIV_ERR_UNSUPPORTED;
+        if (cfg->hidden_width != 16 && cfg->hidden_width != 32 && cfg->hidden_width != 64) return NIV_ERR_UNSUPPORTED;
+    } else if (cfg->n_features == 2) {
         if (cfg->sh_degree != 4 || cfg->n_levels % 4 != 0) return NIV_ERR_UNSUPPORTED;
     } else if (cfg->n_features == 4) {
         if (cfg->sh_degree != 0 || cfg->n_levels % 2 != 0 || cfg->n_levels > 8 || cfg->hidden_width > 64) return NIV_ERR_UNSUPPORTED;
     } else return NIV_ERR_UNSUPPORTED;
     if (cfg->n_params > 2 || (cfg->n_params && cfg->n_frequencies != 8)) return NIV_ERR_UNSUPPORTED;
     if (cfg->n_hidden_layers > 3) return NIV_ERR_UNSUPPORTED;
-    if (cfg->hidden_width != 32 && cfg->hidden_width != 64 && cfg->hidden_width != 128) return NIV_ERR_UNSUPPORTED;
+    if (cfg->hidden_width != 32 && cfg->hidden_width != 64 && cfg->hidden_width != 128 &&
+        !(cfg->n_levels == 0 && cfg->hidden_width == 16)) return NIV_ERR_UNSUPPORTED;
 
     niv_model* m = new (std::nothrow) niv_model();
     if (!m) return NIV_ERR_ALLOC;
@@ -873,13 +898,13 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     P.tmask = (uint32_t)(T - 1);
     P.n_features = cfg->n_features;
     P.raw_dir = cfg->sh_degree == 0 ? 1u : 0u;
-    P.enc_dim = cfg->n_levels * cfg->n_features + (P.raw_dir ? 3u : 16u);
+    P.enc_dim = (cfg->n_levels ? cfg->n_levels * cfg->n_features : 6u * cfg->n_frequencies) + (P.raw_dir ? 3u : 16u);
     P.in_dim = P.enc_dim + 2 * cfg->n_frequencies * cfg->n_params;
     P.n_params = cfg->n_params;
     P.n_layers = cfg->n_hidden_layers + 1;
     P.out_act = cfg->out_activation;
     I.in_dim = P.in_dim;
-    I.table_bytes = (uint64_t)cfg->n_levels * T * cfg->n_features * 2;
+    I.table_bytes = (uint64_t)cfg->n_levels * T * cfg->n_features * 2;      // 0 for the grid-less models
     I.tile_texels = kTile;
 
     // layer shapes and the packed weight blob layout
@@ -926,6 +951,7 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
         int kind = kv ? atoi(kv) : 2;
         if (kind != 1 && kind != 2) kind = 2;
         if (W > 64) kind = 1;                           // width 128: D alone fills the CTA's TMEM budget
+        if (cfg->n_levels == 0 || cfg->n_features == 4) kind = 2;   // the paper's families exist as v2 only
         int tmem_cols = W < 32 ? 32 : (int)W;
         if (kind == 1) m->fused = pick_fused(W, cfg->n_levels, nb);
         else {
@@ -939,7 +965,7 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
         rc = setup_kernel(m, m->fused, tmem_cols, kind == 1 ? "fused_v1" : "fused_v2");
     }
     if (rc != NIV_OK) { delete m; return rc; }
-    e = cudaMalloc(&m->d_table, I.table_bytes);
+    e = cudaMalloc(&m->d_table, I.table_bytes ? I.table_bytes : 16);
     if (e == cudaSuccess) e = cudaMalloc(&m->d_wpack, P.wpack_bytes);
     if (e == cudaSuccess) e = cudaMalloc(&m->d_ctr, kCtrSlots * 128);
     if (e != cudaSuccess) {
@@ -965,7 +991,7 @@ extern "C" int niv_load_params(niv_model* m, const void* table_fp16, size_t tabl
                                const void* weights_fp16, size_t weight_bytes,
                                const float* biases_f32, size_t bias_bytes, int src_on_device, void* stream)
 {
-    if (!m || !table_fp16 || !weights_fp16) return NIV_ERR_INVALID_ARG;
+    if (!m || (!table_fp16 && m->info.table_bytes) || !weights_fp16) return NIV_ERR_INVALID_ARG;
     if (table_bytes != m->info.table_bytes || weight_bytes != m->info.weight_bytes) return NIV_ERR_INVALID_ARG;
     if (biases_f32 ? bias_bytes != m->info.bias_bytes : bias_bytes != 0) return NIV_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
@@ -1018,7 +1044,7 @@ extern "C" int niv_load_params(niv_model* m, const void* table_fp16, size_t tabl
         bsrc += o;
     }
     NIV_CUDA(cudaMemcpyAsync(m->d_wpack, pack.data(), P.wpack_bytes, cudaMemcpyHostToDevice, st));
-    NIV_CUDA(cudaMemcpyAsync(m->d_table, table_fp16, table_bytes,
+    if (table_bytes) NIV_CUDA(cudaMemcpyAsync(m->d_table, table_fp16, table_bytes,
                              src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
     NIV_CUDA(cudaStreamSynchronize(st));
     m->loaded = true;

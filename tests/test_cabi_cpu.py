@@ -49,7 +49,7 @@ def test_argument_validation_happens_before_cuda(L):
     assert L.niv_create(C.byref(cfg), None) == niv.NIV_ERR_INVALID_ARG
     for mutate, want in [
         (lambda c: setattr(c, "api_version", 99), niv.NIV_ERR_INVALID_ARG),
-        (lambda c: setattr(c, "n_levels", 0), niv.NIV_ERR_INVALID_ARG),
+        (lambda c: setattr(c, "n_levels", 0), niv.NIV_ERR_UNSUPPORTED),      # grid-less needs sh_degree 0 (paper family)
         (lambda c: setattr(c, "n_levels", 17), niv.NIV_ERR_INVALID_ARG),
         (lambda c: setattr(c, "log2_table_size", 3), niv.NIV_ERR_INVALID_ARG),
         (lambda c: setattr(c, "log2_table_size", 25), niv.NIV_ERR_INVALID_ARG),

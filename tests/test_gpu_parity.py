@@ -222,6 +222,27 @@ def test_paper_family_full_hd_sampled(torch_cuda, niv, oracle):
     m.close()
 
 
+@pytest.mark.parametrize("width", [16, 32, 64])
+def test_paper_gridless_parity(torch_cuda, niv, oracle, width):
+    """Table 1 rows without a grid: eight-band positional encoding of the position (no table at all)."""
+    torch = torch_cuda
+    spec = I.spec_paper_pe(width)
+    case = Case(spec, 300 + width, bias_scale=0.05)
+    assert case.table.size == 0
+    pos, nrm = _queries(spec, 148 * 128 + 45, 23, coherent=(width == 64))
+    nrm[7] = 0.0
+    m = case.gpu_model(niv)
+    feat = torch.full((pos.shape[0], spec.in_dim), float("nan"), dtype=torch.float32, device="cuda")
+    m.debug_encode(torch.from_numpy(pos).cuda(), torch.from_numpy(nrm).cuda(), features=feat)
+    torch.cuda.synchronize()
+    ref = oracle.encode(spec, case.table, pos, nrm)["features"]
+    assert np.abs(feat.cpu().numpy().astype(np.float64) - ref).max() <= 2e-6
+    got = _gpu_infer(torch, m, pos, nrm)
+    want = oracle.infer(spec, case.table, case.wblob, case.bblob, pos, nrm)
+    _check_irradiance(got, want, nrm, pos, scale=max(1.0, float(want.max() - want.min())))
+    m.close()
+
+
 # ------------------------------------------------------------------------------------------------------
 # edge cases
 # ------------------------------------------------------------------------------------------------------
