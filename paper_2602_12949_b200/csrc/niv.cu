@@ -463,6 +463,10 @@ __global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(const __grid_cons
     if (warp == 0) tmem_dealloc(tmem, TMEM_COLS);
 }
 
+}  // namespace niv
+#include "niv_fused_w128.cuh"
+namespace niv {
+
 // =====================================================================================================
 // stand-alone encode (fp16 features to global) and debug dump
 // =====================================================================================================
@@ -950,11 +954,23 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
         const int nb = nbv ? atoi(nbv) : 4;
         int kind = kv ? atoi(kv) : 2;
         if (kind != 1 && kind != 2) kind = 2;
-        if (W > 64) kind = 1;                           // width 128: D alone fills the CTA's TMEM budget
         if (cfg->n_levels == 0 || cfg->n_features == 4) kind = 2;   // the paper's families exist as v2 only
         int tmem_cols = W < 32 ? 32 : (int)W;
         if (kind == 1) m->fused = pick_fused(W, cfg->n_levels, nb);
-        else {
+        else if (W == 128) {                            // two N = 64 halves per hidden layer (niv_fused_w128.cuh)
+            switch (cfg->n_levels) {
+                case 4:  m->fused = niv_fused_w128_kernel<4, 4>; break;
+                case 8:  m->fused = niv_fused_w128_kernel<8, 4>; break;
+                case 12: m->fused = niv_fused_w128_kernel<12, 4>; break;
+                case 16: m->fused = niv_fused_w128_kernel<16, 4>; break;
+                default: m->fused = nullptr;
+            }
+            tmem_cols = 128;
+            P.ones_off = P.a_off;                        // weights | ones chunk | barriers
+            P.misc_off = P.a_off + 2 * kTile * 16;
+            m->smem_fused = P.misc_off + 2 * 8 + 16;
+            I.smem_bytes = m->smem_fused;
+        } else {
             m->fused = pick_tmem(W, cfg->n_levels, nb, cfg->n_features);
             tmem_cols = 128;
             m->smem_fused = P.a_off + 2 * 8 + 16;        // weights + barriers only
@@ -962,7 +978,7 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
             I.smem_bytes = m->smem_fused;
         }
         if (!m->fused) { delete m; return NIV_ERR_UNSUPPORTED; }
-        rc = setup_kernel(m, m->fused, tmem_cols, kind == 1 ? "fused_v1" : "fused_v2");
+        rc = setup_kernel(m, m->fused, tmem_cols, kind == 1 ? "fused_v1" : W == 128 ? "fused_w128" : "fused_v2");
     }
     if (rc != NIV_OK) { delete m; return rc; }
     e = cudaMalloc(&m->d_table, I.table_bytes ? I.table_bytes : 16);
