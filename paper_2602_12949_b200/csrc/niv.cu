@@ -393,7 +393,7 @@ __global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(const __grid_cons
             if (layer >= (int)n_layers) break;
             const bool last_layer = layer + 1 == (int)n_layers;
             const uint32_t ksteps_ct = layer == 0 ? K1 / 16 : WIDTH / 16;
-            if (tid == 0) {
+            if (warp == 0 && elect_one_sync()) {
                 tc_fence_after_sync();
                 const uint32_t N = last_layer ? 16u : (uint32_t)WIDTH;
                 const uint32_t idesc = make_idesc_f16(kTile, N);
