@@ -321,6 +321,13 @@ __global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(const __grid_cons
         load3(nrm, (size_t)blockIdx.x * kTile + tid, nn);
     }
     uint32_t tile = blockIdx.x, tnext = s_tile[0], it = 0;
+#ifdef NIV_EXPERIMENT_TIMING
+    unsigned long long tacc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    long long tprev = clock64();
+#define NIV_TICK(slot) do { const long long tn__ = clock64(); tacc[slot] += (unsigned long long)(tn__ - tprev); tprev = tn__; } while (0)
+#else
+#define NIV_TICK(slot) do { } while (0)
+#endif
     while (tile < n_tiles) {
         const size_t i = (size_t)tile * kTile + tid;
         const bool valid = i < n;
@@ -374,6 +381,7 @@ __global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(const __grid_cons
                 }
             }
         }
+        NIV_TICK(0);                                  // encode
         __syncwarp();
         if constexpr (AW == 8) tmem_st_x8(lane_taddr + A_COL, a);
         else tmem_st_x16(lane_taddr + A_COL, a);
@@ -384,6 +392,7 @@ __global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(const __grid_cons
         tc_fence_before_sync();
         __syncthreads();
         const uint32_t tnn = s_tile[(it + 1) & 1];
+        NIV_TICK(1);                                  // A store + tile barrier
 
         // ---- a10..a12: the layers.  K depends on the layer's position only (compile time), N on whether it is the
         //      last one (run time, uniform); the descriptors are one add per K-step from values prepared before the
@@ -404,24 +413,36 @@ __global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(const __grid_cons
                 umma_f16_ts2(tmem, tmem + ONES_COL, lo + ksteps_ct * step, 0x4008u, idesc, 1u);        // + bias
                 umma_commit(bar_mma);
             }
+            NIV_TICK(2);                              // MMA issue (thread 0)
             mbar_wait(bar_mma, phase);
             phase ^= 1u;
             tc_fence_after_sync();
+            NIV_TICK(3);                              // MMA wait
 
             if (!last_layer) {
                 // hidden epilogue: D (fp32) -> ReLU + fp16 pack -> A columns of the next layer
-                if constexpr (WIDTH % 32 == 0) {
+                if constexpr (WIDTH == 64) {          // both loads in flight, one wait
+                    uint32_t r0[32], r1[32];
+                    tmem_ld_x32(lane_taddr, r0);
+                    tmem_ld_x32(lane_taddr + 32, r1);
+                    tmem_ld_wait();
+                    uint32_t pk[32];
 #pragma unroll
-                    for (int cc = 0; cc < WIDTH / 32; ++cc) {
-                        uint32_t r[32];
-                        tmem_ld_x32(lane_taddr + cc * 32, r);
-                        tmem_ld_wait();
-                        uint32_t pk[16];
-#pragma unroll
-                        for (int h = 0; h < 16; ++h)
-                            pk[h] = pack_relu_half2(__uint_as_float(r[2 * h]), __uint_as_float(r[2 * h + 1]));
-                        tmem_st_x16(lane_taddr + A_COL + cc * 16, pk);
+                    for (int h = 0; h < 16; ++h) {
+                        pk[h] = pack_relu_half2(__uint_as_float(r0[2 * h]), __uint_as_float(r0[2 * h + 1]));
+                        pk[16 + h] = pack_relu_half2(__uint_as_float(r1[2 * h]), __uint_as_float(r1[2 * h + 1]));
                     }
+                    tmem_st_x16(lane_taddr + A_COL, pk);
+                    tmem_st_x16(lane_taddr + A_COL + 16, pk + 16);
+                } else if constexpr (WIDTH == 32) {
+                    uint32_t r[32];
+                    tmem_ld_x32(lane_taddr, r);
+                    tmem_ld_wait();
+                    uint32_t pk[16];
+#pragma unroll
+                    for (int h = 0; h < 16; ++h)
+                        pk[h] = pack_relu_half2(__uint_as_float(r[2 * h]), __uint_as_float(r[2 * h + 1]));
+                    tmem_st_x16(lane_taddr + A_COL, pk);
                 } else {                              // width 16
                     uint32_t r[16];
                     tmem_ld_x16(lane_taddr, r);
@@ -433,8 +454,10 @@ __global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(const __grid_cons
                     tmem_st_x8(lane_taddr + A_COL, pk);
                 }
                 tmem_st_wait();
+                NIV_TICK(4);                          // hidden epilogue
                 tc_fence_before_sync();
                 __syncthreads();
+                NIV_TICK(5);                          // layer barrier
             } else {
                 uint32_t r[4];
                 tmem_ld_x4(lane_taddr, r);
@@ -454,10 +477,18 @@ __global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(const __grid_cons
                 }
             }
         }
+        NIV_TICK(6);                                  // output layer epilogue + store
         tile = tnext;
         tnext = tnn;
         ++it;
     }
+#ifdef NIV_EXPERIMENT_TIMING
+    if (tid == 0 && P.dbg) {
+        for (int q = 0; q < 7; ++q) atomicAdd(P.dbg + q, tacc[q]);
+        atomicAdd(P.dbg + 7, (unsigned long long)it);
+    }
+#endif
+#undef NIV_TICK
 
     __syncthreads();
     if (warp == 0) tmem_dealloc(tmem, TMEM_COLS);
@@ -991,6 +1022,10 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     }
     P.table = m->d_table;
     P.wpack = m->d_wpack;
+#ifdef NIV_EXPERIMENT_TIMING
+    cudaMalloc(&P.dbg, 8 * sizeof(unsigned long long));
+    cudaMemset(P.dbg, 0, 8 * sizeof(unsigned long long));
+#endif
     for (uint32_t l = 0; l < cfg->n_levels; ++l) P.lv[l].tb = m->d_table + (size_t)P.lv[l].base * (cfg->n_features / 2);
     *out = m;
     return NIV_OK;
@@ -1205,6 +1240,16 @@ extern "C" int niv_destroy(niv_model* m)
 {
     if (!m) return NIV_OK;
     cudaSetDevice(m->cfg.device);
+#ifdef NIV_EXPERIMENT_TIMING
+    {
+        unsigned long long h[8];
+        cudaDeviceSynchronize();
+        cudaMemcpy(h, m->kp.dbg, sizeof(h), cudaMemcpyDeviceToHost);
+        const char* nm[7] = {"encode", "A store + tile barrier", "MMA issue", "MMA wait", "hidden epilogue", "layer barrier", "output"};
+        if (h[7]) for (int q = 0; q < 7; ++q) fprintf(stderr, "[niv timing] %-24s %10.0f cycles per tile (thread 0)\n", nm[q], (double)h[q] / (double)h[7]);
+        cudaFree(m->kp.dbg);
+    }
+#endif
     cudaFree(m->d_table);
     cudaFree(m->d_wpack);
     cudaFree(m->d_ctr);

@@ -36,6 +36,9 @@ struct KParams {
     uint32_t out_act;
     float    t[2];              // per-call scene parameters
     LevelP   lv[kMaxLevels];
+#ifdef NIV_EXPERIMENT_TIMING
+    unsigned long long* dbg;    // timing experiment only: per-phase cycle sums of thread 0 of every CTA
+#endif
     uint32_t* tile_ctr;         // per-launch tile counter (zeroed on the stream before the launch): dynamic tile scheduling
     const uint32_t* table;      // [L][T] entries of 2 x fp16
     const uint8_t*  wpack;      // packed weights + biases (see niv.cu pack_weights)
