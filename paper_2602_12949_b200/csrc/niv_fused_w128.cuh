@@ -10,11 +10,12 @@
 // The "ones" A operand of the bias K-step lives in shared memory (4 KB, SS-form MMA).  128 columns and 62 KB of
 // shared memory per CTA -> three CTAs (12 warps) per SM instead of two with the A tile in shared memory.
 #pragma once
+#include <type_traits>
 
 namespace niv {
 
 template <int L, int NB>
-__global__ void __launch_bounds__(kTile) niv_fused_w128_kernel(const __grid_constant__ KParams P,
+__global__ void __launch_bounds__(kTile, 3) niv_fused_w128_kernel(const __grid_constant__ KParams P,
                                                                const float* __restrict__ pos,
                                                                const float* __restrict__ nrm,
                                                                float* __restrict__ out, size_t n, uint32_t n_tiles)
@@ -86,20 +87,25 @@ __global__ void __launch_bounds__(kTile) niv_fused_w128_kernel(const __grid_cons
     }
     const uint64_t desc_ones = make_smem_desc(smem_u32(sOnes), 2048u, 128u);
 
-    // MMAs of one layer (or of one 64-column half of a hidden layer) into D; issued by thread 0 after a CTA barrier
-    auto issue = [&](int layer, uint32_t ksteps, uint32_t n_mma, uint32_t row0) {
-        if (tid == 0) {
+    // MMAs of one layer (or of one 64-column half of a hidden layer) into D; issued by one elected lane of warp 0
+    // after a CTA barrier.  KSTEPS is a compile-time constant so that the K loop unrolls into back-to-back UTCHMMAs.
+    auto issue = [&](int layer, auto ksteps_c, uint32_t n_mma, uint32_t row0) {
+        constexpr uint32_t KSTEPS = decltype(ksteps_c)::value;
+        if (warp == 0 && elect_one_sync()) {
             tc_fence_after_sync();
             const uint32_t N = (layer + 1 == (int)n_layers) ? 16u : (uint32_t)WIDTH;   // rows of the packed B
             const uint32_t idesc = make_idesc_f16(kTile, n_mma);
             const uint32_t lo = desc_lo0[layer] + row0, step = 2u * N;                // row0 rows x 16 B >> 4
-            for (uint32_t ks = 0; ks < ksteps; ++ks)
+#pragma unroll
+            for (uint32_t ks = 0; ks < KSTEPS; ++ks)
                 umma_f16_ts2(tmem, tmem + A_COL + ks * 8u, lo + ks * step, 0x4008u, idesc, ks > 0 ? 1u : 0u);
-            const uint64_t db = ((uint64_t)0x4008u << 32) | (uint64_t)(lo + ksteps * step);
+            const uint64_t db = ((uint64_t)0x4008u << 32) | (uint64_t)(lo + KSTEPS * step);
             umma_f16_ss(tmem, desc_ones, db, idesc, 1u);                               // + bias
             umma_commit(bar_mma);
         }
     };
+    using KS1 = std::integral_constant<uint32_t, K1 / 16>;
+    using KSH = std::integral_constant<uint32_t, WIDTH / 16>;
 
     uint32_t phase = 0;
     float pn[3] = {0.f, 0.f, 0.f}, nn[3] = {0.f, 0.f, 0.f};
@@ -154,25 +160,26 @@ __global__ void __launch_bounds__(kTile) niv_fused_w128_kernel(const __grid_cons
         __syncthreads();
         const uint32_t tnn = s_tile[(it + 1) & 1];
 
-        for (uint32_t layer = 0; layer < n_layers; ++layer) {
-            const uint32_t ksteps = layer == 0 ? K1 / 16 : WIDTH / 16;
-            if (layer + 1 < n_layers) {
+#pragma unroll
+        for (int layer = 0; layer < kMaxLayers; ++layer) {
+            if (layer >= (int)n_layers) break;
+            if (layer + 1 < (int)n_layers) {
                 uint32_t pk[64];
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
-                    issue((int)layer, ksteps, 64u, 64u * h);
+                    if (layer == 0) issue(layer, KS1{}, 64u, 64u * h);
+                    else issue(layer, KSH{}, 64u, 64u * h);
                     mbar_wait(bar_mma, phase);
                     phase ^= 1u;
                     tc_fence_after_sync();
+                    uint32_t r0[32], r1[32];
+                    tmem_ld_x32(lane_taddr, r0);
+                    tmem_ld_x32(lane_taddr + 32, r1);
+                    tmem_ld_wait();
 #pragma unroll
-                    for (int cc = 0; cc < 2; ++cc) {
-                        uint32_t r[32];
-                        tmem_ld_x32(lane_taddr + cc * 32, r);
-                        tmem_ld_wait();
-#pragma unroll
-                        for (int q = 0; q < 16; ++q)
-                            pk[h * 32 + cc * 16 + q] =
-                                pack_relu_half2(__uint_as_float(r[2 * q]), __uint_as_float(r[2 * q + 1]));
+                    for (int q = 0; q < 16; ++q) {
+                        pk[h * 32 + q] = pack_relu_half2(__uint_as_float(r0[2 * q]), __uint_as_float(r0[2 * q + 1]));
+                        pk[h * 32 + 16 + q] = pack_relu_half2(__uint_as_float(r1[2 * q]), __uint_as_float(r1[2 * q + 1]));
                     }
                     if (h == 0) {                     // D is about to be overwritten by the second half
                         tc_fence_before_sync();
@@ -186,7 +193,8 @@ __global__ void __launch_bounds__(kTile) niv_fused_w128_kernel(const __grid_cons
                 tc_fence_before_sync();
                 __syncthreads();
             } else {
-                issue((int)layer, ksteps, 16u, 0u);
+                if (layer == 0) issue(layer, KS1{}, 16u, 0u);
+                else issue(layer, KSH{}, 16u, 0u);
                 mbar_wait(bar_mma, phase);
                 phase ^= 1u;
                 tc_fence_after_sync();
