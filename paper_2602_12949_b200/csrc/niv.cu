@@ -236,7 +236,12 @@ __global__ void __launch_bounds__(kTile) niv_fused_kernel(const __grid_constant_
 // no generic->async proxy fence), tcgen05.mma reads A from TMEM, and shared memory holds the weights only.
 // TMEM columns per CTA (128 allocated): D [0, WIDTH) fp32 | A [64, 96) packed fp16 pairs | ones [96, 104).
 template <int WIDTH, int L, int NB, int F, bool RAWDIR>
-__global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(const __grid_constant__ KParams P,
+#ifdef NIV_EXPERIMENT_V2_MINB          // timing experiment only: another register budget for the v2 kernel
+__global__ void __launch_bounds__(kTile, NIV_EXPERIMENT_V2_MINB) niv_fused_tmem_kernel(
+#else
+__global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(
+#endif
+                                                               const __grid_constant__ KParams P,
                                                                const float* __restrict__ pos,
                                                                const float* __restrict__ nrm,
                                                                float* __restrict__ out, size_t n, uint32_t n_tiles)
