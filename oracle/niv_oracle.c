@@ -374,3 +374,48 @@ int niv_oracle_max_threads(void)
     return 1;
 #endif
 }
+
+/* ---- f2: deferred compose with optional half-resolution irradiance (Eq. 2 and Fig. 3 234-236:
+ * L = rho/pi * E + D + L_e; "run at reduced resolution ... while still using the full size albedo
+ * buffer"; "E bilinearly upsampled; multiplied by FULL-res albedo; D, emission at full res").
+ * E is [eh][ew][3]; albedo, direct, emission, out are [h][w][3]; direct / emission may be NULL (zero).
+ * (ew, eh) == (w, h): E is used per pixel.  (2 ew, 2 eh) == (w, h): E is upsampled bilinearly with pixel-centre
+ * alignment -- full-res pixel x sits at half-res coordinate x/2 - 1/4, neighbours clamped to the edge (the paper
+ * names no filter beyond "upsampling"; this is the plain bilinear one, identical to
+ * torch.nn.functional.interpolate(scale_factor=2, mode="bilinear", align_corners=False)).  Returns -1 otherwise. ---- */
+int niv_oracle_compose(const float *E, uint32_t ew, uint32_t eh, const float *albedo, const float *direct,
+                       const float *emission, double *out, uint32_t w, uint32_t h)
+{
+    const double PI = 3.14159265358979323846;
+    int half;
+    if (!E || !albedo || !out || w == 0 || h == 0) return -1;
+    if (ew == w && eh == h) half = 0;
+    else if (2 * ew == w && 2 * eh == h) half = 1;
+    else return -1;
+    for (uint32_t y = 0; y < h; ++y)
+        for (uint32_t x = 0; x < w; ++x)
+            for (int c = 0; c < 3; ++c) {
+                double e;
+                if (!half) {
+                    e = (double)E[((size_t)y * ew + x) * 3 + c];
+                } else {
+                    double fx = 0.5 * (double)x - 0.25, fy = 0.5 * (double)y - 0.25;
+                    double x0f = floor(fx), y0f = floor(fy);
+                    double tx = fx - x0f, ty = fy - y0f;
+                    long x0 = (long)x0f, y0 = (long)y0f, x1 = x0 + 1, y1 = y0 + 1;
+                    if (x0 < 0) x0 = 0;
+                    if (y0 < 0) y0 = 0;
+                    if (x1 > (long)ew - 1) x1 = (long)ew - 1;
+                    if (y1 > (long)eh - 1) y1 = (long)eh - 1;
+                    double e00 = (double)E[((size_t)y0 * ew + x0) * 3 + c], e10 = (double)E[((size_t)y0 * ew + x1) * 3 + c];
+                    double e01 = (double)E[((size_t)y1 * ew + x0) * 3 + c], e11 = (double)E[((size_t)y1 * ew + x1) * 3 + c];
+                    e = (1.0 - ty) * ((1.0 - tx) * e00 + tx * e10) + ty * ((1.0 - tx) * e01 + tx * e11);
+                }
+                size_t o = ((size_t)y * w + x) * 3 + c;
+                double v = (double)albedo[o] / PI * e;
+                if (direct) v += (double)direct[o];
+                if (emission) v += (double)emission[o];
+                out[o] = v;
+            }
+    return 0;
+}

@@ -175,3 +175,19 @@ def infer(spec, table, weights_blob, biases_blob, pos, nrm, param=None, n_thread
 
 def max_threads() -> int:
     return int(lib().niv_oracle_max_threads())
+
+
+def compose(E, albedo, direct=None, emission=None) -> np.ndarray:
+    """L = albedo / pi * E + direct + emission; E [eh][ew][3] at full or half resolution (bilinear upsample).
+    -> [h][w][3] fp64."""
+    E = _chk(E, np.float32, "E")
+    albedo = _chk(albedo, np.float32, "albedo")
+    d = None if direct is None else _chk(direct, np.float32, "direct")
+    em = None if emission is None else _chk(emission, np.float32, "emission")
+    h, w = albedo.shape[:2]
+    out = np.zeros((h, w, 3), dtype=np.float64)
+    rc = lib().niv_oracle_compose(_p(E), C.c_uint32(E.shape[1]), C.c_uint32(E.shape[0]), _p(albedo), _p(d), _p(em),
+                                  _p(out), C.c_uint32(w), C.c_uint32(h))
+    if rc:
+        raise ValueError("niv_oracle_compose failed (resolutions must be equal or exactly 2x)")
+    return out

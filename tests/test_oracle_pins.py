@@ -586,3 +586,32 @@ def test_locate_uses_fp32_op_sequence(oracle):
         p64 = (pos.astype(np.float64) - lo.astype(np.float64)) / (hi.astype(np.float64) - lo.astype(np.float64)) * float(N[l])
         n_flip64 += int(np.any(np.minimum(np.floor(p64).astype(np.int32), int(N[l]) - 1) != c, axis=1).sum())
     assert n_flip64 > 0          # the fp64 sequence is a different function: the pin above is not vacuous
+
+
+# ------------------------------------------------------------------ f2: compose + half-resolution upsample
+def test_compose_closed_forms_and_torch_interpolate(oracle):
+    """PAPER.md:269 (Eq. 2), 405-406 (half resolution with the full-size albedo buffer).  Pins: zero albedo ->
+    D + L_e exactly; constant E -> half-res path == full-res path; Eq. 2 by hand on one pixel; the
+    upsample equals torch's bilinear interpolate (align_corners=False), a library routine."""
+    import torch
+    rng = np.random.default_rng(3)
+    h, w = 12, 20
+    alb = rng.uniform(0, 1, (h, w, 3)).astype(np.float32)
+    D = rng.uniform(0, 2, (h, w, 3)).astype(np.float32)
+    Le = rng.uniform(0, 1, (h, w, 3)).astype(np.float32)
+    Eh = rng.uniform(0, 3, (h // 2, w // 2, 3)).astype(np.float32)
+    Ef = rng.uniform(0, 3, (h, w, 3)).astype(np.float32)
+    out = oracle.compose(Ef, np.zeros_like(alb), D, Le)
+    assert np.array_equal(out, D.astype(np.float64) + Le.astype(np.float64))
+    out = oracle.compose(Ef, alb, D, Le)
+    y, x, c = 5, 7, 1
+    assert abs(out[y, x, c] - (float(alb[y, x, c]) / math.pi * float(Ef[y, x, c]) + float(D[y, x, c]) + float(Le[y, x, c]))) < 1e-15
+    const = np.full((h // 2, w // 2, 3), 1.75, dtype=np.float32)
+    np.testing.assert_allclose(oracle.compose(const, alb, D, Le),
+                               oracle.compose(np.full((h, w, 3), 1.75, dtype=np.float32), alb, D, Le), atol=1e-15)
+    up = torch.nn.functional.interpolate(torch.from_numpy(Eh.astype(np.float64)).permute(2, 0, 1)[None], scale_factor=2,
+                                         mode="bilinear", align_corners=False)[0].permute(1, 2, 0).numpy()
+    want = alb.astype(np.float64) / math.pi * up
+    np.testing.assert_allclose(oracle.compose(Eh, alb), want, atol=1e-14)
+    with pytest.raises(ValueError):
+        oracle.compose(Eh[:, :-1], alb)
