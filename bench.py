@@ -465,6 +465,44 @@ def run_sweep(args):
             one(17, 64, w, h, frames)
 
 
+def run_compose(args):
+    """the compose kernel alone (HBM-bound) at full HD, E at full and at half resolution.  One JSON line
+    per case: ms, algorithmic GB/s and its fraction of the measured HBM copy bandwidth."""
+    import torch
+
+    from paper_2602_12949_b200 import build as B
+    from paper_2602_12949_b200 import niv
+
+    B.build()
+    niv.lib()
+    torch.cuda.set_device(0)
+    peaks = load_peaks()
+    h, w = H_PX, W_PX
+    ring = 6                                           # 6 x 100 MB > L2
+    for half in (False, True):
+        eh, ew = (h // 2, w // 2) if half else (h, w)
+        bufs = [[torch.rand((h, w, 3), device="cuda") for _ in range(3)] + [torch.rand((eh, ew, 3), device="cuda"),
+                torch.empty((h, w, 3), device="cuda")] for _ in range(ring)]
+        for k in range(5):
+            a, d, le, e, o = bufs[k % ring]
+            niv.compose(e, a, o, d, le)
+        steps = args.steps or 100
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for k in range(steps):
+            a, d, le, e, o = bufs[k % ring]
+            niv.compose(e, a, o, d, le)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / steps
+        nbytes = (48 + (3 if half else 12)) * h * w
+        print(json.dumps({"op": "niv_compose", "E_resolution": "%dx%d" % (ew, eh), "frame": "%dx%d" % (w, h),
+                          "ms": ms, "algorithmic_bytes": nbytes,
+                          "roofline": {"bound": "hbm", "achieved": nbytes / ms / 1e6, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                                       "frac": nbytes / ms / 1e6 / peaks["hbm_gbs"], "peak_source": peaks["source"]}}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -475,6 +513,8 @@ def main():
     ap.add_argument("--paper-levels", type=int, default=8, choices=[0, 2, 4, 6, 8], help="workload paper: grid levels (0 = none)")
     ap.add_argument("--paper-width", type=int, default=64, choices=[16, 32, 64])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--compose", action="store_true", help="SURVEY 8(f2): time the compose kernel (HBM roofline)")
+    ap.add_argument("--half", action="store_true", help="quarter pixel count: a 960x540 G-buffer (PAPER.md:405, Table 1 'half')")
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[4]: table-size / width / resolution sweep")
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle wall time for cpu_baseline")
     ap.add_argument("--ref-sample", type=int, default=131072, help="texels per step of the reference arm")
@@ -484,6 +524,14 @@ def main():
     if args.sweep:
         run_sweep(args)
         return
+    if args.compose:
+        run_compose(args)
+        return
+    if args.half:
+        global W_PX, H_PX, N_TEXELS, METRIC
+        W_PX, H_PX = 960, 540
+        N_TEXELS = W_PX * H_PX
+        METRIC = "NIV fused inference throughput on a 960x540 (half-resolution) G-buffer (ms_per_step = ms per frame)"
     if args.impl == "reference":
         args.steps = 5 if args.steps is None else args.steps
         args.warmup = 1 if args.warmup is None else args.warmup

@@ -144,6 +144,19 @@ int niv_encode(niv_model *m, const float *pos, const float *nrm, const float *pa
 int niv_debug_encode(niv_model *m, const float *pos, const float *nrm, const float *param, size_t n,
                      uint32_t *idx, int32_t *cell, float *frac, float *features, void *stream);
 
+/* the deferred compose of the paper's frame, L = albedo / pi * E + direct + emission (PAPER.md:269
+ * Eq. 2; Fig. 3, 234-236), with the irradiance at full resolution or at half resolution ("run at
+ * reduced resolution ... while still using the full size albedo buffer").
+ *   E         device, [eh][ew][3] fp32: the output of niv_infer on the full-size or the half-size G-buffer
+ *   albedo    device, [h][w][3] fp32;  direct, emission  device, [h][w][3] fp32 or NULL (zero)
+ *   out       device, [h][w][3] fp32 radiance
+ * (ew, eh) must equal (w, h) or (w/2, h/2) exactly, else NIV_ERR_INVALID_ARG.  Half-resolution E is upsampled
+ * bilinearly with pixel-centre alignment (full-res pixel x at half-res coordinate x/2 - 1/4, edge texels clamped).
+ * 128-bit streaming path when w % 4 == 0 and the full-resolution buffers are 16-byte aligned, a scalar path otherwise.
+ * Asynchronous on `stream`, allocation-free; needs no model.  Runs on the current CUDA device. */
+int niv_compose(const float *E, uint32_t ew, uint32_t eh, const float *albedo, const float *direct,
+                const float *emission, float *out, uint32_t w, uint32_t h, void *stream);
+
 int niv_destroy(niv_model *m);
 
 const char *niv_error_string(int code);

@@ -239,7 +239,9 @@ template <int WIDTH, int L, int NB, int F, bool RAWDIR>
 #ifdef NIV_EXPERIMENT_V2_MINB          // timing experiment only: another register budget for the v2 kernel
 __global__ void __launch_bounds__(kTile, NIV_EXPERIMENT_V2_MINB) niv_fused_tmem_kernel(
 #else
-__global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(
+// width 32 with 16 levels would take 130 registers (3 CTAs per SM): capped at 128; width 64 is left alone, the cap
+// changes its schedule for the worse (0.193 instead of 0.189 ms, profiles/r01_v2.md)
+__global__ void __launch_bounds__(kTile, WIDTH == 32 ? 4 : 0) niv_fused_tmem_kernel(
 #endif
                                                                const __grid_constant__ KParams P,
                                                                const float* __restrict__ pos,
@@ -501,6 +503,7 @@ __global__ void __launch_bounds__(kTile) niv_fused_tmem_kernel(
 
 }  // namespace niv
 #include "niv_fused_w128.cuh"
+#include "niv_compose.cuh"
 namespace niv {
 
 // =====================================================================================================
@@ -1237,6 +1240,35 @@ extern "C" int niv_probe_sectors(niv_model* m, const float* pos, const float* nr
     NIV_CUDA(cudaMemsetAsync(counts, 0, 33 * sizeof(uint64_t), (cudaStream_t)stream));
     const unsigned grid = (unsigned)((n + 127) / 128);
     niv_sector_census_kernel<<<grid, 128, 0, (cudaStream_t)stream>>>(m->kp, pos, nrm, n, (unsigned long long*)counts);
+    NIV_CUDA(cudaGetLastError());
+    return NIV_OK;
+}
+
+extern "C" int niv_compose(const float* E, uint32_t ew, uint32_t eh, const float* albedo, const float* direct,
+                           const float* emission, float* out, uint32_t w, uint32_t h, void* stream)
+{
+    if (!E || !albedo || !out) return NIV_ERR_INVALID_ARG;
+    if (w == 0 || h == 0) return NIV_OK;
+    int half;
+    if (ew == w && eh == h) half = 0;
+    else if (2ull * ew == w && 2ull * eh == h) half = 1;
+    else return NIV_ERR_INVALID_ARG;
+    int dev = 0, sms = 0;
+    NIV_CUDA(cudaGetDevice(&dev));
+    NIV_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    cudaStream_t st = (cudaStream_t)stream;
+    const uintptr_t align = (uintptr_t)albedo | (uintptr_t)out | (uintptr_t)(direct ? direct : albedo) |
+                            (uintptr_t)(emission ? emission : albedo) | (half ? 0 : (uintptr_t)E);
+    const size_t n = (size_t)w * h;
+    if ((w & 3u) == 0 && (align & 15u) == 0) {
+        const size_t groups = n / 4;
+        const unsigned grid = (unsigned)std::min<size_t>((groups + 255) / 256, (size_t)sms * 8);   // 8 x 256 threads per SM
+        if (half) niv_compose_kernel<true><<<grid, 256, 0, st>>>(E, ew, eh, albedo, direct, emission, out, w, h);
+        else niv_compose_kernel<false><<<grid, 256, 0, st>>>(E, ew, eh, albedo, direct, emission, out, w, h);
+    } else {
+        const unsigned grid = (unsigned)std::min<size_t>((n + 255) / 256, (size_t)sms * 8);
+        niv_compose_scalar_kernel<<<grid, 256, 0, st>>>(E, ew, eh, albedo, direct, emission, out, w, h, half);
+    }
     NIV_CUDA(cudaGetLastError());
     return NIV_OK;
 }

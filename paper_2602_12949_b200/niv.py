@@ -25,7 +25,7 @@ NIV_OUT_SIGMOID = 1
 
 # every symbol include/niv.h declares (tests check that the library exports all of them)
 EXPORTS = ("niv_create", "niv_get_info", "niv_load_params", "niv_infer", "niv_infer_host", "niv_encode",
-           "niv_debug_encode", "niv_destroy", "niv_error_string", "niv_last_cuda_error", "niv_probe_gather",
+           "niv_debug_encode", "niv_compose", "niv_destroy", "niv_error_string", "niv_last_cuda_error", "niv_probe_gather",
            "niv_probe_sectors")
 
 
@@ -80,6 +80,7 @@ def lib():
         L.niv_infer_host.argtypes = [vp, vp, vp, C.POINTER(C.c_float), vp, sz, vp]
         L.niv_encode.argtypes = [vp, vp, vp, C.POINTER(C.c_float), vp, sz, vp]
         L.niv_debug_encode.argtypes = [vp, vp, vp, C.POINTER(C.c_float), sz, vp, vp, vp, vp, vp]
+        L.niv_compose.argtypes = [vp, C.c_uint32, C.c_uint32, vp, vp, vp, vp, C.c_uint32, C.c_uint32, vp]
         L.niv_destroy.argtypes = [vp]
         L.niv_error_string.argtypes = [C.c_int]
         L.niv_error_string.restype = C.c_char_p
@@ -276,3 +277,24 @@ def probe_gather(buf, pattern: int, n_ctas: int, loads_per_lane: int, seed: int,
                                 loads_per_lane, seed, sink.data_ptr(), _stream_ptr(stream))
     if rc != NIV_OK:
         raise NivError(rc, "niv_probe_gather")
+
+
+def compose(E, albedo, out, direct=None, emission=None, stream=None):
+    """niv_compose (include/niv.h): out = albedo / pi * E + direct + emission; CUDA fp32 tensors, E [eh][ew][3] at the
+    resolution of albedo [h][w][3] or at half of it.  Asynchronous."""
+    import torch
+    for name, t in (("E", E), ("albedo", albedo), ("out", out), ("direct", direct), ("emission", emission)):
+        if t is None:
+            continue
+        if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous() \
+                or t.dim() != 3 or t.shape[2] != 3:
+            raise TypeError("%s must be a contiguous CUDA float32 tensor [h][w][3]" % name)
+    h, w = albedo.shape[:2]
+    for name, t in (("out", out), ("direct", direct), ("emission", emission)):
+        if t is not None and tuple(t.shape) != (h, w, 3):
+            raise TypeError("%s must have the shape of albedo" % name)
+    rc = lib().niv_compose(E.data_ptr(), E.shape[1], E.shape[0], albedo.data_ptr(),
+                           None if direct is None else direct.data_ptr(),
+                           None if emission is None else emission.data_ptr(), out.data_ptr(), w, h, _stream_ptr(stream))
+    if rc != NIV_OK:
+        raise NivError(rc, "niv_compose")

@@ -432,3 +432,42 @@ def test_full_size_sampled(torch_cuda, niv, oracle, which):
                         param=None if param is None else np.float32(param))
     _check_irradiance(got[sel], want, nrm[sel], pos[sel])
     m.close()
+
+
+# ------------------------------------------------------------------------------------------------------
+# deferred compose, irradiance at full and at half resolution
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("w,h,half", [(64, 36, False), (64, 36, True), (1920, 1080, True), (1920, 1080, False),
+                                      (30, 14, True), (31, 7, False), (2, 2, True)])
+def test_compose_matches_oracle(torch_cuda, niv, oracle, w, h, half):
+    """fp32 kernel against the fp64 oracle: |err| <= 4 fp32 ulps of the largest term (three products / sums);
+    covers the 128-bit path (w % 4 == 0), the scalar path, image borders (clamped upsample) and full HD."""
+    torch = torch_cuda
+    rng = np.random.default_rng(w * 131 + h)
+    ew, eh = (w // 2, h // 2) if half else (w, h)
+    E = rng.uniform(0, 3, (eh, ew, 3)).astype(np.float32)
+    alb = rng.uniform(0, 1, (h, w, 3)).astype(np.float32)
+    D = rng.uniform(0, 2, (h, w, 3)).astype(np.float32)
+    Le = rng.uniform(0, 1, (h, w, 3)).astype(np.float32)
+    want = oracle.compose(E, alb, D, Le)
+    out = torch.full((h, w, 3), float("nan"), dtype=torch.float32, device="cuda")
+    guard = torch.full((h + 1, w, 3), 7.0, dtype=torch.float32, device="cuda")        # writes must stop at h rows
+    niv.compose(torch.from_numpy(E).cuda(), torch.from_numpy(alb).cuda(), out, torch.from_numpy(D).cuda(),
+                torch.from_numpy(Le).cuda())
+    niv.compose(torch.from_numpy(E).cuda(), torch.from_numpy(alb).cuda(), guard[:h])
+    torch.cuda.synchronize()
+    got = out.cpu().numpy().astype(np.float64)
+    assert np.all(np.isfinite(got))
+    assert np.abs(got - want).max() <= 4 * 2.0 ** -23 * 4.0
+    g = guard.cpu().numpy()
+    assert np.all(g[h] == 7.0)
+    assert np.abs(g[:h].astype(np.float64) - oracle.compose(E, alb)).max() <= 4 * 2.0 ** -23 * 4.0
+
+
+def test_compose_rejects_other_ratios(torch_cuda, niv):
+    torch = torch_cuda
+    a = torch.zeros((8, 8, 3), dtype=torch.float32, device="cuda")
+    e = torch.zeros((4, 3, 3), dtype=torch.float32, device="cuda")
+    with pytest.raises(niv.NivError) as ex:
+        niv.compose(e, a, a.clone())
+    assert ex.value.code == niv.NIV_ERR_INVALID_ARG
