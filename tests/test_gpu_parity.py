@@ -471,3 +471,33 @@ def test_compose_rejects_other_ratios(torch_cuda, niv):
     with pytest.raises(niv.NivError) as ex:
         niv.compose(e, a, a.clone())
     assert ex.value.code == niv.NIV_ERR_INVALID_ARG
+
+
+def test_concurrent_streams_share_one_model(torch_cuda, niv, oracle):
+    """niv_infer is safe for concurrent callers on different streams (include/niv.h): every launch draws its own
+    tile counter.  Eight frames on eight streams, in flight together, must each equal the serial result."""
+    torch = torch_cuda
+    case = Case(I.spec_fullhd(), 21)
+    m = case.gpu_model(niv)
+    n = 200000 + 3
+    frames = [_queries(case.spec, n, 50 + k) for k in range(8)]
+    dp = [torch.from_numpy(p).cuda() for p, _ in frames]
+    dn = [torch.from_numpy(q).cuda() for _, q in frames]
+    serial = []
+    for k in range(8):
+        o = torch.empty((n, 3), dtype=torch.float32, device="cuda")
+        m.infer(dp[k], dn[k], o)
+        torch.cuda.synchronize()
+        serial.append(o.cpu().numpy())
+    streams = [torch.cuda.Stream() for _ in range(8)]
+    outs = [torch.full((n, 3), float("nan"), dtype=torch.float32, device="cuda") for _ in range(8)]
+    torch.cuda.synchronize()
+    for rep in range(3):
+        for k in range(8):
+            m.infer(dp[k], dn[k], outs[k], stream=streams[k])
+    torch.cuda.synchronize()
+    for k in range(8):
+        assert np.array_equal(outs[k].cpu().numpy(), serial[k])
+    want = oracle.infer(case.spec, case.table, case.wblob, case.bblob, frames[0][0][:5000], frames[0][1][:5000])
+    _check_irradiance(serial[0][:5000], want, frames[0][1][:5000], frames[0][0][:5000])
+    m.close()
