@@ -29,7 +29,9 @@ def torch_cuda():
 
 @pytest.fixture(scope="module")
 def niv():
+    from paper_2602_12949_b200 import build as B
     from paper_2602_12949_b200 import niv as N
+    B.build()                                  # nvcc, in-tree (a no-op when libniv.so is up to date)
     N.lib()                                    # raises if libniv.so is missing: no fallback
     return N
 
