@@ -299,7 +299,7 @@ int niv_oracle_encode(const niv_oracle_config *cfg, const uint16_t *table,
     if (check_cfg(cfg)) return -1;
     uint32_t N[NIV_ORACLE_MAX_LEVELS], dense[NIV_ORACLE_MAX_LEVELS];
     if (niv_oracle_level_table(cfg, N, dense)) return -1;
-    const uint32_t L = cfg->n_levels, F = cfg->n_features, D = in_dim_of(cfg);
+    const uint32_t L = cfg->n_levels, D = in_dim_of(cfg);
     (void)n_threads;
 #ifdef _OPENMP
     if (n_threads > 0) omp_set_num_threads(n_threads);
@@ -338,7 +338,6 @@ int niv_oracle_infer(const niv_oracle_config *cfg, const uint16_t *table,
     if (check_cfg(cfg)) return -1;
     uint32_t N[NIV_ORACLE_MAX_LEVELS], dense[NIV_ORACLE_MAX_LEVELS];
     if (niv_oracle_level_table(cfg, N, dense)) return -1;
-    const uint32_t L = cfg->n_levels, F = cfg->n_features;
     (void)n_threads;
 #ifdef _OPENMP
     if (n_threads > 0) omp_set_num_threads(n_threads);
