@@ -17,8 +17,8 @@
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream);
  *   - niv_infer / niv_encode / niv_debug_encode are asynchronous on `stream`, allocate nothing, never
  *     synchronise (CUDA-graph capturable), are read-only on the model's parameters and safe for concurrent callers
- *     on different streams (niv_infer draws one of 64 per-launch tile counters round robin and zeroes it on
- *     `stream`: up to 64 launches of one model may be in flight at once);
+ *     on different streams (niv_infer draws one of 64 per-launch tile counters round robin, which the kernel
+ *     itself leaves zeroed: up to 64 launches of one model may be in flight at once);
  *   - there is no CPU fallback: without a CUDA device every entry point that needs one returns NIV_ERR_CUDA.
  */
 #ifndef NIV_H_

@@ -499,6 +499,13 @@ __global__ void __launch_bounds__(kTile, WIDTH == 32 ? 4 : 0) niv_fused_tmem_ker
 
     __syncthreads();
     if (warp == 0) tmem_dealloc(tmem, TMEM_COLS);
+    if (tid == 0) {       // the last CTA to finish leaves the (tile, done) counter pair zero for the slot's next launch
+        __threadfence();
+        if (atomicAdd(P.tile_ctr + 1, 1u) == gridDim.x - 1) {
+            P.tile_ctr[0] = 0u;
+            P.tile_ctr[1] = 0u;
+        }
+    }
 }
 
 }  // namespace niv
@@ -1023,6 +1030,7 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     e = cudaMalloc(&m->d_table, I.table_bytes ? I.table_bytes : 16);
     if (e == cudaSuccess) e = cudaMalloc(&m->d_wpack, P.wpack_bytes);
     if (e == cudaSuccess) e = cudaMalloc(&m->d_ctr, kCtrSlots * 128);
+    if (e == cudaSuccess) e = cudaMemset(m->d_ctr, 0, kCtrSlots * 128);
     if (e != cudaSuccess) {
         g_last_cuda_error = (int)e; (void)cudaGetLastError();
         cudaFree(m->d_table); cudaFree(m->d_wpack); cudaFree(m->d_ctr); delete m;
@@ -1127,7 +1135,7 @@ static int launch_fused(const niv_model* m, const KParams& Pin, const float* pos
 {
     KParams P = Pin;
     P.tile_ctr = m->d_ctr + (size_t)(m->ctr_next.fetch_add(1u) % kCtrSlots) * 32;
-    NIV_CUDA(cudaMemsetAsync(P.tile_ctr, 0, sizeof(uint32_t), st));
+    // (no memset: the kernels leave their counter pair zero, see the end of niv_fused_tmem_kernel)
     const uint32_t n_tiles = (uint32_t)((n + kTile - 1) / kTile);
     const uint32_t grid = n_tiles < m->grid_fused ? n_tiles : m->grid_fused;
     m->fused<<<grid, kTile, m->smem_fused, st>>>(P, pos, nrm, out, n, n_tiles);

@@ -223,6 +223,13 @@ __global__ void __launch_bounds__(kTile, 3) niv_fused_w128_kernel(const __grid_c
 
     __syncthreads();
     if (warp == 0) tmem_dealloc(tmem, TMEM_COLS);
+    if (tid == 0) {       // the last CTA to finish leaves the (tile, done) counter pair zero for the slot's next launch
+        __threadfence();
+        if (atomicAdd(P.tile_ctr + 1, 1u) == gridDim.x - 1) {
+            P.tile_ctr[0] = 0u;
+            P.tile_ctr[1] = 0u;
+        }
+    }
 }
 
 }  // namespace niv
