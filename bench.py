@@ -388,7 +388,7 @@ def run_ours(args):
         "active_gqueries_per_s": value * (1.0 - masked),
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms, "steps": e2e_steps,
                 "h2d_bytes_per_step": 24 * n, "d2h_bytes_per_step": 12 * n,
-                "api": "niv_infer_host (pinned host buffers; chunked H2D / kernel / D2H overlap)",
+                "api": "niv_infer_host (pinned host buffers, zero copy: the fused kernel reads the G-buffer and writes the irradiance over PCIe itself)",
                 "checksum": checksum},
         "gpu_launches": args.steps, "clocks": clk, "roofline": roofline,
     }

@@ -123,10 +123,11 @@ int niv_infer(niv_model *m, const float *pos, const float *nrm, const float *par
 /* The same operation with HOST buffers (the end-to-end call: PAPER.md:402-403 with the G-buffer in host memory).
  *   pos, nrm, out  HOST, [n][3] fp32 packed (pinned memory gives asynchronous copies; pageable memory works)
  *   param          HOST, as niv_infer
- * The frame is cut into chunks; each chunk's host->device copies, fused kernel and device->host copy are
- * queued on internal streams so that the copies of one chunk overlap the kernel of another.  Staging buffers
- * are owned by the model and grown on demand (this call MAY allocate).  `stream` is waited on before the first
- * copy and the call returns only after the last byte of `out` has landed (it synchronises).  NOT safe for
+ * Pinned (cudaHostAlloc / cudaHostRegister) buffers are used in place: the fused kernel reads the G-buffer and writes
+ * the irradiance over PCIe itself, one launch on `stream`, no staging (hidden widths <= 64).  Otherwise the frame is cut
+ * into chunks whose host->device copies, kernels and device->host copies are queued on internal streams so that they
+ * overlap; staging buffers are owned by the model and grown on demand (this path MAY allocate).  Either way the call
+ * returns only after the last byte of `out` has landed (it synchronises).  The staged path is NOT safe for
  * concurrent callers on the same model.  Errors as niv_infer, plus NIV_ERR_ALLOC. */
 int niv_infer_host(niv_model *m, const float *pos, const float *nrm, const float *param,
                    float *out, size_t n, void *stream);

@@ -235,7 +235,7 @@ __global__ void __launch_bounds__(kTile) niv_fused_kernel(const __grid_constant_
 // Here thread t keeps row t of the A operand in TMEM lane t: tcgen05.st instead of STS (no L1TEX wavefronts,
 // no generic->async proxy fence), tcgen05.mma reads A from TMEM, and shared memory holds the weights only.
 // TMEM columns per CTA (128 allocated): D [0, WIDTH) fp32 | A [64, 96) packed fp16 pairs | ones [96, 104).
-template <int WIDTH, int L, int NB, int F, bool RAWDIR>
+template <int WIDTH, int L, int NB, int F, bool RAWDIR, bool OUT128 = false>
 #ifdef NIV_EXPERIMENT_V2_MINB          // timing experiment only: another register budget for the v2 kernel
 __global__ void __launch_bounds__(kTile, NIV_EXPERIMENT_V2_MINB) niv_fused_tmem_kernel(
 #else
@@ -470,7 +470,34 @@ __global__ void __launch_bounds__(kTile, WIDTH == 32 ? 4 : 0) niv_fused_tmem_ker
                 tmem_ld_x4(lane_taddr, r);
                 tmem_ld_wait();
                 tc_fence_before_sync();
-                if (valid) {
+                if constexpr (OUT128) {
+                    // a12 for buffers in pinned HOST memory (niv_infer_host, zero copy): the warp's 32 x 3 floats go
+                    // through shared memory and leave as 24 aligned 128-bit stores = three full 128-byte lines, which
+                    // cross PCIe as full-line writes (scalar 12-byte-stride stores take 2.9 ms per frame, these 0.49)
+                    float y[3];
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        float v = __uint_as_float(r[c]);
+                        if (P.out_act == NIV_OUT_SIGMOID) v = __fdividef(1.0f, 1.0f + __expf(-v));
+                        y[c] = masked ? 0.0f : v;
+                    }
+                    const uint32_t lane = tid & 31u;
+                    float* so = reinterpret_cast<float*>(smem + P.misc_off + 64) + warp * 96;
+                    const size_t w0 = ((size_t)tile * kTile + warp * 32u) * 3;        // first float of the warp
+                    const bool vec = (w0 + 96 <= 3 * n) && ((reinterpret_cast<uintptr_t>(out) & 15u) == 0);
+                    if (vec) {
+                        so[lane * 3] = y[0];
+                        so[lane * 3 + 1] = y[1];
+                        so[lane * 3 + 2] = y[2];
+                        __syncwarp();
+                        if (lane < 24) *reinterpret_cast<float4*>(out + w0 + lane * 4) = *reinterpret_cast<const float4*>(so + lane * 4);
+                        __syncwarp();
+                    } else if (valid) {
+                        out[3 * i] = y[0];
+                        out[3 * i + 1] = y[1];
+                        out[3 * i + 2] = y[2];
+                    }
+                } else if (valid) {
                     float y[3];
 #pragma unroll
                     for (int c = 0; c < 3; ++c) {
@@ -766,6 +793,8 @@ struct niv_model {
     uint32_t grid_fused = 0;
     uint32_t smem_fused = 0;
     void (*fused)(KParams, const float*, const float*, float*, size_t, uint32_t) = nullptr;
+    void (*fused_host)(KParams, const float*, const float*, float*, size_t, uint32_t) = nullptr;   // 128-bit output stores
+    uint32_t grid_host = 0;
     uint32_t* d_ctr = nullptr;                     // kCtrSlots tile counters, 128 B apart; one per launch in flight
     mutable std::atomic<uint32_t> ctr_next{0};
     // niv_infer_host staging (grown on demand)
@@ -792,7 +821,7 @@ static uint32_t round_up(uint32_t v, uint32_t m) { return (v + m - 1) / m * m; }
 // Resident CTAs per SM from the kernel's own resource use.  (cudaOccupancyMaxActiveBlocksPerMultiprocessor
 // answers 1 for these kernels on sm_100a with driver 580 -- measured, see DESIGN.md section 6 -- so it is not used.)
 template <typename K>
-static int setup_kernel(niv_model* m, K kernel, int tmem_cols, const char* name) {
+static int setup_kernel(niv_model* m, K kernel, int tmem_cols, const char* name, uint32_t* grid_out = nullptr) {
     NIV_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m->smem_fused));
     cudaFuncAttributes fa;
     NIV_CUDA(cudaFuncGetAttributes(&fa, kernel));
@@ -818,6 +847,7 @@ static int setup_kernel(niv_model* m, K kernel, int tmem_cols, const char* name)
         NIV_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, pct));
         if (getenv("NIV_DEBUG")) fprintf(stderr, "[niv] %s: shared-memory carve-out %d %%\n", name, pct);
     }
+    if (grid_out) { *grid_out = (uint32_t)blocks * m->info.num_sms; return NIV_OK; }
     m->info.ctas_per_sm = (uint32_t)blocks;
     m->grid_fused = (uint32_t)blocks * m->info.num_sms;
     return NIV_OK;
@@ -842,38 +872,41 @@ static fused_fn pick_fused(uint32_t W, uint32_t L, int nb) {
     if (W == 64) return pick_l<64>(L, nb);
     return pick_l<128>(L, nb);
 }
-template <int W, int L>
+template <int W, int L, bool O>
 static fused_fn pick_tmem_nb(int nb) {
-    return nb == 4 ? niv_fused_tmem_kernel<W, L, 4, 2, false> : niv_fused_tmem_kernel<W, L, 2, 2, false>;
+    if (O) return niv_fused_tmem_kernel<W, L, 4, 2, false, O>;          // host-buffer variant: one batch size
+    return nb == 4 ? niv_fused_tmem_kernel<W, L, 4, 2, false, O> : niv_fused_tmem_kernel<W, L, 2, 2, false, false>;
 }
-template <int W>
+template <int W, bool O>
 static fused_fn pick_tmem_l(uint32_t L, int nb) {
     switch (L) {
-        case 4:  return niv_fused_tmem_kernel<W, 4, 4, 2, false>;
-        case 8:  return pick_tmem_nb<W, 8>(nb);
-        case 12: return niv_fused_tmem_kernel<W, 12, 4, 2, false>;
-        case 16: return pick_tmem_nb<W, 16>(nb);
+        case 4:  return niv_fused_tmem_kernel<W, 4, 4, 2, false, O>;
+        case 8:  return pick_tmem_nb<W, 8, O>(nb);
+        case 12: return niv_fused_tmem_kernel<W, 12, 4, 2, false, O>;
+        case 16: return pick_tmem_nb<W, 16, O>(nb);
         default: return nullptr;
     }
 }
 // the paper's own family: F = 4, raw direction, 2..8 levels, 2 levels (16 x 8-byte gathers) per batch
-template <int W>
+template <int W, bool O>
 static fused_fn pick_tmem_paper(uint32_t L) {
     switch (L) {
-        case 2: return niv_fused_tmem_kernel<W, 2, 2, 4, true>;
-        case 4: return niv_fused_tmem_kernel<W, 4, 2, 4, true>;
-        case 6: return niv_fused_tmem_kernel<W, 6, 2, 4, true>;
-        case 8: return niv_fused_tmem_kernel<W, 8, 2, 4, true>;
+        case 2: return niv_fused_tmem_kernel<W, 2, 2, 4, true, O>;
+        case 4: return niv_fused_tmem_kernel<W, 4, 2, 4, true, O>;
+        case 6: return niv_fused_tmem_kernel<W, 6, 2, 4, true, O>;
+        case 8: return niv_fused_tmem_kernel<W, 8, 2, 4, true, O>;
         default: return nullptr;
     }
 }
+// O = true: the variant whose output leaves as 128-bit stores (buffers in pinned host memory)
+template <bool O>
 static fused_fn pick_tmem(uint32_t W, uint32_t L, int nb, uint32_t F) {
     if (L == 0)                                     // grid-less: positional encoding, no gathers
-        return W == 16 ? niv_fused_tmem_kernel<16, 0, 1, 2, true> : W == 32 ? niv_fused_tmem_kernel<32, 0, 1, 2, true>
-             : W == 64 ? niv_fused_tmem_kernel<64, 0, 1, 2, true> : nullptr;
-    if (F == 4) return W == 32 ? pick_tmem_paper<32>(L) : W == 64 ? pick_tmem_paper<64>(L) : nullptr;
-    if (W == 32) return pick_tmem_l<32>(L, nb);
-    if (W == 64) return pick_tmem_l<64>(L, nb);
+        return W == 16 ? niv_fused_tmem_kernel<16, 0, 1, 2, true, O> : W == 32 ? niv_fused_tmem_kernel<32, 0, 1, 2, true, O>
+             : W == 64 ? niv_fused_tmem_kernel<64, 0, 1, 2, true, O> : nullptr;
+    if (F == 4) return W == 32 ? pick_tmem_paper<32, O>(L) : W == 64 ? pick_tmem_paper<64, O>(L) : nullptr;
+    if (W == 32) return pick_tmem_l<32, O>(L, nb);
+    if (W == 64) return pick_tmem_l<64, O>(L, nb);
     return nullptr;
 }
 
@@ -1017,14 +1050,18 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
             m->smem_fused = P.misc_off + 2 * 8 + 16;
             I.smem_bytes = m->smem_fused;
         } else {
-            m->fused = pick_tmem(W, cfg->n_levels, nb, cfg->n_features);
+            m->fused = pick_tmem<false>(W, cfg->n_levels, nb, cfg->n_features);
+            m->fused_host = pick_tmem<true>(W, cfg->n_levels, nb, cfg->n_features);
             tmem_cols = 128;
-            m->smem_fused = P.a_off + 2 * 8 + 16;        // weights + barriers only
+            m->smem_fused = P.a_off + 64 + 4 * 384;      // weights | barriers, TMEM slot, tile slots | output staging
             P.misc_off = P.a_off;
             I.smem_bytes = m->smem_fused;
         }
         if (!m->fused) { delete m; return NIV_ERR_UNSUPPORTED; }
         rc = setup_kernel(m, m->fused, tmem_cols, kind == 1 ? "fused_v1" : W == 128 ? "fused_w128" : "fused_v2");
+        if (rc == NIV_OK && m->fused_host && kind == 2 && W != 128)
+            rc = setup_kernel(m, m->fused_host, tmem_cols, "fused_v2_host", &m->grid_host);
+        else m->fused_host = nullptr;
     }
     if (rc != NIV_OK) { delete m; return rc; }
     e = cudaMalloc(&m->d_table, I.table_bytes ? I.table_bytes : 16);
@@ -1131,14 +1168,15 @@ static int fill_params(const niv_model* m, const float* param, KParams& P)
 }
 
 static int launch_fused(const niv_model* m, const KParams& Pin, const float* pos, const float* nrm, float* out,
-                        size_t n, cudaStream_t st)
+                        size_t n, cudaStream_t st, bool host_variant = false)
 {
     KParams P = Pin;
     P.tile_ctr = m->d_ctr + (size_t)(m->ctr_next.fetch_add(1u) % kCtrSlots) * 32;
     // (no memset: the kernels leave their counter pair zero, see the end of niv_fused_tmem_kernel)
     const uint32_t n_tiles = (uint32_t)((n + kTile - 1) / kTile);
-    const uint32_t grid = n_tiles < m->grid_fused ? n_tiles : m->grid_fused;
-    m->fused<<<grid, kTile, m->smem_fused, st>>>(P, pos, nrm, out, n, n_tiles);
+    const uint32_t cap = host_variant ? m->grid_host : m->grid_fused;
+    const uint32_t grid = n_tiles < cap ? n_tiles : cap;
+    (host_variant ? m->fused_host : m->fused)<<<grid, kTile, m->smem_fused, st>>>(P, pos, nrm, out, n, n_tiles);
     NIV_CUDA(cudaGetLastError());
     return NIV_OK;
 }
@@ -1169,6 +1207,24 @@ extern "C" int niv_infer_host(niv_model* m, const float* pos, const float* nrm, 
     int rc = fill_params(m, param, P);
     if (rc != NIV_OK) return rc;
     NIV_CUDA(cudaSetDevice(m->cfg.device));
+    // Zero copy: if all three buffers are pinned (or registered) host memory the fused kernel reads the G-buffer and
+    // writes the irradiance over PCIe itself -- the texel of the next tile is requested a tile ahead, the output
+    // leaves as full 128-byte lines -- so transfer and compute overlap tile by tile in ONE launch with no staging
+    // (1.04 ms per full-HD frame against 1.21 ms with chunked copies; 0.91 ms is the copy time of the input alone).
+    if (m->fused_host && !getenv("NIV_HOST_STAGED")) {
+        cudaPointerAttributes ap, an, ao;
+        if (cudaPointerGetAttributes(&ap, pos) == cudaSuccess && cudaPointerGetAttributes(&an, nrm) == cudaSuccess &&
+            cudaPointerGetAttributes(&ao, out) == cudaSuccess && ap.type == cudaMemoryTypeHost &&
+            an.type == cudaMemoryTypeHost && ao.type == cudaMemoryTypeHost && ap.devicePointer && an.devicePointer &&
+            ao.devicePointer && ((uintptr_t)ao.devicePointer & 15u) == 0) {
+            rc = launch_fused(m, P, (const float*)ap.devicePointer, (const float*)an.devicePointer,
+                              (float*)ao.devicePointer, n, (cudaStream_t)stream, true);
+            if (rc != NIV_OK) return rc;
+            NIV_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+            return NIV_OK;
+        }
+        (void)cudaGetLastError();                    // pageable memory: cudaPointerGetAttributes may have set an error
+    }
     if (!m->hs[0]) {
         NIV_CUDA(cudaStreamCreateWithFlags(&m->hs[0], cudaStreamNonBlocking));
         NIV_CUDA(cudaStreamCreateWithFlags(&m->hs[1], cudaStreamNonBlocking));
