@@ -50,6 +50,7 @@ def _env_int(name, default):
 PAPER_LEVELS, PAPER_WIDTH = 8, 64        # --paper-levels / --paper-width (workload "paper")
 # PAPER.md:383-389 (Table 1, RTX 4090, full HD): ms per frame by (grid levels, width)
 PAPER_TABLE1_MS = {(0, 16): 0.19, (0, 32): 0.20, (0, 64): 0.25, (2, 64): 0.31, (4, 64): 0.67, (6, 64): 1.06, (8, 64): 1.35}
+PAPER_TABLE1_HALF_MS = {(0, 16): 0.029, (0, 32): 0.031, (0, 64): 0.069, (2, 64): 0.088, (4, 64): 0.18, (6, 64): 0.26, (8, 64): 0.37}
 
 
 def make_workload(name: str, frame: int):
@@ -373,7 +374,8 @@ def run_ours(args):
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
         # BASELINE.md holds a paper number only for the paper's own model: 1.35 ms per full-HD frame on an RTX 4090
         # = 1.536 Gqueries/s -- another machine's, context not target
-        "vs_baseline": (value / (N_TEXELS / (PAPER_TABLE1_MS[(PAPER_LEVELS, PAPER_WIDTH)] * 1e-3) / 1e9))
+        "vs_baseline": (value / (N_TEXELS / ((PAPER_TABLE1_HALF_MS if args.half else PAPER_TABLE1_MS)[(PAPER_LEVELS, PAPER_WIDTH)]
+                                             * 1e-3) / 1e9))
         if (args.workload == "paper" and world == 1 and (PAPER_LEVELS, PAPER_WIDTH) in PAPER_TABLE1_MS) else None,
         "dtype": "f16 operands / f32 accumulate (index path: f32 + u32)", "data": "synthetic",
         "config": {"workload": args.workload, "description": desc, "model": _model_str(spec),
