@@ -479,30 +479,30 @@ def run_compose(args):
     niv.lib()
     torch.cuda.set_device(0)
     peaks = load_peaks()
-    h, w = H_PX, W_PX
-    ring = 6                                           # 6 x 100 MB > L2
-    for half in (False, True):
-        eh, ew = (h // 2, w // 2) if half else (h, w)
-        bufs = [[torch.rand((h, w, 3), device="cuda") for _ in range(3)] + [torch.rand((eh, ew, 3), device="cuda"),
-                torch.empty((h, w, 3), device="cuda")] for _ in range(ring)]
-        for k in range(5):
-            a, d, le, e, o = bufs[k % ring]
-            niv.compose(e, a, o, d, le)
-        steps = args.steps or 100
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        torch.cuda.synchronize()
-        e0.record()
-        for k in range(steps):
-            a, d, le, e, o = bufs[k % ring]
-            niv.compose(e, a, o, d, le)
-        e1.record()
-        torch.cuda.synchronize()
-        ms = e0.elapsed_time(e1) / steps
-        nbytes = (48 + (3 if half else 12)) * h * w
-        print(json.dumps({"op": "niv_compose", "E_resolution": "%dx%d" % (ew, eh), "frame": "%dx%d" % (w, h),
-                          "ms": ms, "algorithmic_bytes": nbytes,
-                          "roofline": {"bound": "hbm", "achieved": nbytes / ms / 1e6, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                                       "frac": nbytes / ms / 1e6 / peaks["hbm_gbs"], "peak_source": peaks["source"]}}), flush=True)
+    for (h, w) in ((H_PX, W_PX), (2 * H_PX, 2 * W_PX)):
+        ring = 6 if h == H_PX else 2                     # 6 x 100 MB / 2 x 400 MB > L2
+        for half in (False, True):
+            eh, ew = (h // 2, w // 2) if half else (h, w)
+            bufs = [[torch.rand((h, w, 3), device="cuda") for _ in range(3)] + [torch.rand((eh, ew, 3), device="cuda"),
+                    torch.empty((h, w, 3), device="cuda")] for _ in range(ring)]
+            for k in range(5):
+                a, d, le, e, o = bufs[k % ring]
+                niv.compose(e, a, o, d, le)
+            steps = args.steps or 100
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            for k in range(steps):
+                a, d, le, e, o = bufs[k % ring]
+                niv.compose(e, a, o, d, le)
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / steps
+            nbytes = (48 + (3 if half else 12)) * h * w
+            print(json.dumps({"op": "niv_compose", "E_resolution": "%dx%d" % (ew, eh), "frame": "%dx%d" % (w, h),
+                              "ms": ms, "algorithmic_bytes": nbytes,
+                              "roofline": {"bound": "hbm", "achieved": nbytes / ms / 1e6, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                                           "frac": nbytes / ms / 1e6 / peaks["hbm_gbs"], "peak_source": peaks["source"]}}), flush=True)
 
 
 def main():
