@@ -503,3 +503,25 @@ def test_concurrent_streams_share_one_model(torch_cuda, niv, oracle):
     want = oracle.infer(case.spec, case.table, case.wblob, case.bblob, frames[0][0][:5000], frames[0][1][:5000])
     _check_irradiance(serial[0][:5000], want, frames[0][1][:5000], frames[0][0][:5000])
     m.close()
+
+
+def test_sweep_extremes_sampled(torch_cuda, niv, oracle):
+    """BASELINE.json configs[4] extremes at full size: the largest table (T = 2^20, 64 MiB) with width 128 on a 2560x1440
+    frame, and two frames in one call with width 32 and the smallest table; sampled outputs against the oracle."""
+    torch = torch_cuda
+    for log2_T, width, frames in ((20, 128, 1), (14, 32, 2)):
+        spec = I.spec_fullhd(log2_T, width, 2)
+        case = Case(spec, 400 + width)
+        gs = [I.make_gbuffer(2560, 1440, 0, frame=f) for f in range(frames)]
+        pos = np.concatenate([g["pos"] for g in gs])
+        nrm = np.concatenate([g["nrm"] for g in gs])
+        n = pos.shape[0]
+        m = case.gpu_model(niv)
+        got = _gpu_infer(torch, m, pos, nrm)
+        masked = np.all(nrm == 0, axis=1)
+        assert np.all(got[masked] == 0) and np.all(np.isfinite(got))
+        sel = np.unique(np.concatenate([(I.random_u64(5, 2, 20000) % np.uint64(n)).astype(np.int64),
+                                        np.arange(0, 200), np.arange(n - 200, n)]))
+        want = oracle.infer(spec, case.table, case.wblob, case.bblob, pos[sel], nrm[sel])
+        _check_irradiance(got[sel], want, nrm[sel], pos[sel])
+        m.close()
