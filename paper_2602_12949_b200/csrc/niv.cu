@@ -537,6 +537,7 @@ __global__ void __launch_bounds__(kTile, WIDTH == 32 ? 4 : 0) niv_fused_tmem_ker
 
 }  // namespace niv
 #include "niv_fused_w128.cuh"
+#include "niv_fused_mma.cuh"
 #include "niv_compose.cuh"
 namespace niv {
 
@@ -795,6 +796,8 @@ struct niv_model {
     void (*fused)(KParams, const float*, const float*, float*, size_t, uint32_t) = nullptr;
     void (*fused_host)(KParams, const float*, const float*, float*, size_t, uint32_t) = nullptr;   // 128-bit output stores
     uint32_t grid_host = 0;
+    bool mma_kernel = false;                       // NIV_KERNEL=6: the per-warp mma.sync A/B kernel (32-texel tiles)
+    uint32_t* d_wmma = nullptr;
     uint32_t* d_ctr = nullptr;                     // kCtrSlots tile counters, 128 B apart; one per launch in flight
     mutable std::atomic<uint32_t> ctr_next{0};
     // niv_infer_host staging (grown on demand)
@@ -1032,11 +1035,18 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
         const char* nbv = getenv("NIV_NB");             // levels per gather batch: 2 or 4
         const int nb = nbv ? atoi(nbv) : 4;
         int kind = kv ? atoi(kv) : 2;
-        if (kind != 1 && kind != 2) kind = 2;
+        if (kind != 1 && kind != 2 && kind != 6) kind = 2;
         if (cfg->n_levels == 0 || cfg->n_features == 4) kind = 2;   // the paper's families exist as v2 only
         int tmem_cols = W < 32 ? 32 : (int)W;
         if (kind == 1) m->fused = pick_fused(W, cfg->n_levels, nb);
-        else if (W == 128) {                            // two N = 64 halves per hidden layer (niv_fused_w128.cuh)
+        else if (kind == 6 && W == 64 && cfg->n_levels == 16 && cfg->n_features == 2 && cfg->n_hidden_layers == 2 &&
+                 cfg->n_params == 0) {
+            m->fused = niv_fused_mma_kernel<4, 4>;       // 4 levels per gather batch, 128 registers, 4 CTAs per SM
+            m->mma_kernel = true;
+            tmem_cols = 32;                              // no tensor memory: do not let it limit the occupancy
+            m->smem_fused = (kMmaWords + 4 * kMmaStage) * 4;
+            I.smem_bytes = m->smem_fused;
+        } else if (W == 128) {                            // two N = 64 halves per hidden layer (niv_fused_w128.cuh)
             switch (cfg->n_levels) {
                 case 4:  m->fused = niv_fused_w128_kernel<4, 4>; break;
                 case 8:  m->fused = niv_fused_w128_kernel<8, 4>; break;
@@ -1058,8 +1068,8 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
             I.smem_bytes = m->smem_fused;
         }
         if (!m->fused) { delete m; return NIV_ERR_UNSUPPORTED; }
-        rc = setup_kernel(m, m->fused, tmem_cols, kind == 1 ? "fused_v1" : W == 128 ? "fused_w128" : "fused_v2");
-        if (rc == NIV_OK && m->fused_host && kind == 2 && W != 128)
+        rc = setup_kernel(m, m->fused, tmem_cols, kind == 1 ? "fused_v1" : m->mma_kernel ? "fused_mma" : W == 128 ? "fused_w128" : "fused_v2");
+        if (rc == NIV_OK && m->fused_host && kind == 2 && W != 128 && !m->mma_kernel)
             rc = setup_kernel(m, m->fused_host, tmem_cols, "fused_v2_host", &m->grid_host);
         else m->fused_host = nullptr;
     }
@@ -1148,6 +1158,24 @@ extern "C" int niv_load_params(niv_model* m, const void* table_fp16, size_t tabl
         bsrc += o;
     }
     NIV_CUDA(cudaMemcpyAsync(m->d_wpack, pack.data(), P.wpack_bytes, cudaMemcpyHostToDevice, st));
+    std::vector<uint32_t> wm;
+    if (m->mma_kernel) {                                // row-major padded weights + fp32 biases (niv_fused_mma.cuh)
+        wm.assign(kMmaWords, 0u);
+        uint16_t* h = reinterpret_cast<uint16_t*>(wm.data());
+        const size_t o2 = (size_t)64 * P.in_dim, o3 = o2 + 64 * 64;
+        for (uint32_t r = 0; r < 64; ++r) {
+            for (uint32_t c2 = 0; c2 < 48; ++c2) h[(kMmaW1 + r * kMmaS1) * 2 + c2] = w[(size_t)r * P.in_dim + c2];
+            for (uint32_t c2 = 0; c2 < 64; ++c2) h[(kMmaW2 + r * kMmaS2) * 2 + c2] = w[o2 + (size_t)r * 64 + c2];
+        }
+        for (uint32_t r = 0; r < 3; ++r)
+            for (uint32_t c2 = 0; c2 < 64; ++c2) h[(kMmaW3 + r * kMmaS2) * 2 + c2] = w[o3 + (size_t)r * 64 + c2];
+        float* bf = reinterpret_cast<float*>(wm.data() + kMmaB1);
+        for (uint32_t r = 0; r < 64; ++r) { bf[r] = b[r]; bf[64 + r] = b[64 + r]; }
+        for (uint32_t r = 0; r < 3; ++r) bf[128 + r] = b[128 + r];
+        if (!m->d_wmma) NIV_CUDA(cudaMalloc(&m->d_wmma, kMmaWords * 4));
+        NIV_CUDA(cudaMemcpyAsync(m->d_wmma, wm.data(), kMmaWords * 4, cudaMemcpyHostToDevice, st));
+        m->kp.wmma = m->d_wmma;
+    }
     if (table_bytes) NIV_CUDA(cudaMemcpyAsync(m->d_table, table_fp16, table_bytes,
                              src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
     NIV_CUDA(cudaStreamSynchronize(st));
@@ -1173,6 +1201,12 @@ static int launch_fused(const niv_model* m, const KParams& Pin, const float* pos
     KParams P = Pin;
     P.tile_ctr = m->d_ctr + (size_t)(m->ctr_next.fetch_add(1u) % kCtrSlots) * 32;
     // (no memset: the kernels leave their counter pair zero, see the end of niv_fused_tmem_kernel)
+    if (m->mma_kernel) {                                // warp-granular 32-texel tiles, four per CTA
+        const uint32_t nt32 = (uint32_t)((n + 31) / 32), ctas = (nt32 + 3) / 4;
+        m->fused<<<ctas < m->grid_fused ? ctas : m->grid_fused, kTile, m->smem_fused, st>>>(P, pos, nrm, out, n, nt32);
+        NIV_CUDA(cudaGetLastError());
+        return NIV_OK;
+    }
     const uint32_t n_tiles = (uint32_t)((n + kTile - 1) / kTile);
     const uint32_t cap = host_variant ? m->grid_host : m->grid_fused;
     const uint32_t grid = n_tiles < cap ? n_tiles : cap;
@@ -1354,6 +1388,7 @@ extern "C" int niv_destroy(niv_model* m)
     cudaFree(m->d_table);
     cudaFree(m->d_wpack);
     cudaFree(m->d_ctr);
+    cudaFree(m->d_wmma);
     cudaFree(m->d_stage);
     if (m->hs[0]) cudaStreamDestroy(m->hs[0]);
     if (m->hs[1]) cudaStreamDestroy(m->hs[1]);

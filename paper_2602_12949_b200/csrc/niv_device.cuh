@@ -51,6 +51,7 @@ struct KParams {
     uint32_t a_off;             // byte offset of the A tile in shared memory
     uint32_t ones_off;          // byte offset of the constant "ones" A chunk of the bias K-step (v1 kernel)
     uint32_t misc_off;          // byte offset of folded bias / barriers
+    const uint32_t* wmma;       // weights in the layout of the mma.sync A/B kernel (niv_fused_mma.cuh), else NULL
 };
 
 // ---------------------------------------------------------------- O0: background / non-finite mask

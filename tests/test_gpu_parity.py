@@ -525,3 +525,24 @@ def test_sweep_extremes_sampled(torch_cuda, niv, oracle):
         want = oracle.infer(spec, case.table, case.wblob, case.bblob, pos[sel], nrm[sel])
         _check_irradiance(got[sel], want, nrm[sel], pos[sel])
         m.close()
+
+
+def test_mma_sync_ab_kernel_parity(torch_cuda, niv, oracle, monkeypatch):
+    """The per-warp mma.sync A/B kernel (NIV_KERNEL=6, csrc/niv_fused_mma.cuh) computes the same function: parity with
+    the oracle on the full-HD model, and agreement with the default tcgen05 kernel to fp16-activation rounding."""
+    torch = torch_cuda
+    case = Case(I.spec_fullhd(), 31, bias_scale=0.1)
+    n = 148 * 128 * 3 + 77
+    pos, nrm = _queries(case.spec, n, 61, coherent=True)
+    nrm[5] = 0.0
+    want = oracle.infer(case.spec, case.table, case.wblob, case.bblob, pos, nrm)
+    m = case.gpu_model(niv)
+    ref = _gpu_infer(torch, m, pos, nrm)
+    m.close()
+    monkeypatch.setenv("NIV_KERNEL", "6")
+    m = case.gpu_model(niv)
+    got = _gpu_infer(torch, m, pos, nrm)
+    m.close()
+    monkeypatch.delenv("NIV_KERNEL")
+    _check_irradiance(got, want, nrm, pos)
+    assert np.abs(got.astype(np.float64) - ref.astype(np.float64)).max() <= 2e-3
