@@ -331,10 +331,13 @@ def run_ours(args):
     t_tensor = flop_texel * n / (peaks["tflops_sustained"] * 1e12)
     t_hbm = hbm_bytes / (peaks["hbm_gbs"] * 1e9)
     traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    tp = os.path.join(ROOT, "profiles", "traffic.csv")             # ncu DRAM bytes per launch (profiles/traffic.md)
     if os.path.exists(tp):
         with open(tp) as f:
-            traffic = json.load(f).get(args.workload)
+            for ln in f.read().splitlines()[1:]:
+                k, _, v = ln.partition(",")
+                if k == args.workload and v.strip().isdigit():
+                    traffic = int(v)
     t_all = {"l2-gather": t_gather, "tensor": t_tensor, "hbm": t_hbm}
     bound = max(t_all, key=t_all.get)                # the slowest roofline bounds the kernel (north_star)
     roofline = {
