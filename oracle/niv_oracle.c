@@ -330,10 +330,10 @@ int niv_oracle_encode(const niv_oracle_config *cfg, const uint16_t *table,
 }
 
 /* ---- full path O0..O9.  out_f32 [n][3] and/or out_f64 [n][3] (either may be NULL). ---- */
-int niv_oracle_infer(const niv_oracle_config *cfg, const uint16_t *table,
-                     const uint16_t *weights, const float *biases,
-                     const float *pos, const float *nrm, const float *param,
-                     float *out_f32, double *out_f64, size_t n, int n_threads)
+static int infer_impl(const niv_oracle_config *cfg, const uint16_t *table,
+                      const uint16_t *weights, const float *biases,
+                      const float *pos, const float *nrm, const float *param_base, size_t param_stride,
+                      float *out_f32, double *out_f64, size_t n, int n_threads)
 {
     if (check_cfg(cfg)) return -1;
     uint32_t N[NIV_ORACLE_MAX_LEVELS], dense[NIV_ORACLE_MAX_LEVELS];
@@ -345,6 +345,7 @@ int niv_oracle_infer(const niv_oracle_config *cfg, const uint16_t *table,
     #pragma omp parallel for schedule(static)
     for (long long i = 0; i < (long long)n; ++i) {
         double y[3] = { 0.0, 0.0, 0.0 };
+        const float *param = param_base ? param_base + (size_t)i * param_stride : NULL;   /* this texel's scalars */
         if (!texel_masked(pos + 3 * i, nrm + 3 * i)) {               /* O0 */
             double x[NIV_ORACLE_MAX_DIM];
             encode_one(cfg, N, dense, table, pos + 3 * i, NULL, NULL, NULL, x);   /* O1-O4 */
@@ -363,6 +364,28 @@ int niv_oracle_infer(const niv_oracle_config *cfg, const uint16_t *table,
         }
     }
     return 0;
+}
+
+/* the scene parameters are the same for every texel of the call (one frame, one time of day: PAPER.md:669-671) */
+int niv_oracle_infer(const niv_oracle_config *cfg, const uint16_t *table,
+                     const uint16_t *weights, const float *biases,
+                     const float *pos, const float *nrm, const float *param,
+                     float *out_f32, double *out_f64, size_t n, int n_threads)
+{
+    return infer_impl(cfg, table, weights, biases, pos, nrm, param, 0, out_f32, out_f64, n, n_threads);
+}
+
+/* ---- f3: every texel carries its own scene parameters, tparam [n][n_params] f32 (several frames with different
+ * t in one call, or a parameter that varies over the image).  The network input of texel i is O7 with
+ * gamma(tparam[i][q]) in place of gamma(t[q]) -- the paper's "new inputs to the model" evaluated per
+ * shading point; nothing else changes. ---- */
+int niv_oracle_infer_texel_params(const niv_oracle_config *cfg, const uint16_t *table,
+                                  const uint16_t *weights, const float *biases,
+                                  const float *pos, const float *nrm, const float *tparam,
+                                  float *out_f32, double *out_f64, size_t n, int n_threads)
+{
+    if (!cfg || cfg->n_params == 0 || !tparam) return -1;
+    return infer_impl(cfg, table, weights, biases, pos, nrm, tparam, cfg->n_params, out_f32, out_f64, n, n_threads);
 }
 
 int niv_oracle_max_threads(void)

@@ -173,6 +173,28 @@ def infer(spec, table, weights_blob, biases_blob, pos, nrm, param=None, n_thread
     return (out32, out64) if want_f64 else out32
 
 
+def infer_texel_params(spec, table, weights_blob, biases_blob, pos, nrm, tparam, n_threads: int = 0,
+                       want_f64: bool = False):
+    """as infer(), every texel with its own scene parameters tparam [n][n_params]."""
+    cfg = make_config(spec)
+    table = _chk(table, np.float16, "table")
+    w = _chk(weights_blob, np.float16, "weights")
+    b = None if biases_blob is None else _chk(biases_blob, np.float32, "biases")
+    pos = _chk(pos, np.float32, "pos")
+    nrm = _chk(nrm, np.float32, "nrm")
+    tp = _chk(tparam, np.float32, "tparam")
+    n = pos.shape[0]
+    if spec.n_params == 0 or tp.size != n * spec.n_params:
+        raise ValueError("tparam must hold n * n_params values")
+    out32 = np.zeros((n, 3), dtype=np.float32)
+    out64 = np.zeros((n, 3), dtype=np.float64) if want_f64 else None
+    rc = lib().niv_oracle_infer_texel_params(C.byref(cfg), _p(table), _p(w), _p(b), _p(pos), _p(nrm), _p(tp),
+                                             _p(out32), _p(out64), C.c_size_t(n), C.c_int(n_threads))
+    if rc:
+        raise ValueError("niv_oracle_infer_texel_params failed")
+    return (out32, out64) if want_f64 else out32
+
+
 def max_threads() -> int:
     return int(lib().niv_oracle_max_threads())
 

@@ -565,6 +565,40 @@ def test_infer_is_composition_of_parts_and_masks(oracle):
     assert np.array_equal(out32, again)
 
 
+def test_texel_params_are_the_per_call_function_row_by_row(oracle):
+    """with per-texel parameters, texel i is the per-call function (pinned above)
+    evaluated at t = tparam[i]; a constant buffer reproduces the per-call result bit for bit; two parameters keep their
+    order (reading #12: parameter q at input columns enc_dim + 16 q .. + 16), checked through the MLP composition."""
+    for n_params in (1, 2):
+        spec = dataclasses.replace(I.spec_param(), n_params=n_params)
+        table = I.make_table(spec, 4)
+        weights, biases = I.make_mlp(spec, 4, bias_scale=0.1)
+        wb, bb = I.pack_weights(weights), I.pack_biases(biases)
+        n = 48
+        pos = I.positions_uniform(n, I.ROOM_AABB, 5)
+        nrm = I.normals_uniform(n, 5)
+        nrm[3] = 0.0                                   # a background texel stays zero whatever its parameter
+        tp = I.uniform01(17, 3, n * n_params).astype(np.float32).reshape(n, n_params)
+        out = oracle.infer_texel_params(spec, table, wb, bb, pos, nrm, tp, want_f64=True)[1]
+        for i in range(n):
+            row = oracle.infer(spec, table, wb, bb, pos[i:i + 1], nrm[i:i + 1], tp[i], want_f64=True)[1]
+            assert np.array_equal(out[i], row[0])
+        assert np.all(out[3] == 0)
+        const = np.tile(tp[7], (n, 1))
+        a = oracle.infer_texel_params(spec, table, wb, bb, pos, nrm, const)
+        b = oracle.infer(spec, table, wb, bb, pos, nrm, tp[7])
+        assert np.array_equal(a, b)
+        # composition of parts: features of texel 0 with ITS parameters through the MLP
+        enc = oracle.encode(spec, table, pos[:1], nrm[:1], tp[0])
+        x = enc["features"][0]
+        for q in range(n_params):
+            np.testing.assert_array_equal(x[48 + 16 * q:64 + 16 * q], oracle.param_encode(float(tp[0, q]), 8))
+        y = oracle.mlp(spec, wb, bb, x)
+        np.testing.assert_allclose(out[0], 1.0 / (1.0 + np.exp(-y)), rtol=0, atol=3e-16)
+    # the parameter really enters: two different t give different irradiance
+    assert not np.array_equal(out[0], oracle.infer(spec, table, wb, bb, pos[:1], nrm[:1], tp[1], want_f64=True)[1][0])
+
+
 def test_locate_uses_fp32_op_sequence(oracle):
     """Reading #10: the cell is decided by fl32(fl32(fl32(x-min)*inv)*N) -- compare with the same sequence in
     numpy float32 (an all-fp64 evaluation flips cells on ~1e-3 of full-HD texels)."""
