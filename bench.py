@@ -262,6 +262,18 @@ def run_ours(args):
     d_nrm = [torch.from_numpy(nrm).cuda() for _ in range(RING)]
     d_out = [torch.empty((n, 3), dtype=torch.float32, device="cuda") for _ in range(RING)]
     stream = torch.cuda.current_stream()
+    d_tp = None
+    if args.texel_params:                            # the parameter varies over the image, one value per texel
+        if not spec.n_params:
+            raise SystemExit("--texel-params needs a model with scene parameters (--workload param)")
+        tp = (np.float32(param)[None, :] + np.float32(0.25) * (np.arange(n, dtype=np.float32) / np.float32(n))[:, None])
+        d_tp = torch.from_numpy(np.ascontiguousarray(tp, dtype=np.float32)).cuda()
+
+    def infer_dev(k):
+        if d_tp is not None:
+            model.infer_texel_params(d_pos[k], d_nrm[k], d_tp, d_out[k])
+        else:
+            model.infer(d_pos[k], d_nrm[k], d_out[k], param=param)
 
     def barrier():
         if world > 1:
@@ -270,14 +282,14 @@ def run_ours(args):
 
     # ---- device-resident timing ---------------------------------------------------------------------
     for s in range(args.warmup):
-        model.infer(d_pos[s % RING], d_nrm[s % RING], d_out[s % RING], param=param)
+        infer_dev(s % RING)
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     barrier()
     clocks = ClockSampler(local) if rank == 0 else None
     ev[0].record(stream)
     for s in range(args.steps):
         k = s % RING
-        model.infer(d_pos[k], d_nrm[k], d_out[k], param=param)
+        infer_dev(k)
         ev[s + 1].record(stream)
     barrier()
     total_ms = ev[0].elapsed_time(ev[-1])
@@ -285,7 +297,7 @@ def run_ours(args):
     # clocks keep sampling a little longer so that short runs still get a few samples under load
     t_end = time.time() + 0.3
     while time.time() < t_end:
-        model.infer(d_pos[0], d_nrm[0], d_out[0], param=param)
+        infer_dev(0)
         torch.cuda.synchronize()
     clk = clocks.stop() if clocks else None
     total_ms = D.reduce_max(total_ms, "cuda")
@@ -366,7 +378,7 @@ def run_ours(args):
     }
 
     cpu = None
-    if world == 1 and not args.no_cpu_baseline:
+    if world == 1 and not args.no_cpu_baseline and d_tp is None:
         n_s, dt, cores = time_oracle(spec, table, wb, bb, pos, nrm, param, args.cpu_budget)
         cpu = {"value": n_s / dt / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": "%d of %d texels (every k-th 128-texel tile of the frame), %.1f s" % (n_s, n, dt),
@@ -389,7 +401,10 @@ def run_ours(args):
                          (RING, RING * 36 * n / 1e6, info.table_bytes / 2 ** 20),
                    "grid": "%d CTAs = %d SMs x %d, %d texels per tile" % (info.num_sms * info.ctas_per_sm,
                                                                          info.num_sms, info.ctas_per_sm,
-                                                                         info.tile_texels)},
+                                                                         info.tile_texels),
+                   **({"texel_params": "device timing through niv_infer_texel_params, t = %s + 0.25 i/n per texel; "
+                                       "e2e stays the per-call entry point; no cpu_baseline on this line" % list(param)}
+                      if d_tp is not None else {})},
         "active_gqueries_per_s": value * (1.0 - masked),
         "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": e2e_ms, "steps": e2e_steps,
                 "h2d_bytes_per_step": 24 * n, "d2h_bytes_per_step": 12 * n,
@@ -519,6 +534,8 @@ def main():
     ap.add_argument("--paper-width", type=int, default=64, choices=[16, 32, 64])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--compose", action="store_true", help="SURVEY 8(f2): time the compose kernel (HBM roofline)")
+    ap.add_argument("--texel-params", action="store_true",
+                    help="--workload param only: time niv_infer_texel_params (one scene parameter value per texel, SURVEY 8 f3)")
     ap.add_argument("--half", action="store_true", help="quarter pixel count: a 960x540 G-buffer (PAPER.md:405, Table 1 'half')")
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[4]: table-size / width / resolution sweep")
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle wall time for cpu_baseline")

@@ -120,6 +120,19 @@ int niv_load_params(niv_model *m, const void *table_fp16, size_t table_bytes,
 int niv_infer(niv_model *m, const float *pos, const float *nrm, const float *param,
               float *out, size_t n, void *stream);
 
+/* the hot path with scene parameters PER TEXEL -- several frames with different t in one call, or a
+ * parameter that varies over the image.  The paper extends the field "by introducing new inputs to the model, e.g. the
+ * current position of the moving emitters" and frequency-encodes them; here the input of
+ * texel i is [latents | SH-16 | gamma(tparam[i][0]) | gamma(tparam[i][1])], gamma(t) = (sin, cos)(2^k pi t), k = 0..7.
+ *   pos, nrm, out  device, as niv_infer
+ *   tparam         DEVICE, [n][n_params] fp32 packed (borrowed for the duration of the launch)
+ * The encoding enters the first layer as 16 fp16 columns per parameter (one more tensor-core K-step each), where
+ * niv_infer folds it into the bias in fp32: with the same t in every row the two calls agree to the fp16 rounding of
+ * gamma, ~1e-4 in irradiance.  Models: n_params 1 or 2, F = 2 with SH-16, 8 or 16 levels, hidden width 32 or 64
+ * (else NIV_ERR_UNSUPPORTED); n_params == 0 -> NIV_ERR_INVALID_ARG.  Other errors and masking as niv_infer. */
+int niv_infer_texel_params(niv_model *m, const float *pos, const float *nrm, const float *tparam,
+                           float *out, size_t n, void *stream);
+
 /* The same operation with HOST buffers (the end-to-end call: PAPER.md:402-403 with the G-buffer in host memory).
  *   pos, nrm, out  HOST, [n][3] fp32 packed (pinned memory gives asynchronous copies; pageable memory works)
  *   param          HOST, as niv_infer

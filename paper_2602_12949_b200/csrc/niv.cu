@@ -235,13 +235,18 @@ __global__ void __launch_bounds__(kTile) niv_fused_kernel(const __grid_constant_
 // Here thread t keeps row t of the A operand in TMEM lane t: tcgen05.st instead of STS (no L1TEX wavefronts,
 // no generic->async proxy fence), tcgen05.mma reads A from TMEM, and shared memory holds the weights only.
 // TMEM columns per CTA (128 allocated): D [0, WIDTH) fp32 | A [64, 96) packed fp16 pairs | ones [96, 104).
-template <int WIDTH, int L, int NB, int F, bool RAWDIR, bool OUT128 = false>
+// NPT > 0: every texel carries its own NPT scene parameters (P.tparam [n][NPT]); their sin/cos encoding
+// becomes 16 * NPT more columns of the layer-1 A row (K1 grows by one K-step per parameter) instead of the per-call
+// fold into the bias row.  TMEM columns then: A [64, 96 + 8 (NPT - 1)), ones behind it.
+template <int WIDTH, int L, int NB, int F, bool RAWDIR, bool OUT128 = false, int NPT = 0>
 #ifdef NIV_EXPERIMENT_V2_MINB          // timing experiment only: another register budget for the v2 kernel
 __global__ void __launch_bounds__(kTile, NIV_EXPERIMENT_V2_MINB) niv_fused_tmem_kernel(
 #else
 // width 32 with 16 levels would take 130 registers (3 CTAs per SM): capped at 128; width 64 is left alone, the cap
-// changes its schedule for the worse (0.193 instead of 0.189 ms, profiles/r01_v2.md)
-__global__ void __launch_bounds__(kTile, WIDTH == 32 ? 4 : 0) niv_fused_tmem_kernel(
+// changes its schedule for the worse (0.193 instead of 0.189 ms, profiles/r01_v2.md); the per-texel-parameter
+// variants are capped too (two parameters at width 64 would take 140 registers; with one the capped schedule is the
+// faster one, 0.162 against 0.177 ms)
+__global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_fused_tmem_kernel(
 #endif
                                                                const __grid_constant__ KParams P,
                                                                const float* __restrict__ pos,
@@ -249,12 +254,14 @@ __global__ void __launch_bounds__(kTile, WIDTH == 32 ? 4 : 0) niv_fused_tmem_ker
                                                                float* __restrict__ out, size_t n, uint32_t n_tiles)
 {
     static_assert(WIDTH <= 64, "A-in-TMEM kernel: D + A + ones must fit 128 columns");
-    constexpr uint32_t TMEM_COLS = 128, A_COL = 64, ONES_COL = 96;
+    constexpr uint32_t TMEM_COLS = 128, A_COL = 64, ONES_COL = NPT == 2 ? 104 : 96;
     constexpr int NG = L / NB;
     constexpr int HW = L ? L * F / 2 : 24;            // 32-bit words of hash latents in one A row (L = 0: the
                                                       // 3 x 8 (sin, cos) pairs of the positional encoding)
     constexpr int DW = RAWDIR ? 2 : 8;                // ... of the direction input: (x, y | z, 0) or SH-16
-    constexpr int AW = (HW + DW + 7) / 8 * 8;         // ... of one layer-1 A row (K1 = 2 * AW)
+    constexpr int AW = (HW + DW + 7) / 8 * 8;         // ... of the position + direction part of a layer-1 A row
+    constexpr int AWT = AW + 8 * NPT;                 // ... of the whole row (K1 = 2 * AWT)
+    static_assert(AWT <= 40 && A_COL + AWT <= ONES_COL, "layer-1 A row must end before the ones chunk");
     extern __shared__ __align__(1024) uint8_t smem[];
     uint8_t* sW = smem;
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + P.misc_off);
@@ -292,7 +299,7 @@ __global__ void __launch_bounds__(kTile, WIDTH == 32 ? 4 : 0) niv_fused_tmem_ker
     mbar_wait(bar_w, 0);
 
     // ---- a8: fold the per-call parameter encoding into layer 1's bias K-row (hi, lo) in shared memory
-    if (P.n_params != 0 && tid < WIDTH) {
+    if (NPT == 0 && P.n_params != 0 && tid < WIDTH) {
         float b = reinterpret_cast<const float*>(sW + P.b_off[0])[tid];
         const uint32_t np16 = 16 * P.n_params;
         for (uint32_t q = 0; q < P.n_params; ++q) {
@@ -311,7 +318,7 @@ __global__ void __launch_bounds__(kTile, WIDTH == 32 ? 4 : 0) niv_fused_tmem_ker
 
     // shared-memory descriptor (low half) of every layer's B operand at K-step 0: (address >> 4) | (N * 16 >> 4) << 16,
     // the high half is the constant 0x4008 = SBO 128 B >> 4 | descriptor version 1 << 14 (niv_tc.cuh make_smem_desc)
-    constexpr uint32_t K1 = 2 * AW;
+    constexpr uint32_t K1 = 2 * AWT;
     const uint32_t n_layers = P.n_layers;
     uint32_t desc_lo0[kMaxLayers];
 #pragma unroll
@@ -323,9 +330,12 @@ __global__ void __launch_bounds__(kTile, WIDTH == 32 ? 4 : 0) niv_fused_tmem_ker
     // G-buffer texel of the first tile; inside the loop the NEXT tile's texel is requested before the current
     // one is encoded, so its HBM latency hides under a whole tile of work (a1 prefetch)
     float pn[3] = {0.f, 0.f, 0.f}, nn[3] = {0.f, 0.f, 0.f};
+    float tn[NPT > 0 ? NPT : 1] = {0.f};              // per-texel scene parameters, prefetched like the G-buffer
     if ((size_t)blockIdx.x * kTile + tid < n) {
         load3(pos, (size_t)blockIdx.x * kTile + tid, pn);
         load3(nrm, (size_t)blockIdx.x * kTile + tid, nn);
+#pragma unroll
+        for (int q = 0; q < NPT; ++q) tn[q] = __ldg(P.tparam + ((size_t)blockIdx.x * kTile + tid) * NPT + q);
     }
     uint32_t tile = blockIdx.x, tnext = s_tile[0], it = 0;
 #ifdef NIV_EXPERIMENT_TIMING
@@ -339,6 +349,9 @@ __global__ void __launch_bounds__(kTile, WIDTH == 32 ? 4 : 0) niv_fused_tmem_ker
         const size_t i = (size_t)tile * kTile + tid;
         const bool valid = i < n;
         const float p[3] = {pn[0], pn[1], pn[2]}, nv[3] = {nn[0], nn[1], nn[2]};
+        float tv[NPT > 0 ? NPT : 1];
+#pragma unroll
+        for (int q = 0; q < NPT; ++q) tv[q] = tn[q];
         uint32_t tnn_mine = 0;
         if (tid == 0) tnn_mine = gridDim.x + atomicAdd(P.tile_ctr, 1u);       // the tile after next
         {
@@ -348,15 +361,17 @@ __global__ void __launch_bounds__(kTile, WIDTH == 32 ? 4 : 0) niv_fused_tmem_ker
             if (inext < n) {
                 load3(pos, inext, pn);
                 load3(nrm, inext, nn);
+#pragma unroll
+                for (int q = 0; q < NPT; ++q) tn[q] = __ldg(P.tparam + inext * NPT + q);
             }
         }
         const bool masked = !valid || texel_masked(p, nv);
 
         // ---- a2..a9: this thread's A row in registers.  Rows are independent in the GEMMs and masked rows are
         //      overwritten with zeros at the store, so a masked thread just passes zeros.
-        uint32_t a[AW];
+        uint32_t a[AWT];
 #pragma unroll
-        for (int k = 0; k < AW; ++k) a[k] = 0u;
+        for (int k = 0; k < AWT; ++k) a[k] = 0u;
         if (!masked) {
             float u[3];
             normalise(P, p, u);
@@ -387,6 +402,9 @@ __global__ void __launch_bounds__(kTile, WIDTH == 32 ? 4 : 0) niv_fused_tmem_ker
                     if (g + 1 < NG) batch_blend<NB, F>(bb, a + (g + 1) * NB * (F / 2));
                 }
             }
+            // a8 per texel: gamma(t) = (sin, cos)(2^k pi t), k = 0..7, as fp16 pairs
+#pragma unroll
+            for (int q = 0; q < NPT; ++q) param_encode8_packed(tv[q], a + AW + 8 * q);
         }
         NIV_TICK(0);                                  // encode
         __syncwarp();
@@ -394,6 +412,8 @@ __global__ void __launch_bounds__(kTile, WIDTH == 32 ? 4 : 0) niv_fused_tmem_ker
         else tmem_st_x16(lane_taddr + A_COL, a);
         if constexpr (AW == 24) tmem_st_x8(lane_taddr + A_COL + 16, a + 16);
         if constexpr (AW == 32) tmem_st_x16(lane_taddr + A_COL + 16, a + 16);
+        if constexpr (NPT >= 1) tmem_st_x8(lane_taddr + A_COL + AW, a + AW);
+        if constexpr (NPT == 2) tmem_st_x8(lane_taddr + A_COL + AW + 8, a + AW + 8);
         tmem_st_wait();
         if (tid == 0) s_tile[(it + 1) & 1] = tnn_mine;
         tc_fence_before_sync();
@@ -796,6 +816,12 @@ struct niv_model {
     void (*fused)(KParams, const float*, const float*, float*, size_t, uint32_t) = nullptr;
     void (*fused_host)(KParams, const float*, const float*, float*, size_t, uint32_t) = nullptr;   // 128-bit output stores
     uint32_t grid_host = 0;
+    // per-texel scene parameters (niv_infer_texel_params): a kernel whose layer 1 has the parameter columns as K-steps,
+    // with its own packed weights and shared-memory layout
+    void (*fused_tp)(KParams, const float*, const float*, float*, size_t, uint32_t) = nullptr;
+    KParams kp_tp;
+    uint8_t* d_wpack_tp = nullptr;
+    uint32_t grid_tp = 0, smem_tp = 0;
     bool mma_kernel = false;                       // NIV_KERNEL=6: the per-warp mma.sync A/B kernel (32-texel tiles)
     uint32_t* d_wmma = nullptr;
     uint32_t* d_ctr = nullptr;                     // kCtrSlots tile counters, 128 B apart; one per launch in flight
@@ -824,14 +850,16 @@ static uint32_t round_up(uint32_t v, uint32_t m) { return (v + m - 1) / m * m; }
 // Resident CTAs per SM from the kernel's own resource use.  (cudaOccupancyMaxActiveBlocksPerMultiprocessor
 // answers 1 for these kernels on sm_100a with driver 580 -- measured, see DESIGN.md section 6 -- so it is not used.)
 template <typename K>
-static int setup_kernel(niv_model* m, K kernel, int tmem_cols, const char* name, uint32_t* grid_out = nullptr) {
-    NIV_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)m->smem_fused));
+static int setup_kernel(niv_model* m, K kernel, int tmem_cols, const char* name, uint32_t* grid_out = nullptr,
+                        uint32_t smem_override = 0) {
+    const uint32_t smem_dyn = smem_override ? smem_override : m->smem_fused;
+    NIV_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_dyn));
     cudaFuncAttributes fa;
     NIV_CUDA(cudaFuncGetAttributes(&fa, kernel));
     cudaDeviceProp prop;
     NIV_CUDA(cudaGetDeviceProperties(&prop, m->cfg.device));
     const int regs_per_cta = ((fa.numRegs + 7) / 8 * 8) * kTile;
-    const int smem_per_cta = (int)round_up(m->smem_fused + (uint32_t)fa.sharedSizeBytes + (uint32_t)prop.reservedSharedMemPerBlock, 128);
+    const int smem_per_cta = (int)round_up(smem_dyn + (uint32_t)fa.sharedSizeBytes + (uint32_t)prop.reservedSharedMemPerBlock, 128);
     int blocks = prop.regsPerMultiprocessor / regs_per_cta;
     blocks = std::min(blocks, (int)prop.sharedMemPerMultiprocessor / smem_per_cta);
     blocks = std::min(blocks, prop.maxThreadsPerMultiProcessor / kTile);
@@ -910,6 +938,22 @@ static fused_fn pick_tmem(uint32_t W, uint32_t L, int nb, uint32_t F) {
     if (F == 4) return W == 32 ? pick_tmem_paper<32, O>(L) : W == 64 ? pick_tmem_paper<64, O>(L) : nullptr;
     if (W == 32) return pick_tmem_l<32, O>(L, nb);
     if (W == 64) return pick_tmem_l<64, O>(L, nb);
+    return nullptr;
+}
+
+// per-texel scene parameters: BASELINE.json's family (F = 2, SH-16), 8 or 16 levels, width 32 / 64, 1 or 2 parameters
+template <int W, int NPT>
+static fused_fn pick_tmem_tp_l(uint32_t L) {
+    switch (L) {
+        case 8:  return niv_fused_tmem_kernel<W, 8, 4, 2, false, false, NPT>;
+        case 16: return niv_fused_tmem_kernel<W, 16, 4, 2, false, false, NPT>;
+        default: return nullptr;
+    }
+}
+static fused_fn pick_tmem_tp(uint32_t W, uint32_t L, uint32_t F, uint32_t sh_degree, uint32_t n_params) {
+    if (F != 2 || sh_degree != 4) return nullptr;
+    if (n_params == 1) return W == 32 ? pick_tmem_tp_l<32, 1>(L) : W == 64 ? pick_tmem_tp_l<64, 1>(L) : nullptr;
+    if (n_params == 2) return W == 32 ? pick_tmem_tp_l<32, 2>(L) : W == 64 ? pick_tmem_tp_l<64, 2>(L) : nullptr;
     return nullptr;
 }
 
@@ -1072,24 +1116,50 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
         if (rc == NIV_OK && m->fused_host && kind == 2 && W != 128 && !m->mma_kernel)
             rc = setup_kernel(m, m->fused_host, tmem_cols, "fused_v2_host", &m->grid_host);
         else m->fused_host = nullptr;
+        if (rc == NIV_OK && cfg->n_params && kind == 2 && W != 128)
+            m->fused_tp = pick_tmem_tp(W, cfg->n_levels, cfg->n_features, cfg->sh_degree, cfg->n_params);
+        if (m->fused_tp) {
+            // layout of the per-texel-parameter variant: layer 1 with K = round16(enc_dim) + 16 n_params, no fold blob
+            KParams& T = m->kp_tp;
+            T = P;
+            uint32_t o2 = 0;
+            for (uint32_t k = 0; k < P.n_layers; ++k) {
+                if (k == 0) T.kdim[0] = round_up(P.enc_dim, 16) + 16 * cfg->n_params;
+                T.w_off[k] = o2;
+                o2 += (T.kdim[k] + 16) * T.npad[k] * 2;
+            }
+            for (uint32_t k = 0; k < P.n_layers; ++k) { T.b_off[k] = o2; o2 += T.npad[k] * 4; }
+            T.wparam_off = o2;
+            T.wpack_bytes = round_up(o2, 16);
+            T.a_off = round_up(T.wpack_bytes, 128);
+            T.misc_off = T.a_off;
+            m->smem_tp = T.a_off + 64 + 4 * 384;
+            rc = setup_kernel(m, m->fused_tp, 128, "fused_v2_texel_params", &m->grid_tp, m->smem_tp);
+        }
     }
     if (rc != NIV_OK) { delete m; return rc; }
     e = cudaMalloc(&m->d_table, I.table_bytes ? I.table_bytes : 16);
     if (e == cudaSuccess) e = cudaMalloc(&m->d_wpack, P.wpack_bytes);
+    if (e == cudaSuccess && m->fused_tp) e = cudaMalloc(&m->d_wpack_tp, m->kp_tp.wpack_bytes);
     if (e == cudaSuccess) e = cudaMalloc(&m->d_ctr, kCtrSlots * 128);
     if (e == cudaSuccess) e = cudaMemset(m->d_ctr, 0, kCtrSlots * 128);
     if (e != cudaSuccess) {
         g_last_cuda_error = (int)e; (void)cudaGetLastError();
-        cudaFree(m->d_table); cudaFree(m->d_wpack); cudaFree(m->d_ctr); delete m;
+        cudaFree(m->d_table); cudaFree(m->d_wpack); cudaFree(m->d_wpack_tp); cudaFree(m->d_ctr); delete m;
         return NIV_ERR_ALLOC;
     }
     P.table = m->d_table;
     P.wpack = m->d_wpack;
+    m->kp_tp.table = m->d_table;
+    m->kp_tp.wpack = m->d_wpack_tp;
 #ifdef NIV_EXPERIMENT_TIMING
     cudaMalloc(&P.dbg, 8 * sizeof(unsigned long long));
     cudaMemset(P.dbg, 0, 8 * sizeof(unsigned long long));
 #endif
-    for (uint32_t l = 0; l < cfg->n_levels; ++l) P.lv[l].tb = m->d_table + (size_t)P.lv[l].base * (cfg->n_features / 2);
+    for (uint32_t l = 0; l < cfg->n_levels; ++l) {
+        P.lv[l].tb = m->d_table + (size_t)P.lv[l].base * (cfg->n_features / 2);
+        m->kp_tp.lv[l].tb = P.lv[l].tb;
+    }
     *out = m;
     return NIV_OK;
 }
@@ -1126,6 +1196,8 @@ extern "C" int niv_load_params(niv_model* m, const void* table_fp16, size_t tabl
 
     // pack: per layer, the UMMA K-major no-swizzle layout of B = W[out][in]:
     //   element (n, k) at  (k/8) * (Npad*16) + n*16 + (k%8)*2  bytes; rows n >= out and columns k >= in are zero.
+    //   texel_params: layer 1 keeps its parameter columns, as K rows round16(enc_dim) .. + 16 n_params (kp_tp layout)
+    auto pack_blob = [&](const KParams& P, bool texel_params) {
     std::vector<uint8_t> pack(P.wpack_bytes, 0);
     size_t wsrc = 0, bsrc = 0;
     for (uint32_t k = 0; k < P.n_layers; ++k) {
@@ -1135,7 +1207,12 @@ extern "C" int niv_load_params(niv_model* m, const void* table_fp16, size_t tabl
         for (uint32_t r = 0; r < o; ++r)
             for (uint32_t c = 0; c < kuse; ++c)
                 dst[(size_t)(c >> 3) * (P.npad[k] * 8) + r * 8 + (c & 7)] = w[wsrc + (size_t)r * in + c];
-        if (k == 0 && P.n_params) {
+        if (k == 0 && texel_params) {
+            const uint32_t k0 = round_up(P.enc_dim, 16);
+            for (uint32_t r = 0; r < o; ++r)
+                for (uint32_t c = 0; c < 16 * P.n_params; ++c)
+                    dst[(size_t)((k0 + c) >> 3) * (P.npad[k] * 8) + r * 8 + ((k0 + c) & 7)] = w[wsrc + (size_t)r * in + P.enc_dim + c];
+        } else if (k == 0 && P.n_params) {
             float* wp = reinterpret_cast<float*>(pack.data() + P.wparam_off);
             const uint32_t np16 = 16 * P.n_params;
             for (uint32_t r = 0; r < o; ++r)
@@ -1157,7 +1234,15 @@ extern "C" int niv_load_params(niv_model* m, const void* table_fp16, size_t tabl
         wsrc += (size_t)o * in;
         bsrc += o;
     }
+    return pack;
+    };
+    const std::vector<uint8_t> pack = pack_blob(P, false);
     NIV_CUDA(cudaMemcpyAsync(m->d_wpack, pack.data(), P.wpack_bytes, cudaMemcpyHostToDevice, st));
+    std::vector<uint8_t> pack_tp;                       // (alive until the stream is synchronised below)
+    if (m->fused_tp) {
+        pack_tp = pack_blob(m->kp_tp, true);
+        NIV_CUDA(cudaMemcpyAsync(m->d_wpack_tp, pack_tp.data(), m->kp_tp.wpack_bytes, cudaMemcpyHostToDevice, st));
+    }
     std::vector<uint32_t> wm;
     if (m->mma_kernel) {                                // row-major padded weights + fp32 biases (niv_fused_mma.cuh)
         wm.assign(kMmaWords, 0u);
@@ -1227,6 +1312,26 @@ extern "C" int niv_infer(niv_model* m, const float* pos, const float* nrm, const
     int rc = fill_params(m, param, P);
     if (rc != NIV_OK) return rc;
     return launch_fused(m, P, pos, nrm, out, n, (cudaStream_t)stream);
+}
+
+extern "C" int niv_infer_texel_params(niv_model* m, const float* pos, const float* nrm, const float* tparam,
+                                      float* out, size_t n, void* stream)
+{
+    if (!m) return NIV_ERR_INVALID_ARG;
+    if (!m->loaded) return NIV_ERR_NOT_LOADED;
+    if (m->cfg.n_params == 0) return NIV_ERR_INVALID_ARG;
+    if (!m->fused_tp) return NIV_ERR_UNSUPPORTED;
+    if (n == 0) return NIV_OK;
+    if (!pos || !nrm || !tparam || !out) return NIV_ERR_INVALID_ARG;
+    if (n > ((size_t)1 << 31)) return NIV_ERR_INVALID_ARG;
+    KParams P = m->kp_tp;
+    P.tparam = tparam;
+    P.tile_ctr = m->d_ctr + (size_t)(m->ctr_next.fetch_add(1u) % kCtrSlots) * 32;
+    const uint32_t n_tiles = (uint32_t)((n + kTile - 1) / kTile);
+    const uint32_t grid = n_tiles < m->grid_tp ? n_tiles : m->grid_tp;
+    m->fused_tp<<<grid, kTile, m->smem_tp, (cudaStream_t)stream>>>(P, pos, nrm, out, n, n_tiles);
+    NIV_CUDA(cudaGetLastError());
+    return NIV_OK;
 }
 
 extern "C" int niv_infer_host(niv_model* m, const float* pos, const float* nrm, const float* param,
@@ -1387,6 +1492,7 @@ extern "C" int niv_destroy(niv_model* m)
 #endif
     cudaFree(m->d_table);
     cudaFree(m->d_wpack);
+    cudaFree(m->d_wpack_tp);
     cudaFree(m->d_ctr);
     cudaFree(m->d_wmma);
     cudaFree(m->d_stage);

@@ -52,6 +52,7 @@ struct KParams {
     uint32_t ones_off;          // byte offset of the constant "ones" A chunk of the bias K-step (v1 kernel)
     uint32_t misc_off;          // byte offset of folded bias / barriers
     const uint32_t* wmma;       // weights in the layout of the mma.sync A/B kernel (niv_fused_mma.cuh), else NULL
+    const float* tparam;        // per-texel scene parameters [n][n_params] (niv_infer_texel_params), else NULL
 };
 
 // ---------------------------------------------------------------- O0: background / non-finite mask
@@ -263,6 +264,11 @@ __device__ __forceinline__ void param_encode8(float t, float o[16]) {
         o[2 * k + 1] = c;
     }
 }
+
+// the same values as fp16 pairs (sin, cos) per band: one A-row chunk of 8 words (per-texel parameters)
+// One sincospif and seven angle doublings (as the positional encoding above): the doubling error, < 2^7 * 2^-23 = 1.5e-5,
+// is far below the fp16 rounding of the stored value (2.4e-4 at |v| ~ 1); 22 instead of ~90 instructions per parameter.
+__device__ __forceinline__ void param_encode8_packed(float t, uint32_t o[8]) { posenc8_packed(t, o); }
 
 __device__ __forceinline__ void load3(const float* __restrict__ p, size_t i, float v[3]) {
     v[0] = __ldg(p + 3 * i);

@@ -24,7 +24,8 @@ NIV_OUT_LINEAR = 0
 NIV_OUT_SIGMOID = 1
 
 # every symbol include/niv.h declares (tests check that the library exports all of them)
-EXPORTS = ("niv_create", "niv_get_info", "niv_load_params", "niv_infer", "niv_infer_host", "niv_encode",
+EXPORTS = ("niv_create", "niv_get_info", "niv_load_params", "niv_infer", "niv_infer_texel_params", "niv_infer_host",
+           "niv_encode",
            "niv_debug_encode", "niv_compose", "niv_destroy", "niv_error_string", "niv_last_cuda_error", "niv_probe_gather",
            "niv_probe_sectors")
 
@@ -78,6 +79,7 @@ def lib():
         L.niv_load_params.argtypes = [vp, vp, sz, vp, sz, vp, sz, C.c_int, vp]
         L.niv_infer.argtypes = [vp, vp, vp, C.POINTER(C.c_float), vp, sz, vp]
         L.niv_infer_host.argtypes = [vp, vp, vp, C.POINTER(C.c_float), vp, sz, vp]
+        L.niv_infer_texel_params.argtypes = [vp, vp, vp, vp, vp, sz, vp]
         L.niv_encode.argtypes = [vp, vp, vp, C.POINTER(C.c_float), vp, sz, vp]
         L.niv_debug_encode.argtypes = [vp, vp, vp, C.POINTER(C.c_float), sz, vp, vp, vp, vp, vp]
         L.niv_compose.argtypes = [vp, C.c_uint32, C.c_uint32, vp, vp, vp, vp, C.c_uint32, C.c_uint32, vp]
@@ -201,6 +203,18 @@ class NivModel:
                              _dev(out, torch.float32, "out", 3) if n else None, n, _stream_ptr(stream))
         if rc != NIV_OK:
             raise NivError(rc, "niv_infer")
+        return out
+
+    def infer_texel_params(self, pos, nrm, tparam, out, stream=None):
+        """as infer(), every texel with its own scene parameters; tparam device [n][n_params] fp32."""
+        import torch
+        n = pos.shape[0]
+        rc = lib().niv_infer_texel_params(self._h, _dev(pos, torch.float32, "pos", 3) if n else None,
+                                          _dev(nrm, torch.float32, "nrm", 3) if n else None,
+                                          _dev(tparam, torch.float32, "tparam", self.spec.n_params) if n else None,
+                                          _dev(out, torch.float32, "out", 3) if n else None, n, _stream_ptr(stream))
+        if rc != NIV_OK:
+            raise NivError(rc, "niv_infer_texel_params")
         return out
 
     def infer_host(self, pos, nrm, out, param=None, stream=None):

@@ -191,6 +191,57 @@ def test_two_parameters(torch_cuda, niv, oracle):
 
 
 # ------------------------------------------------------------------------------------------------------
+# scene parameters per texel (several frames with different t in one call)
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n_params,width,L", [(1, 64, 16), (2, 64, 16), (1, 32, 16), (2, 32, 8), (1, 64, 8)])
+def test_texel_params_parity(torch_cuda, niv, oracle, n_params, width, L):
+    torch = torch_cuda
+    spec = dataclasses.replace(I.spec_param(), n_params=n_params, hidden_width=width, n_levels=L, log2_table_size=16)
+    case = Case(spec, 31 + n_params + width, bias_scale=0.1)
+    n = 3 * 4000 + 77                                  # three "frames" with their own t, and a ragged tail
+    pos, nrm = _queries(spec, n, 23, coherent=True)
+    nrm[5] = 0.0                                       # background texels keep (0, 0, 0)
+    pos[130, 2] = np.nan
+    tp = np.zeros((n, n_params), dtype=np.float32)
+    for f, t in enumerate((0.125, 0.37, 0.93)):
+        tp[f * 4000:(f + 1) * 4000] = t + 0.01 * np.arange(n_params, dtype=np.float32)
+    tp[12000:] = I.uniform01(5, 9, (n - 12000) * n_params).astype(np.float32).reshape(-1, n_params)   # varies per texel
+    m = case.gpu_model(niv)
+    dp, dn, dt = (torch.from_numpy(a).cuda() for a in (pos, nrm, tp))
+    out = torch.full((n, 3), float("nan"), dtype=torch.float32, device="cuda")
+    m.infer_texel_params(dp, dn, dt, out)
+    torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    want = oracle.infer_texel_params(spec, case.table, case.wblob, case.bblob, pos, nrm, tp)
+    _check_irradiance(got, want, nrm, pos)
+    # a frame's slice agrees with the per-call entry point (fp32 fold) to the fp16 rounding of the encoding
+    ref = torch.full((4000, 3), float("nan"), dtype=torch.float32, device="cuda")
+    m.infer(dp[4000:8000].contiguous(), dn[4000:8000].contiguous(), ref, param=[float(v) for v in tp[4000]])
+    torch.cuda.synchronize()
+    assert np.abs(ref.cpu().numpy() - got[4000:8000]).max() <= MAX_ABS
+    # the same launch twice: identical bits
+    out2 = torch.full((n, 3), float("nan"), dtype=torch.float32, device="cuda")
+    m.infer_texel_params(dp, dn, dt, out2)
+    torch.cuda.synchronize()
+    assert torch.equal(out, out2)
+    m.close()
+
+
+def test_texel_params_error_codes(torch_cuda, niv):
+    torch = torch_cuda
+    z = torch.zeros((4, 3), dtype=torch.float32, device="cuda")
+    m0 = Case(I.spec_fullhd(14), 1).gpu_model(niv)     # a model without scene parameters
+    rc = niv.lib().niv_infer_texel_params(m0._h, z.data_ptr(), z.data_ptr(), z.data_ptr(), z.data_ptr(), 4, None)
+    assert rc == niv.NIV_ERR_INVALID_ARG
+    m0.close()
+    spec = dataclasses.replace(I.spec_param(), hidden_width=128, log2_table_size=14)   # no per-texel kernel at width 128
+    m1 = Case(spec, 1).gpu_model(niv)
+    rc = niv.lib().niv_infer_texel_params(m1._h, z.data_ptr(), z.data_ptr(), z.data_ptr(), z.data_ptr(), 4, None)
+    assert rc == niv.NIV_ERR_UNSUPPORTED
+    m1.close()
+
+
+# ------------------------------------------------------------------------------------------------------
 # the paper's own model family: F = 4, sqrt(2) levels, raw direction, four weight matrices, linear output
 # ------------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("L,width", [(8, 64), (6, 64), (4, 32), (2, 64), (8, 32)])
