@@ -18,7 +18,10 @@
  *   - niv_infer / niv_encode / niv_debug_encode are asynchronous on `stream`, allocate nothing, never
  *     synchronise (CUDA-graph capturable), are read-only on the model's parameters and safe for concurrent callers
  *     on different streams (niv_infer draws one of 64 per-launch tile counters round robin, which the kernel
- *     itself leaves zeroed: up to 64 launches of one model may be in flight at once);
+ *     itself leaves zeroed: up to 64 launches of one model may be in flight at once; a launch recorded into a CUDA
+ *     graph keeps, for all its replays, one of 64 further counters that live launches never use, so up to 64 captured
+ *     launches per model may replay concurrently with each other and with live launches; replays of one graph are
+ *     serialised by CUDA itself);
  *   - there is no CPU fallback: without a CUDA device every entry point that needs one returns NIV_ERR_CUDA.
  */
 #ifndef NIV_H_

@@ -826,6 +826,7 @@ struct niv_model {
     uint32_t* d_wmma = nullptr;
     uint32_t* d_ctr = nullptr;                     // kCtrSlots tile counters, 128 B apart; one per launch in flight
     mutable std::atomic<uint32_t> ctr_next{0};
+    mutable std::atomic<uint32_t> ctr_next_captured{0};   // launches recorded into a CUDA graph draw from their own pool
     // niv_infer_host staging (grown on demand)
     float* d_stage = nullptr;          // [pos | nrm | out], each 3*stage_cap floats
     size_t stage_cap = 0;
@@ -1141,8 +1142,8 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     e = cudaMalloc(&m->d_table, I.table_bytes ? I.table_bytes : 16);
     if (e == cudaSuccess) e = cudaMalloc(&m->d_wpack, P.wpack_bytes);
     if (e == cudaSuccess && m->fused_tp) e = cudaMalloc(&m->d_wpack_tp, m->kp_tp.wpack_bytes);
-    if (e == cudaSuccess) e = cudaMalloc(&m->d_ctr, kCtrSlots * 128);
-    if (e == cudaSuccess) e = cudaMemset(m->d_ctr, 0, kCtrSlots * 128);
+    if (e == cudaSuccess) e = cudaMalloc(&m->d_ctr, 2 * kCtrSlots * 128);
+    if (e == cudaSuccess) e = cudaMemset(m->d_ctr, 0, 2 * kCtrSlots * 128);
     if (e != cudaSuccess) {
         g_last_cuda_error = (int)e; (void)cudaGetLastError();
         cudaFree(m->d_table); cudaFree(m->d_wpack); cudaFree(m->d_wpack_tp); cudaFree(m->d_ctr); delete m;
@@ -1280,11 +1281,24 @@ static int fill_params(const niv_model* m, const float* param, KParams& P)
     return NIV_OK;
 }
 
+// The tile counter of one launch.  A launch recorded into a CUDA graph keeps its slot for every replay, so captured
+// launches take theirs from a second pool of kCtrSlots that live launches never touch: a replay cannot meet a live
+// launch on the same counter.
+static uint32_t* draw_tile_counter(const niv_model* m, cudaStream_t st)
+{
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cs) != cudaSuccess) { (void)cudaGetLastError(); cs = cudaStreamCaptureStatusNone; }
+    const uint32_t slot = cs == cudaStreamCaptureStatusActive
+                              ? kCtrSlots + m->ctr_next_captured.fetch_add(1u) % kCtrSlots
+                              : m->ctr_next.fetch_add(1u) % kCtrSlots;
+    return m->d_ctr + (size_t)slot * 32;
+}
+
 static int launch_fused(const niv_model* m, const KParams& Pin, const float* pos, const float* nrm, float* out,
                         size_t n, cudaStream_t st, bool host_variant = false)
 {
     KParams P = Pin;
-    P.tile_ctr = m->d_ctr + (size_t)(m->ctr_next.fetch_add(1u) % kCtrSlots) * 32;
+    P.tile_ctr = draw_tile_counter(m, st);
     // (no memset: the kernels leave their counter pair zero, see the end of niv_fused_tmem_kernel)
     if (m->mma_kernel) {                                // warp-granular 32-texel tiles, four per CTA
         const uint32_t nt32 = (uint32_t)((n + 31) / 32), ctas = (nt32 + 3) / 4;
@@ -1326,7 +1340,7 @@ extern "C" int niv_infer_texel_params(niv_model* m, const float* pos, const floa
     if (n > ((size_t)1 << 31)) return NIV_ERR_INVALID_ARG;
     KParams P = m->kp_tp;
     P.tparam = tparam;
-    P.tile_ctr = m->d_ctr + (size_t)(m->ctr_next.fetch_add(1u) % kCtrSlots) * 32;
+    P.tile_ctr = draw_tile_counter(m, (cudaStream_t)stream);
     const uint32_t n_tiles = (uint32_t)((n + kTile - 1) / kTile);
     const uint32_t grid = n_tiles < m->grid_tp ? n_tiles : m->grid_tp;
     m->fused_tp<<<grid, kTile, m->smem_tp, (cudaStream_t)stream>>>(P, pos, nrm, out, n, n_tiles);

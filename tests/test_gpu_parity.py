@@ -437,6 +437,20 @@ def test_device_resident_params_and_determinism(torch_cuda, niv, oracle):
     g.replay()
     torch.cuda.synchronize()
     assert np.array_equal(out.cpu().numpy(), a)
+    # replays of the graph next to more live launches than there are live tile counters (64): the captured launch
+    # has a counter of its own, so neither side loses or repeats a tile
+    s2 = torch.cuda.Stream()
+    big_p, big_n = dp.repeat(8, 1).contiguous(), dn.repeat(8, 1).contiguous()
+    live = torch.zeros((400000, 3), dtype=torch.float32, device="cuda")
+    torch.cuda.synchronize()
+    for r in range(70):
+        m.infer(big_p, big_n, live, stream=s2)
+        if r % 7 == 0:
+            out.zero_()
+            g.replay()
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy(), a)
+    assert np.array_equal(live.cpu().numpy(), np.tile(a, (8, 1)))
     m.close()
 
 
