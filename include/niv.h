@@ -22,6 +22,10 @@
  *     graph keeps, for all its replays, one of 64 further counters that live launches never use, so up to 64 captured
  *     launches per model may replay concurrently with each other and with live launches; replays of one graph are
  *     serialised by CUDA itself);
+ *   - the fused kernels of hidden width <= 64 are launched with programmatic stream serialisation: their prologue
+ *     (model-owned memory only) may overlap the tail of the previous kernel of the stream, and they wait for that
+ *     kernel's completion (griddepcontrol.wait) before the first access to any buffer of the caller, so stream order
+ *     holds for every buffer passed in; NIV_PDL=0 in the environment at niv_create turns this off;
  *   - there is no CPU fallback: without a CUDA device every entry point that needs one returns NIV_ERR_CUDA.
  */
 #ifndef NIV_H_

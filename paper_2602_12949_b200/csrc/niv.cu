@@ -327,6 +327,12 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
         desc_lo0[l] = (((sW_u32 + P.w_off[l]) & 0x3FFFFu) >> 4) | (N << 16);
     }
     uint32_t phase = 0;
+    // Programmatic dependent launch (launch_fused sets the stream-serialisation attribute): everything above touches
+    // only the model's own memory, so this launch's CTAs may take the place of the previous launch's as those drain,
+    // with TMEM allocated and weights staged; from here on the caller's buffers are read and written, which needs the
+    // previous kernel of the stream complete.  The next launch may start filling in behind this one right away.
+    pdl_launch_dependents();
+    pdl_wait();
     // G-buffer texel of the first tile; inside the loop the NEXT tile's texel is requested before the current
     // one is encoded, so its HBM latency hides under a whole tile of work (a1 prefetch)
     float pn[3] = {0.f, 0.f, 0.f}, nn[3] = {0.f, 0.f, 0.f};
@@ -826,6 +832,7 @@ struct niv_model {
     uint32_t* d_wmma = nullptr;
     uint32_t* d_ctr = nullptr;                     // kCtrSlots tile counters, 128 B apart; one per launch in flight
     mutable std::atomic<uint32_t> ctr_next{0};
+    bool pdl = true;                               // NIV_PDL=0: launch without programmatic stream serialisation (A/B knob)
     mutable std::atomic<uint32_t> ctr_next_captured{0};   // launches recorded into a CUDA graph draw from their own pool
     // niv_infer_host staging (grown on demand)
     float* d_stage = nullptr;          // [pos | nrm | out], each 3*stage_cap floats
@@ -1076,6 +1083,7 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     if (prop.major != 10) { delete m; return NIV_ERR_UNSUPPORTED; }           // sm_100a only; no fallback
     I.num_sms = (uint32_t)prop.multiProcessorCount;
     {
+        if (const char* pv = getenv("NIV_PDL")) m->pdl = atoi(pv) != 0;
         const char* kv = getenv("NIV_KERNEL");          // A-B knob: 1 = v1 (A operand in shared memory), 2 = v2 (A in TMEM)
         const char* nbv = getenv("NIV_NB");             // levels per gather batch: 2 or 4
         const int nb = nbv ? atoi(nbv) : 4;
@@ -1294,6 +1302,26 @@ static uint32_t* draw_tile_counter(const niv_model* m, cudaStream_t st)
     return m->d_ctr + (size_t)slot * 32;
 }
 
+// One launch of a fused kernel; `pdl`: with the programmatic-stream-serialisation attribute (v2 kernels, which hold
+// their griddepcontrol.wait before the first access to a caller's buffer).
+static int launch_v2(fused_fn fn, uint32_t grid, uint32_t smem, cudaStream_t st, bool pdl, const KParams& P,
+                     const float* pos, const float* nrm, float* out, size_t n, uint32_t n_tiles)
+{
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(kTile);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = pdl ? 1 : 0;
+    NIV_CUDA(cudaLaunchKernelEx(&cfg, fn, P, pos, nrm, out, n, n_tiles));
+    return NIV_OK;
+}
+
 static int launch_fused(const niv_model* m, const KParams& Pin, const float* pos, const float* nrm, float* out,
                         size_t n, cudaStream_t st, bool host_variant = false)
 {
@@ -1309,9 +1337,8 @@ static int launch_fused(const niv_model* m, const KParams& Pin, const float* pos
     const uint32_t n_tiles = (uint32_t)((n + kTile - 1) / kTile);
     const uint32_t cap = host_variant ? m->grid_host : m->grid_fused;
     const uint32_t grid = n_tiles < cap ? n_tiles : cap;
-    (host_variant ? m->fused_host : m->fused)<<<grid, kTile, m->smem_fused, st>>>(P, pos, nrm, out, n, n_tiles);
-    NIV_CUDA(cudaGetLastError());
-    return NIV_OK;
+    return launch_v2(host_variant ? m->fused_host : m->fused, grid, m->smem_fused, st, m->pdl && m->fused_host, P, pos,
+                     nrm, out, n, n_tiles);
 }
 
 extern "C" int niv_infer(niv_model* m, const float* pos, const float* nrm, const float* param,
@@ -1343,9 +1370,7 @@ extern "C" int niv_infer_texel_params(niv_model* m, const float* pos, const floa
     P.tile_ctr = draw_tile_counter(m, (cudaStream_t)stream);
     const uint32_t n_tiles = (uint32_t)((n + kTile - 1) / kTile);
     const uint32_t grid = n_tiles < m->grid_tp ? n_tiles : m->grid_tp;
-    m->fused_tp<<<grid, kTile, m->smem_tp, (cudaStream_t)stream>>>(P, pos, nrm, out, n, n_tiles);
-    NIV_CUDA(cudaGetLastError());
-    return NIV_OK;
+    return launch_v2(m->fused_tp, grid, m->smem_tp, (cudaStream_t)stream, m->pdl, P, pos, nrm, out, n, n_tiles);
 }
 
 extern "C" int niv_infer_host(niv_model* m, const float* pos, const float* nrm, const float* param,
