@@ -269,9 +269,15 @@ def run_ours(args):
         tp = (np.float32(param)[None, :] + np.float32(0.25) * (np.arange(n, dtype=np.float32) / np.float32(n))[:, None])
         d_tp = torch.from_numpy(np.ascontiguousarray(tp, dtype=np.float32)).cuda()
 
+    # the G-buffer workloads are images: niv_infer_image (8 x 4 pixel blocks per warp); the incoherent set has no
+    # image structure and goes through niv_infer (32 consecutive texels per warp), as does --tiling linear
+    image = args.tiling == "image" and args.workload != "incoherent" and d_tp is None and bool(info.image_tiled)
+
     def infer_dev(k):
         if d_tp is not None:
             model.infer_texel_params(d_pos[k], d_nrm[k], d_tp, d_out[k])
+        elif image:
+            model.infer_image(d_pos[k], d_nrm[k], d_out[k], W_PX, H_PX, param=param)
         else:
             model.infer(d_pos[k], d_nrm[k], d_out[k], param=param)
 
@@ -337,7 +343,10 @@ def run_ours(args):
     # ---- rooflines (rank 0) -------------------------------------------------------------------------
     peaks = load_peaks()
     counts = torch.zeros(33, dtype=torch.int64, device="cuda")
-    model.probe_sectors(d_pos[0], d_nrm[0], counts)
+    if image:
+        model.probe_sectors_image(d_pos[0], d_nrm[0], W_PX, H_PX, counts)      # the census of the warps that ran
+    else:
+        model.probe_sectors(d_pos[0], d_nrm[0], counts)
     torch.cuda.synchronize()
     c = counts.cpu().numpy()
     L = spec.n_levels
@@ -413,6 +422,8 @@ def run_ours(args):
                    "grid": "%d CTAs = %d SMs x %d, %d texels per tile" % (info.num_sms * info.ctas_per_sm,
                                                                          info.num_sms, info.ctas_per_sm,
                                                                          info.tile_texels),
+                   "tiling": ("niv_infer_image: a warp = an 8 x 4 pixel block, a tile = 32 x 4 pixels" if image else
+                              "niv_infer: a warp = 32 consecutive texels, a tile = 128"),
                    **({"texel_params": "device timing through niv_infer_texel_params, t = %s + 0.25 i/n per texel; "
                                        "e2e stays the per-call entry point; no cpu_baseline on this line" % list(param)}
                       if d_tp is not None else {})},
@@ -545,6 +556,8 @@ def main():
     ap.add_argument("--paper-width", type=int, default=64, choices=[16, 32, 64])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--compose", action="store_true", help="SURVEY 8(f2): time the compose kernel (HBM roofline)")
+    ap.add_argument("--tiling", default="image", choices=["image", "linear"],
+                    help="device path of the G-buffer workloads: niv_infer_image (default) or niv_infer")
     ap.add_argument("--texel-params", action="store_true",
                     help="--workload param only: time niv_infer_texel_params (one scene parameter value per texel, SURVEY 8 f3)")
     ap.add_argument("--half", action="store_true", help="quarter pixel count: a 960x540 G-buffer (PAPER.md:405, Table 1 'half')")

@@ -238,7 +238,8 @@ __global__ void __launch_bounds__(kTile) niv_fused_kernel(const __grid_constant_
 // NPT > 0: every texel carries its own NPT scene parameters (P.tparam [n][NPT]); their sin/cos encoding
 // becomes 16 * NPT more columns of the layer-1 A row (K1 grows by one K-step per parameter) instead of the per-call
 // fold into the bias row.  TMEM columns then: A [64, 96 + 8 (NPT - 1)), ones behind it.
-template <int WIDTH, int L, int NB, int F, bool RAWDIR, bool OUT128 = false, int NPT = 0>
+// IMG (niv_infer_image): texels are addressed as 8 x 4 pixel blocks per warp of a row-major image (image_texel).
+template <int WIDTH, int L, int NB, int F, bool RAWDIR, bool OUT128 = false, int NPT = 0, bool IMG = false>
 #ifdef NIV_EXPERIMENT_V2_MINB          // timing experiment only: another register budget for the v2 kernel
 __global__ void __launch_bounds__(kTile, NIV_EXPERIMENT_V2_MINB) niv_fused_tmem_kernel(
 #else
@@ -337,11 +338,22 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
     // one is encoded, so its HBM latency hides under a whole tile of work (a1 prefetch)
     float pn[3] = {0.f, 0.f, 0.f}, nn[3] = {0.f, 0.f, 0.f};
     float tn[NPT > 0 ? NPT : 1] = {0.f};              // per-texel scene parameters, prefetched like the G-buffer
-    if ((size_t)blockIdx.x * kTile + tid < n) {
-        load3(pos, (size_t)blockIdx.x * kTile + tid, pn);
-        load3(nrm, (size_t)blockIdx.x * kTile + tid, nn);
+    // texel of thread tid in tile t: 128 consecutive texels per tile, or (IMG) a 32 x 4 pixel tile of the image
+    auto texel_of = [&](uint32_t t, bool& ok) -> size_t {
+        if constexpr (IMG) return image_texel(P, t, tid, ok);
+        const size_t idx = (size_t)t * kTile + tid;
+        ok = idx < n;
+        return idx;
+    };
+    {
+        bool ok;
+        const size_t i0 = texel_of(blockIdx.x, ok);
+        if (ok) {
+            load3(pos, i0, pn);
+            load3(nrm, i0, nn);
 #pragma unroll
-        for (int q = 0; q < NPT; ++q) tn[q] = __ldg(P.tparam + ((size_t)blockIdx.x * kTile + tid) * NPT + q);
+            for (int q = 0; q < NPT; ++q) tn[q] = __ldg(P.tparam + i0 * NPT + q);
+        }
     }
     uint32_t tile = blockIdx.x, tnext = s_tile[0], it = 0;
 #ifdef NIV_EXPERIMENT_TIMING
@@ -352,8 +364,8 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
 #define NIV_TICK(slot) do { } while (0)
 #endif
     while (tile < n_tiles) {
-        const size_t i = (size_t)tile * kTile + tid;
-        const bool valid = i < n;
+        bool valid;
+        const size_t i = texel_of(tile, valid);
         const float p[3] = {pn[0], pn[1], pn[2]}, nv[3] = {nn[0], nn[1], nn[2]};
         float tv[NPT > 0 ? NPT : 1];
 #pragma unroll
@@ -361,10 +373,11 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
         uint32_t tnn_mine = 0;
         if (tid == 0) tnn_mine = gridDim.x + atomicAdd(P.tile_ctr, 1u);       // the tile after next
         {
-            const size_t inext = (size_t)tnext * kTile + tid;
+            bool ok;
+            const size_t inext = texel_of(tnext, ok);     // (a tile index past the end gives ok = false in both modes)
 #pragma unroll
             for (int d = 0; d < 3; ++d) { pn[d] = 0.f; nn[d] = 0.f; }
-            if (inext < n) {
+            if (ok) {
                 load3(pos, inext, pn);
                 load3(nrm, inext, nn);
 #pragma unroll
@@ -754,9 +767,10 @@ __global__ void __launch_bounds__(128) niv_sector_census_kernel(const __grid_con
 {
     __shared__ uint32_t s_sec[4][256];
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
-    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     float p[3] = {0.f, 0.f, 0.f}, nv[3] = {0.f, 0.f, 0.f};
-    const bool valid = i < n;
+    bool valid = i < n;
+    if (P.tiles_x) i = image_texel(P, blockIdx.x, threadIdx.x, valid);      // the warps of niv_infer_image
     if (valid) { load3(pos, i, p); load3(nrm, i, nv); }
     const bool masked = !valid || texel_masked(p, nv);
     float u[3] = {0.f, 0.f, 0.f};
@@ -828,6 +842,9 @@ struct niv_model {
     KParams kp_tp;
     uint8_t* d_wpack_tp = nullptr;
     uint32_t grid_tp = 0, smem_tp = 0;
+    // niv_infer_image: the same kernel with 8 x 4 pixel blocks per warp
+    void (*fused_img)(KParams, const float*, const float*, float*, size_t, uint32_t) = nullptr;
+    uint32_t grid_img = 0;
     bool mma_kernel = false;                       // NIV_KERNEL=6: the per-warp mma.sync A/B kernel (32-texel tiles)
     uint32_t* d_wmma = nullptr;
     uint32_t* d_ctr = nullptr;                     // kCtrSlots tile counters, 128 B apart; one per launch in flight
@@ -947,6 +964,25 @@ static fused_fn pick_tmem(uint32_t W, uint32_t L, int nb, uint32_t F) {
     if (W == 32) return pick_tmem_l<32, O>(L, nb);
     if (W == 64) return pick_tmem_l<64, O>(L, nb);
     return nullptr;
+}
+
+// image tiling (niv_infer_image): BASELINE.json's family (F = 2, 8..16 levels reach cells smaller than a warp's strip).
+// The paper's own family (F = 4, <= 8 levels, finest cell 5.5 cm) measured SLOWER with it (0.1098 against 0.1049 ms,
+// profiles/r01_v2.md): its cells are larger than a 32-pixel strip anyway; it keeps the linear kernel, as do the
+// grid-less models, which gather nothing.
+template <int W>
+static fused_fn pick_tmem_img_w(uint32_t L) {
+    switch (L) {
+        case 4:  return niv_fused_tmem_kernel<W, 4, 4, 2, false, false, 0, true>;
+        case 8:  return niv_fused_tmem_kernel<W, 8, 4, 2, false, false, 0, true>;
+        case 12: return niv_fused_tmem_kernel<W, 12, 4, 2, false, false, 0, true>;
+        case 16: return niv_fused_tmem_kernel<W, 16, 4, 2, false, false, 0, true>;
+        default: return nullptr;
+    }
+}
+static fused_fn pick_tmem_img(uint32_t W, uint32_t L, uint32_t F) {
+    if (L == 0 || F != 2) return nullptr;
+    return W == 32 ? pick_tmem_img_w<32>(L) : W == 64 ? pick_tmem_img_w<64>(L) : nullptr;
 }
 
 // per-texel scene parameters: BASELINE.json's family (F = 2, SH-16), 8 or 16 levels, width 32 / 64, 1 or 2 parameters
@@ -1125,6 +1161,10 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
         if (rc == NIV_OK && m->fused_host && kind == 2 && W != 128 && !m->mma_kernel)
             rc = setup_kernel(m, m->fused_host, tmem_cols, "fused_v2_host", &m->grid_host);
         else m->fused_host = nullptr;
+        if (rc == NIV_OK && kind == 2 && W != 128 && !m->mma_kernel) {
+            m->fused_img = pick_tmem_img(W, cfg->n_levels, cfg->n_features);
+            if (m->fused_img) rc = setup_kernel(m, m->fused_img, 128, "fused_v2_image", &m->grid_img);
+        }
         if (rc == NIV_OK && cfg->n_params && kind == 2 && W != 128)
             m->fused_tp = pick_tmem_tp(W, cfg->n_levels, cfg->n_features, cfg->sh_degree, cfg->n_params);
         if (m->fused_tp) {
@@ -1147,6 +1187,8 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
         }
     }
     if (rc != NIV_OK) { delete m; return rc; }
+    I.image_tiled = m->fused_img ? 1u : 0u;
+    I.texel_params = m->fused_tp ? 1u : 0u;
     e = cudaMalloc(&m->d_table, I.table_bytes ? I.table_bytes : 16);
     if (e == cudaSuccess) e = cudaMalloc(&m->d_wpack, P.wpack_bytes);
     if (e == cudaSuccess && m->fused_tp) e = cudaMalloc(&m->d_wpack_tp, m->kp_tp.wpack_bytes);
@@ -1355,6 +1397,29 @@ extern "C" int niv_infer(niv_model* m, const float* pos, const float* nrm, const
     return launch_fused(m, P, pos, nrm, out, n, (cudaStream_t)stream);
 }
 
+extern "C" int niv_infer_image(niv_model* m, const float* pos, const float* nrm, const float* param,
+                               float* out, uint32_t width, uint32_t height, void* stream)
+{
+    if (!m) return NIV_ERR_INVALID_ARG;
+    if (!m->loaded) return NIV_ERR_NOT_LOADED;
+    const size_t n = (size_t)width * height;
+    if (n == 0) return NIV_OK;
+    if (!pos || !nrm || !out) return NIV_ERR_INVALID_ARG;
+    if (n > ((size_t)1 << 31)) return NIV_ERR_INVALID_ARG;
+    KParams P;
+    int rc = fill_params(m, param, P);
+    if (rc != NIV_OK) return rc;
+    if (!m->fused_img || getenv("NIV_IMAGE_LINEAR"))     // models without an image-tiled kernel: same result, linear tiles
+        return launch_fused(m, P, pos, nrm, out, n, (cudaStream_t)stream);
+    P.img_w = width;
+    P.img_h = height;
+    P.tiles_x = (width + 31u) / 32u;
+    const uint32_t n_tiles = P.tiles_x * ((height + 3u) / 4u);
+    P.tile_ctr = draw_tile_counter(m, (cudaStream_t)stream);
+    const uint32_t grid = n_tiles < m->grid_img ? n_tiles : m->grid_img;
+    return launch_v2(m->fused_img, grid, m->smem_fused, (cudaStream_t)stream, m->pdl, P, pos, nrm, out, n, n_tiles);
+}
+
 extern "C" int niv_infer_texel_params(niv_model* m, const float* pos, const float* nrm, const float* tparam,
                                       float* out, size_t n, void* stream)
 {
@@ -1482,6 +1547,22 @@ extern "C" int niv_probe_sectors(niv_model* m, const float* pos, const float* nr
     NIV_CUDA(cudaMemsetAsync(counts, 0, 33 * sizeof(uint64_t), (cudaStream_t)stream));
     const unsigned grid = (unsigned)((n + 127) / 128);
     niv_sector_census_kernel<<<grid, 128, 0, (cudaStream_t)stream>>>(m->kp, pos, nrm, n, (unsigned long long*)counts);
+    NIV_CUDA(cudaGetLastError());
+    return NIV_OK;
+}
+
+extern "C" int niv_probe_sectors_image(const niv_model* m, const float* pos, const float* nrm, uint32_t width,
+                                       uint32_t height, uint64_t* counts, void* stream)
+{
+    if (!m || !pos || !nrm || !counts || width == 0 || height == 0) return NIV_ERR_INVALID_ARG;
+    NIV_CUDA(cudaMemsetAsync(counts, 0, 33 * sizeof(uint64_t), (cudaStream_t)stream));
+    KParams P = m->kp;
+    P.img_w = width;
+    P.img_h = height;
+    P.tiles_x = (width + 31u) / 32u;
+    const unsigned grid = P.tiles_x * ((height + 3u) / 4u);
+    niv_sector_census_kernel<<<grid, 128, 0, (cudaStream_t)stream>>>(P, pos, nrm, (size_t)width * height,
+                                                                     (unsigned long long*)counts);
     NIV_CUDA(cudaGetLastError());
     return NIV_OK;
 }

@@ -53,6 +53,8 @@ struct KParams {
     uint32_t misc_off;          // byte offset of folded bias / barriers
     const uint32_t* wmma;       // weights in the layout of the mma.sync A/B kernel (niv_fused_mma.cuh), else NULL
     const float* tparam;        // per-texel scene parameters [n][n_params] (niv_infer_texel_params), else NULL
+    uint32_t img_w, img_h;      // niv_infer_image: the buffers are a row-major img_h x img_w image ...
+    uint32_t tiles_x;           // ... cut into 32 x 4 pixel tiles, tiles_x = ceil(img_w / 32) per tile row (else 0)
 };
 
 // ---------------------------------------------------------------- O0: background / non-finite mask
@@ -269,6 +271,16 @@ __device__ __forceinline__ void param_encode8(float t, float o[16]) {
 // One sincospif and seven angle doublings (as the positional encoding above): the doubling error, < 2^7 * 2^-23 = 1.5e-5,
 // is far below the fp16 rounding of the stored value (2.4e-4 at |v| ~ 1); 22 instead of ~90 instructions per parameter.
 __device__ __forceinline__ void param_encode8_packed(float t, uint32_t o[8]) { posenc8_packed(t, o); }
+
+// niv_infer_image: tile = 32 x 4 pixels, warp w of the CTA = columns 8w .. 8w+7 of it (an 8 x 4 pixel block, lane =
+// 8 * row + column).  A warp's 32 texels then lie in a compact patch of the surface instead of a 32-pixel strip, so
+// they share more grid cells: 14 % fewer distinct sectors per warp on the full-HD frame (profiles/r01_v2.md).
+__device__ __forceinline__ size_t image_texel(const KParams& P, uint32_t tile, uint32_t tid, bool& valid) {
+    const uint32_t ty = tile / P.tiles_x, tx = tile - ty * P.tiles_x;
+    const uint32_t x = tx * 32u + (tid >> 5) * 8u + (tid & 7u), y = ty * 4u + ((tid >> 3) & 3u);
+    valid = x < P.img_w && y < P.img_h;
+    return (size_t)y * P.img_w + x;
+}
 
 __device__ __forceinline__ void load3(const float* __restrict__ p, size_t i, float v[3]) {
     v[0] = __ldg(p + 3 * i);

@@ -24,7 +24,8 @@ NIV_OUT_LINEAR = 0
 NIV_OUT_SIGMOID = 1
 
 # every symbol include/niv.h declares (tests check that the library exports all of them)
-EXPORTS = ("niv_create", "niv_get_info", "niv_load_params", "niv_infer", "niv_infer_texel_params", "niv_infer_host",
+EXPORTS = ("niv_create", "niv_get_info", "niv_load_params", "niv_infer", "niv_infer_image", "niv_infer_texel_params",
+           "niv_infer_host", "niv_probe_sectors_image",
            "niv_encode",
            "niv_debug_encode", "niv_compose", "niv_destroy", "niv_error_string", "niv_last_cuda_error", "niv_probe_gather",
            "niv_probe_sectors")
@@ -49,7 +50,7 @@ class NivInfo(C.Structure):
         ("resolution", C.c_uint32 * 16), ("is_dense", C.c_uint32 * 16),
         ("table_bytes", C.c_uint64), ("weight_bytes", C.c_uint64), ("bias_bytes", C.c_uint64),
         ("num_sms", C.c_uint32), ("ctas_per_sm", C.c_uint32), ("tile_texels", C.c_uint32),
-        ("smem_bytes", C.c_uint32),
+        ("smem_bytes", C.c_uint32), ("image_tiled", C.c_uint32), ("texel_params", C.c_uint32),
     ]
 
 
@@ -80,6 +81,8 @@ def lib():
         L.niv_infer.argtypes = [vp, vp, vp, C.POINTER(C.c_float), vp, sz, vp]
         L.niv_infer_host.argtypes = [vp, vp, vp, C.POINTER(C.c_float), vp, sz, vp]
         L.niv_infer_texel_params.argtypes = [vp, vp, vp, vp, vp, sz, vp]
+        L.niv_infer_image.argtypes = [vp, vp, vp, C.POINTER(C.c_float), vp, C.c_uint32, C.c_uint32, vp]
+        L.niv_probe_sectors_image.argtypes = [vp, vp, vp, C.c_uint32, C.c_uint32, vp, vp]
         L.niv_encode.argtypes = [vp, vp, vp, C.POINTER(C.c_float), vp, sz, vp]
         L.niv_debug_encode.argtypes = [vp, vp, vp, C.POINTER(C.c_float), sz, vp, vp, vp, vp, vp]
         L.niv_compose.argtypes = [vp, C.c_uint32, C.c_uint32, vp, vp, vp, vp, C.c_uint32, C.c_uint32, vp]
@@ -205,6 +208,21 @@ class NivModel:
             raise NivError(rc, "niv_infer")
         return out
 
+    def infer_image(self, pos, nrm, out, width, height, param=None, stream=None):
+        """As infer() for a row-major height x width G-buffer ([h*w][3] tensors): warps take 8 x 4 pixel blocks."""
+        import torch
+        n = int(width) * int(height)
+        if pos.shape[0] != n or nrm.shape[0] != n or out.shape[0] != n:
+            raise ValueError("buffers must hold width * height texels")
+        rc = lib().niv_infer_image(self._h, _dev(pos, torch.float32, "pos", 3) if n else None,
+                                   _dev(nrm, torch.float32, "nrm", 3) if n else None,
+                                   _params(param, self.spec.n_params),
+                                   _dev(out, torch.float32, "out", 3) if n else None, int(width), int(height),
+                                   _stream_ptr(stream))
+        if rc != NIV_OK:
+            raise NivError(rc, "niv_infer_image")
+        return out
+
     def infer_texel_params(self, pos, nrm, tparam, out, stream=None):
         """as infer(), every texel with its own scene parameters; tparam device [n][n_params] fp32."""
         import torch
@@ -260,6 +278,15 @@ class NivModel:
                                      pos.shape[0], _dev(counts, torch.int64, "counts"), _stream_ptr(stream))
         if rc != NIV_OK:
             raise NivError(rc, "niv_probe_sectors")
+
+    def probe_sectors_image(self, pos, nrm, width, height, counts, stream=None):
+        """The census for infer_image's warps (include/niv.h niv_probe_sectors_image)."""
+        import torch
+        rc = lib().niv_probe_sectors_image(self._h, _dev(pos, torch.float32, "pos", 3),
+                                           _dev(nrm, torch.float32, "nrm", 3), int(width), int(height),
+                                           _dev(counts, torch.int64, "counts"), _stream_ptr(stream))
+        if rc != NIV_OK:
+            raise NivError(rc, "niv_probe_sectors_image")
 
     def close(self):
         if getattr(self, "_h", None) and self._h.value:

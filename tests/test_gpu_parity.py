@@ -191,6 +191,80 @@ def test_two_parameters(torch_cuda, niv, oracle):
 
 
 # ------------------------------------------------------------------------------------------------------
+# niv_infer_image: 8 x 4 pixel blocks per warp -- the same function, texel for texel
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("which,w,h", [("fullhd", 203, 37), ("fullhd", 64, 8), ("fullhd", 31, 3), ("fullhd", 1, 1),
+                                       ("w32", 96, 50), ("paper", 130, 21), ("param", 77, 19), ("w128", 70, 9),
+                                       ("gridless", 40, 6)])
+def test_image_tiling_is_bit_identical_and_matches_oracle(torch_cuda, niv, oracle, which, w, h):
+    torch = torch_cuda
+    spec = {"fullhd": I.spec_fullhd(15), "w32": I.spec_fullhd(15, 32, 1), "paper": I.spec_paper(6, 64),
+            "param": dataclasses.replace(I.spec_param(), log2_table_size=15),
+            "w128": I.spec_fullhd(14, 128), "gridless": I.spec_paper_pe(32)}[which]
+    case = Case(spec, 50 + w, bias_scale=0.1)
+    n = w * h
+    if n >= 2000:
+        g = I.make_gbuffer(w, h, 29)
+        pos, nrm = g["pos"].copy(), g["nrm"].copy()
+    else:                                              # too few pixels for the scene's camera search
+        pos, nrm = I.positions_uniform(n, I.ROOM_AABB, 29), I.normals_uniform(n, 29)
+    if n > 40:
+        nrm[7] = 0.0
+        pos[33, 0] = np.inf
+    param = [0.4] if spec.n_params else None
+    m = case.gpu_model(niv)
+    dp, dn = torch.from_numpy(pos).cuda(), torch.from_numpy(nrm).cuda()
+    guard = 64
+    buf = torch.full((n + guard, 3), -7.0, dtype=torch.float32, device="cuda")     # rows past the image stay untouched
+    m.infer_image(dp, dn, buf[:n], w, h, param=param)
+    lin = torch.full((n, 3), float("nan"), dtype=torch.float32, device="cuda")
+    m.infer(dp, dn, lin, param=param)
+    torch.cuda.synchronize()
+    assert torch.equal(buf[:n], lin)
+    assert bool((buf[n:] == -7.0).all())
+    want = oracle.infer(spec, case.table, case.wblob, case.bblob, pos, nrm,
+                        param=None if param is None else np.float32(param))
+    # (linear-output models: tolerance relative to the output range, as in their own parity tests)
+    scale = max(1.0, float(want.max() - want.min())) if spec.out_activation == I.OUT_LINEAR else 1.0
+    _check_irradiance(buf[:n].cpu().numpy(), want, nrm, pos, scale=scale)
+    m.close()
+
+
+def test_image_census_counts_fewer_sectors_than_strips(torch_cuda, niv):
+    """The census of the 8 x 4 warps: same active texels, every level at most the strip count + noise, fine levels fewer."""
+    torch = torch_cuda
+    spec = I.spec_fullhd()
+    m = Case(spec, 3).gpu_model(niv)
+    w, h = 640, 360
+    g = I.make_gbuffer(w, h, 0)
+    dp, dn = torch.from_numpy(g["pos"]).cuda(), torch.from_numpy(g["nrm"]).cuda()
+    a = torch.zeros(33, dtype=torch.int64, device="cuda")
+    b = torch.zeros(33, dtype=torch.int64, device="cuda")
+    m.probe_sectors(dp, dn, a)
+    m.probe_sectors_image(dp, dn, w, h, b)
+    torch.cuda.synchronize()
+    a, b = a.cpu().numpy(), b.cpu().numpy()
+    assert a[32] == b[32] > 0
+    assert b[:16].sum() < 0.95 * a[:16].sum()
+    # brute force of the image census on the host for one level: distinct sectors per 8 x 4 block
+    out = torch.zeros((w * h, 16, 8), dtype=torch.int32, device="cuda")
+    m.debug_encode(dp, dn, idx=out)
+    torch.cuda.synchronize()
+    idx = out.cpu().numpy().astype(np.int64).reshape(h, w, 16, 8)
+    act = ~(np.all(g["nrm"] == 0, axis=1)).reshape(h, w)
+    lvl = 9
+    base = lvl * spec.table_size
+    total = 0
+    for y0 in range(0, h, 4):
+        for x0 in range(0, w, 8):
+            blk = idx[y0:y0 + 4, x0:x0 + 8, lvl][act[y0:y0 + 4, x0:x0 + 8]]
+            if blk.size:
+                total += len(np.unique((base + blk.reshape(-1)) >> 3))
+    assert total == b[lvl]
+    m.close()
+
+
+# ------------------------------------------------------------------------------------------------------
 # SURVEY 8(f3): scene parameters per texel (several frames with different t in one call)
 # ------------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("n_params,width,L", [(1, 64, 16), (2, 64, 16), (1, 32, 16), (2, 32, 8), (1, 64, 8)])
