@@ -268,6 +268,7 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + P.misc_off);
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2);
     uint32_t* s_tile = tmem_slot + 1;                 // [2]: the tile after next, handed from thread 0 to the CTA
+    uint32_t* s_txy = s_tile + 2;                     // [2]: IMG: its (tile column | tile row << 16)
 
     const uint32_t tid = threadIdx.x;
     const uint32_t warp = tid >> 5;
@@ -283,7 +284,11 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
     if (warp == 0) tmem_alloc(smem_u32(tmem_slot), TMEM_COLS);
     // dynamic tile scheduling: tile blockIdx.x is static, every further tile comes from a global counter, so a CTA
     // that drew cheap (background) tiles or a fast SM simply draws more of them and the grid drains together
-    if (tid == 0) s_tile[0] = gridDim.x + atomicAdd(P.tile_ctr, 1u);
+    if (tid == 0) {
+        const uint32_t t1 = gridDim.x + atomicAdd(P.tile_ctr, 1u);
+        s_tile[0] = t1;
+        if constexpr (IMG) s_txy[0] = image_tile_xy(P, t1);
+    }
     tc_fence_before_sync();
     __syncthreads();
     tc_fence_after_sync();
@@ -339,15 +344,18 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
     float pn[3] = {0.f, 0.f, 0.f}, nn[3] = {0.f, 0.f, 0.f};
     float tn[NPT > 0 ? NPT : 1] = {0.f};              // per-texel scene parameters, prefetched like the G-buffer
     // texel of thread tid in tile t: 128 consecutive texels per tile, or (IMG) a 32 x 4 pixel tile of the image
-    auto texel_of = [&](uint32_t t, bool& ok) -> size_t {
-        if constexpr (IMG) return image_texel(P, t, tid, ok);
+    //   (txy: the tile's packed image coordinates, which thread 0 works out with the tile index; unused otherwise)
+    auto texel_of = [&](uint32_t t, uint32_t txy, bool& ok) -> size_t {
+        if constexpr (IMG) return image_texel_xy(P, txy, tid, ok);
         const size_t idx = (size_t)t * kTile + tid;
         ok = idx < n;
         return idx;
     };
+    uint32_t txy = 0, txy_next = 0;
+    if constexpr (IMG) { txy = image_tile_xy(P, blockIdx.x); txy_next = s_txy[0]; }
     {
         bool ok;
-        const size_t i0 = texel_of(blockIdx.x, ok);
+        const size_t i0 = texel_of(blockIdx.x, txy, ok);
         if (ok) {
             load3(pos, i0, pn);
             load3(nrm, i0, nn);
@@ -365,16 +373,20 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
 #endif
     while (tile < n_tiles) {
         bool valid;
-        const size_t i = texel_of(tile, valid);
+        const size_t i = texel_of(tile, txy, valid);
         const float p[3] = {pn[0], pn[1], pn[2]}, nv[3] = {nn[0], nn[1], nn[2]};
         float tv[NPT > 0 ? NPT : 1];
 #pragma unroll
         for (int q = 0; q < NPT; ++q) tv[q] = tn[q];
         uint32_t tnn_mine = 0;
-        if (tid == 0) tnn_mine = gridDim.x + atomicAdd(P.tile_ctr, 1u);       // the tile after next
+        uint32_t txy_mine = 0;
+        if (tid == 0) {
+            tnn_mine = gridDim.x + atomicAdd(P.tile_ctr, 1u);                 // the tile after next
+            if constexpr (IMG) txy_mine = image_tile_xy(P, tnn_mine);
+        }
         {
             bool ok;
-            const size_t inext = texel_of(tnext, ok);     // (a tile index past the end gives ok = false in both modes)
+            const size_t inext = texel_of(tnext, txy_next, ok);   // (a tile index past the end gives ok = false)
 #pragma unroll
             for (int d = 0; d < 3; ++d) { pn[d] = 0.f; nn[d] = 0.f; }
             if (ok) {
@@ -434,10 +446,15 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
         if constexpr (NPT >= 1) tmem_st_x8(lane_taddr + A_COL + AW, a + AW);
         if constexpr (NPT == 2) tmem_st_x8(lane_taddr + A_COL + AW + 8, a + AW + 8);
         tmem_st_wait();
-        if (tid == 0) s_tile[(it + 1) & 1] = tnn_mine;
+        if (tid == 0) {
+            s_tile[(it + 1) & 1] = tnn_mine;
+            if constexpr (IMG) s_txy[(it + 1) & 1] = txy_mine;
+        }
         tc_fence_before_sync();
         __syncthreads();
         const uint32_t tnn = s_tile[(it + 1) & 1];
+        uint32_t txy_nn = 0;
+        if constexpr (IMG) txy_nn = s_txy[(it + 1) & 1];
         NIV_TICK(1);                                  // A store + tile barrier
 
         // ---- a10..a12: the layers.  K depends on the layer's position only (compile time), N on whether it is the
@@ -553,6 +570,7 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
         NIV_TICK(6);                                  // output layer epilogue + store
         tile = tnext;
         tnext = tnn;
+        if constexpr (IMG) { txy = txy_next; txy_next = txy_nn; }
         ++it;
     }
 #ifdef NIV_EXPERIMENT_TIMING
@@ -1409,7 +1427,8 @@ extern "C" int niv_infer_image(niv_model* m, const float* pos, const float* nrm,
     KParams P;
     int rc = fill_params(m, param, P);
     if (rc != NIV_OK) return rc;
-    if (!m->fused_img || getenv("NIV_IMAGE_LINEAR"))     // models without an image-tiled kernel: same result, linear tiles
+    // models without an image-tiled kernel (and images beyond the packed tile coordinates): same result, linear tiles
+    if (!m->fused_img || width > (1u << 20) || height > (1u << 17) || getenv("NIV_IMAGE_LINEAR"))
         return launch_fused(m, P, pos, nrm, out, n, (cudaStream_t)stream);
     P.img_w = width;
     P.img_h = height;

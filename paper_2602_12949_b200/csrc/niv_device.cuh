@@ -275,11 +275,18 @@ __device__ __forceinline__ void param_encode8_packed(float t, uint32_t o[8]) { p
 // niv_infer_image: tile = 32 x 4 pixels, warp w of the CTA = columns 8w .. 8w+7 of it (an 8 x 4 pixel block, lane =
 // 8 * row + column).  A warp's 32 texels then lie in a compact patch of the surface instead of a 32-pixel strip, so
 // they share more grid cells: 14 % fewer distinct sectors per warp on the full-HD frame (profiles/r01_v2.md).
-__device__ __forceinline__ size_t image_texel(const KParams& P, uint32_t tile, uint32_t tid, bool& valid) {
+// (tile column | tile row << 16) of a tile index: the one division, done by one thread per tile in the fused kernel
+__device__ __forceinline__ uint32_t image_tile_xy(const KParams& P, uint32_t tile) {
     const uint32_t ty = tile / P.tiles_x, tx = tile - ty * P.tiles_x;
-    const uint32_t x = tx * 32u + (tid >> 5) * 8u + (tid & 7u), y = ty * 4u + ((tid >> 3) & 3u);
+    return tx | (min(ty, 0xFFFFu) << 16);            // rows past the image (tile indices past the end) stay invalid
+}
+__device__ __forceinline__ size_t image_texel_xy(const KParams& P, uint32_t txy, uint32_t tid, bool& valid) {
+    const uint32_t x = (txy & 0xFFFFu) * 32u + (tid >> 5) * 8u + (tid & 7u), y = (txy >> 16) * 4u + ((tid >> 3) & 3u);
     valid = x < P.img_w && y < P.img_h;
     return (size_t)y * P.img_w + x;
+}
+__device__ __forceinline__ size_t image_texel(const KParams& P, uint32_t tile, uint32_t tid, bool& valid) {
+    return image_texel_xy(P, image_tile_xy(P, tile), tid, valid);
 }
 
 __device__ __forceinline__ void load3(const float* __restrict__ p, size_t i, float v[3]) {
