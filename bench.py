@@ -474,24 +474,36 @@ def run_sweep(args):
         d_pos = [torch.from_numpy(pos).cuda() for _ in range(ring)]
         d_nrm = [torch.from_numpy(nrm).cuda() for _ in range(ring)]
         d_out = [torch.empty((n, 3), dtype=torch.float32, device="cuda") for _ in range(ring)]
+        # frames stacked in one call form one taller image (every height here is a multiple of the 4-row tile)
+        image = args.tiling == "image" and bool(model.info.image_tiled)
+
+        def call(k):
+            if image:
+                model.infer_image(d_pos[k % ring], d_nrm[k % ring], d_out[k % ring], w, h * frames)
+            else:
+                model.infer(d_pos[k % ring], d_nrm[k % ring], d_out[k % ring])
+
         for k in range(5):
-            model.infer(d_pos[k % ring], d_nrm[k % ring], d_out[k % ring])
+            call(k)
         steps = 30
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         torch.cuda.synchronize()
         e0.record()
         for k in range(steps):
-            model.infer(d_pos[k % ring], d_nrm[k % ring], d_out[k % ring])
+            call(k)
         e1.record()
         torch.cuda.synchronize()
         ms = e0.elapsed_time(e1) / steps
         counts = torch.zeros(33, dtype=torch.int64, device="cuda")
-        model.probe_sectors(d_pos[0], d_nrm[0], counts)
+        if image:
+            model.probe_sectors_image(d_pos[0], d_nrm[0], w, h * frames, counts)
+        else:
+            model.probe_sectors(d_pos[0], d_nrm[0], counts)
         torch.cuda.synchronize()
         sectors = int(counts[:16].sum().item())
         info = model.info
         row = {"log2_T": log2_T, "table_MiB": info.table_bytes / 2 ** 20, "width": width, "res": "%dx%d" % (w, h),
-               "frames_per_call": frames, "texels": n, "masked": masked, "ms_per_call": ms, "ms_per_frame": ms / frames,
+               "frames_per_call": frames, "tiling": "image" if image else "linear", "texels": n, "masked": masked, "ms_per_call": ms, "ms_per_frame": ms / frames,
                "gqueries_per_s": n / ms / 1e6, "gather_sector_GBs": sectors * 32 / ms / 1e6,
                "hbm_io_GBs": 36.0 * n / ms / 1e6, "ctas_per_sm": info.ctas_per_sm, "smem_bytes": info.smem_bytes}
         print(json.dumps(row), flush=True)
