@@ -563,7 +563,15 @@ def test_full_size_sampled(torch_cuda, niv, oracle, which):
         pos, nrm = g["pos"], g["nrm"]
         assert 0.12 <= g["masked_fraction"] <= 0.18
     m = case.gpu_model(niv)
-    got = _gpu_infer(torch, m, pos, nrm, param=param)
+    if which == "incoherent":
+        got = _gpu_infer(torch, m, pos, nrm, param=param)
+    else:                                              # bench.py's launch for the G-buffer workloads: niv_infer_image
+        dp, dn = torch.from_numpy(pos).cuda(), torch.from_numpy(nrm).cuda()
+        out = torch.full((n, 3), float("nan"), dtype=torch.float32, device="cuda")
+        m.infer_image(dp, dn, out, 1920, 1080, param=param)
+        torch.cuda.synchronize()
+        got = out.cpu().numpy()
+        assert np.array_equal(got, _gpu_infer(torch, m, pos, nrm, param=param))      # and --tiling linear: same bits
     masked = np.all(nrm == 0, axis=1)
     assert np.all(got[masked] == 0) and np.all(np.isfinite(got))
     assert np.all((got[~masked] > 0) & (got[~masked] < 1))            # sigmoid range, at any size
