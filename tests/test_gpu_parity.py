@@ -230,6 +230,40 @@ def test_image_tiling_is_bit_identical_and_matches_oracle(torch_cuda, niv, oracl
     m.close()
 
 
+def test_image_entry_point_edge_cases(torch_cuda, niv):
+    torch = torch_cuda
+    case = Case(I.spec_fullhd(14), 4)
+    m = case.gpu_model(niv)
+    z = torch.zeros((8, 3), dtype=torch.float32, device="cuda")
+    L = niv.lib()
+    assert L.niv_infer_image(m._h, None, None, None, None, 0, 5, None) == niv.NIV_OK          # empty image: no-op
+    assert L.niv_infer_image(m._h, z.data_ptr(), z.data_ptr(), None, z.data_ptr(), 0, 0, None) == niv.NIV_OK
+    assert L.niv_infer_image(m._h, None, z.data_ptr(), None, z.data_ptr(), 4, 2, None) == niv.NIV_ERR_INVALID_ARG
+    assert L.niv_infer_image(m._h, z.data_ptr(), z.data_ptr(), None, z.data_ptr(), 1 << 16, 1 << 16, None) == niv.NIV_ERR_INVALID_ARG
+    import ctypes
+    p1 = (ctypes.c_float * 1)(0.5)
+    assert L.niv_infer_image(m._h, z.data_ptr(), z.data_ptr(), p1, z.data_ptr(), 4, 2, None) == niv.NIV_ERR_INVALID_ARG   # model has no parameter
+    # a one-row image wider than the packed tile coordinates reach: served by the linear kernel, same function
+    w = (1 << 20) + 40
+    pos, nrm = I.positions_uniform(w, I.ROOM_AABB, 3), I.normals_uniform(w, 3)
+    dp, dn = torch.from_numpy(pos).cuda(), torch.from_numpy(nrm).cuda()
+    a = torch.full((w, 3), float("nan"), dtype=torch.float32, device="cuda")
+    b = torch.full((w, 3), float("nan"), dtype=torch.float32, device="cuda")
+    m.infer_image(dp, dn, a, w, 1)
+    m.infer(dp, dn, b)
+    torch.cuda.synchronize()
+    assert torch.equal(a, b) and bool(torch.isfinite(a).all())
+    # a tall, narrow image: one tile column, partial in x
+    h = 4099
+    a2 = torch.full((3 * h, 3), float("nan"), dtype=torch.float32, device="cuda")
+    b2 = torch.full((3 * h, 3), float("nan"), dtype=torch.float32, device="cuda")
+    m.infer_image(dp[:3 * h], dn[:3 * h], a2, 3, h)
+    m.infer(dp[:3 * h], dn[:3 * h], b2)
+    torch.cuda.synchronize()
+    assert torch.equal(a2, b2)
+    m.close()
+
+
 def test_image_census_counts_fewer_sectors_than_strips(torch_cuda, niv):
     """The census of the 8 x 4 warps: same active texels, every level at most the strip count + noise, fine levels fewer."""
     torch = torch_cuda
