@@ -17,15 +17,20 @@
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream);
  *   - niv_infer / niv_encode / niv_debug_encode are asynchronous on `stream`, allocate nothing, never
  *     synchronise (CUDA-graph capturable), are read-only on the model's parameters and safe for concurrent callers
- *     on different streams (niv_infer draws one of 64 per-launch tile counters round robin, which the kernel
- *     itself leaves zeroed: up to 64 launches of one model may be in flight at once; a launch recorded into a CUDA
- *     graph keeps, for all its replays, one of 64 further counters that live launches never use, so up to 64 captured
- *     launches per model may replay concurrently with each other and with live launches; replays of one graph are
- *     serialised by CUDA itself);
+ *     on different streams.  Tiles are scheduled dynamically through one of 64 per-model tile counters: a counter is
+ *     handed to a launch only while no earlier launch is still running on it (the last CTA of a launch reports its
+ *     counter free through a host-mapped word), so any number of launches may be in flight; a launch that finds all
+ *     64 busy, and every launch recorded into a CUDA graph (its replays are invisible to the host), uses static tile
+ *     striding instead -- the same result, only less even on frames with large background regions;
+ *   - n <= 2^31 texels per call (NIV_ERR_INVALID_ARG beyond);
  *   - the fused kernels of hidden width <= 64 are launched with programmatic stream serialisation: their prologue
  *     (model-owned memory only) may overlap the tail of the previous kernel of the stream, and they wait for that
  *     kernel's completion (griddepcontrol.wait) before the first access to any buffer of the caller, so stream order
- *     holds for every buffer passed in; NIV_PDL=0 in the environment at niv_create turns this off;
+ *     holds for every buffer passed in;
+ *   - environment knobs, all read ONCE at niv_create and never on the call path: NIV_PDL=0 (no programmatic stream
+ *     serialisation), NIV_IMAGE_LINEAR=1 (niv_infer_image through the linear-tile kernel), NIV_HOST_STAGED=1
+ *     (niv_infer_host through staging copies even for pinned buffers), NIV_MMA_SYNC=1 (the mma.sync A/B kernel for the
+ *     BASELINE.json configs[1] shape), NIV_DEBUG=1 (resource report on stderr);
  *   - there is no CPU fallback: without a CUDA device every entry point that needs one returns NIV_ERR_CUDA.
  */
 #ifndef NIV_H_

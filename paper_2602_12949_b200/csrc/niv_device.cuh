@@ -36,10 +36,10 @@ struct KParams {
     uint32_t out_act;
     float    t[2];              // per-call scene parameters
     LevelP   lv[kMaxLevels];
-#ifdef NIV_EXPERIMENT_TIMING
-    unsigned long long* dbg;    // timing experiment only: per-phase cycle sums of thread 0 of every CTA
-#endif
-    uint32_t* tile_ctr;         // per-launch tile counter (zeroed on the stream before the launch): dynamic tile scheduling
+    uint32_t* tile_ctr;         // this launch's (tile, done) counter pair, left zero by the launch's last CTA: dynamic
+                                // tile scheduling; NULL = static striding (launches recorded into a CUDA graph)
+    volatile uint32_t* slot_done; // host-mapped word of the counter slot: the last CTA writes slot_gen (slot free again)
+    uint32_t slot_gen;
     const uint32_t* table;      // [L][T] entries of 2 x fp16
     const uint8_t*  wpack;      // packed weights + biases (see niv.cu pack_weights)
     uint32_t wpack_bytes;
@@ -49,7 +49,7 @@ struct KParams {
     uint32_t b_off[kMaxLayers];
     uint32_t wparam_off;        // fp32 [width][16*n_params] columns of W1 that multiply the parameter encoding
     uint32_t a_off;             // byte offset of the A tile in shared memory
-    uint32_t ones_off;          // byte offset of the constant "ones" A chunk of the bias K-step (v1 kernel)
+    uint32_t ones_off;          // byte offset of the constant "ones" A chunk of the bias K-step
     uint32_t misc_off;          // byte offset of folded bias / barriers
     const uint32_t* wmma;       // weights in the layout of the mma.sync A/B kernel (niv_fused_mma.cuh), else NULL
     const float* tparam;        // per-texel scene parameters [n][n_params] (niv_infer_texel_params), else NULL
@@ -141,11 +141,12 @@ __device__ __forceinline__ uint32_t pack_half2(float a, float b) {
 // each lerp = HADD2 (b - a) + HFMA2 (w * d + a) -> 14 instructions per level instead of 16 conversions +
 // 16 FFMA + 15 weight ops, and the result is already the packed fp16 pair the A operand wants.
 // Error: <= 15 * 2^-11 * max|table| worst case, ~2e-4 * max|table| rms.
+// The three fractions of a level travel as fp16 in 1.5 registers: (w_x, w_y) in one word, w_z of two levels in
+// another; the lerps read them through the .H0_H0 / .H1_H1 operand selectors of HFMA2 (no unpacking instruction).
 __device__ __forceinline__ __half2 u2h(uint32_t v) { return *reinterpret_cast<__half2*>(&v); }
 __device__ __forceinline__ uint32_t h2u(__half2 v) { return *reinterpret_cast<uint32_t*>(&v); }
 __device__ __forceinline__ __half2 lerp2(__half2 a, __half2 b, __half2 w) { return __hfma2(w, __hsub2(b, a), a); }
-__device__ __forceinline__ uint32_t blend8_h2(const uint32_t v[8], const uint32_t w2[3]) {
-    const __half2 wx = u2h(w2[0]), wy = u2h(w2[1]), wz = u2h(w2[2]);
+__device__ __forceinline__ uint32_t blend8_h2(const uint32_t v[8], __half2 wx, __half2 wy, __half2 wz) {
     const __half2 a0 = lerp2(u2h(v[0]), u2h(v[1]), wx), a1 = lerp2(u2h(v[2]), u2h(v[3]), wx);
     const __half2 a2 = lerp2(u2h(v[4]), u2h(v[5]), wx), a3 = lerp2(u2h(v[6]), u2h(v[7]), wx);
     const __half2 b0 = lerp2(a0, a1, wy), b1 = lerp2(a2, a3, wy);
@@ -158,7 +159,8 @@ __device__ __forceinline__ uint32_t blend8_h2(const uint32_t v[8], const uint32_
 template <int NB, int F>
 struct Batch {
     uint32_t v[NB][8][F / 2];   // gathered entries (F/2 x half2 each)
-    uint32_t w2[NB][3];         // interpolation fractions, each duplicated into a half2
+    uint32_t wxy[NB];           // (w_x, w_y) of a level as one fp16 pair
+    uint32_t wz[(NB + 1) / 2];  // w_z of levels 2k (low half) and 2k + 1 (high half)
 };
 // The per-level dense / hashed branch is uniform; it also keeps ptxas from sinking a batch's gathers down to their
 // first use (measured: with the split known at compile time ptxas interleaves loads and blends, 72 registers, and
@@ -166,6 +168,8 @@ struct Batch {
 template <int NB, int F>
 __device__ __forceinline__ void batch_issue(const KParams& P, int l0, const float u[3], Batch<NB, F>& b) {
     static_assert(F == 2 || F == 4, "F = 2 or 4");
+    float wzf[NB + 1];
+    wzf[NB] = 0.0f;
 #pragma unroll
     for (int q = 0; q < NB; ++q) {
         const LevelP& lv = P.lv[l0 + q];
@@ -176,13 +180,6 @@ __device__ __forceinline__ void batch_issue(const KParams& P, int l0, const floa
         corner_entries(lv, P.tmask, c, e);
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
-#ifdef NIV_EXPERIMENT_SKIPX1          // timing experiment only (wrong results): what the +x corner loads cost
-            if (j & 1) { for (int h = 0; h < F / 2; ++h) b.v[q][j][h] = b.v[q][j - 1][h]; continue; }
-#endif
-#ifdef NIV_EXPERIMENT_NOGATHER        // timing experiment only: index arithmetic kept, no table access
-            for (int h = 0; h < F / 2; ++h) b.v[q][j][h] = e[j];
-            continue;
-#endif
             if (F == 2) {
                 b.v[q][j][0] = __ldg(lv.tb + e[j]);
             } else {
@@ -191,21 +188,27 @@ __device__ __forceinline__ void batch_issue(const KParams& P, int l0, const floa
                 b.v[q][j][F / 2 - 1] = t.y;
             }
         }
-#pragma unroll
-        for (int d = 0; d < 3; ++d) b.w2[q][d] = pack_half2(w[d], w[d]);
+        b.wxy[q] = pack_half2(w[0], w[1]);
+        wzf[q] = w[2];
     }
+#pragma unroll
+    for (int q = 0; q < NB; q += 2) b.wz[q / 2] = pack_half2(wzf[q], wzf[q + 1]);
 }
 template <int NB, int F>
 __device__ __forceinline__ void batch_blend(const Batch<NB, F>& b, uint32_t* f) {
 #pragma unroll
-    for (int q = 0; q < NB; ++q)
+    for (int q = 0; q < NB; ++q) {
+        const __half2 wxy = u2h(b.wxy[q]), wzz = u2h(b.wz[q / 2]);
+        const __half2 wx = __low2half2(wxy), wy = __high2half2(wxy);
+        const __half2 wz = (q & 1) ? __high2half2(wzz) : __low2half2(wzz);
 #pragma unroll
         for (int h = 0; h < F / 2; ++h) {
             uint32_t v[8];
 #pragma unroll
             for (int j = 0; j < 8; ++j) v[j] = b.v[q][j][h];
-            f[q * (F / 2) + h] = blend8_h2(v, b.w2[q]);
+            f[q * (F / 2) + h] = blend8_h2(v, wx, wy, wz);
         }
+    }
 }
 
 // One group of 4 levels (8 latents = one 16-byte fp16 chunk of the A operand), gathers issued together (F = 2).

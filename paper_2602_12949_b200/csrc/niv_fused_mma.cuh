@@ -1,5 +1,5 @@
 // niv_fused_mma.cuh -- the fused encode + MLP with per-warp mma.sync (legacy HMMA) instead of tcgen05 / TMEM.
-// Included by niv.cu.  An A/B kernel (NIV_KERNEL=6) for the question north_star (3) leaves to the measurements:
+// Included by niv.cu.  An A/B kernel (NIV_MMA_SYNC=1 at niv_create) for the question north_star (3) leaves to the measurements:
 // "tcgen05/TMEM or mma.sync, whichever ncu shows is faster".  BASELINE.json configs[1] shape only: L = 16, F = 2, SH-16,
 // 48 -> 64 -> 64 -> 3, no scene parameter.
 //
@@ -51,7 +51,7 @@ __global__ void __launch_bounds__(kTile, MINB) niv_fused_mma_kernel(const __grid
     uint32_t tile = blockIdx.x * 4u + warp;
     while (tile < n_tiles32) {
         uint32_t tnext = 0;
-        if (lane == 0) tnext = gridDim.x * 4u + atomicAdd(P.tile_ctr, 1u);
+        if (lane == 0) tnext = P.tile_ctr ? gridDim.x * 4u + atomicAdd(P.tile_ctr, 1u) : tile + gridDim.x * 4u;   // NULL: static striding
         tnext = __shfl_sync(0xffffffffu, tnext, 0);
         const size_t i = (size_t)tile * 32u + lane;
         const bool valid = i < n;
@@ -192,9 +192,13 @@ __global__ void __launch_bounds__(kTile, MINB) niv_fused_mma_kernel(const __grid
     }
     // leave the (tile, done) counter pair zero for the slot's next launch
     __syncthreads();
-    if (tid == 0) {
+    if (tid == 0 && P.tile_ctr) {
         __threadfence();
-        if (atomicAdd(P.tile_ctr + 1, 1u) == gridDim.x - 1) { P.tile_ctr[0] = 0u; P.tile_ctr[1] = 0u; }
+        if (atomicAdd(P.tile_ctr + 1, 1u) == gridDim.x - 1) {
+            P.tile_ctr[0] = 0u;
+            P.tile_ctr[1] = 0u;
+            if (P.slot_done) *P.slot_done = P.slot_gen;
+        }
     }
 }
 

@@ -45,7 +45,10 @@ __global__ void __launch_bounds__(kTile, 3) niv_fused_w128_kernel(const __grid_c
         mbar_fence_init();
     }
     if (warp == 0) tmem_alloc(smem_u32(tmem_slot), TMEM_COLS);
-    if (tid == 0) s_tile[0] = gridDim.x + atomicAdd(P.tile_ctr, 1u);
+    auto next_tile = [&](uint32_t after) -> uint32_t {     // NULL counter = static striding (niv_fused.cuh)
+        return P.tile_ctr ? gridDim.x + atomicAdd(P.tile_ctr, 1u) : after + gridDim.x;
+    };
+    if (tid == 0) s_tile[0] = next_tile(blockIdx.x);
     *reinterpret_cast<uint4*>(sOnes + tid * 16) = make_uint4(0x3C003C00u, 0u, 0u, 0u);      // fp16 (1, 1, 0, ...)
     *reinterpret_cast<uint4*>(sOnes + 2048 + tid * 16) = make_uint4(0u, 0u, 0u, 0u);
     tc_fence_before_sync();
@@ -119,7 +122,7 @@ __global__ void __launch_bounds__(kTile, 3) niv_fused_w128_kernel(const __grid_c
         const bool valid = i < n;
         const float p[3] = {pn[0], pn[1], pn[2]}, nv[3] = {nn[0], nn[1], nn[2]};
         uint32_t tnn_mine = 0;
-        if (tid == 0) tnn_mine = gridDim.x + atomicAdd(P.tile_ctr, 1u);
+        if (tid == 0) tnn_mine = next_tile(tnext);
         {
             const size_t inext = (size_t)tnext * kTile + tid;
 #pragma unroll
@@ -223,11 +226,12 @@ __global__ void __launch_bounds__(kTile, 3) niv_fused_w128_kernel(const __grid_c
 
     __syncthreads();
     if (warp == 0) tmem_dealloc(tmem, TMEM_COLS);
-    if (tid == 0) {       // the last CTA to finish leaves the (tile, done) counter pair zero for the slot's next launch
+    if (tid == 0 && P.tile_ctr) {   // the last CTA to finish leaves the (tile, done) counter pair zero and reports the slot free
         __threadfence();
         if (atomicAdd(P.tile_ctr + 1, 1u) == gridDim.x - 1) {
             P.tile_ctr[0] = 0u;
             P.tile_ctr[1] = 0u;
+            if (P.slot_done) *P.slot_done = P.slot_gen;
         }
     }
 }

@@ -709,7 +709,7 @@ def test_sweep_extremes_sampled(torch_cuda, niv, oracle):
 
 
 def test_mma_sync_ab_kernel_parity(torch_cuda, niv, oracle, monkeypatch):
-    """The per-warp mma.sync A/B kernel (NIV_KERNEL=6, csrc/niv_fused_mma.cuh) computes the same function: parity with
+    """The per-warp mma.sync A/B kernel (NIV_MMA_SYNC=1 at niv_create, csrc/niv_fused_mma.cuh) computes the same function: parity with
     the oracle on the full-HD model, and agreement with the default tcgen05 kernel to fp16-activation rounding."""
     torch = torch_cuda
     case = Case(I.spec_fullhd(), 31, bias_scale=0.1)
@@ -720,10 +720,10 @@ def test_mma_sync_ab_kernel_parity(torch_cuda, niv, oracle, monkeypatch):
     m = case.gpu_model(niv)
     ref = _gpu_infer(torch, m, pos, nrm)
     m.close()
-    monkeypatch.setenv("NIV_KERNEL", "6")
+    monkeypatch.setenv("NIV_MMA_SYNC", "1")
     m = case.gpu_model(niv)
     got = _gpu_infer(torch, m, pos, nrm)
     m.close()
-    monkeypatch.delenv("NIV_KERNEL")
+    monkeypatch.delenv("NIV_MMA_SYNC")
     _check_irradiance(got, want, nrm, pos)
     assert np.abs(got.astype(np.float64) - ref.astype(np.float64)).max() <= 2e-3
