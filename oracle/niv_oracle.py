@@ -14,6 +14,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "niv_oracle.c")
+_SRCS = [_SRC, os.path.join(_HERE, "niv_oracle_ext.c")]
 _LIB = os.path.join(_HERE, "libniv_oracle.so")
 
 
@@ -30,9 +31,9 @@ class OracleConfig(C.Structure):
 
 def build(force: bool = False) -> str:
     """gcc -O2 -ffp-contract=off -fopenmp (no -ffast-math): the fp32 index path must not be contracted."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(f) for f in _SRCS):
         cmd = ["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-fPIC", "-shared",
-               "-Wall", "-Wextra", "-o", _LIB, _SRC, "-lm"]
+               "-Wall", "-Wextra", "-o", _LIB] + _SRCS + ["-lm"]
         subprocess.run(cmd, check=True)
     return _LIB
 
@@ -213,3 +214,28 @@ def compose(E, albedo, direct=None, emission=None) -> np.ndarray:
     if rc:
         raise ValueError("niv_oracle_compose failed (resolutions must be equal or exactly 2x)")
     return out
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# the paper's probe baseline (niv_oracle_ext.c)
+def probe_query(dims, bbox_min, bbox_max, coeffs, pos, nrm, cosine_falloff=True, n_threads: int = 0, debug=False):
+    """coeffs [nz][ny][nx][9][3] fp16 (27 per probe, x fastest) -> E [n][3] fp32
+    (debug: also fp64 E, the 8 normalised weights and the 8 probe indices per texel)."""
+    d = (C.c_uint32 * 3)(*[int(v) for v in dims])
+    lo = (C.c_float * 3)(*[float(v) for v in bbox_min])
+    hi = (C.c_float * 3)(*[float(v) for v in bbox_max])
+    coeffs = _chk(coeffs, np.float16, "coeffs")
+    if coeffs.size != int(dims[0]) * int(dims[1]) * int(dims[2]) * 27:
+        raise ValueError("coeffs must hold 27 values per probe")
+    pos = _chk(pos, np.float32, "pos")
+    nrm = _chk(nrm, np.float32, "nrm")
+    n = pos.shape[0]
+    out32 = np.zeros((n, 3), dtype=np.float32)
+    out64 = np.zeros((n, 3), dtype=np.float64) if debug else None
+    w = np.zeros((n, 8), dtype=np.float64) if debug else None
+    pi = np.zeros((n, 8), dtype=np.uint32) if debug else None
+    rc = lib().niv_oracle_probe_query(d, lo, hi, C.c_int(1 if cosine_falloff else 0), _p(coeffs), _p(pos), _p(nrm),
+                                      C.c_size_t(n), _p(out32), _p(out64), _p(w), _p(pi), C.c_int(n_threads))
+    if rc:
+        raise ValueError("niv_oracle_probe_query failed")
+    return (out32, out64, w, pi) if debug else out32

@@ -328,3 +328,27 @@ def make_gbuffer(width: int, height: int, seed: int, frame: int = 0) -> Dict[str
                         "eye": eye, "target": target, "width": width, "height": height}
         sub += 1
     raise RuntimeError("no camera with 12-18 % background found")
+
+
+# ----------------------------------------------------------------------------
+# a synthetic probe grid (stands in for a baked DDGI-like grid)
+# ----------------------------------------------------------------------------
+PROBE_STREAM = 0x7000
+
+
+def make_probe_grid(dims: Tuple[int, int, int], seed: int, scale: float = 1.0) -> np.ndarray:
+    """-> coefficients [nz][ny][nx][9][3] fp16: 27 values per probe, x fastest.  A baked grid is not
+    available (no scenes, no path tracer), so the values are seeded noise with the magnitudes of an irradiance field:
+    a positive band-0 term of order one, bands 1 and 2 a half and a quarter of it, both signs."""
+    nx, ny, nz = (int(v) for v in dims)
+    n = nx * ny * nz
+    r = uniform01(seed, PROBE_STREAM, n * 27).reshape(nz, ny, nx, 9, 3)
+    band = np.array([1.0] + [0.5] * 3 + [0.25] * 5)[None, None, None, :, None]
+    c = (2.0 * r - 1.0) * band
+    c[..., 0, :] = 1.0 + 2.0 * r[..., 0, :]                      # band 0 in [1, 3)
+    return (scale * c).astype(np.float16)
+
+
+def probe_grid_dims_for_spacing(aabb_min, aabb_max, spacing: float) -> Tuple[int, int, int]:
+    """Probes on a regular lattice over the box, faces included, about `spacing` apart."""
+    return tuple(int(max(2, round((float(hi) - float(lo)) / spacing) + 1)) for lo, hi in zip(aabb_min, aabb_max))
