@@ -230,6 +230,34 @@ int niv_probe_sectors(niv_model *m, const float *pos, const float *nrm, size_t n
 int niv_probe_sectors_image(const niv_model *m, const float *pos, const float *nrm, uint32_t width, uint32_t height,
                             uint64_t *counts, void *stream);
 
+/* ---- the paper's probe baseline as a second workload over the same G-buffers --------------------------
+ * A regular grid of irradiance probes, "similar to DDGI" (App. A): per probe second-order
+ * spherical harmonics (9 coefficients x 3 channels) in half precision, 54 bytes; a query blends the 8 probes of the
+ * enclosing cell with trilinear weights x a cosine fall-off ("probes behind the sampled normal do not contribute"),
+ * clamps every weight to 1e-6 and renormalises, then reconstructs E(n) = sum_k c_k Y_k(n) with the basis of
+ * SPEC.md:341-345.  Steps P0..P7 and the readings taken are in DESIGN.md 3.6.  Ray-traced visibility is not built.
+ * "Probes should always hold a performance edge" is the claim this lets one measure. */
+typedef struct niv_probe_grid niv_probe_grid;    /* opaque; owns the device copy of the probes */
+typedef struct {
+    uint32_t struct_size;        /* = sizeof(niv_probe_config)                                          */
+    uint32_t dims[3];            /* probes per axis, >= 2; lattice over the box, faces included         */
+    float    bbox_min[3], bbox_max[3];
+    uint32_t cosine_falloff;     /* 1: App. A's fall-off, 0: plain trilinear weights (still clamped)    */
+    int32_t  device;
+} niv_probe_config;
+
+int niv_probes_create(const niv_probe_config *cfg, niv_probe_grid **out);
+/* coeffs_fp16: [nz][ny][nx][9][3] fp16 = 27 values per probe, x fastest, host or device;
+ * bytes must equal 54 * nx * ny * nz.  Synchronises `stream`. */
+int niv_probes_load(niv_probe_grid *g, const void *coeffs_fp16, size_t bytes, int src_on_device, void *stream);
+/* out[i] = E_probes(pos[i], nrm[i]); device pointers, [n][3] fp32 packed; background / non-finite texels -> 0 (as
+ * niv_infer); positions outside the box are clamped into it.  Asynchronous on `stream`, allocation-free. */
+int niv_probes_query(niv_probe_grid *g, const float *pos, const float *nrm, float *out, size_t n, void *stream);
+/* Roofline numerator of the query: counts (device, uint64[2]) = { distinct 32-byte sectors of probe records per warp of
+ * 32 consecutive texels, summed; active texels }. */
+int niv_probes_census(niv_probe_grid *g, const float *pos, const float *nrm, size_t n, uint64_t *counts, void *stream);
+int niv_probes_destroy(niv_probe_grid *g);
+
 #ifdef __cplusplus
 }
 #endif

@@ -43,8 +43,12 @@ static int masked6(const float *p, const float *n)
  *   P2 locate      p_d = fl32(u_d * (float)(n_d - 1)); c_d = min(floor(p_d), n_d - 2); w_d = fl32(p_d - c_d)    (fp32, as O2)
  *   P3 trilinear   probe j (bit d of j = +1 on axis d) at lattice point c + bits, weight prod_d (bit ? w_d : 1 - w_d);
  *                  probes stored x fastest: index vx + nx (vy + ny vz)
- *   P4 fall-off    weight *= max(0, dot(normalize(q_j - xc), n)), q_j = min + v (max - min) / (n - 1) the probe
- *                  position, xc = x clamped into the box; a probe AT xc (zero vector) keeps its weight (factor 1)
+ *   P4 fall-off    weight *= max(0, dot(normalize(q_j - xc), n)), q_j the probe position, xc = x clamped into the box;
+ *                  a probe AT xc (zero vector) keeps its weight (factor 1).  The vector q_j - xc is evaluated in fp32
+ *                  with a pinned op sequence (step_d = fl32(fl32(max_d - min_d) / (float)(n_d - 1)),
+ *                  q = fl32(fl32((float)v * step_d) + min_d), d = fl32(q - xc)): next to a probe the direction is
+ *                  ill-conditioned in the probe position, and where its cosine crosses zero the weights are not
+ *                  Lipschitz in it, so the precision of this one vector is part of the definition (reading P-e)
  *   P5 clamp       weight = max(weight, 1e-6);  P6 renormalise to sum 1
  *   P7 reconstruct E = sum_j weight_j sum_k c_jk Y_k(n), Y the real SH of bands 0..2 in the order and with the
  *                  constants of SPEC.md:341-345 (= the first nine of niv_oracle_sh16); coefficients [9][3] fp16 per probe
@@ -56,11 +60,13 @@ int niv_oracle_probe_query(const uint32_t dims[3], const float bmin[3], const fl
     if (!dims || !bmin || !bmax || !coeffs || !pos || !nrm) return -1;
     for (int d = 0; d < 3; ++d)
         if (dims[d] < 2 || !(bmax[d] > bmin[d])) return -1;
-    float inv[3];
+    float inv[3], step[3];
     for (int d = 0; d < 3; ++d) {
         volatile float ext = bmax[d] - bmin[d];
         volatile float iv = 1.0f / ext;
+        volatile float st = ext / (float)(dims[d] - 1);
         inv[d] = iv;
+        step[d] = st;
     }
 #ifdef _OPENMP
     if (n_threads > 0) omp_set_num_threads(n_threads);
@@ -99,8 +105,10 @@ int niv_oracle_probe_query(const uint32_t dims[3], const float bmin[3], const fl
                     const int bit = (j >> d) & 1;
                     v[d] = (uint32_t)(c[d] + bit);
                     wt *= bit ? (double)w[d] : 1.0 - (double)w[d];        /* P3 */
-                    const double q = (double)bmin[d] + (double)v[d] * ((double)bmax[d] - (double)bmin[d]) / (double)(dims[d] - 1);
-                    dvec[d] = q - (double)xc[d];
+                    volatile float q0 = (float)v[d] * step[d];            /* P4: pinned fp32 sequence */
+                    volatile float q1 = q0 + bmin[d];
+                    volatile float dd = q1 - xc[d];
+                    dvec[d] = (double)dd;
                     len2 += dvec[d] * dvec[d];
                 }
                 if (cosine_falloff && len2 > 0.0) {                       /* P4 */

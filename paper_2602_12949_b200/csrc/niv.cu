@@ -31,6 +31,7 @@
 #include "niv_fused_w128.cuh"
 #include "niv_fused_mma.cuh"
 #include "niv_compose.cuh"
+#include "niv_probes.cuh"
 namespace niv {
 
 // =====================================================================================================
@@ -1030,6 +1031,112 @@ extern "C" int niv_compose(const float* E, uint32_t ew, uint32_t eh, const float
         niv_compose_scalar_kernel<<<grid, 256, 0, st>>>(E, ew, eh, albedo, direct, emission, out, w, h, half);
     }
     NIV_CUDA(cudaGetLastError());
+    return NIV_OK;
+}
+
+// =====================================================================================================
+// the probe-grid baseline
+// =====================================================================================================
+struct niv_probe_grid {
+    niv_probe_config cfg;
+    ProbeParams gp;
+    uint4* d_probes = nullptr;
+    size_t n_probes = 0;
+    bool loaded = false;
+};
+
+extern "C" int niv_probes_create(const niv_probe_config* cfg, niv_probe_grid** out)
+{
+    if (!cfg || !out) return NIV_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (cfg->struct_size != sizeof(niv_probe_config)) return NIV_ERR_INVALID_ARG;
+    size_t n_probes = 1;
+    for (int d = 0; d < 3; ++d) {
+        if (cfg->dims[d] < 2 || cfg->dims[d] > 4096) return NIV_ERR_INVALID_ARG;
+        if (!std::isfinite(cfg->bbox_min[d]) || !std::isfinite(cfg->bbox_max[d]) || !(cfg->bbox_max[d] > cfg->bbox_min[d]))
+            return NIV_ERR_INVALID_ARG;
+        n_probes *= cfg->dims[d];
+    }
+    if (n_probes > ((size_t)1 << 30) || cfg->cosine_falloff > 1) return NIV_ERR_INVALID_ARG;
+    niv_probe_grid* g = new (std::nothrow) niv_probe_grid();
+    if (!g) return NIV_ERR_ALLOC;
+    g->cfg = *cfg;
+    g->n_probes = n_probes;
+    ProbeParams& G = g->gp;
+    memset(&G, 0, sizeof(G));
+    for (int d = 0; d < 3; ++d) {
+        G.amin[d] = cfg->bbox_min[d];
+        G.amax[d] = cfg->bbox_max[d];
+        volatile float ext = cfg->bbox_max[d] - cfg->bbox_min[d];
+        volatile float inv = 1.0f / ext;
+        volatile float step = ext / (float)(cfg->dims[d] - 1);
+        G.ainv[d] = inv;
+        G.step[d] = step;
+        G.nf[d] = (float)(cfg->dims[d] - 1);
+        G.nm2[d] = (int32_t)cfg->dims[d] - 2;
+        G.dims[d] = cfg->dims[d];
+    }
+    G.falloff = cfg->cosine_falloff;
+    g_last_cuda_error = 0;
+    cudaError_t e = cudaSetDevice(cfg->device);
+    if (e == cudaSuccess) e = cudaMalloc(&g->d_probes, n_probes * 64);
+    if (e != cudaSuccess) { g_last_cuda_error = (int)e; (void)cudaGetLastError(); delete g; return e == cudaErrorMemoryAllocation ? NIV_ERR_ALLOC : NIV_ERR_CUDA; }
+    G.probes = g->d_probes;
+    *out = g;
+    return NIV_OK;
+}
+
+extern "C" int niv_probes_load(niv_probe_grid* g, const void* coeffs_fp16, size_t bytes, int src_on_device, void* stream)
+{
+    if (!g || !coeffs_fp16 || bytes != g->n_probes * 54) return NIV_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    NIV_CUDA(cudaSetDevice(g->cfg.device));
+    const uint16_t* src = (const uint16_t*)coeffs_fp16;
+    uint16_t* tmp = nullptr;
+    if (!src_on_device) {
+        NIV_CUDA(cudaMalloc(&tmp, bytes));
+        cudaError_t e = cudaMemcpyAsync(tmp, coeffs_fp16, bytes, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) { cudaFree(tmp); g_last_cuda_error = (int)e; return NIV_ERR_CUDA; }
+        src = tmp;
+    }
+    const size_t total = g->n_probes * 32;
+    niv_probes_pack_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(src, (uint16_t*)g->d_probes, g->n_probes);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (tmp) cudaFree(tmp);
+    if (e != cudaSuccess) { g_last_cuda_error = (int)e; (void)cudaGetLastError(); return NIV_ERR_CUDA; }
+    g->loaded = true;
+    return NIV_OK;
+}
+
+extern "C" int niv_probes_query(niv_probe_grid* g, const float* pos, const float* nrm, float* out, size_t n, void* stream)
+{
+    if (!g) return NIV_ERR_INVALID_ARG;
+    if (!g->loaded) return NIV_ERR_NOT_LOADED;
+    if (n == 0) return NIV_OK;
+    if (!pos || !nrm || !out || n > ((size_t)1 << 31)) return NIV_ERR_INVALID_ARG;
+    niv_probes_query_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(g->gp, pos, nrm, out, n);
+    NIV_CUDA(cudaGetLastError());
+    return NIV_OK;
+}
+
+extern "C" int niv_probes_census(niv_probe_grid* g, const float* pos, const float* nrm, size_t n, uint64_t* counts,
+                                 void* stream)
+{
+    if (!g || !pos || !nrm || !counts || n == 0) return NIV_ERR_INVALID_ARG;
+    NIV_CUDA(cudaMemsetAsync(counts, 0, 2 * sizeof(uint64_t), (cudaStream_t)stream));
+    niv_probes_census_kernel<<<(unsigned)((n + 127) / 128), 128, 0, (cudaStream_t)stream>>>(g->gp, pos, nrm, n,
+                                                                                           (unsigned long long*)counts);
+    NIV_CUDA(cudaGetLastError());
+    return NIV_OK;
+}
+
+extern "C" int niv_probes_destroy(niv_probe_grid* g)
+{
+    if (!g) return NIV_OK;
+    cudaSetDevice(g->cfg.device);
+    cudaFree(g->d_probes);
+    delete g;
     return NIV_OK;
 }
 

@@ -28,7 +28,8 @@ EXPORTS = ("niv_create", "niv_get_info", "niv_load_params", "niv_infer", "niv_in
            "niv_infer_host", "niv_probe_sectors_image",
            "niv_encode",
            "niv_debug_encode", "niv_compose", "niv_destroy", "niv_error_string", "niv_last_cuda_error", "niv_probe_gather",
-           "niv_probe_sectors")
+           "niv_probe_sectors",
+           "niv_probes_create", "niv_probes_load", "niv_probes_query", "niv_probes_census", "niv_probes_destroy")
 
 
 class NivConfig(C.Structure):
@@ -52,6 +53,11 @@ class NivInfo(C.Structure):
         ("num_sms", C.c_uint32), ("ctas_per_sm", C.c_uint32), ("tile_texels", C.c_uint32),
         ("smem_bytes", C.c_uint32), ("image_tiled", C.c_uint32), ("texel_params", C.c_uint32),
     ]
+
+
+class NivProbeConfig(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("dims", C.c_uint32 * 3), ("bbox_min", C.c_float * 3),
+                ("bbox_max", C.c_float * 3), ("cosine_falloff", C.c_uint32), ("device", C.c_int32)]
 
 
 class NivError(RuntimeError):
@@ -92,6 +98,11 @@ def lib():
         L.niv_last_cuda_error.argtypes = []
         L.niv_probe_gather.argtypes = [vp, sz, C.c_int, C.c_uint32, C.c_uint32, C.c_uint32, vp, vp]
         L.niv_probe_sectors.argtypes = [vp, vp, vp, sz, vp, vp]
+        L.niv_probes_create.argtypes = [C.POINTER(NivProbeConfig), C.POINTER(vp)]
+        L.niv_probes_load.argtypes = [vp, vp, sz, C.c_int, vp]
+        L.niv_probes_query.argtypes = [vp, vp, vp, vp, sz, vp]
+        L.niv_probes_census.argtypes = [vp, vp, vp, sz, vp, vp]
+        L.niv_probes_destroy.argtypes = [vp]
         for name in EXPORTS:
             if name != "niv_error_string":
                 getattr(L, name).restype = C.c_int
@@ -142,6 +153,13 @@ def _dev(t, dtype, name: str, cols: Optional[int] = None):
     if cols is not None and (t.dim() != 2 or t.shape[1] != cols):
         raise TypeError("%s must have shape [n][%d]" % (name, cols))
     return t.data_ptr()
+
+
+def _same_rows(n: int, **bufs):
+    """Every per-texel buffer of a call must hold n rows (a shorter one would be read or written out of bounds)."""
+    for name, t in bufs.items():
+        if t.shape[0] != n:
+            raise ValueError("%s holds %d rows, pos holds %d" % (name, t.shape[0], n))
 
 
 def _params(param: Optional[Sequence[float]], n_params: int):
@@ -200,6 +218,7 @@ class NivModel:
         """out[i] = E_theta(pos[i], nrm[i][, param]); device tensors [n][3] fp32; asynchronous."""
         import torch
         n = pos.shape[0]
+        _same_rows(n, nrm=nrm, out=out)
         rc = lib().niv_infer(self._h, _dev(pos, torch.float32, "pos", 3) if n else None,
                              _dev(nrm, torch.float32, "nrm", 3) if n else None,
                              _params(param, self.spec.n_params),
@@ -227,6 +246,7 @@ class NivModel:
         """as infer(), every texel with its own scene parameters; tparam device [n][n_params] fp32."""
         import torch
         n = pos.shape[0]
+        _same_rows(n, nrm=nrm, tparam=tparam, out=out)
         rc = lib().niv_infer_texel_params(self._h, _dev(pos, torch.float32, "pos", 3) if n else None,
                                           _dev(nrm, torch.float32, "nrm", 3) if n else None,
                                           _dev(tparam, torch.float32, "tparam", self.spec.n_params) if n else None,
@@ -239,6 +259,7 @@ class NivModel:
         """Same, with HOST buffers (numpy arrays or pinned CPU tensors, [n][3] fp32): the library stages
         them through its own device buffers (H2D, kernel, D2H) and synchronises the stream."""
         n = pos.shape[0]
+        _same_rows(n, nrm=nrm, out=out)
         rc = lib().niv_infer_host(self._h, _host_ptr(pos, "pos"), _host_ptr(nrm, "nrm"),
                                   _params(param, self.spec.n_params), _host_ptr(out, "out"), n,
                                   _stream_ptr(stream))
@@ -339,3 +360,67 @@ def compose(E, albedo, out, direct=None, emission=None, stream=None):
                            None if emission is None else emission.data_ptr(), out.data_ptr(), w, h, _stream_ptr(stream))
     if rc != NIV_OK:
         raise NivError(rc, "niv_compose")
+
+
+class NivProbeGrid:
+    """Handle on a niv_probe_grid (the paper's probe baseline).  Methods mirror the C ABI one to one."""
+
+    def __init__(self, dims, bbox_min, bbox_max, cosine_falloff: bool = True, device: int = 0):
+        cfg = NivProbeConfig()
+        cfg.struct_size = C.sizeof(NivProbeConfig)
+        for d in range(3):
+            cfg.dims[d] = int(dims[d])
+            cfg.bbox_min[d] = float(bbox_min[d])
+            cfg.bbox_max[d] = float(bbox_max[d])
+        cfg.cosine_falloff = 1 if cosine_falloff else 0
+        cfg.device = device
+        self.dims = tuple(int(v) for v in dims)
+        self._h = C.c_void_p()
+        rc = lib().niv_probes_create(C.byref(cfg), C.byref(self._h))
+        if rc != NIV_OK:
+            self._h = C.c_void_p()
+            raise NivError(rc, "niv_probes_create")
+
+    def load(self, coeffs, stream=None):
+        """coeffs [nz][ny][nx][9][3] fp16: numpy array (host) or CUDA tensor."""
+        import numpy as np
+        if isinstance(coeffs, np.ndarray):
+            coeffs = np.ascontiguousarray(coeffs, dtype=np.float16)
+            ptr, nbytes, dev = coeffs.ctypes.data, coeffs.nbytes, 0
+        else:
+            import torch
+            ptr, nbytes, dev = _dev(coeffs, torch.float16, "coeffs"), coeffs.numel() * 2, 1
+        rc = lib().niv_probes_load(self._h, ptr, nbytes, dev, _stream_ptr(stream))
+        if rc != NIV_OK:
+            raise NivError(rc, "niv_probes_load")
+
+    def query(self, pos, nrm, out, stream=None):
+        import torch
+        n = pos.shape[0]
+        if nrm.shape[0] != n or out.shape[0] != n:
+            raise ValueError("pos, nrm and out must hold the same number of texels")
+        rc = lib().niv_probes_query(self._h, _dev(pos, torch.float32, "pos", 3) if n else None,
+                                    _dev(nrm, torch.float32, "nrm", 3) if n else None,
+                                    _dev(out, torch.float32, "out", 3) if n else None, n, _stream_ptr(stream))
+        if rc != NIV_OK:
+            raise NivError(rc, "niv_probes_query")
+        return out
+
+    def census(self, pos, nrm, counts, stream=None):
+        """counts: device int64[2] = (distinct probe sectors per warp, summed; active texels)."""
+        import torch
+        rc = lib().niv_probes_census(self._h, _dev(pos, torch.float32, "pos", 3), _dev(nrm, torch.float32, "nrm", 3),
+                                     pos.shape[0], _dev(counts, torch.int64, "counts"), _stream_ptr(stream))
+        if rc != NIV_OK:
+            raise NivError(rc, "niv_probes_census")
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            lib().niv_probes_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -138,7 +138,7 @@ def test_probe_query_matches_numpy_brute_force(oracle):
             got, e64, _, _ = oracle.probe_query(dims, lo, hi, c, pos, nrm, cosine_falloff=falloff, debug=True)
             for i in range(60):
                 want = _brute(dims, lo, hi, c, pos[i], nrm[i], falloff)
-                assert np.allclose(e64[i], want, rtol=0, atol=3e-6), (dims, falloff, i)
+                assert np.allclose(e64[i], want, rtol=0, atol=1e-5), (dims, falloff, i)    # (fp32 probe offsets, P-e)
             assert np.abs(got - e64).max() < 1e-6
 
 
