@@ -342,7 +342,7 @@ def run_ours(args):
 
     # ---- rooflines (rank 0) -------------------------------------------------------------------------
     peaks = load_peaks()
-    counts = torch.zeros(33, dtype=torch.int64, device="cuda")
+    counts = torch.zeros(niv.NIV_CENSUS_COUNTS, dtype=torch.int64, device="cuda")
     if image:
         model.probe_sectors_image(d_pos[0], d_nrm[0], W_PX, H_PX, counts)      # the census of the warps that ran
     else:
@@ -351,6 +351,7 @@ def run_ours(args):
     c = counts.cpu().numpy()
     L = spec.n_levels
     sectors, lines, n_active = int(c[:L].sum()), int(c[16:16 + L].sum()), int(c[32])
+    touched = int(c[33:33 + L].sum())                   # sectors the kernel's own layout touches (cell-block levels)
     gpeak, probe_bytes = measure_gather_peak(torch, niv, info.table_bytes, info.num_sms)
     kernel_s = kernel_ms_timed * 1e-3                   # one fused kernel per step: timed region / K (gaps included)
     dims = [spec.in_dim] + [spec.hidden_width] * spec.n_hidden_layers + [3]
@@ -383,7 +384,15 @@ def run_ours(args):
                        % (probe_bytes >> 20),
         "algorithmic": {"sectors_per_launch": sectors, "sectors_per_active_texel": sectors / max(n_active, 1),
                         "lines_per_active_texel": lines / max(n_active, 1), "active_texels": n_active,
-                        "gathers_per_active_texel": 8 * L, "sectors_per_level": [int(v) for v in c[:L]]},
+                        "gathers_per_active_texel": 8 * L, "sectors_per_level": [int(v) for v in c[:L]],
+                        "definition": "distinct 32 B sectors per (warp, level) among the corner addresses of the [L][T] "
+                                      "table as loaded (SURVEY.md 8(d)); independent of the library's internal layout"},
+        "touched": {"sectors_per_launch": touched, "sectors_per_active_texel": touched / max(n_active, 1),
+                    "sectors_per_level": [int(v) for v in c[33:33 + L]], "cell_block_levels": int(info.cell_levels),
+                    "cell_block_bytes": int(info.cell_bytes), "achieved_gbs": touched * 32 / kernel_s / 1e9,
+                    "frac_of_probe_peak": touched * 32 / kernel_s / 1e9 / gpeak["random_sector"]["sector_gbs"],
+                    "note": "what the kernel's own layout reads: levels held as cell blocks cost one sector per "
+                            "distinct cell instead of the 8 corners' sectors"},
         "gather_rate_ggathers_per_s": 8 * L * n_active / kernel_s / 1e9,
         "probe": gpeak,
         "t_roofline_us": {"l2_gather": t_gather * 1e6, "tensor": t_tensor * 1e6, "hbm": t_hbm * 1e6},
@@ -494,7 +503,7 @@ def run_sweep(args):
         e1.record()
         torch.cuda.synchronize()
         ms = e0.elapsed_time(e1) / steps
-        counts = torch.zeros(33, dtype=torch.int64, device="cuda")
+        counts = torch.zeros(niv.NIV_CENSUS_COUNTS, dtype=torch.int64, device="cuda")
         if image:
             model.probe_sectors_image(d_pos[0], d_nrm[0], w, h * frames, counts)
         else:

@@ -98,6 +98,10 @@ typedef struct {
     uint32_t smem_bytes;                   /* dynamic shared memory per CTA of the fused kernel     */
     uint32_t image_tiled;                  /* 1: niv_infer_image has its own 8 x 4-block kernel, 0: it runs niv_infer's */
     uint32_t texel_params;                 /* 1: niv_infer_texel_params is available for this model */
+    uint32_t cell_levels;                  /* levels 0 .. cell_levels-1 are also held as cell blocks (8 corner
+                                              entries per cell, one 32- / 64-byte load per texel and level) */
+    uint32_t reserved0;
+    uint64_t cell_bytes;                   /* device bytes of those copies (budget: NIV_CELL_MB at niv_create) */
 } niv_info;
 
 /* Validate `cfg` completely and allocate device storage for the parameters (uninitialised).
@@ -222,8 +226,12 @@ int niv_probe_gather(const void *buf, size_t buf_bytes, int pattern, uint32_t n_
 /* niv_probe_sectors: the sector census behind the gather roofline ("S = number of 32-byte sectors
  * the frame algorithmically needs at warp granularity").  For every group of 32 consecutive texels (the fused
  * kernel's texel -> warp map) and every level, counts the DISTINCT 32-byte sectors and 128-byte lines among the
- * group's <= 256 corner addresses.  counts is device, 33 x uint64: [0,16) sectors per level, [16,32) lines per
- * level, [32] active (unmasked) texels.  Asynchronous; counts is zeroed first on `stream`. */
+ * group's <= 256 corner addresses in the table as niv_load_params receives it ([L][T] entries): the algorithmic
+ * figure, independent of how the library lays the table out.  counts is device, NIV_CENSUS_COUNTS x uint64:
+ * [0,16) sectors per level, [16,32) lines per level, [32] active (unmasked) texels, [33,49) the sectors the fused
+ * kernel really touches per level (the same on gathered levels; distinct cell blocks on the levels niv_info.cell_levels
+ * holds as cell blocks).  Asynchronous; counts is zeroed first on `stream`. */
+#define NIV_CENSUS_COUNTS 49
 int niv_probe_sectors(niv_model *m, const float *pos, const float *nrm, size_t n, uint64_t *counts, void *stream);
 
 /* The same census for niv_infer_image's texel -> warp map (8 x 4 pixel blocks of a height x width image). */

@@ -15,7 +15,7 @@ SRC = os.path.join(_HERE, "csrc", "niv.cu")
 LIB = os.path.join(_HERE, "libniv.so")
 DEPS = [SRC] + glob.glob(os.path.join(_HERE, "csrc", "*.cuh")) + [os.path.join(_ROOT, "include", "niv.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "--shared", "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall", "-cudart", "shared"]
+              "-split-compile", "0", "--shared", "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall", "-cudart", "shared"]
 
 
 def stale() -> bool:

@@ -145,6 +145,25 @@ __global__ void __launch_bounds__(128) niv_debug_kernel(const __grid_constant__ 
 }
 
 // =====================================================================================================
+// cell-block copy of a coarse level: block (cx, cy, cz) = the 8 corner entries of that cell, found
+// through the same corner_entries() as every other kernel.  One thread per cell; run once per niv_load_params.
+// =====================================================================================================
+__global__ void __launch_bounds__(256) niv_build_cells_kernel(const __grid_constant__ KParams P, uint32_t level,
+                                                              uint32_t* __restrict__ dst, uint32_t n_cells)
+{
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_cells) return;
+    const LevelP& lv = P.lv[level];
+    const uint32_t N = lv.cs;
+    const int c[3] = {(int)(i % N), (int)((i / N) % N), (int)(i / (N * N))};
+    uint32_t e[8];
+    corner_entries(lv, P.tmask, c, e);
+    const uint32_t FW = P.n_features >> 1;
+    for (int j = 0; j < 8; ++j)
+        for (uint32_t h = 0; h < FW; ++h) dst[((size_t)i * 8 + j) * FW + h] = lv.tb[(size_t)e[j] * FW + h];
+}
+
+// =====================================================================================================
 // gather micro-benchmark
 // =====================================================================================================
 __device__ __forceinline__ uint32_t mix32(uint32_t x) {
@@ -219,11 +238,13 @@ __global__ void __launch_bounds__(256) niv_probe_gather_kernel(const uint32_t* _
 // One warp per group of 32 consecutive texels (the fused kernel's own texel -> warp map).  For every level the
 // warp's <= 256 corner addresses are reduced to the number of DISTINCT 32-byte sectors (and distinct 128-byte
 // lines); the per-level counts are summed over the grid.  counts[0..L) = sectors, counts[16..16+L) = lines,
-// counts[32] = active texels.
+// counts[32] = active texels.  These are the addresses of the table as niv_load_params receives it ([L][T] entries):
+// the algorithmic figure of SURVEY.md 8(d).  counts[33..33+L) = the sectors the fused kernel really touches: the same
+// on gathered levels, the distinct cell blocks (32 B, or 64 B = 2 sectors for F = 4) on cell-block levels.
 __global__ void __launch_bounds__(128) niv_sector_census_kernel(const __grid_constant__ KParams P,
                                                                 const float* __restrict__ pos,
                                                                 const float* __restrict__ nrm, size_t n,
-                                                                unsigned long long* __restrict__ counts)
+                                                                unsigned long long* __restrict__ counts, int with_cells)
 {
     __shared__ uint32_t s_sec[4][256];
     const uint32_t lane = threadIdx.x & 31u, warp = threadIdx.x >> 5;
@@ -271,6 +292,16 @@ __global__ void __launch_bounds__(128) niv_sector_census_kernel(const __grid_con
             atomicAdd(&counts[16 + l], (unsigned long long)lin);
         }
         __syncwarp();
+        uint32_t touched = sec;
+        if (with_cells && P.lv[l].cs) {                                       // distinct cells among the warp's texels
+            int c[3] = {0, 0, 0}; float w[3];
+            if (!masked) locate(P.lv[l], u, c, w);
+            const uint32_t ci = masked ? 0xFFFFFFFFu : (uint32_t)c[0] + P.lv[l].cs * (uint32_t)c[1] + P.lv[l].cs2 * (uint32_t)c[2];
+            const uint32_t same = __match_any_sync(0xffffffffu, ci);
+            const bool first = !masked && (__ffs(same) - 1 == (int)lane);
+            touched = __popc(__ballot_sync(0xffffffffu, first)) * (P.n_features == 4 ? 2u : 1u);
+        }
+        if (lane == 0 && touched && with_cells) atomicAdd(&counts[33 + l], (unsigned long long)touched);
     }
 }
 
@@ -281,6 +312,7 @@ __global__ void __launch_bounds__(128) niv_sector_census_kernel(const __grid_con
 // =====================================================================================================
 using namespace niv;
 
+constexpr int kCellBudgetMB = 32;       // default budget of the cell-block copies of the coarse levels
 constexpr uint32_t kCtrSlots = 64;      // dynamically scheduled launches of one model that may be in flight at once
 
 typedef void (*fused_fn)(KParams, const float*, const float*, float*, size_t, uint32_t);
@@ -295,6 +327,8 @@ struct niv_model {
     niv_info info;
     KParams kp;
     uint32_t* d_table = nullptr;
+    uint32_t* d_cells = nullptr;                   // cell-block copies of the coarse levels (KParams::lv[].cells)
+    uint64_t cell_off[kMaxLevels] = {};            //   byte offset of a level's blocks in d_cells
     uint8_t* d_wpack = nullptr;
     std::vector<uint32_t> layer_out, layer_in;     // true (unpadded) shapes
     bool loaded = false;
@@ -375,58 +409,65 @@ static int setup_kernel(niv_model* m, FusedKernel& k, int tmem_cols, const char*
 }
 
 // ---- which instantiation serves which model -----------------------------------------------------------------------
-// O = output as 128-bit stores (pinned host buffers), NPT = per-texel parameters, IMG = image tiling
-template <int W, int L, int F, bool RAWDIR, bool O, int NPT, bool IMG>
+// O = output as 128-bit stores (pinned host buffers), NPT = per-texel parameters, IMG = image tiling,
+// C = read the coarsest min(L, kCellLevels) levels from their cell-block copies
+// how many: BASELINE.json's family (F = 2) five (0.1673 -> 0.1613 / 0.1585 / 0.1567 ms per full-HD frame with 3 / 4 / 5
+// levels; a sixth would take 57 MB); the paper's family (F = 4, 64-byte blocks) four (its 8-level model: 0.1093 ms
+// without, 0.0998 with four, 0.119 with five) -- profiles/r02_cells.md
+constexpr int cell_levels_of(int L, int F) { return F == 4 ? (L < 4 ? L : 4) : (L < 5 ? L : 5); }
+template <int W, int L, int F, bool RAWDIR, bool O, int NPT, bool IMG, bool C>
 static fused_fn fused_inst() {
     // levels per gather batch (two batches in flight): BASELINE.json's family four = 32 gathers; the paper's family
     // (8-byte entries) two = 32 registers
     constexpr int NB = L == 0 ? 1 : F == 4 ? 2 : 4;
-    return niv_fused_kernel<W, L, NB, F, RAWDIR, O, NPT, IMG>;
+    return niv_fused_kernel<W, L, NB, F, RAWDIR, O, NPT, IMG, C ? cell_levels_of(L, F) : 0>;
 }
-template <int W, bool O, int NPT, bool IMG>
+template <int W, bool O, int NPT, bool IMG, bool C>
 static fused_fn pick_levels_f2(uint32_t L) {        // BASELINE.json's family: F = 2, SH-16
     switch (L) {
-        case 4:  return fused_inst<W, 4, 2, false, O, NPT, IMG>();
-        case 8:  return fused_inst<W, 8, 2, false, O, NPT, IMG>();
-        case 12: return fused_inst<W, 12, 2, false, O, NPT, IMG>();
-        case 16: return fused_inst<W, 16, 2, false, O, NPT, IMG>();
+        case 4:  return fused_inst<W, 4, 2, false, O, NPT, IMG, C>();
+        case 8:  return fused_inst<W, 8, 2, false, O, NPT, IMG, C>();
+        case 12: return fused_inst<W, 12, 2, false, O, NPT, IMG, C>();
+        case 16: return fused_inst<W, 16, 2, false, O, NPT, IMG, C>();
         default: return nullptr;
     }
 }
-template <int W, bool O>
+template <int W, bool O, bool C>
 static fused_fn pick_levels_f4(uint32_t L) {        // the paper's own family: F = 4, raw direction
     switch (L) {
-        case 2: return fused_inst<W, 2, 4, true, O, 0, false>();
-        case 4: return fused_inst<W, 4, 4, true, O, 0, false>();
-        case 6: return fused_inst<W, 6, 4, true, O, 0, false>();
-        case 8: return fused_inst<W, 8, 4, true, O, 0, false>();
+        case 2: return fused_inst<W, 2, 4, true, O, 0, false, C>();
+        case 4: return fused_inst<W, 4, 4, true, O, 0, false, C>();
+        case 6: return fused_inst<W, 6, 4, true, O, 0, false, C>();
+        case 8: return fused_inst<W, 8, 4, true, O, 0, false, C>();
         default: return nullptr;
     }
 }
-template <bool O>
+template <bool O, bool C>
 static fused_fn pick_fused(uint32_t W, uint32_t L, uint32_t F) {
     if (L == 0)                                     // grid-less: positional encoding, no gathers
-        return W == 16 ? fused_inst<16, 0, 2, true, O, 0, false>() : W == 32 ? fused_inst<32, 0, 2, true, O, 0, false>()
-             : W == 64 ? fused_inst<64, 0, 2, true, O, 0, false>() : nullptr;
-    if (F == 4) return W == 32 ? pick_levels_f4<32, O>(L) : W == 64 ? pick_levels_f4<64, O>(L) : nullptr;
-    return W == 32 ? pick_levels_f2<32, O, 0, false>(L) : W == 64 ? pick_levels_f2<64, O, 0, false>(L) : nullptr;
+        return W == 16 ? fused_inst<16, 0, 2, true, O, 0, false, false>() : W == 32 ? fused_inst<32, 0, 2, true, O, 0, false, false>()
+             : W == 64 ? fused_inst<64, 0, 2, true, O, 0, false, false>() : nullptr;
+    if (F == 4) return W == 32 ? pick_levels_f4<32, O, C>(L) : W == 64 ? pick_levels_f4<64, O, C>(L) : nullptr;
+    return W == 32 ? pick_levels_f2<32, O, 0, false, C>(L) : W == 64 ? pick_levels_f2<64, O, 0, false, C>(L) : nullptr;
 }
 // image tiling (niv_infer_image): BASELINE.json's family (F = 2, 8..16 levels reach cells smaller than a warp's strip).
 // The paper's own family (F = 4, <= 8 levels, finest cell 5.5 cm) measured SLOWER with it (profiles/r01_v2.md): its
 // cells are larger than a 32-pixel strip anyway; it keeps the linear kernel, as do the grid-less models.
+template <bool C>
 static fused_fn pick_fused_img(uint32_t W, uint32_t L, uint32_t F) {
     if (L == 0 || F != 2) return nullptr;
-    return W == 32 ? pick_levels_f2<32, false, 0, true>(L) : W == 64 ? pick_levels_f2<64, false, 0, true>(L) : nullptr;
+    return W == 32 ? pick_levels_f2<32, false, 0, true, C>(L) : W == 64 ? pick_levels_f2<64, false, 0, true, C>(L) : nullptr;
 }
 // per-texel scene parameters: BASELINE.json's family, 8 or 16 levels, width 32 / 64, 1 or 2 parameters
-template <int W, int NPT>
+template <int W, int NPT, bool C>
 static fused_fn pick_tp_levels(uint32_t L) {
-    return L == 8 ? fused_inst<W, 8, 2, false, false, NPT, false>() : L == 16 ? fused_inst<W, 16, 2, false, false, NPT, false>() : nullptr;
+    return L == 8 ? fused_inst<W, 8, 2, false, false, NPT, false, C>() : L == 16 ? fused_inst<W, 16, 2, false, false, NPT, false, C>() : nullptr;
 }
+template <bool C>
 static fused_fn pick_fused_tp(uint32_t W, uint32_t L, uint32_t F, uint32_t sh_degree, uint32_t n_params) {
     if (F != 2 || sh_degree != 4) return nullptr;
-    if (n_params == 1) return W == 32 ? pick_tp_levels<32, 1>(L) : W == 64 ? pick_tp_levels<64, 1>(L) : nullptr;
-    if (n_params == 2) return W == 32 ? pick_tp_levels<32, 2>(L) : W == 64 ? pick_tp_levels<64, 2>(L) : nullptr;
+    if (n_params == 1) return W == 32 ? pick_tp_levels<32, 1, C>(L) : W == 64 ? pick_tp_levels<64, 1, C>(L) : nullptr;
+    if (n_params == 2) return W == 32 ? pick_tp_levels<32, 2, C>(L) : W == 64 ? pick_tp_levels<64, 2, C>(L) : nullptr;
     return nullptr;
 }
 
@@ -504,13 +545,14 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
         uint64_t N;
         if (explicit_res) N = cfg->resolutions[l];
         else N = (uint64_t)std::floor((double)cfg->base_resolution * std::pow(cfg->per_level_scale, (double)l));
-        if (N == 0 || N >= (1u << 24)) { delete m; return NIV_ERR_INVALID_ARG; }
+        if (N == 0 || N > (1u << 22)) { delete m; return NIV_ERR_INVALID_ARG; }   // locate_bits: N + 2^23 exact in fp32
         const uint64_t R = N + 1;
         const bool dense = R * R * R <= T;
         I.resolution[l] = (uint32_t)N;
         I.is_dense[l] = dense ? 1u : 0u;
         P.lv[l].Nf = (float)N;
         P.lv[l].Nm1 = (int32_t)N - 1;
+        P.lv[l].cmaxf = (float)(8388608u + (uint32_t)N - 1u);               // exact: < 2^24
         P.lv[l].R = (uint32_t)R;
         P.lv[l].R2 = dense ? (uint32_t)(R * R) : 0u;
         P.lv[l].base = (uint32_t)(l * T);
@@ -533,6 +575,31 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     P.out_act = cfg->out_activation;
     I.in_dim = P.in_dim;
     I.table_bytes = (uint64_t)cfg->n_levels * T * cfg->n_features * 2;      // 0 for the grid-less models
+    // cell-block copies of the coarsest min(L, kCellLevels) levels, if their N^3 blocks of 8 entries fit
+    // the budget (NIV_CELL_MB, read once here; 0 = none): the kernels that read them are compiled for exactly that
+    // many levels, so it is all of them or none.  (width 128 and the mma.sync A/B kernel gather from the table)
+    bool use_cells = false;
+    if (cfg->n_levels && cfg->hidden_width <= 64 && !want_mma_sync) {
+        const char* s_mb = getenv("NIV_CELL_MB");
+        const uint64_t budget = (uint64_t)(s_mb ? std::max(0, atoi(s_mb)) : kCellBudgetMB) << 20;
+        const uint32_t want = (uint32_t)cell_levels_of((int)cfg->n_levels, (int)cfg->n_features);
+        uint64_t off = 0;
+        use_cells = true;
+        for (uint32_t l = 0; l < want; ++l) {
+            const uint64_t N = I.resolution[l], bytes = N * N * N * 8 * cfg->n_features * 2;
+            if (N * N * N >= (1u << 24) || off + bytes > budget) { use_cells = false; break; }
+            m->cell_off[l] = off;
+            off += bytes;
+        }
+        if (use_cells) {
+            for (uint32_t l = 0; l < want; ++l) {
+                P.lv[l].cs = I.resolution[l];
+                P.lv[l].cs2 = I.resolution[l] * I.resolution[l];
+            }
+            I.cell_levels = want;
+            I.cell_bytes = off;
+        }
+    }
     I.tile_texels = kTile;
 
     // layer shapes and the packed weight blob layout
@@ -579,21 +646,24 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
         rc = m->fused.fn ? setup_kernel(m, m->fused, 128, "fused_w128") : NIV_ERR_UNSUPPORTED;
     } else {
         const int tmem_cols = 128;                       // D | A | ones in one allocation
-        m->fused.fn = pick_fused<false>(W, cfg->n_levels, cfg->n_features);
+        m->fused.fn = use_cells ? pick_fused<false, true>(W, cfg->n_levels, cfg->n_features)
+                                : pick_fused<false, false>(W, cfg->n_levels, cfg->n_features);
         m->fused.smem = smem_dev;
         rc = m->fused.fn ? setup_kernel(m, m->fused, tmem_cols, "fused") : NIV_ERR_UNSUPPORTED;
         if (rc == NIV_OK) {
-            m->fused_host.fn = pick_fused<true>(W, cfg->n_levels, cfg->n_features);
+            m->fused_host.fn = pick_fused<true, false>(W, cfg->n_levels, cfg->n_features);   // PCIe-bound: table gathers
             m->fused_host.smem = smem_host;
             rc = setup_kernel(m, m->fused_host, tmem_cols, "fused_host");
         }
         if (rc == NIV_OK) {
-            m->fused_img.fn = pick_fused_img(W, cfg->n_levels, cfg->n_features);
+            m->fused_img.fn = use_cells ? pick_fused_img<true>(W, cfg->n_levels, cfg->n_features)
+                                        : pick_fused_img<false>(W, cfg->n_levels, cfg->n_features);
             m->fused_img.smem = smem_dev;
             rc = setup_kernel(m, m->fused_img, tmem_cols, "fused_image");
         }
         if (rc == NIV_OK && cfg->n_params) {
-            m->fused_tp.fn = pick_fused_tp(W, cfg->n_levels, cfg->n_features, cfg->sh_degree, cfg->n_params);
+            m->fused_tp.fn = use_cells ? pick_fused_tp<true>(W, cfg->n_levels, cfg->n_features, cfg->sh_degree, cfg->n_params)
+                                       : pick_fused_tp<false>(W, cfg->n_levels, cfg->n_features, cfg->sh_degree, cfg->n_params);
             if (m->fused_tp.fn) {
                 // layout of the per-texel-parameter variant: layer 1 with K = round16(enc_dim) + 16 n_params, no fold blob
                 m->kp_tp = P;
@@ -609,6 +679,7 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     I.image_tiled = m->fused_img.fn ? 1u : 0u;
     I.texel_params = m->fused_tp.fn ? 1u : 0u;
     e = cudaMalloc(&m->d_table, I.table_bytes ? I.table_bytes : 16);
+    if (e == cudaSuccess && I.cell_bytes) e = cudaMalloc(&m->d_cells, I.cell_bytes);
     if (e == cudaSuccess) e = cudaMalloc(&m->d_wpack, P.wpack_bytes);
     if (e == cudaSuccess && m->fused_tp.fn) e = cudaMalloc(&m->d_wpack_tp, m->kp_tp.wpack_bytes);
     if (e == cudaSuccess) e = cudaMalloc(&m->d_ctr, kCtrSlots * 128);
@@ -629,7 +700,8 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     m->kp_tp.wpack = m->d_wpack_tp;
     for (uint32_t l = 0; l < cfg->n_levels; ++l) {
         P.lv[l].tb = m->d_table + (size_t)P.lv[l].base * (cfg->n_features / 2);
-        m->kp_tp.lv[l].tb = P.lv[l].tb;
+        if (l < I.cell_levels) P.lv[l].cells = reinterpret_cast<const uint4*>(reinterpret_cast<const uint8_t*>(m->d_cells) + m->cell_off[l]);
+        m->kp_tp.lv[l] = P.lv[l];
     }
     *out = m;
     return NIV_OK;
@@ -740,6 +812,12 @@ extern "C" int niv_load_params(niv_model* m, const void* table_fp16, size_t tabl
     }
     if (table_bytes) NIV_CUDA(cudaMemcpyAsync(m->d_table, table_fp16, table_bytes,
                              src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+    for (uint32_t l = 0; l < m->info.cell_levels; ++l) {            // cell-block copies of the coarse levels
+        const uint32_t n_cells = P.lv[l].cs * P.lv[l].cs2;
+        niv_build_cells_kernel<<<(n_cells + 255) / 256, 256, 0, st>>>(
+            P, l, reinterpret_cast<uint32_t*>(reinterpret_cast<uint8_t*>(m->d_cells) + m->cell_off[l]), n_cells);
+        NIV_CUDA(cudaGetLastError());
+    }
     NIV_CUDA(cudaStreamSynchronize(st));
     m->loaded = true;
     return NIV_OK;
@@ -982,9 +1060,9 @@ extern "C" int niv_probe_sectors(niv_model* m, const float* pos, const float* nr
     if (!m) return NIV_ERR_INVALID_ARG;
     if (!m->loaded) return NIV_ERR_NOT_LOADED;
     if (!pos || !nrm || !counts || n == 0) return NIV_ERR_INVALID_ARG;
-    NIV_CUDA(cudaMemsetAsync(counts, 0, 33 * sizeof(uint64_t), (cudaStream_t)stream));
+    NIV_CUDA(cudaMemsetAsync(counts, 0, NIV_CENSUS_COUNTS * sizeof(uint64_t), (cudaStream_t)stream));
     const unsigned grid = (unsigned)((n + 127) / 128);
-    niv_sector_census_kernel<<<grid, 128, 0, (cudaStream_t)stream>>>(m->kp, pos, nrm, n, (unsigned long long*)counts);
+    niv_sector_census_kernel<<<grid, 128, 0, (cudaStream_t)stream>>>(m->kp, pos, nrm, n, (unsigned long long*)counts, 1);
     NIV_CUDA(cudaGetLastError());
     return NIV_OK;
 }
@@ -993,14 +1071,14 @@ extern "C" int niv_probe_sectors_image(const niv_model* m, const float* pos, con
                                        uint32_t height, uint64_t* counts, void* stream)
 {
     if (!m || !pos || !nrm || !counts || width == 0 || height == 0) return NIV_ERR_INVALID_ARG;
-    NIV_CUDA(cudaMemsetAsync(counts, 0, 33 * sizeof(uint64_t), (cudaStream_t)stream));
+    NIV_CUDA(cudaMemsetAsync(counts, 0, NIV_CENSUS_COUNTS * sizeof(uint64_t), (cudaStream_t)stream));
     KParams P = m->kp;
     P.img_w = width;
     P.img_h = height;
     P.tiles_x = (width + 31u) / 32u;
     const unsigned grid = P.tiles_x * ((height + 3u) / 4u);
     niv_sector_census_kernel<<<grid, 128, 0, (cudaStream_t)stream>>>(P, pos, nrm, (size_t)width * height,
-                                                                     (unsigned long long*)counts);
+                                                                     (unsigned long long*)counts, 1);
     NIV_CUDA(cudaGetLastError());
     return NIV_OK;
 }
@@ -1145,6 +1223,7 @@ extern "C" int niv_destroy(niv_model* m)
     if (!m) return NIV_OK;
     cudaSetDevice(m->cfg.device);
     cudaFree(m->d_table);
+    cudaFree(m->d_cells);
     cudaFree(m->d_wpack);
     cudaFree(m->d_wpack_tp);
     cudaFree(m->d_ctr);

@@ -14,12 +14,16 @@ constexpr int kTile = 128;          // texels per CTA tile = MMA M = TMEM lanes
 
 struct LevelP {
     float    Nf;        // (float)N_l, exact
+    float    cmaxf;     // 2^23 + (N_l - 1) as a float: the clamp of the cell in the "floor by addition" form (locate_bits)
     int32_t  Nm1;       // N_l - 1
     uint32_t R;         // N_l + 1 vertices per side (dense stride)
     uint32_t R2;        // R*R
     uint32_t base;      // first table entry of this level = l*T
     uint32_t dense;     // 1 dense, 0 hashed
+    uint32_t cs, cs2;   // cell-block levels: N_l and N_l^2 (cell (cx, cy, cz) is block cx + cs cy + cs2 cz)
     const uint32_t* tb; // this level's first entry = table + base * (F/2) words (a gather address is ONE IMAD.WIDE)
+    const uint4* cells; // cell-block copy of the level: per cell its 8 corner entries, corner j at
+                        // word j * F/2, i.e. 32 B (F = 2) or 64 B (F = 4) per cell; NULL = gather from tb
 };
 
 struct KParams {
@@ -74,14 +78,29 @@ __device__ __forceinline__ void normalise(const KParams& P, const float p[3], fl
 }
 
 // ---------------------------------------------------------------- O2: locate the cell on one level
-__device__ __forceinline__ void locate(const LevelP& lv, const float u[3], int c[3], float w[3]) {
+// c = min(floor(p), N - 1), w = p - (float)c with p = fl32(u N) in [0, N], N <= 2^22, evaluated without a float -> int
+// conversion (F2I / I2F run on the quarter-rate conversion pipe; these are five full-rate FP32 instructions per axis):
+//   t  = p + 2^23 rounded toward -inf  = 2^23 + floor(p) exactly (one ulp at 2^23 is 1)
+//   tc = min(t, 2^23 + N - 1)          = 2^23 + c
+//   cf = tc - 2^23                     = (float)c exactly;   w = fl32(p - cf): the subtraction of step O2
+// The bits of tc are 0x4B000000 + c: locate_bits hands them out as they are (the low 24 bits of 0x4B000000 are zero and
+// so are those of any multiple of it, which is all the hashed and cell-block index arithmetic needs, see below);
+// locate() masks them to the integer cell.
+constexpr float kTwo23 = 8388608.0f;
+__device__ __forceinline__ void locate_bits(const LevelP& lv, const float u[3], uint32_t cb[3], float w[3]) {
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
-        float p = __fmul_rn(u[d], lv.Nf);
-        int ci = min(__float2int_rd(p), lv.Nm1);
-        c[d] = ci;
-        w[d] = __fsub_rn(p, (float)ci);
+        const float p = __fmul_rn(u[d], lv.Nf);
+        const float tc = fminf(__fadd_rd(p, kTwo23), lv.cmaxf);
+        cb[d] = __float_as_uint(tc);
+        w[d] = __fsub_rn(p, __fsub_rn(tc, kTwo23));
     }
+}
+__device__ __forceinline__ void locate(const LevelP& lv, const float u[3], int c[3], float w[3]) {
+    uint32_t cb[3];
+    locate_bits(lv, u, cb, w);
+#pragma unroll
+    for (int d = 0; d < 3; ++d) c[d] = (int)(cb[d] & 0x007FFFFFu);
 }
 
 // ---------------------------------------------------------------- O3: the 8 corner entries, relative to the level's first entry
@@ -99,6 +118,8 @@ __device__ __forceinline__ void corner_entries_dense(const LevelP& lv, const int
     for (int j = 0; j < 8; ++j)
         e[j] = b + (j & 1) + ((j >> 1) & 1) * lv.R + ((j >> 2) & 1) * lv.R2;
 }
+// (c may carry the 0x4B000000 of locate_bits: every term then changes by a multiple of 2^24, which `& tmask` removes,
+//  tmask < 2^24)
 __device__ __forceinline__ void corner_entries_hashed(uint32_t tmask, const int c[3], uint32_t e[8]) {
     uint32_t x0 = (uint32_t)c[0], x1 = x0 + 1u;
     uint32_t y0 = (uint32_t)c[1] * 2654435761u, y1 = y0 + 2654435761u;   // (c+1)*p == c*p + p  (mod 2^32)
@@ -165,7 +186,16 @@ struct Batch {
 // The per-level dense / hashed branch is uniform; it also keeps ptxas from sinking a batch's gathers down to their
 // first use (measured: with the split known at compile time ptxas interleaves loads and blends, 72 registers, and
 // the frame takes 0.208 instead of 0.193 ms even with a warp-level fence between issue and blend).
-template <int NB, int F>
+// 256-bit load (sm_100: one LDG.E.256): a whole F = 2 cell block, or half of an F = 4 one
+__device__ __forceinline__ void ldg256(const void* p, uint32_t* r0, uint32_t* r1, uint32_t* r2, uint32_t* r3,
+                                       uint32_t* r4, uint32_t* r5, uint32_t* r6, uint32_t* r7) {
+    const uint4 a = __ldg(reinterpret_cast<const uint4*>(p)), b = __ldg(reinterpret_cast<const uint4*>(p) + 1);
+    *r0 = a.x; *r1 = a.y; *r2 = a.z; *r3 = a.w; *r4 = b.x; *r5 = b.y; *r6 = b.z; *r7 = b.w;
+}
+// NC: levels 0 .. NC-1 are read from their cell-block copies (known at compile time: a run-time test per level costs
+// ten predicated-off instructions on every level and measured 0.198 instead of 0.167 ms per frame; the dense / hashed
+// test of the other levels stays a run-time uniform branch, see above)
+template <int NB, int F, int NC = 0>
 __device__ __forceinline__ void batch_issue(const KParams& P, int l0, const float u[3], Batch<NB, F>& b) {
     static_assert(F == 2 || F == 4, "F = 2 or 4");
     float wzf[NB + 1];
@@ -173,19 +203,41 @@ __device__ __forceinline__ void batch_issue(const KParams& P, int l0, const floa
 #pragma unroll
     for (int q = 0; q < NB; ++q) {
         const LevelP& lv = P.lv[l0 + q];
-        int c[3];
+        uint32_t cb[3];
         float w[3];
-        uint32_t e[8];
-        locate(lv, u, c, w);
-        corner_entries(lv, P.tmask, c, e);
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
+        locate_bits(lv, u, cb, w);
+        if (l0 + q < NC) {
+            // cell-block level: the 8 corner entries of the cell are one 32-byte (F = 2) / 64-byte (F = 4) block, no
+            // corner indices at all.  (the 0x4B000000 of locate_bits leaves the low 24 bits of the sum alone)
+            const uint32_t ci = (cb[0] + lv.cs * cb[1] + lv.cs2 * cb[2]) & 0x00FFFFFFu;
+            const uint4* blk = lv.cells + (size_t)ci * F;
             if (F == 2) {
-                b.v[q][j][0] = __ldg(lv.tb + e[j]);
+                ldg256(blk, &b.v[q][0][0], &b.v[q][1][0], &b.v[q][2][0], &b.v[q][3][0],
+                       &b.v[q][4][0], &b.v[q][5][0], &b.v[q][6][0], &b.v[q][7][0]);
             } else {
-                const uint2 t = __ldg(reinterpret_cast<const uint2*>(lv.tb) + e[j]);
-                b.v[q][j][0] = t.x;
-                b.v[q][j][F / 2 - 1] = t.y;
+                ldg256(blk, &b.v[q][0][0], &b.v[q][0][F / 2 - 1], &b.v[q][1][0], &b.v[q][1][F / 2 - 1],
+                       &b.v[q][2][0], &b.v[q][2][F / 2 - 1], &b.v[q][3][0], &b.v[q][3][F / 2 - 1]);
+                ldg256(blk + 2, &b.v[q][4][0], &b.v[q][4][F / 2 - 1], &b.v[q][5][0], &b.v[q][5][F / 2 - 1],
+                       &b.v[q][6][0], &b.v[q][6][F / 2 - 1], &b.v[q][7][0], &b.v[q][7][F / 2 - 1]);
+            }
+        } else {
+            uint32_t e[8];
+            if (lv.dense) {
+                const int c[3] = {(int)(cb[0] & 0x007FFFFFu), (int)(cb[1] & 0x007FFFFFu), (int)(cb[2] & 0x007FFFFFu)};
+                corner_entries_dense(lv, c, e);
+            } else {
+                const int c[3] = {(int)cb[0], (int)cb[1], (int)cb[2]};
+                corner_entries_hashed(P.tmask, c, e);
+            }
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                if (F == 2) {
+                    b.v[q][j][0] = __ldg(lv.tb + e[j]);
+                } else {
+                    const uint2 t = __ldg(reinterpret_cast<const uint2*>(lv.tb) + e[j]);
+                    b.v[q][j][0] = t.x;
+                    b.v[q][j][F / 2 - 1] = t.y;
+                }
             }
         }
         b.wxy[q] = pack_half2(w[0], w[1]);
@@ -281,7 +333,8 @@ __device__ __forceinline__ void param_encode8_packed(float t, uint32_t o[8]) { p
 // (tile column | tile row << 16) of a tile index: the one division, done by one thread per tile in the fused kernel
 __device__ __forceinline__ uint32_t image_tile_xy(const KParams& P, uint32_t tile) {
     const uint32_t ty = tile / P.tiles_x, tx = tile - ty * P.tiles_x;
-    return tx | (min(ty, 0xFFFFu) << 16);            // rows past the image (tile indices past the end) stay invalid
+    return tx | (min(ty, 0xFFFFu) << 16);
+           // rows past the image (tile indices past the end) stay invalid
 }
 __device__ __forceinline__ size_t image_texel_xy(const KParams& P, uint32_t txy, uint32_t tid, bool& valid) {
     const uint32_t x = (txy & 0xFFFFu) * 32u + (tid >> 5) * 8u + (tid & 7u), y = (txy >> 16) * 4u + ((tid >> 3) & 3u);

@@ -26,7 +26,8 @@ __device__ __forceinline__ uint32_t pack_relu_half2(float lo, float hi) {
 // width 32 with 16 levels would take 130 registers (3 CTAs per SM): capped at 128; width 64 is left alone, the cap
 // changes its schedule for the worse (0.193 instead of 0.189 ms, profiles/r01_v2.md); the per-texel-parameter
 // variants are capped too (two parameters at width 64 would take 140 registers)
-template <int WIDTH, int L, int NB, int F, bool RAWDIR, bool OUT128, int NPT, bool IMG>
+// NC: the coarsest NC levels are read from their cell-block copies, one 32- / 64-byte load per level
+template <int WIDTH, int L, int NB, int F, bool RAWDIR, bool OUT128, int NPT, bool IMG, int NC>
 __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_fused_kernel(
                                                                const __grid_constant__ KParams P,
                                                                const float* __restrict__ pos,
@@ -34,6 +35,7 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
                                                                float* __restrict__ out, size_t n, uint32_t n_tiles)
 {
     static_assert(WIDTH <= 64, "A-in-TMEM kernel: D + A + ones must fit 128 columns");
+    static_assert(NC <= L, "cell-block levels are the leading levels");
     constexpr uint32_t TMEM_COLS = 128, A_COL = 64, ONES_COL = NPT == 2 ? 104 : 96;
     constexpr int NG = L / NB;
     constexpr int HW = L ? L * F / 2 : 24;            // 32-bit words of hash latents in one A row (L = 0: the
@@ -198,13 +200,13 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
                 for (int d = 0; d < 3; ++d) posenc8_packed(u[d], a + 8 * d);
             } else {
                 Batch<NB, F> ba, bb;
-                batch_issue<NB, F>(P, 0, u, ba);
+                batch_issue<NB, F, NC>(P, 0, u, ba);
                 encode_direction();                   // arithmetic under the first batch's latency
 #pragma unroll
                 for (int g = 0; g < NG; g += 2) {
-                    if (g + 1 < NG) batch_issue<NB, F>(P, (g + 1) * NB, u, bb);
+                    if (g + 1 < NG) batch_issue<NB, F, NC>(P, (g + 1) * NB, u, bb);
                     batch_blend<NB, F>(ba, a + g * NB * (F / 2));
-                    if (g + 2 < NG) batch_issue<NB, F>(P, (g + 2) * NB, u, ba);
+                    if (g + 2 < NG) batch_issue<NB, F, NC>(P, (g + 2) * NB, u, ba);
                     if (g + 1 < NG) batch_blend<NB, F>(bb, a + (g + 1) * NB * (F / 2));
                 }
             }

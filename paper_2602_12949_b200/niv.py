@@ -22,6 +22,7 @@ NIV_ERR_CUDA = -4
 NIV_ERR_ALLOC = -5
 NIV_OUT_LINEAR = 0
 NIV_OUT_SIGMOID = 1
+NIV_CENSUS_COUNTS = 49      # niv_probe_sectors: [0,16) sectors, [16,32) lines, [32] active texels, [33,49) touched
 
 # every symbol include/niv.h declares (tests check that the library exports all of them)
 EXPORTS = ("niv_create", "niv_get_info", "niv_load_params", "niv_infer", "niv_infer_image", "niv_infer_texel_params",
@@ -52,6 +53,7 @@ class NivInfo(C.Structure):
         ("table_bytes", C.c_uint64), ("weight_bytes", C.c_uint64), ("bias_bytes", C.c_uint64),
         ("num_sms", C.c_uint32), ("ctas_per_sm", C.c_uint32), ("tile_texels", C.c_uint32),
         ("smem_bytes", C.c_uint32), ("image_tiled", C.c_uint32), ("texel_params", C.c_uint32),
+        ("cell_levels", C.c_uint32), ("reserved0", C.c_uint32), ("cell_bytes", C.c_uint64),
     ]
 
 
@@ -293,7 +295,7 @@ class NivModel:
             raise NivError(rc, "niv_debug_encode")
 
     def probe_sectors(self, pos, nrm, counts, stream=None):
-        """counts: device int64[33] (include/niv.h niv_probe_sectors)."""
+        """counts: device int64[NIV_CENSUS_COUNTS] (include/niv.h niv_probe_sectors)."""
         import torch
         rc = lib().niv_probe_sectors(self._h, _dev(pos, torch.float32, "pos", 3), _dev(nrm, torch.float32, "nrm", 3),
                                      pos.shape[0], _dev(counts, torch.int64, "counts"), _stream_ptr(stream))

@@ -272,8 +272,8 @@ def test_image_census_counts_fewer_sectors_than_strips(torch_cuda, niv):
     w, h = 640, 360
     g = I.make_gbuffer(w, h, 0)
     dp, dn = torch.from_numpy(g["pos"]).cuda(), torch.from_numpy(g["nrm"]).cuda()
-    a = torch.zeros(33, dtype=torch.int64, device="cuda")
-    b = torch.zeros(33, dtype=torch.int64, device="cuda")
+    a = torch.zeros(niv.NIV_CENSUS_COUNTS, dtype=torch.int64, device="cuda")
+    b = torch.zeros(niv.NIV_CENSUS_COUNTS, dtype=torch.int64, device="cuda")
     m.probe_sectors(dp, dn, a)
     m.probe_sectors_image(dp, dn, w, h, b)
     torch.cuda.synchronize()
@@ -407,6 +407,59 @@ def test_paper_gridless_parity(torch_cuda, niv, oracle, width):
 # ------------------------------------------------------------------------------------------------------
 # edge cases
 # ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("which", ["fullhd", "tiny", "paper8", "paper2", "param_tp"])
+def test_cell_block_levels_are_exact_copies(torch_cuda, niv, oracle, monkeypatch, which):
+    """the coarsest levels are also held as cell blocks (8 corner entries per cell, built at load time
+    through the same corner-index function) and the fused kernels read those instead of gathering.  The values are
+    copies, so the result must be BIT-identical to the same model created with the copies disabled (NIV_CELL_MB=0,
+    read at niv_create), on a loud table (every entry different) -- and both match the oracle."""
+    torch = torch_cuda
+    spec = {"fullhd": I.spec_fullhd(), "tiny": I.spec_tiny(), "paper8": I.spec_paper(8, 64), "paper2": I.spec_paper(2, 32),
+            "param_tp": I.spec_param()}[which]
+    case = Case(spec, 21, table_amp=1.0, bias_scale=0.1)
+    n = 20011
+    pos, nrm = _queries(spec, n, 5, coherent=False)
+    pos[:4000], nrm[:4000] = _queries(spec, 4000, 6, coherent=True)
+    pos[7] = np.asarray(spec.aabb_max, dtype=np.float32)          # u = 1 on every axis: the clamped last cell
+    pos[8] = np.asarray(spec.aabb_min, dtype=np.float32)
+    param = [0.3] if spec.n_params else None
+    m_on = case.gpu_model(niv)
+    want_levels = min(spec.n_levels, 4 if spec.n_features == 4 else 5)
+    assert m_on.info.cell_levels == want_levels and m_on.info.cell_bytes > 0
+    monkeypatch.setenv("NIV_CELL_MB", "0")
+    m_off = case.gpu_model(niv)
+    monkeypatch.delenv("NIV_CELL_MB")
+    assert m_off.info.cell_levels == 0 and m_off.info.cell_bytes == 0
+    a = _gpu_infer(torch, m_on, pos, nrm, param)
+    b = _gpu_infer(torch, m_off, pos, nrm, param)
+    assert np.array_equal(a, b)
+    want = oracle.infer(spec, case.table, case.wblob, case.bblob, pos, nrm,
+                        param=None if param is None else np.float32(param))
+    scale = 1.0 if spec.out_activation == I.OUT_SIGMOID else max(1.0, float(want.max() - want.min()))
+    _check_irradiance(a, want, nrm, pos, scale)
+    if which == "fullhd":                                          # the image-tiled kernel has its own instantiation
+        w, h = 211, 95
+        g = I.make_gbuffer(w, h, 3)
+        dp, dn = torch.from_numpy(g["pos"]).cuda(), torch.from_numpy(g["nrm"]).cuda()
+        oa = torch.full((w * h, 3), float("nan"), device="cuda")
+        ob = torch.full((w * h, 3), float("nan"), device="cuda")
+        m_on.infer_image(dp, dn, oa, w, h)
+        m_off.infer_image(dp, dn, ob, w, h)
+        torch.cuda.synchronize()
+        assert torch.equal(oa, ob)
+    if which == "param_tp":                                        # ... and so has the per-texel-parameter kernel
+        dp, dn = torch.from_numpy(pos).cuda(), torch.from_numpy(nrm).cuda()
+        tp = torch.from_numpy(I.uniform01(77, 3, n).astype(np.float32).reshape(n, 1)).cuda()
+        oa = torch.full((n, 3), float("nan"), device="cuda")
+        ob = torch.full((n, 3), float("nan"), device="cuda")
+        m_on.infer_texel_params(dp, dn, tp, oa)
+        m_off.infer_texel_params(dp, dn, tp, ob)
+        torch.cuda.synchronize()
+        assert torch.equal(oa, ob)
+    m_on.close()
+    m_off.close()
+
+
 @pytest.mark.parametrize("n", [1, 31, 127, 128, 129, 257])
 def test_ragged_sizes(torch_cuda, niv, oracle, n):
     case = Case(I.spec_tiny(), 0)
