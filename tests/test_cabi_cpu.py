@@ -95,3 +95,46 @@ def test_binding_does_not_import_the_oracle():
     assert "import oracle" not in src and "from oracle" not in src
     for f in os.listdir(os.path.join(ROOT, "paper_2602_12949_b200", "csrc")):
         assert "oracle" not in open(os.path.join(ROOT, "paper_2602_12949_b200", "csrc", f)).read().lower()
+
+
+def test_fused_kernels_keep_the_descriptor_uniform(L):
+    """Code-generation guard (profiles/r02_cells.md): when ptxas runs out of uniform registers it keeps the global-memory
+    descriptor in vector registers and re-creates it with two R2UR in front of every gather (+250 instructions, 6 % of a
+    frame).  Counted here: loads `LDG ... desc[URx]` with an `R2UR URx` among the eight instructions before them; a
+    healthy kernel has none or a handful.  Also: the hot kernels must really be tcgen05 / TMEM code (UTCHMMA, LDTM) and
+    the headline ones must not spill."""
+    import shutil
+    import subprocess
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump):
+        pytest.skip("cuobjdump not available")
+    sass = subprocess.run([cuobjdump, "-sass", B.LIB], capture_output=True, text=True, check=True).stdout
+    stats, name, recent = {}, None, []
+    for line in sass.splitlines():
+        m = re.search(r"Function : (\S+)", line)
+        if m:
+            name, recent = m.group(1), []
+            stats[name] = {"recreated": 0, "ldg": 0, "mma": 0, "ldtm": 0, "local": 0}
+            continue
+        if name is None or not re.match(r"\s+/\*[0-9a-f]{4,5}\*/", line):
+            continue
+        st = stats[name]
+        st["mma"] += "UTCHMMA" in line
+        st["ldtm"] += " LDTM" in line
+        st["local"] += (" LDL" in line) or (" STL" in line)
+        g = re.search(r" LDG\.\S* .*desc\[(UR\d+)\]", line)
+        if g:
+            st["ldg"] += 1
+            st["recreated"] += any(re.search(r" R2UR %s," % g.group(1), r) for r in recent)
+        recent = (recent + [line])[-8:]
+    fused = {k: v for k, v in stats.items() if "niv_fused_kernel" in k or "niv_fused_w128_kernel" in k}
+    assert len(fused) >= 40
+    for k, v in fused.items():
+        assert v["mma"] > 0 and v["ldtm"] > 0, k
+        assert v["recreated"] <= max(8, v["ldg"] // 8), (k, v)
+    # the headline kernels (BASELINE.json configs[1]: width 64, 16 levels, F = 2; device path, linear and image tiling,
+    # five cell-block levels) keep everything in registers
+    head = [k for k in fused if re.search(r"ILi64ELi16ELi4ELi2ELb0ELb0ELi0ELb[01]ELi5E", k)]
+    assert len(head) == 2
+    for k in head:
+        assert fused[k]["local"] == 0, (k, fused[k])
