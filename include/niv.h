@@ -17,18 +17,24 @@
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream);
  *   - niv_infer / niv_encode / niv_debug_encode are asynchronous on `stream`, allocate nothing, never
  *     synchronise (CUDA-graph capturable), are read-only on the model's parameters and safe for concurrent callers
- *     on different streams.  Tiles are scheduled dynamically through one of 64 per-model tile counters: a counter is
+ *     on different streams.  Tiles are scheduled dynamically through one of 2048 per-model tile counters: a counter is
  *     handed to a launch only while no earlier launch is still running on it (the last CTA of a launch reports its
  *     counter free through a host-mapped word), so any number of launches may be in flight; a launch that finds all
- *     64 busy, and every launch recorded into a CUDA graph (its replays are invisible to the host), uses static tile
+ *     2048 busy, and every launch recorded into a CUDA graph (its replays are invisible to the host), uses static tile
  *     striding instead -- the same result, only less even on frames with large background regions;
  *   - n <= 2^31 texels per call (NIV_ERR_INVALID_ARG beyond);
  *   - the fused kernels of hidden width <= 64 are launched with programmatic stream serialisation: their prologue
  *     (model-owned memory only) may overlap the tail of the previous kernel of the stream, and they wait for that
  *     kernel's completion (griddepcontrol.wait) before the first access to any buffer of the caller, so stream order
- *     holds for every buffer passed in;
+ *     holds for every buffer passed in.  One case skips that wait: the previous launch on the stream was issued by this
+ *     library and none of its buffers overlaps a buffer of this launch in a way that matters (nothing this launch
+ *     touches is written by it, nothing this launch writes is read by it) -- the two then run beside each other for
+ *     the previous launch's last tiles, and the launches two and three back are known complete (completion words
+ *     polled on the device) before this one touches a buffer.  The result is that of serial execution in every case
+ *     (tests: back-to-back calls on aliased buffers); NIV_OVERLAP=0 turns it off;
  *   - environment knobs, all read ONCE at niv_create and never on the call path: NIV_PDL=0 (no programmatic stream
- *     serialisation), NIV_IMAGE_LINEAR=1 (niv_infer_image through the linear-tile kernel), NIV_HOST_STAGED=1
+ *     serialisation), NIV_OVERLAP=0 (every launch waits for the previous kernel of its stream), NIV_CELL_MB=<n> (budget of
+ *     the cell-block copies of the coarse levels, default 32, 0 = none), NIV_IMAGE_LINEAR=1 (niv_infer_image through the linear-tile kernel), NIV_HOST_STAGED=1
  *     (niv_infer_host through staging copies even for pinned buffers), NIV_MMA_SYNC=1 (the mma.sync A/B kernel for the
  *     BASELINE.json configs[1] shape), NIV_DEBUG=1 (resource report on stderr);
  *   - there is no CPU fallback: without a CUDA device every entry point that needs one returns NIV_ERR_CUDA.

@@ -18,6 +18,7 @@
 #include <mutex>
 #include <new>
 #include <type_traits>
+#include <unordered_map>
 #include <vector>
 
 #include <cuda_fp16.h>
@@ -313,7 +314,7 @@ __global__ void __launch_bounds__(128) niv_sector_census_kernel(const __grid_con
 using namespace niv;
 
 constexpr int kCellBudgetMB = 32;       // default budget of the cell-block copies of the coarse levels
-constexpr uint32_t kCtrSlots = 64;      // dynamically scheduled launches of one model that may be in flight at once
+constexpr uint32_t kCtrSlots = 2048;     // dynamically scheduled launches of one model that may be in flight at once
 
 typedef void (*fused_fn)(KParams, const float*, const float*, float*, size_t, uint32_t);
 
@@ -342,6 +343,7 @@ struct niv_model {
     uint32_t* d_wmma = nullptr;
     // knobs read ONCE, at niv_create (never on the call path)
     bool pdl = true;                               // NIV_PDL=0: no programmatic stream serialisation
+    bool overlap = true;                           // NIV_OVERLAP=0: every launch waits for the previous kernel of its stream
     bool image_linear = false;                     // NIV_IMAGE_LINEAR=1: niv_infer_image through the linear kernel
     bool host_staged = false;                      // NIV_HOST_STAGED=1: niv_infer_host always through staging copies
     bool debug = false;                            // NIV_DEBUG=1: resource report on stderr
@@ -529,6 +531,7 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     if (!m) return NIV_ERR_ALLOC;
     m->cfg = *cfg;
     m->pdl = env_flag("NIV_PDL", true);
+    m->overlap = env_flag("NIV_OVERLAP", true);
     m->image_linear = env_flag("NIV_IMAGE_LINEAR", false);
     m->host_staged = env_flag("NIV_HOST_STAGED", false);
     m->debug = env_flag("NIV_DEBUG", false);
@@ -863,11 +866,71 @@ static void draw_tile_counter(niv_model* m, cudaStream_t st, KParams& P)
     }
 }
 
+// ---- launch overlap -------------------------------------------------------------------------------------------------
+// Back-to-back launches on one stream (one frame per call): with programmatic stream serialisation the
+// CTAs of launch n take the SM slots of launch n-1 as those drain, but griddepcontrol.wait holds them until ALL of n-1
+// has finished, so every launch pays the drain of the last tiles and the fill of the first ones (8 us of a 156 us
+// frame).  If n-1 is a launch of this library whose buffers are disjoint from those of n (nothing n reads or writes is
+// written by n-1, nothing n writes is read by n-1), n does not need that wait: it starts on its own buffers beside the
+// last tiles of n-1.  What keeps this exact:
+//   * the host keeps, per stream, the buffer ranges and completion words of the last three launches it issued there;
+//     any other kernel or copy the caller puts between two launches only adds ordering (it does not trigger early);
+//   * launch n polls the completion words (tile_ctr[2], written with release by the last CTA) of launches n-2 and n-3
+//     before it touches a caller's buffer, so at most two launches ever run beside each other, and it skips the
+//     griddepcontrol.wait only if n-1, n-2 and n-3 all have such a word (launches recorded into a CUDA graph, on the
+//     static-striding fallback or through another kernel have none: the next launches wait in full);
+//   * niv_destroy forgets all history (cudaFree has synchronised the device by then).
+struct LaunchRec {
+    bool tracked = false;
+    uintptr_t lo[4] = {0, 0, 0, 0}, hi[4] = {0, 0, 0, 0};    // pos, nrm, tparam (read), out (written)
+    const uint32_t* done = nullptr;
+    uint32_t gen = 0;
+};
+struct StreamHist { LaunchRec r[3]; };                        // r[0] = the previous launch on the stream, r[1], r[2] before it
+static std::mutex g_hist_mu;
+static std::unordered_map<cudaStream_t, StreamHist> g_hist;
+
+static bool ranges_overlap(const LaunchRec& a, int i, const LaunchRec& b, int j) {
+    return a.lo[i] < b.hi[j] && b.lo[j] < a.hi[i];
+}
+static bool launches_conflict(const LaunchRec& prev, const LaunchRec& cur) {
+    for (int j = 0; j < 4; ++j)
+        if (ranges_overlap(prev, 3, cur, j)) return true;     // cur touches what prev writes
+    for (int i = 0; i < 3; ++i)
+        if (ranges_overlap(prev, i, cur, 3)) return true;     // cur writes what prev reads
+    return false;
+}
+static void forget_history() {
+    std::lock_guard<std::mutex> lock(g_hist_mu);
+    g_hist.clear();
+}
+
 // One launch of a fused kernel; `pdl`: with the programmatic-stream-serialisation attribute (the tcgen05 kernels of
 // width <= 64, which hold their griddepcontrol.wait before the first access to a caller's buffer).
-static int launch_one(const FusedKernel& k, cudaStream_t st, bool pdl, const KParams& P, const float* pos,
+static int launch_one(const niv_model* m, const FusedKernel& k, cudaStream_t st, bool pdl, KParams& P, const float* pos,
                       const float* nrm, float* out, size_t n, uint32_t n_tiles)
 {
+    LaunchRec cur;
+    const void* base[4] = {pos, nrm, P.tparam, out};
+    const size_t bytes[4] = {n * 12, n * 12, P.tparam ? n * 4 * m->cfg.n_params : 0, n * 12};
+    for (int i = 0; i < 4; ++i) { cur.lo[i] = (uintptr_t)base[i]; cur.hi[i] = cur.lo[i] + bytes[i]; }
+    cur.tracked = pdl && m->overlap && P.tile_ctr != nullptr;
+    cur.done = P.tile_ctr ? P.tile_ctr + 2 : nullptr;
+    cur.gen = P.slot_gen;
+    P.grid_wait = 1;
+    P.wait_a = P.wait_b = nullptr;
+    P.gen_a = P.gen_b = 0;
+
+    std::lock_guard<std::mutex> lock(g_hist_mu);
+    if (g_hist.size() > 4096) g_hist.clear();                 // stream handles come and go
+    StreamHist& h = g_hist[st];
+    if (cur.tracked) {                                        // (a launch without a counter slot is being captured: no polls)
+        const LaunchRec *a = &h.r[1], *b = &h.r[2];
+        if (!a->tracked) { a = b; b = nullptr; }
+        if (a && a->tracked) { P.wait_a = a->done; P.gen_a = a->gen; }
+        if (b && b->tracked && P.wait_a) { P.wait_b = b->done; P.gen_b = b->gen; }
+        if (h.r[0].tracked && h.r[1].tracked && h.r[2].tracked && !launches_conflict(h.r[0], cur)) P.grid_wait = 0;
+    }
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
     cfg.gridDim = dim3(n_tiles < k.grid ? n_tiles : k.grid);
@@ -879,8 +942,25 @@ static int launch_one(const FusedKernel& k, cudaStream_t st, bool pdl, const KPa
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = pdl ? 1 : 0;
-    NIV_CUDA(cudaLaunchKernelEx(&cfg, k.fn, P, pos, nrm, out, n, n_tiles));
+    const cudaError_t e = cudaLaunchKernelEx(&cfg, k.fn, P, pos, nrm, out, n, n_tiles);
+    h.r[2] = h.r[1];
+    h.r[1] = h.r[0];
+    h.r[0] = cur;
+    if (e != cudaSuccess) {
+        h.r[0].tracked = false;
+        g_last_cuda_error = (int)e;
+        (void)cudaGetLastError();
+        return NIV_ERR_CUDA;
+    }
     return NIV_OK;
+}
+// a launch that goes around launch_one (the mma.sync A/B kernel, the staged host path): the next ones wait in full
+static void note_untracked_launch(cudaStream_t st) {
+    std::lock_guard<std::mutex> lock(g_hist_mu);
+    StreamHist& h = g_hist[st];
+    h.r[2] = h.r[1];
+    h.r[1] = h.r[0];
+    h.r[0] = LaunchRec();
 }
 
 static int launch_fused(niv_model* m, const KParams& Pin, const float* pos, const float* nrm, float* out,
@@ -890,13 +970,15 @@ static int launch_fused(niv_model* m, const KParams& Pin, const float* pos, cons
     draw_tile_counter(m, st, P);
     if (m->mma_kernel) {                                // warp-granular 32-texel tiles, four per CTA
         const uint32_t nt32 = (uint32_t)((n + 31) / 32), ctas = (nt32 + 3) / 4;
+        note_untracked_launch(st);
         m->fused.fn<<<ctas < m->fused.grid ? ctas : m->fused.grid, kTile, m->fused.smem, st>>>(P, pos, nrm, out, n, nt32);
         NIV_CUDA(cudaGetLastError());
         return NIV_OK;
     }
     const uint32_t n_tiles = (uint32_t)((n + kTile - 1) / kTile);
     const bool tc5 = m->cfg.hidden_width <= 64;          // the kernels with the griddepcontrol pair
-    return launch_one(host_variant ? m->fused_host : m->fused, st, m->pdl && tc5, P, pos, nrm, out, n, n_tiles);
+    // (the zero-copy host variant is followed by a stream synchronisation: it has nothing to overlap with)
+    return launch_one(m, host_variant ? m->fused_host : m->fused, st, m->pdl && tc5 && !host_variant, P, pos, nrm, out, n, n_tiles);
 }
 
 static int check_call(const niv_model* m, const void* pos, const void* nrm, const void* out, size_t n)
@@ -937,7 +1019,7 @@ extern "C" int niv_infer_image(niv_model* m, const float* pos, const float* nrm,
     P.tiles_x = (width + 31u) / 32u;
     const uint32_t n_tiles = P.tiles_x * ((height + 3u) / 4u);
     draw_tile_counter(m, (cudaStream_t)stream, P);
-    return launch_one(m->fused_img, (cudaStream_t)stream, m->pdl, P, pos, nrm, out, n, n_tiles);
+    return launch_one(m, m->fused_img, (cudaStream_t)stream, m->pdl, P, pos, nrm, out, n, n_tiles);
 }
 
 extern "C" int niv_infer_texel_params(niv_model* m, const float* pos, const float* nrm, const float* tparam,
@@ -954,7 +1036,7 @@ extern "C" int niv_infer_texel_params(niv_model* m, const float* pos, const floa
     P.tparam = tparam;
     draw_tile_counter(m, (cudaStream_t)stream, P);
     const uint32_t n_tiles = (uint32_t)((n + kTile - 1) / kTile);
-    return launch_one(m->fused_tp, (cudaStream_t)stream, m->pdl, P, pos, nrm, out, n, n_tiles);
+    return launch_one(m, m->fused_tp, (cudaStream_t)stream, m->pdl, P, pos, nrm, out, n, n_tiles);
 }
 
 extern "C" int niv_infer_host(niv_model* m, const float* pos, const float* nrm, const float* param,
@@ -1221,6 +1303,7 @@ extern "C" int niv_probes_destroy(niv_probe_grid* g)
 extern "C" int niv_destroy(niv_model* m)
 {
     if (!m) return NIV_OK;
+    forget_history();                       // launch records point at this model's completion words
     cudaSetDevice(m->cfg.device);
     cudaFree(m->d_table);
     cudaFree(m->d_cells);

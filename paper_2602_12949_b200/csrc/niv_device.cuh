@@ -43,7 +43,15 @@ struct KParams {
     uint32_t* tile_ctr;         // this launch's (tile, done) counter pair, left zero by the launch's last CTA: dynamic
                                 // tile scheduling; NULL = static striding (launches recorded into a CUDA graph)
     volatile uint32_t* slot_done; // host-mapped word of the counter slot: the last CTA writes slot_gen (slot free again)
-    uint32_t slot_gen;
+    uint32_t slot_gen;          //   (tile_ctr[2] receives it too: the device-visible "launch complete" word)
+    // launch overlap (niv.cu plan_overlap): grid_wait = 1: griddepcontrol.wait before the first access to a caller's
+    // buffer (the previous kernel of the stream is complete); 0: the previous launch is one of this library's on
+    // disjoint buffers, so this one may run beside its last tiles.  wait_a / wait_b: completion words of the two
+    // launches before that one, polled until they reach gen_a / gen_b (NULL: nothing to poll)
+    uint32_t grid_wait;
+    uint32_t gen_a, gen_b;
+    const uint32_t* wait_a;
+    const uint32_t* wait_b;
     const uint32_t* table;      // [L][T] entries of 2 x fp16
     const uint8_t*  wpack;      // packed weights + biases (see niv.cu pack_weights)
     uint32_t wpack_bytes;

@@ -122,7 +122,15 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
     // with TMEM allocated and weights staged; from here on the caller's buffers are read and written, which needs the
     // previous kernel of the stream complete.  The next launch may start filling in behind this one right away.
     pdl_launch_dependents();
-    pdl_wait();
+    if (P.grid_wait) pdl_wait();
+    if (P.wait_a) {                    // launches two and three back: complete before this one touches a buffer
+        if (tid == 0) {
+            while ((int32_t)(ld_acquire_gpu(P.wait_a) - P.gen_a) < 0) __nanosleep(64);
+            if (P.wait_b)
+                while ((int32_t)(ld_acquire_gpu(P.wait_b) - P.gen_b) < 0) __nanosleep(64);
+        }
+        __syncthreads();
+    }
     // G-buffer texel of the first tile; inside the loop the NEXT tile's texel is requested before the current
     // one is encoded, so its HBM latency hides under a whole tile of work (a1 prefetch)
     float pn[3] = {0.f, 0.f, 0.f}, nn[3] = {0.f, 0.f, 0.f};
@@ -351,6 +359,8 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
         if (atomicAdd(P.tile_ctr + 1, 1u) == gridDim.x - 1) {
             P.tile_ctr[0] = 0u;
             P.tile_ctr[1] = 0u;
+            __threadfence();
+            st_release_gpu(P.tile_ctr + 2, P.slot_gen);        // "this launch is complete", for the launches after the next
             if (P.slot_done) *P.slot_done = P.slot_gen;
         }
     }

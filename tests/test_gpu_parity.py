@@ -460,6 +460,63 @@ def test_cell_block_levels_are_exact_copies(torch_cuda, niv, oracle, monkeypatch
     m_off.close()
 
 
+@pytest.mark.parametrize("n", [300, 70001])
+def test_back_to_back_launches_overlap_safely(torch_cuda, niv, monkeypatch, n):
+    """a launch whose buffers are disjoint from those of the launch before it (same stream, this library)
+    does not wait for that launch to finish.  Whatever the aliasing between consecutive calls, the results must be those
+    of strictly serial execution (the same calls with NIV_OVERLAP=0): rotating disjoint buffers (the case that overlaps),
+    one output buffer written by every call, each call reading the previous call's output as its positions, and a
+    foreign kernel between two calls.  n = 300 keeps the grid below the machine size (several launches resident at
+    once), n = 70001 is a few tiles per CTA."""
+    torch = torch_cuda
+    spec = I.spec_fullhd()
+    case = Case(spec, 4, table_amp=1.0, bias_scale=0.1)
+    K = 24
+    rng_pos = [_queries(spec, n, 100 + k)[0] for k in range(4)]
+    nrm = _queries(spec, n, 7)[1]
+
+    def scenario(model):
+        res = {}
+        dn = torch.from_numpy(nrm).cuda()
+        dps = [torch.from_numpy(p).cuda() for p in rng_pos]
+        # (a) rotating disjoint buffers
+        outs = [torch.full((n, 3), float("nan"), device="cuda") for _ in range(K)]
+        for k in range(K):
+            model.infer(dps[k % 4], dn, outs[k])
+        res["rot"] = torch.stack(outs).clone()
+        # (b) every call writes the same output buffer: the last one must win, and every call's result is checked
+        #     through a copy the stream makes right after it
+        out = torch.full((n, 3), float("nan"), device="cuda")
+        snaps = []
+        for k in range(K):
+            model.infer(dps[k % 4], dn, out)
+            if k % 5 == 0:
+                snaps.append(out.clone())              # a foreign kernel between two launches
+        res["same_out"] = out.clone()
+        res["snaps"] = torch.stack(snaps)
+        # (c) a chain: call k reads call k-1's output (values in [0, 1], scaled into the box) as its positions
+        chain = [torch.full((n, 3), float("nan"), device="cuda") for _ in range(3)]
+        model.infer(dps[0], dn, chain[0])
+        for k in range(1, K):
+            src, dst = chain[(k - 1) % 3], chain[k % 3]
+            model.infer(src, dn, dst)
+        res["chain"] = chain[(K - 1) % 3].clone()
+        torch.cuda.synchronize()
+        return res
+
+    m_on = case.gpu_model(niv)
+    a = scenario(m_on)
+    monkeypatch.setenv("NIV_OVERLAP", "0")
+    m_off = case.gpu_model(niv)
+    monkeypatch.delenv("NIV_OVERLAP")
+    b = scenario(m_off)
+    for key in a:
+        assert torch.equal(a[key], b[key]), key
+        assert bool(torch.isfinite(a[key]).all()), key
+    m_on.close()
+    m_off.close()
+
+
 @pytest.mark.parametrize("n", [1, 31, 127, 128, 129, 257])
 def test_ragged_sizes(torch_cuda, niv, oracle, n):
     case = Case(I.spec_tiny(), 0)
