@@ -482,9 +482,13 @@ static void layout_blob(const niv_model* m, KParams& P, uint32_t k1, bool fold_p
         P.kdim[k] = (k == 0) ? k1 : in;
         P.npad[k] = round_up(o, 16);
         P.w_off[k] = off;
-        off += (P.kdim[k] + 16) * P.npad[k] * 2;                 // + the bias K-step: rows (bias_hi, bias_lo, 0, ..)
+        // + the bias K-step.  Only its first group of 8 K rows is stored: (bias_hi, bias_lo, 0 x 6).  Rows 8..15 of
+        // the step are whatever follows in the blob (the next layer's weights, finite by niv_load_params' check; a
+        // zero block after the last layer): the A side of the step is (1, 1, 0 x 14), so they are multiplied by zero.
+        off += (P.kdim[k] + 8) * P.npad[k] * 2;
         in = o;
     }
+    off += P.npad[P.n_layers - 1] * 16;
     for (uint32_t k = 0; k < P.n_layers; ++k) { P.b_off[k] = off; off += P.npad[k] * 4; }
     P.wparam_off = off;
     if (fold_params) off += W * 16 * m->cfg.n_params * 4;
