@@ -37,6 +37,7 @@ W_PX, H_PX = 1920, 1080
 N_TEXELS = W_PX * H_PX
 METRIC = "NIV fused inference throughput on a 1920x1080 G-buffer (ms_per_step = ms per frame)"
 UNIT = "Gqueries/s"
+PROBES_METRIC = "probe-grid query throughput on a 1920x1080 G-buffer (SURVEY 8 f4; ms_per_step = ms per frame)"
 RING = 8                      # distinct input/output buffer sets rotated between steps (8 x 74.6 MB > 126 MB L2)
 
 
@@ -171,24 +172,41 @@ def run_reference(args):
         return
     from oracle import niv_oracle
     niv_oracle.build()
-    spec, table, wb, bb, pos, nrm, param, desc, masked = make_workload(args.workload, 0)
-    prm = None if param is None else np.float32(param)
+    if args.workload == "probes":
+        aabb = I.ROOM_AABB
+        dims = I.probe_grid_dims_for_spacing(aabb[0], aabb[1], args.probe_spacing)
+        coeffs = I.make_probe_grid(dims, 0)
+        g = I.make_gbuffer(W_PX, H_PX, 0, frame=0)
+        pos, nrm = g["pos"], g["nrm"]
+        desc = "configs[1] G-buffer queried in a %dx%dx%d grid of SH-2 probes" % dims
+
+        spec = None
+
+        def once(sp, sn):
+            niv_oracle.probe_query(dims, aabb[0], aabb[1], coeffs, sp, sn)
+    else:
+        spec, table, wb, bb, pos, nrm, param, desc, masked = make_workload(args.workload, 0)
+        prm = None if param is None else np.float32(param)
+
+        def once(sp, sn):
+            niv_oracle.infer(spec, table, wb, bb, sp, sn, param=prm)
     sp, sn, n_s = oracle_sample(pos, nrm, args.ref_sample)
     for _ in range(args.warmup):
-        niv_oracle.infer(spec, table, wb, bb, sp, sn, param=prm)
+        once(sp, sn)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        niv_oracle.infer(spec, table, wb, bb, sp, sn, param=prm)
+        once(sp, sn)
     dt = (time.perf_counter() - t0) / args.steps
     val = n_s / dt / 1e9
     cores = niv_oracle.max_threads()
     sample = "%d of %d texels per step (every k-th 128-texel tile of the frame)" % (n_s, N_TEXELS)
     print(json.dumps({
-        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "impl": "reference", "metric": PROBES_METRIC if args.workload == "probes" else METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "ms_per_frame_extrapolated":
         dt * 1e3 * N_TEXELS / n_s, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
-        "config": {"workload": args.workload, "description": desc, "model": _model_str(spec)},
+        "config": {"workload": args.workload, "description": desc,
+                   "model": _model_str(spec) if spec is not None else "SH-2 probe grid, 27 fp16 per probe"},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -451,6 +469,134 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_probes(args):
+    """the paper's probe-grid baseline as a second workload over the configs[1] G-buffer:
+    a regular SH-2 probe grid at the memory budget the paper compares at ("5.4 MB budget": 54 B per probe
+    -> ~100 k probes, 0.16 m apart in the 10 x 4 x 10 m room), queried once per texel.  Same JSON contract."""
+    import torch
+
+    from paper_2602_12949_b200 import build as B
+    from paper_2602_12949_b200 import niv
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    if _env_int("WORLD_SIZE", 1) != 1:
+        raise SystemExit("--workload probes is a one-GPU line")
+    torch.cuda.set_device(0)
+    B.build()
+    niv.lib()
+    aabb = I.ROOM_AABB
+    dims = I.probe_grid_dims_for_spacing(aabb[0], aabb[1], args.probe_spacing)
+    coeffs = I.make_probe_grid(dims, 0)
+    g = I.make_gbuffer(W_PX, H_PX, 0, frame=0)
+    pos, nrm, masked = g["pos"], g["nrm"], g["masked_fraction"]
+    n = pos.shape[0]
+    grid = niv.NivProbeGrid(dims, aabb[0], aabb[1], cosine_falloff=True)
+    grid.load(coeffs)
+    d_pos = [torch.from_numpy(pos).cuda() for _ in range(RING)]
+    d_nrm = [torch.from_numpy(nrm).cuda() for _ in range(RING)]
+    d_out = [torch.empty((n, 3), dtype=torch.float32, device="cuda") for _ in range(RING)]
+    stream = torch.cuda.current_stream()
+    for s in range(args.warmup):
+        grid.query(d_pos[s % RING], d_nrm[s % RING], d_out[s % RING])
+    ev_a, ev_b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    clocks = ClockSampler(0)
+    ev_a.record(stream)
+    for s in range(args.steps):
+        grid.query(d_pos[s % RING], d_nrm[s % RING], d_out[s % RING])
+    ev_b.record(stream)
+    torch.cuda.synchronize()
+    ms_step = ev_a.elapsed_time(ev_b) / args.steps
+    t_end = time.time() + 0.3
+    while time.time() < t_end:
+        grid.query(d_pos[0], d_nrm[0], d_out[0])
+        torch.cuda.synchronize()
+    clk = clocks.stop()
+    # end to end: pinned host buffers, copies inside the timed region (the probe query has no host entry point of its own)
+    h_pos, h_nrm = torch.from_numpy(pos).pin_memory(), torch.from_numpy(nrm).pin_memory()
+    h_out = torch.empty((n, 3), dtype=torch.float32).pin_memory()
+    e2e_steps = max(3, min(args.steps, 20))
+
+    def e2e_once():
+        d_pos[0].copy_(h_pos, non_blocking=True)
+        d_nrm[0].copy_(h_nrm, non_blocking=True)
+        grid.query(d_pos[0], d_nrm[0], d_out[0])
+        h_out.copy_(d_out[0], non_blocking=True)
+        torch.cuda.synchronize()
+
+    for _ in range(2):
+        e2e_once()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        e2e_once()
+    e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
+
+    peaks = load_peaks()
+    counts = torch.zeros(2, dtype=torch.int64, device="cuda")
+    grid.census(d_pos[0], d_nrm[0], counts)
+    torch.cuda.synchronize()
+    sectors, n_active = int(counts[0].item()), int(counts[1].item())
+    grid_bytes = 64 * dims[0] * dims[1] * dims[2]
+    info_sms = torch.cuda.get_device_properties(0).multi_processor_count
+    gpeak, probe_bytes = measure_gather_peak(torch, niv, grid_bytes, info_sms)
+    kernel_s = ms_step * 1e-3
+    hbm_bytes = 36 * n
+    t_gather = sectors * 32 / (gpeak["random_sector"]["sector_gbs"] * 1e9)
+    t_hbm = hbm_bytes / (peaks["hbm_gbs"] * 1e9)
+    t_all = {"l2-gather": t_gather, "hbm": t_hbm}
+    bound = max(t_all, key=t_all.get)
+    roofline = {
+        "bound": bound, "kernel": "niv_probes_query_kernel",
+        "achieved": {"l2-gather": sectors * 32 / kernel_s / 1e9, "hbm": hbm_bytes / kernel_s / 1e9}[bound],
+        "peak": {"l2-gather": gpeak["random_sector"]["sector_gbs"], "hbm": peaks["hbm_gbs"]}[bound], "unit": "GB/s",
+        "frac": t_all[bound] / kernel_s, "traffic": None,
+        "peak_source": ("measured in this run: niv_probe_gather, random 32 B sectors of a resident %d MiB buffer" % (probe_bytes >> 20))
+        if bound == "l2-gather" else peaks["source"],
+        "algorithmic": {"sectors_per_launch": sectors, "sectors_per_active_texel": sectors / max(n_active, 1),
+                        "active_texels": n_active, "probes_per_texel": 8, "bytes_per_probe_record": 64,
+                        "hbm_bytes_per_texel": 36},
+        "t_roofline_us": {"l2_gather": t_gather * 1e6, "hbm": t_hbm * 1e6},
+        "hbm": {"achieved": hbm_bytes / kernel_s / 1e9, "peak": peaks["hbm_gbs"], "frac": t_hbm / kernel_s},
+        "l2_gather": {"achieved": sectors * 32 / kernel_s / 1e9, "peak": gpeak["random_sector"]["sector_gbs"],
+                      "frac": t_gather / kernel_s},
+    }
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import niv_oracle
+        niv_oracle.build()
+        sp, sn, n_s = oracle_sample(pos, nrm, 262144)
+        t0 = time.perf_counter()
+        niv_oracle.probe_query(dims, aabb[0], aabb[1], coeffs, sp, sn)
+        rate = n_s / (time.perf_counter() - t0)
+        sp, sn, n_s = oracle_sample(pos, nrm, int(min(n, max(262144, rate * args.cpu_budget))))
+        t0 = time.perf_counter()
+        niv_oracle.probe_query(dims, aabb[0], aabb[1], coeffs, sp, sn)
+        dt = time.perf_counter() - t0
+        cpu = {"value": n_s / dt / 1e9, "unit": UNIT, "cores": niv_oracle.max_threads(), "kind": "oracle",
+               "sample": "%d of %d texels (every k-th 128-texel tile of the frame), %.1f s" % (n_s, n, dt)}
+    out = {
+        "metric": PROBES_METRIC,
+        "value": n / kernel_s / 1e9, "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f16 probes / f32 arithmetic (cell: f32 + u32)", "data": "synthetic",
+        "config": {"workload": "probes", "description": "configs[1] G-buffer (%.1f%% background) queried in a %dx%dx%d grid of "
+                   "SH-2 probes, %.2f m apart (%.2f MB at the paper's 54 B per probe; 64 B records on the device), cosine "
+                   "fall-off on" % (100 * masked, dims[0], dims[1], dims[2], args.probe_spacing,
+                                    54 * dims[0] * dims[1] * dims[2] / 1e6),
+                   "texels_per_gpu_per_step": n, "masked_fraction": masked,
+                   "l2": "inputs/outputs rotate over %d distinct buffer sets (%.0f MB > 126 MB L2)" % (RING, RING * 36 * n / 1e6)},
+        "e2e": {"value": n / (e2e_ms * 1e-3) / 1e9, "unit": UNIT, "ms_per_step": e2e_ms, "steps": e2e_steps,
+                "h2d_bytes_per_step": 24 * n, "d2h_bytes_per_step": 12 * n,
+                "api": "pinned host buffers -> cudaMemcpyAsync -> niv_probes_query -> cudaMemcpyAsync, synchronised per step"},
+        "gpu_launches": args.steps, "clocks": clk, "roofline": roofline,
+    }
+    if cpu:
+        out["cpu_baseline"] = cpu
+    print(json.dumps(out))
+    grid.close()
+
+
 def run_sweep(args):
     """BASELINE.json configs[4]: table size x MLP width at full HD, and resolution x frames per call.  One JSON line
     per case on stdout (NOT the contract line: a table for profiles/)."""
@@ -572,7 +718,9 @@ def main():
     ap.add_argument("--steps", type=int, default=None)
     ap.add_argument("--warmup", type=int, default=None)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="fullhd", choices=["fullhd", "incoherent", "param", "paper"])
+    ap.add_argument("--workload", default="fullhd", choices=["fullhd", "incoherent", "param", "paper", "probes"])
+    ap.add_argument("--probe-spacing", type=float, default=0.16, help="workload probes: probe spacing in metres (0.16 m = "
+                    "the 5.4 MB budget of PAPER.md:462 in the 10 x 4 x 10 m room)")
     ap.add_argument("--paper-levels", type=int, default=8, choices=[0, 2, 4, 6, 8], help="workload paper: grid levels (0 = none)")
     ap.add_argument("--paper-width", type=int, default=64, choices=[16, 32, 64])
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -606,7 +754,10 @@ def main():
     else:
         args.steps = 200 if args.steps is None else args.steps
         args.warmup = 20 if args.warmup is None else max(args.warmup, 3)
-        run_ours(args)
+        if args.workload == "probes":
+            run_probes(args)
+        else:
+            run_ours(args)
 
 
 if __name__ == "__main__":
