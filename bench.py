@@ -353,6 +353,29 @@ def run_ours(args):
     e2e_value = D.whole_job_gqps(n, world, e2e_ms)
     checksum = float(h_out[0].sum())
 
+    # ---- the same end-to-end call on the compact G-buffer formats / fp16 output: fewer bytes per
+    #      texel over PCIe.  Formats of include/niv.h; the packing is the producer's job and is not timed.
+    e2e_compact = []
+    if spec.hidden_width <= 64 and spec.n_levels and not args.no_compact_e2e:
+        aabb = (spec.aabb_min, spec.aabb_max)
+        for gf, of, name in ((I.GBUF_P32_OCT16, I.OUTFMT_F16X4, "pos fp32 x 3 + oct16 normal (16 B) -> fp16 x 4 (8 B)"),
+                             (I.GBUF_P16_OCT8, I.OUTFMT_F16X4, "pos unorm16 x 3 + oct8 normal (8 B) -> fp16 x 4 (8 B)")):
+            a, b = I.pack_gbuffer(gf, pos, nrm, aabb)
+            ha = [torch.from_numpy(a).pin_memory() for _ in range(2)]
+            ho = [torch.empty((n, 4), dtype=torch.int16).pin_memory() for _ in range(2)]
+            for s in range(3):
+                model.infer_host_packed(gf, ha[s % 2], None, ho[s % 2], n, out_format=of, param=param)
+            barrier()
+            t0 = time.perf_counter()
+            for s in range(e2e_steps):
+                model.infer_host_packed(gf, ha[s % 2], None, ho[s % 2], n, out_format=of, param=param)
+            torch.cuda.synchronize()
+            ms = D.reduce_max((time.perf_counter() - t0) * 1e3 / e2e_steps, "cuda")
+            e2e_compact.append({"formats": name, "gbuf_format": gf, "out_format": of, "value": D.whole_job_gqps(n, world, ms),
+                                "unit": UNIT, "ms_per_step": ms, "h2d_bytes_per_step": int(a.nbytes), "d2h_bytes_per_step": 8 * n,
+                                "api": "niv_infer_host_packed (pinned host buffers, zero copy)"})
+            del ha, ho
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -461,6 +484,8 @@ def run_ours(args):
                 "checksum": checksum},
         "gpu_launches": args.steps, "clocks": clk, "roofline": roofline,
     }
+    if e2e_compact:
+        out["e2e_compact"] = e2e_compact
     if cpu:
         out["cpu_baseline"] = cpu
     print(json.dumps(out))
@@ -724,6 +749,7 @@ def main():
     ap.add_argument("--paper-levels", type=int, default=8, choices=[0, 2, 4, 6, 8], help="workload paper: grid levels (0 = none)")
     ap.add_argument("--paper-width", type=int, default=64, choices=[16, 32, 64])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-compact-e2e", action="store_true", help="skip the end-to-end legs on the compact G-buffer formats")
     ap.add_argument("--compose", action="store_true", help="SURVEY 8(f2): time the compose kernel (HBM roofline)")
     ap.add_argument("--tiling", default="image", choices=["image", "linear"],
                     help="device path of the G-buffer workloads: niv_infer_image (default) or niv_infer")

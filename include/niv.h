@@ -63,6 +63,16 @@ enum {
     NIV_ERR_ALLOC       = -5    /* host or device allocation failed                               */
 };
 
+/* G-buffer and output formats of the *_packed entry points (readings in DESIGN.md 3.4, 3.5) */
+enum { NIV_GBUF_F32X3 = 0,        /* pos[n][3], nrm[n][3] fp32: the format of niv_infer                                */
+       NIV_GBUF_F32X4 = 1,        /* pos[n][4], nrm[n][4] fp32 (xyzw, stride 16 bytes, w ignored)                      */
+       NIV_GBUF_P32_OCT16 = 2,    /* one array, 16 bytes per texel: x, y, z fp32 | octahedral normal 2 x snorm16
+                                     (low half = x); both halves 0x8000 = background                                  */
+       NIV_GBUF_P16_OCT8 = 3 };   /* one array, 8 bytes per texel: position 3 x unorm16 of the model's AABB |
+                                     octahedral normal 2 x snorm8; both 0x80 = background                            */
+enum { NIV_OUTFMT_F32X3 = 0,      /* out[n][3] fp32                                                                    */
+       NIV_OUTFMT_F16X4 = 1 };    /* out[n][4] fp16: (r, g, b, 0), round to nearest even of the fp32 result           */
+
 enum { NIV_OUT_LINEAR = 0,      /* the paper: no activation on the final layer     */
        NIV_OUT_SIGMOID = 1 };   /* BASELINE.json configs[0]                                       */
 
@@ -180,6 +190,29 @@ int niv_infer_texel_params(niv_model *m, const float *pos, const float *nrm, con
  * concurrent callers on the same model.  Errors as niv_infer, plus NIV_ERR_ALLOC. */
 int niv_infer_host(niv_model *m, const float *pos, const float *nrm, const float *param,
                    float *out, size_t n, void *stream);
+
+/* ---- compact G-buffer formats and fp16 output -------------------------------------------------
+ * The paper only says "position and normal buffers"; engines keep G-buffers in many layouts, and on the
+ * end-to-end path every byte per texel crosses PCIe.  The *_packed entry points are niv_infer / niv_infer_image /
+ * niv_infer_host with the layouts named by NIV_GBUF_* and NIV_OUTFMT_* above (readings and decode steps in DESIGN.md
+ * 3.4 / 3.5):
+ *   gbuf_a, gbuf_b  F32X3, F32X4: the position and the normal array; P32_OCT16, P16_OCT8: gbuf_a = the one array of
+ *                   n records, gbuf_b ignored (may be NULL).  Alignment: 4 / 16 / 16 / 8 bytes.
+ *   out             F32X3: [n][3] fp32;  F16X4: [n][4] fp16 (8-byte aligned)
+ * A texel is decoded to an fp32 position and an fp32 unit normal first -- the position by a pinned fp32 op sequence,
+ * so the cells and hash indices are those of niv_infer on the decoded values, bit for bit -- and then takes the path of
+ * niv_infer.  Grid models of hidden width <= 64 only (NIV_ERR_UNSUPPORTED for width 128 and for the grid-less models);
+ * niv_infer_image_packed runs the linear-tile kernel for every format but fp32 x 3 in and out; unknown formats and
+ * misaligned buffers -> NIV_ERR_INVALID_ARG; otherwise as the unpacked entry points. */
+int niv_infer_packed(niv_model *m, int gbuf_format, const void *gbuf_a, const void *gbuf_b, const float *param,
+                     int out_format, void *out, size_t n, void *stream);
+int niv_infer_image_packed(niv_model *m, int gbuf_format, const void *gbuf_a, const void *gbuf_b, const float *param,
+                           int out_format, void *out, uint32_t width, uint32_t height, void *stream);
+int niv_infer_host_packed(niv_model *m, int gbuf_format, const void *gbuf_a, const void *gbuf_b, const float *param,
+                          int out_format, void *out, size_t n, void *stream);
+/* The fp32 position and normal ([n][3] each, device) the fused kernels decode from a compact G-buffer (device). */
+int niv_decode_gbuffer(niv_model *m, int gbuf_format, const void *gbuf_a, const void *gbuf_b, float *pos, float *nrm,
+                       size_t n, void *stream);
 
 /* Stand-alone encoding kernel (rows a1..a9 without the MLP): features_fp16 is device, [n][in_dim] fp16
  * row-major = [latents | SH-16 | parameter encoding], zero rows for background texels.  F = 2 family only

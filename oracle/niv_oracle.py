@@ -239,3 +239,31 @@ def probe_query(dims, bbox_min, bbox_max, coeffs, pos, nrm, cosine_falloff=True,
     if rc:
         raise ValueError("niv_oracle_probe_query failed")
     return (out32, out64, w, pi) if debug else out32
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# compact G-buffer formats and fp16 output (niv_oracle_ext.c)
+def decode_gbuffer(fmt: int, bbox_min, bbox_max, a, b=None):
+    """-> (pos [n][3] fp32, nrm [n][3] fp32) of a G-buffer in format 0..3."""
+    a = np.ascontiguousarray(a)
+    rec = {0: 12, 1: 16, 2: 16, 3: 8}[int(fmt)]
+    n = a.nbytes // rec
+    if b is not None:
+        b = np.ascontiguousarray(b)
+    lo = (C.c_float * 3)(*[float(v) for v in bbox_min])
+    hi = (C.c_float * 3)(*[float(v) for v in bbox_max])
+    pos = np.zeros((n, 3), dtype=np.float32)
+    nrm = np.zeros((n, 3), dtype=np.float32)
+    rc = lib().niv_oracle_decode_gbuffer(C.c_int(int(fmt)), lo, hi, _p(a), _p(b), C.c_size_t(n), _p(pos), _p(nrm))
+    if rc:
+        raise ValueError("niv_oracle_decode_gbuffer failed")
+    return pos, nrm
+
+
+def quantise_f16x4(e) -> np.ndarray:
+    """[n][3] fp32 -> [n][4] uint16: (r, g, b, 0) as binary16 bit patterns, round to nearest even."""
+    e = _chk(e, np.float32, "e")
+    out = np.zeros((e.shape[0], 4), dtype=np.uint16)
+    if lib().niv_oracle_quantise_f16x4(_p(e), C.c_size_t(e.shape[0]), _p(out)):
+        raise ValueError("niv_oracle_quantise_f16x4 failed")
+    return out

@@ -139,3 +139,113 @@ int niv_oracle_probe_query(const uint32_t dims[3], const float bmin[3], const fl
     }
     return 0;
 }
+
+/* =====================================================================================================
+ * Compact G-buffer formats.  PAPER.md:402-403 says "position and normal buffers" and nothing about
+ * their layout; the formats are this build's readings.  A texel is DECODED to an fp32 position and
+ * an fp32 normal, and everything downstream (O0..O9) is defined on the decoded values.
+ *   format 0  pos[n][3], nrm[n][3] fp32                                   (the layout of niv_oracle_infer)
+ *   format 1  pos[n][4], nrm[n][4] fp32, w ignored
+ *   format 2  one array of 16-byte records: x, y, z fp32 | oct, 2 x snorm16 (low half = first component)
+ *   format 3  one array of 8-byte records: qx, qy, qz unorm16 of the box | oct, 2 x snorm8
+ * D1 position, format 3 (fp32, one rounded operation per line -- it decides cells):
+ *        u = fl32((float)q * fl32(1 / 65535));  t = fl32(u * fl32(max - min));  x = fl32(t + min)
+ * D2 normal, formats 2 / 3: components v in [-32767, 32767] / [-127, 127] -> f = v / 32767 (/ 127); the reserved code
+ *        (-32768, -32768) / (-128, -128) is "background": normal (0, 0, 0), which O0 masks.  Octahedral map:
+ *        z = 1 - |fx| - |fy|;  if z < 0: (x, y) = ((1 - |fy|) sgn fx, (1 - |fx|) sgn fy) with sgn 0 = +1, else (fx, fy);
+ *        n = (x, y, z) / |(x, y, z)|   in fp64, rounded to fp32 at the end.
+ * ===================================================================================================== */
+static void oct_decode(double fx, double fy, double n[3])
+{
+    double z = 1.0 - fabs(fx) - fabs(fy), x = fx, y = fy;
+    if (z < 0.0) {
+        x = copysign(1.0 - fabs(fy), fx);
+        y = copysign(1.0 - fabs(fx), fy);
+    }
+    const double r = sqrt(x * x + y * y + z * z);
+    n[0] = x / r; n[1] = y / r; n[2] = z / r;
+}
+
+int niv_oracle_decode_gbuffer(int format, const float bmin[3], const float bmax[3], const void *a, const void *b,
+                              size_t n, float *pos, float *nrm)
+{
+    if (!a || !pos || !nrm || format < 0 || format > 3) return -1;
+    if (format <= 1 && !b) return -1;
+    if (format == 3 && (!bmin || !bmax)) return -1;
+    for (size_t i = 0; i < n; ++i) {
+        if (format <= 1) {
+            const size_t s = format == 0 ? 3 : 4;
+            for (int d = 0; d < 3; ++d) {
+                pos[3 * i + d] = ((const float *)a)[s * i + d];
+                nrm[3 * i + d] = ((const float *)b)[s * i + d];
+            }
+        } else if (format == 2) {
+            const uint8_t *r = (const uint8_t *)a + 16 * i;
+            uint32_t o;
+            memcpy(pos + 3 * i, r, 12);
+            memcpy(&o, r + 12, 4);
+            const int ox = (int16_t)(o & 0xFFFFu), oy = (int16_t)(o >> 16);
+            if (ox == -32768 && oy == -32768) {
+                nrm[3 * i] = nrm[3 * i + 1] = nrm[3 * i + 2] = 0.0f;
+            } else {
+                double v[3];
+                oct_decode(ox / 32767.0, oy / 32767.0, v);
+                for (int d = 0; d < 3; ++d) nrm[3 * i + d] = (float)v[d];
+            }
+        } else {
+            const uint8_t *r = (const uint8_t *)a + 8 * i;
+            uint16_t q[3];
+            memcpy(q, r, 6);
+            const float k = 1.0f / 65535.0f;
+            for (int d = 0; d < 3; ++d) {                        /* D1 */
+                const float ext = bmax[d] - bmin[d];
+                const float u = (float)q[d] * k;
+                const float t = u * ext;
+                pos[3 * i + d] = t + bmin[d];
+            }
+            const int ox = (int8_t)r[6], oy = (int8_t)r[7];
+            if (ox == -128 && oy == -128) {
+                nrm[3 * i] = nrm[3 * i + 1] = nrm[3 * i + 2] = 0.0f;
+            } else {
+                double v[3];
+                oct_decode(ox / 127.0, oy / 127.0, v);
+                for (int d = 0; d < 3; ++d) nrm[3 * i + d] = (float)v[d];
+            }
+        }
+    }
+    return 0;
+}
+
+/* =====================================================================================================
+ * fp16 output ("fp16 / packed output formats"): out[i] = (r, g, b, 0) as four IEEE
+ * binary16 values, each the round-to-nearest-even of the fp32 result (overflow -> infinity, subnormals kept).
+ * ===================================================================================================== */
+static uint16_t float_to_half_rne(float f)
+{
+    uint32_t x;
+    memcpy(&x, &f, 4);
+    const uint32_t sign = (x >> 16) & 0x8000u;
+    const uint32_t mag = x & 0x7FFFFFFFu;
+    if (mag >= 0x7F800000u) return (uint16_t)(sign | 0x7C00u | ((mag > 0x7F800000u) ? 0x200u : 0u));   /* inf / nan */
+    if (mag >= 0x477FF000u) return (uint16_t)(sign | 0x7C00u);            /* >= 65520 rounds to infinity */
+    if (mag < 0x33000001u) return (uint16_t)sign;                         /* <= 2^-25: rounds to zero (ties to even) */
+    int e = (int)(mag >> 23) - 127;
+    uint32_t m = (mag & 0x7FFFFFu) | 0x800000u;                           /* 24-bit significand */
+    int shift = (e < -14) ? (13 + (-14 - e)) : 13;                        /* bits dropped */
+    uint32_t half = m >> shift;
+    const uint32_t rem = m & ((1u << shift) - 1u), halfway = 1u << (shift - 1);
+    if (rem > halfway || (rem == halfway && (half & 1u))) ++half;
+    if (e < -14) return (uint16_t)(sign | half);                          /* subnormal (a carry makes it the smallest normal) */
+    /* normal: half holds 1.mantissa (11 bits); a carry out of the mantissa bumps the exponent by itself */
+    return (uint16_t)(sign | ((uint32_t)((e + 15) << 10) + (half - 0x400u)));
+}
+
+int niv_oracle_quantise_f16x4(const float *e, size_t n, uint16_t *out)
+{
+    if (!e || !out) return -1;
+    for (size_t i = 0; i < n; ++i) {
+        for (int c = 0; c < 3; ++c) out[4 * i + c] = float_to_half_rne(e[3 * i + c]);
+        out[4 * i + 3] = 0;
+    }
+    return 0;
+}

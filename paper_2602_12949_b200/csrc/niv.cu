@@ -335,6 +335,7 @@ struct niv_model {
     bool loaded = false;
     FusedKernel fused;                             // niv_infer
     FusedKernel fused_host;                        // niv_infer_host, pinned buffers: 128-bit output stores
+    FusedKernel fused_pk, fused_host_pk;           // *_packed entry points: compact G-buffer formats / fp16 output
     FusedKernel fused_img;                         // niv_infer_image: 8 x 4 pixel blocks per warp
     FusedKernel fused_tp;                          // niv_infer_texel_params: parameter columns as K-steps of layer 1,
     KParams kp_tp;                                 //   with its own packed weights and shared-memory layout
@@ -417,40 +418,43 @@ static int setup_kernel(niv_model* m, FusedKernel& k, int tmem_cols, const char*
 // levels; a sixth would take 57 MB); the paper's family (F = 4, 64-byte blocks) four (its 8-level model: 0.1093 ms
 // without, 0.0998 with four, 0.119 with five) -- profiles/r02_cells.md
 constexpr int cell_levels_of(int L, int F) { return F == 4 ? (L < 4 ? L : 4) : (L < 5 ? L : 5); }
-template <int W, int L, int F, bool RAWDIR, bool O, int NPT, bool IMG, bool C>
+template <int W, int L, int F, bool RAWDIR, bool O, int NPT, bool IMG, bool C, bool PK = false>
 static fused_fn fused_inst() {
     // levels per gather batch (two batches in flight): BASELINE.json's family four = 32 gathers; the paper's family
     // (8-byte entries) two = 32 registers
     constexpr int NB = L == 0 ? 1 : F == 4 ? 2 : 4;
-    return niv_fused_kernel<W, L, NB, F, RAWDIR, O, NPT, IMG, C ? cell_levels_of(L, F) : 0>;
+    return niv_fused_kernel<W, L, NB, F, RAWDIR, O, NPT, IMG, C ? cell_levels_of(L, F) : 0, PK>;
 }
-template <int W, bool O, int NPT, bool IMG, bool C>
+template <int W, bool O, int NPT, bool IMG, bool C, bool PK = false>
 static fused_fn pick_levels_f2(uint32_t L) {        // BASELINE.json's family: F = 2, SH-16
     switch (L) {
-        case 4:  return fused_inst<W, 4, 2, false, O, NPT, IMG, C>();
-        case 8:  return fused_inst<W, 8, 2, false, O, NPT, IMG, C>();
-        case 12: return fused_inst<W, 12, 2, false, O, NPT, IMG, C>();
-        case 16: return fused_inst<W, 16, 2, false, O, NPT, IMG, C>();
+        case 4:  return fused_inst<W, 4, 2, false, O, NPT, IMG, C, PK>();
+        case 8:  return fused_inst<W, 8, 2, false, O, NPT, IMG, C, PK>();
+        case 12: return fused_inst<W, 12, 2, false, O, NPT, IMG, C, PK>();
+        case 16: return fused_inst<W, 16, 2, false, O, NPT, IMG, C, PK>();
         default: return nullptr;
     }
 }
-template <int W, bool O, bool C>
+template <int W, bool O, bool C, bool PK = false>
 static fused_fn pick_levels_f4(uint32_t L) {        // the paper's own family: F = 4, raw direction
     switch (L) {
-        case 2: return fused_inst<W, 2, 4, true, O, 0, false, C>();
-        case 4: return fused_inst<W, 4, 4, true, O, 0, false, C>();
-        case 6: return fused_inst<W, 6, 4, true, O, 0, false, C>();
-        case 8: return fused_inst<W, 8, 4, true, O, 0, false, C>();
+        case 2: return fused_inst<W, 2, 4, true, O, 0, false, C, PK>();
+        case 4: return fused_inst<W, 4, 4, true, O, 0, false, C, PK>();
+        case 6: return fused_inst<W, 6, 4, true, O, 0, false, C, PK>();
+        case 8: return fused_inst<W, 8, 4, true, O, 0, false, C, PK>();
         default: return nullptr;
     }
 }
-template <bool O, bool C>
+// PK: the variant that reads the compact G-buffer formats / writes fp16 (linear tiles; the grid models of both families)
+template <bool O, bool C, bool PK = false>
 static fused_fn pick_fused(uint32_t W, uint32_t L, uint32_t F) {
-    if (L == 0)                                     // grid-less: positional encoding, no gathers
+    if (L == 0) {                                   // grid-less: positional encoding, no gathers
+        if (PK) return nullptr;
         return W == 16 ? fused_inst<16, 0, 2, true, O, 0, false, false>() : W == 32 ? fused_inst<32, 0, 2, true, O, 0, false, false>()
              : W == 64 ? fused_inst<64, 0, 2, true, O, 0, false, false>() : nullptr;
-    if (F == 4) return W == 32 ? pick_levels_f4<32, O, C>(L) : W == 64 ? pick_levels_f4<64, O, C>(L) : nullptr;
-    return W == 32 ? pick_levels_f2<32, O, 0, false, C>(L) : W == 64 ? pick_levels_f2<64, O, 0, false, C>(L) : nullptr;
+    }
+    if (F == 4) return W == 32 ? pick_levels_f4<32, O, C, PK>(L) : W == 64 ? pick_levels_f4<64, O, C, PK>(L) : nullptr;
+    return W == 32 ? pick_levels_f2<32, O, 0, false, C, PK>(L) : W == 64 ? pick_levels_f2<64, O, 0, false, C, PK>(L) : nullptr;
 }
 // image tiling (niv_infer_image): BASELINE.json's family (F = 2, 8..16 levels reach cells smaller than a warp's strip).
 // The paper's own family (F = 4, <= 8 levels, finest cell 5.5 cm) measured SLOWER with it (profiles/r01_v2.md): its
@@ -661,6 +665,17 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
             m->fused_host.fn = pick_fused<true, false>(W, cfg->n_levels, cfg->n_features);   // PCIe-bound: table gathers
             m->fused_host.smem = smem_host;
             rc = setup_kernel(m, m->fused_host, tmem_cols, "fused_host");
+        }
+        if (rc == NIV_OK) {
+            m->fused_pk.fn = use_cells ? pick_fused<false, true, true>(W, cfg->n_levels, cfg->n_features)
+                                       : pick_fused<false, false, true>(W, cfg->n_levels, cfg->n_features);
+            m->fused_pk.smem = smem_dev;
+            rc = setup_kernel(m, m->fused_pk, tmem_cols, "fused_packed");
+        }
+        if (rc == NIV_OK) {
+            m->fused_host_pk.fn = pick_fused<true, false, true>(W, cfg->n_levels, cfg->n_features);
+            m->fused_host_pk.smem = smem_host;
+            rc = setup_kernel(m, m->fused_host_pk, tmem_cols, "fused_host_packed");
         }
         if (rc == NIV_OK) {
             m->fused_img.fn = use_cells ? pick_fused_img<true>(W, cfg->n_levels, cfg->n_features)
@@ -915,8 +930,10 @@ static int launch_one(const niv_model* m, const FusedKernel& k, cudaStream_t st,
                       const float* nrm, float* out, size_t n, uint32_t n_tiles)
 {
     LaunchRec cur;
+    static const size_t kA[4] = {12, 16, 16, 8}, kB[4] = {12, 16, 0, 0}, kO[2] = {12, 8};   // bytes per texel by format
     const void* base[4] = {pos, nrm, P.tparam, out};
-    const size_t bytes[4] = {n * 12, n * 12, P.tparam ? n * 4 * m->cfg.n_params : 0, n * 12};
+    const size_t bytes[4] = {n * kA[P.gbuf_fmt & 3], n * kB[P.gbuf_fmt & 3], P.tparam ? n * 4 * m->cfg.n_params : 0,
+                             n * kO[P.out_fmt & 1]};
     for (int i = 0; i < 4; ++i) { cur.lo[i] = (uintptr_t)base[i]; cur.hi[i] = cur.lo[i] + bytes[i]; }
     cur.tracked = pdl && m->overlap && P.tile_ctr != nullptr;
     cur.done = P.tile_ctr ? P.tile_ctr + 2 : nullptr;
@@ -982,7 +999,10 @@ static int launch_fused(niv_model* m, const KParams& Pin, const float* pos, cons
     const uint32_t n_tiles = (uint32_t)((n + kTile - 1) / kTile);
     const bool tc5 = m->cfg.hidden_width <= 64;          // the kernels with the griddepcontrol pair
     // (the zero-copy host variant is followed by a stream synchronisation: it has nothing to overlap with)
-    return launch_one(m, host_variant ? m->fused_host : m->fused, st, m->pdl && tc5 && !host_variant, P, pos, nrm, out, n, n_tiles);
+    const bool packed = P.gbuf_fmt != NIV_GBUF_F32X3 || P.out_fmt != NIV_OUTFMT_F32X3;
+    const FusedKernel& k = packed ? (host_variant ? m->fused_host_pk : m->fused_pk) : (host_variant ? m->fused_host : m->fused);
+    if (!k.fn) return NIV_ERR_UNSUPPORTED;
+    return launch_one(m, k, st, m->pdl && tc5 && !host_variant, P, pos, nrm, out, n, n_tiles);
 }
 
 static int check_call(const niv_model* m, const void* pos, const void* nrm, const void* out, size_t n)
@@ -995,35 +1015,96 @@ static int check_call(const niv_model* m, const void* pos, const void* nrm, cons
     return NIV_OK;
 }
 
+// ---- G-buffer / output formats (include/niv.h NIV_GBUF_*, NIV_OUTFMT_*) ---------------------------------------------
+struct FmtInfo { size_t a_bytes, b_bytes, out_bytes; uintptr_t in_align, out_align; };
+static bool fmt_info(int gf, int of, FmtInfo& f)
+{
+    switch (gf) {
+        case NIV_GBUF_F32X3:     f.a_bytes = 12; f.b_bytes = 12; f.in_align = 4;  break;
+        case NIV_GBUF_F32X4:     f.a_bytes = 16; f.b_bytes = 16; f.in_align = 16; break;
+        case NIV_GBUF_P32_OCT16: f.a_bytes = 16; f.b_bytes = 0;  f.in_align = 16; break;
+        case NIV_GBUF_P16_OCT8:  f.a_bytes = 8;  f.b_bytes = 0;  f.in_align = 8;  break;
+        default: return false;
+    }
+    switch (of) {
+        case NIV_OUTFMT_F32X3: f.out_bytes = 12; f.out_align = 4; break;
+        case NIV_OUTFMT_F16X4: f.out_bytes = 8;  f.out_align = 8; break;
+        default: return false;
+    }
+    return true;
+}
+// common argument checks of the *_packed entry points; > 0: nothing to do
+static int check_packed(const niv_model* m, int gf, const void* a, const void* b, int of, const void* out, size_t n, FmtInfo& f)
+{
+    if (!fmt_info(gf, of, f)) return NIV_ERR_INVALID_ARG;
+    int rc = check_call(m, a, f.b_bytes ? b : a, out, n);
+    if (rc != NIV_OK) return rc;
+    if (((uintptr_t)a & (f.in_align - 1)) || (f.b_bytes && ((uintptr_t)b & (f.in_align - 1))) ||
+        ((uintptr_t)out & (f.out_align - 1))) return NIV_ERR_INVALID_ARG;
+    // the compact formats live in the tcgen05 kernels of width <= 64 (the width-128 and mma.sync kernels load fp32 x 3)
+    if ((gf != NIV_GBUF_F32X3 || of != NIV_OUTFMT_F32X3) && (m->cfg.hidden_width > 64 || m->mma_kernel || !m->fused_pk.fn))
+        return NIV_ERR_UNSUPPORTED;
+    return NIV_OK;
+}
+static void set_formats(const niv_model* m, KParams& P, int gf, int of)
+{
+    P.gbuf_fmt = (uint32_t)gf;
+    P.out_fmt = (uint32_t)of;
+    for (int d = 0; d < 3; ++d) {
+        volatile float ext = m->cfg.aabb_max[d] - m->cfg.aabb_min[d];
+        P.aext[d] = ext;
+    }
+}
+
+extern "C" int niv_infer_packed(niv_model* m, int gbuf_format, const void* gbuf_a, const void* gbuf_b, const float* param,
+                                int out_format, void* out, size_t n, void* stream)
+{
+    FmtInfo f;
+    int rc = check_packed(m, gbuf_format, gbuf_a, gbuf_b, out_format, out, n, f);
+    if (rc != NIV_OK) return rc > 0 ? NIV_OK : rc;
+    KParams P;
+    rc = fill_params(m, param, P);
+    if (rc != NIV_OK) return rc;
+    set_formats(m, P, gbuf_format, out_format);
+    return launch_fused(m, P, (const float*)gbuf_a, (const float*)gbuf_b, (float*)out, n, (cudaStream_t)stream);
+}
+
 extern "C" int niv_infer(niv_model* m, const float* pos, const float* nrm, const float* param,
                          float* out, size_t n, void* stream)
 {
-    int rc = check_call(m, pos, nrm, out, n);
-    if (rc != NIV_OK) return rc > 0 ? NIV_OK : rc;
-    KParams P;
-    rc = fill_params(m, param, P);
-    if (rc != NIV_OK) return rc;
-    return launch_fused(m, P, pos, nrm, out, n, (cudaStream_t)stream);
+    return niv_infer_packed(m, NIV_GBUF_F32X3, pos, nrm, param, NIV_OUTFMT_F32X3, out, n, stream);
 }
 
-extern "C" int niv_infer_image(niv_model* m, const float* pos, const float* nrm, const float* param,
-                               float* out, uint32_t width, uint32_t height, void* stream)
+extern "C" int niv_infer_image_packed(niv_model* m, int gbuf_format, const void* gbuf_a, const void* gbuf_b,
+                                      const float* param, int out_format, void* out, uint32_t width, uint32_t height,
+                                      void* stream)
 {
     const size_t n = (size_t)width * height;
-    int rc = check_call(m, pos, nrm, out, n);
+    FmtInfo f;
+    int rc = check_packed(m, gbuf_format, gbuf_a, gbuf_b, out_format, out, n, f);
     if (rc != NIV_OK) return rc > 0 ? NIV_OK : rc;
     KParams P;
     rc = fill_params(m, param, P);
     if (rc != NIV_OK) return rc;
+    set_formats(m, P, gbuf_format, out_format);
     // models without an image-tiled kernel (and images beyond the packed tile coordinates): same result, linear tiles
-    if (!m->fused_img.fn || width > (1u << 20) || height > (1u << 17) || m->image_linear)
-        return launch_fused(m, P, pos, nrm, out, n, (cudaStream_t)stream);
+    // (and the compact formats, whose kernels are linear-tile ones)
+    const bool packed = gbuf_format != NIV_GBUF_F32X3 || out_format != NIV_OUTFMT_F32X3;
+    if (!m->fused_img.fn || width > (1u << 20) || height > (1u << 17) || m->image_linear || packed)
+        return launch_fused(m, P, (const float*)gbuf_a, (const float*)gbuf_b, (float*)out, n, (cudaStream_t)stream);
     P.img_w = width;
     P.img_h = height;
     P.tiles_x = (width + 31u) / 32u;
     const uint32_t n_tiles = P.tiles_x * ((height + 3u) / 4u);
     draw_tile_counter(m, (cudaStream_t)stream, P);
-    return launch_one(m, m->fused_img, (cudaStream_t)stream, m->pdl, P, pos, nrm, out, n, n_tiles);
+    return launch_one(m, m->fused_img, (cudaStream_t)stream, m->pdl, P, (const float*)gbuf_a, (const float*)gbuf_b,
+                      (float*)out, n, n_tiles);
+}
+
+extern "C" int niv_infer_image(niv_model* m, const float* pos, const float* nrm, const float* param,
+                               float* out, uint32_t width, uint32_t height, void* stream)
+{
+    return niv_infer_image_packed(m, NIV_GBUF_F32X3, pos, nrm, param, NIV_OUTFMT_F32X3, out, width, height, stream);
 }
 
 extern "C" int niv_infer_texel_params(niv_model* m, const float* pos, const float* nrm, const float* tparam,
@@ -1043,26 +1124,34 @@ extern "C" int niv_infer_texel_params(niv_model* m, const float* pos, const floa
     return launch_one(m, m->fused_tp, (cudaStream_t)stream, m->pdl, P, pos, nrm, out, n, n_tiles);
 }
 
-extern "C" int niv_infer_host(niv_model* m, const float* pos, const float* nrm, const float* param,
-                              float* out, size_t n, void* stream)
+extern "C" int niv_infer_host_packed(niv_model* m, int gbuf_format, const void* gbuf_a, const void* gbuf_b,
+                                     const float* param, int out_format, void* out, size_t n, void* stream)
 {
-    int rc = check_call(m, pos, nrm, out, n);
+    FmtInfo f;
+    int rc = check_packed(m, gbuf_format, gbuf_a, gbuf_b, out_format, out, n, f);
     if (rc != NIV_OK) return rc > 0 ? NIV_OK : rc;
     KParams P;
     rc = fill_params(m, param, P);
     if (rc != NIV_OK) return rc;
+    set_formats(m, P, gbuf_format, out_format);
     NIV_CUDA(cudaSetDevice(m->cfg.device));
-    // Zero copy: if all three buffers are pinned (or registered) host memory the fused kernel reads the G-buffer and
-    // writes the irradiance over PCIe itself -- the texel of the next tile is requested a tile ahead, the output
-    // leaves as full 128-byte lines -- so transfer and compute overlap tile by tile in ONE launch with no staging
-    // (1.04 ms per full-HD frame against 1.21 ms with chunked copies; 0.91 ms is the copy time of the input alone).
-    if (m->fused_host.fn && !m->host_staged) {
+    const uint8_t* a = (const uint8_t*)gbuf_a;
+    const uint8_t* b = (const uint8_t*)gbuf_b;
+    uint8_t* o = (uint8_t*)out;
+    // Zero copy: if all buffers are pinned (or registered) host memory the fused kernel reads the G-buffer and
+    // writes the irradiance over PCIe itself -- the texel of the next tile is requested ahead, the output leaves as
+    // full lines -- so transfer and compute overlap tile by tile in ONE launch with no staging (1.04 ms per full-HD
+    // frame against 1.21 ms with chunked copies for fp32 x 3 in and out; the compact formats move 16 + 8 or 8 + 8
+    // bytes per texel instead of 24 + 12).
+    const bool packed = gbuf_format != NIV_GBUF_F32X3 || out_format != NIV_OUTFMT_F32X3;
+    if ((packed ? m->fused_host_pk.fn : m->fused_host.fn) && !m->host_staged) {
         cudaPointerAttributes ap, an, ao;
-        if (cudaPointerGetAttributes(&ap, pos) == cudaSuccess && cudaPointerGetAttributes(&an, nrm) == cudaSuccess &&
-            cudaPointerGetAttributes(&ao, out) == cudaSuccess && ap.type == cudaMemoryTypeHost &&
-            an.type == cudaMemoryTypeHost && ao.type == cudaMemoryTypeHost && ap.devicePointer && an.devicePointer &&
-            ao.devicePointer && ((uintptr_t)ao.devicePointer & 15u) == 0) {
-            rc = launch_fused(m, P, (const float*)ap.devicePointer, (const float*)an.devicePointer,
+        const bool ok_a = cudaPointerGetAttributes(&ap, a) == cudaSuccess && ap.type == cudaMemoryTypeHost && ap.devicePointer;
+        const bool ok_b = !f.b_bytes || (cudaPointerGetAttributes(&an, b) == cudaSuccess && an.type == cudaMemoryTypeHost && an.devicePointer);
+        const bool ok_o = cudaPointerGetAttributes(&ao, o) == cudaSuccess && ao.type == cudaMemoryTypeHost && ao.devicePointer &&
+                          ((uintptr_t)ao.devicePointer & 15u) == 0;
+        if (ok_a && ok_b && ok_o) {
+            rc = launch_fused(m, P, (const float*)ap.devicePointer, f.b_bytes ? (const float*)an.devicePointer : nullptr,
                               (float*)ao.devicePointer, n, (cudaStream_t)stream, true);
             if (rc != NIV_OK) return rc;
             NIV_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
@@ -1075,16 +1164,16 @@ extern "C" int niv_infer_host(niv_model* m, const float* pos, const float* nrm, 
         NIV_CUDA(cudaStreamCreateWithFlags(&m->hs[1], cudaStreamNonBlocking));
         NIV_CUDA(cudaEventCreateWithFlags(&m->hev, cudaEventDisableTiming));
     }
-    if (n > m->stage_cap) {
+    if (n > m->stage_cap) {                          // [a | b | out], each 16 bytes per texel at most
         if (m->d_stage) { NIV_CUDA(cudaFree(m->d_stage)); m->d_stage = nullptr; m->stage_cap = 0; }
         const size_t cap = (n + 1023) / 1024 * 1024;
-        cudaError_t e = cudaMalloc(&m->d_stage, cap * 9 * sizeof(float));
+        cudaError_t e = cudaMalloc(&m->d_stage, cap * 48);
         if (e != cudaSuccess) { g_last_cuda_error = (int)e; (void)cudaGetLastError(); return NIV_ERR_ALLOC; }
         m->stage_cap = cap;
     }
-    float* d_pos = m->d_stage;
-    float* d_nrm = m->d_stage + 3 * m->stage_cap;
-    float* d_out = m->d_stage + 6 * m->stage_cap;
+    uint8_t* d_a = reinterpret_cast<uint8_t*>(m->d_stage);
+    uint8_t* d_b = d_a + 16 * m->stage_cap;
+    uint8_t* d_o = d_a + 32 * m->stage_cap;
     // order after the caller's stream
     NIV_CUDA(cudaEventRecord(m->hev, (cudaStream_t)stream));
     NIV_CUDA(cudaStreamWaitEvent(m->hs[0], m->hev, 0));
@@ -1093,17 +1182,53 @@ extern "C" int niv_infer_host(niv_model* m, const float* pos, const float* nrm, 
     size_t chunk = (n / 8 + kTile - 1) / kTile * kTile;
     if (chunk < 32768) chunk = 32768;
     int k = 0;
-    for (size_t o = 0; o < n; o += chunk, ++k) {
-        const size_t c = (n - o < chunk) ? n - o : chunk;
+    for (size_t t0 = 0; t0 < n; t0 += chunk, ++k) {
+        const size_t c = (n - t0 < chunk) ? n - t0 : chunk;
         cudaStream_t st = m->hs[k & 1];
-        NIV_CUDA(cudaMemcpyAsync(d_pos + 3 * o, pos + 3 * o, c * 12, cudaMemcpyHostToDevice, st));
-        NIV_CUDA(cudaMemcpyAsync(d_nrm + 3 * o, nrm + 3 * o, c * 12, cudaMemcpyHostToDevice, st));
-        rc = launch_fused(m, P, d_pos + 3 * o, d_nrm + 3 * o, d_out + 3 * o, c, st);
+        NIV_CUDA(cudaMemcpyAsync(d_a + f.a_bytes * t0, a + f.a_bytes * t0, c * f.a_bytes, cudaMemcpyHostToDevice, st));
+        if (f.b_bytes) NIV_CUDA(cudaMemcpyAsync(d_b + f.b_bytes * t0, b + f.b_bytes * t0, c * f.b_bytes, cudaMemcpyHostToDevice, st));
+        rc = launch_fused(m, P, (const float*)(d_a + f.a_bytes * t0), (const float*)(d_b + f.b_bytes * t0),
+                          (float*)(d_o + f.out_bytes * t0), c, st);
         if (rc != NIV_OK) return rc;
-        NIV_CUDA(cudaMemcpyAsync(out + 3 * o, d_out + 3 * o, c * 12, cudaMemcpyDeviceToHost, st));
+        NIV_CUDA(cudaMemcpyAsync(o + f.out_bytes * t0, d_o + f.out_bytes * t0, c * f.out_bytes, cudaMemcpyDeviceToHost, st));
     }
     NIV_CUDA(cudaStreamSynchronize(m->hs[0]));
     NIV_CUDA(cudaStreamSynchronize(m->hs[1]));
+    return NIV_OK;
+}
+
+extern "C" int niv_infer_host(niv_model* m, const float* pos, const float* nrm, const float* param,
+                              float* out, size_t n, void* stream)
+{
+    return niv_infer_host_packed(m, NIV_GBUF_F32X3, pos, nrm, param, NIV_OUTFMT_F32X3, out, n, stream);
+}
+
+// The decoded fp32 position and normal of every texel of a compact G-buffer (what the fused kernels work on): for tests
+// (bit-exact positions against the CPU decode) and for callers that want the fp32 buffers.
+__global__ void __launch_bounds__(256) niv_decode_kernel(const __grid_constant__ KParams P, const float* __restrict__ a,
+                                                         const float* __restrict__ b, float* __restrict__ pos,
+                                                         float* __restrict__ nrm, size_t n)
+{
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float pr[3] = {0.f, 0.f, 0.f}, nr[3] = {0.f, 0.f, 0.f}, p[3], nv[3];
+    load_texel_raw(P.gbuf_fmt, a, b, i, pr, nr);
+    decode_texel(P, pr, nr, p, nv);
+    for (int d = 0; d < 3; ++d) { pos[3 * i + d] = p[d]; nrm[3 * i + d] = nv[d]; }
+}
+extern "C" int niv_decode_gbuffer(niv_model* m, int gbuf_format, const void* gbuf_a, const void* gbuf_b, float* pos,
+                                  float* nrm, size_t n, void* stream)
+{
+    FmtInfo f;
+    if (!m || !pos || !nrm) return NIV_ERR_INVALID_ARG;
+    if (!fmt_info(gbuf_format, NIV_OUTFMT_F32X3, f)) return NIV_ERR_INVALID_ARG;
+    if (n == 0) return NIV_OK;
+    if (!gbuf_a || (f.b_bytes && !gbuf_b)) return NIV_ERR_INVALID_ARG;
+    if (((uintptr_t)gbuf_a & (f.in_align - 1)) || (f.b_bytes && ((uintptr_t)gbuf_b & (f.in_align - 1)))) return NIV_ERR_INVALID_ARG;
+    KParams P = m->kp;
+    set_formats(m, P, gbuf_format, NIV_OUTFMT_F32X3);
+    niv_decode_kernel<<<(unsigned)((n + 255) / 256), 256, 0, (cudaStream_t)stream>>>(P, (const float*)gbuf_a, (const float*)gbuf_b, pos, nrm, n);
+    NIV_CUDA(cudaGetLastError());
     return NIV_OK;
 }
 

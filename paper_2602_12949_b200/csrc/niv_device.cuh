@@ -65,6 +65,9 @@ struct KParams {
     uint32_t misc_off;          // byte offset of folded bias / barriers
     const uint32_t* wmma;       // weights in the layout of the mma.sync A/B kernel (niv_fused_mma.cuh), else NULL
     const float* tparam;        // per-texel scene parameters [n][n_params] (niv_infer_texel_params), else NULL
+    uint32_t gbuf_fmt;          // NIV_GBUF_*: how the caller's G-buffer texels are stored (load_texel_raw / decode_texel)
+    uint32_t out_fmt;           // NIV_OUTFMT_*: fp32 x 3 or fp16 x 4 per texel
+    float    aext[3];           // fl32(max - min): the scale of the unorm16 position format
     uint32_t img_w, img_h;      // niv_infer_image: the buffers are a row-major img_h x img_w image ...
     uint32_t tiles_x;           // ... cut into 32 x 4 pixel tiles, tiles_x = ceil(img_w / 32) per tile row (else 0)
 };
@@ -357,6 +360,66 @@ __device__ __forceinline__ void load3(const float* __restrict__ p, size_t i, flo
     v[0] = __ldg(p + 3 * i);
     v[1] = __ldg(p + 3 * i + 1);
     v[2] = __ldg(p + 3 * i + 2);
+}
+
+// ---------------------------------------------------------------- a1 for the compact G-buffer formats
+// DESIGN.md 3.4.  The raw words of texel i travel in the six registers the fp32 texel takes (they are requested a tile
+// ahead); decode_texel turns them into the fp32 position and normal the rest of the path is defined on.
+//   NIV_GBUF_F32X3      pos[i] = 3 floats, nrm[i] = 3 floats (two arrays)
+//   NIV_GBUF_F32X4      the same with a stride of 16 bytes (xyzw, w ignored): one 128-bit load per array
+//   NIV_GBUF_P32_OCT16  one array, 16 bytes per texel: x, y, z fp32 | octahedral normal, 2 x snorm16: one 128-bit load
+//   NIV_GBUF_P16_OCT8   one array, 8 bytes per texel: position 3 x unorm16 of the model's box | octahedral normal,
+//                       2 x snorm8: one 64-bit load
+// The position decode is a pinned fp32 sequence (it decides cells): x = fl32(fl32(fl32((float)q * fl32(1/65535)) * ext) + min).
+__device__ __forceinline__ void load_texel_raw(uint32_t fmt, const float* __restrict__ a, const float* __restrict__ b,
+                                               size_t i, float pr[3], float nr[3]) {
+    if (fmt == 0) {
+        load3(a, i, pr);
+        load3(b, i, nr);
+    } else if (fmt == 1) {
+        const float4 p4 = __ldg(reinterpret_cast<const float4*>(a) + i), n4 = __ldg(reinterpret_cast<const float4*>(b) + i);
+        pr[0] = p4.x; pr[1] = p4.y; pr[2] = p4.z;
+        nr[0] = n4.x; nr[1] = n4.y; nr[2] = n4.z;
+    } else if (fmt == 2) {
+        const uint4 t = __ldg(reinterpret_cast<const uint4*>(a) + i);
+        pr[0] = __uint_as_float(t.x); pr[1] = __uint_as_float(t.y); pr[2] = __uint_as_float(t.z);
+        nr[0] = __uint_as_float(t.w);
+    } else {
+        const uint2 t = __ldg(reinterpret_cast<const uint2*>(a) + i);
+        pr[0] = __uint_as_float(t.x); pr[1] = __uint_as_float(t.y);
+    }
+}
+// octahedral direction: (fx, fy) in [-1, 1]^2 -> unit vector
+__device__ __forceinline__ void oct_decode(float fx, float fy, float n[3]) {
+    float z = 1.0f - fabsf(fx) - fabsf(fy), x = fx, y = fy;
+    if (z < 0.0f) {
+        x = copysignf(1.0f - fabsf(fy), fx);
+        y = copysignf(1.0f - fabsf(fx), fy);
+    }
+    const float r = rsqrtf(x * x + y * y + z * z);
+    n[0] = x * r; n[1] = y * r; n[2] = z * r;
+}
+__device__ __forceinline__ void decode_texel(const KParams& P, const float pr[3], const float nr[3], float p[3], float n[3]) {
+    if (P.gbuf_fmt <= 1) {
+#pragma unroll
+        for (int d = 0; d < 3; ++d) { p[d] = pr[d]; n[d] = nr[d]; }
+    } else if (P.gbuf_fmt == 2) {
+#pragma unroll
+        for (int d = 0; d < 3; ++d) p[d] = pr[d];
+        const uint32_t o = __float_as_uint(nr[0]);
+        const int ox = (int)(short)(o & 0xFFFFu), oy = (int)(short)(o >> 16);
+        if (ox == -32768 && oy == -32768) { n[0] = n[1] = n[2] = 0.0f; }           // background
+        else oct_decode((float)ox * (1.0f / 32767.0f), (float)oy * (1.0f / 32767.0f), n);
+    } else {
+        const uint32_t w0 = __float_as_uint(pr[0]), w1 = __float_as_uint(pr[1]);
+        const uint32_t q[3] = {w0 & 0xFFFFu, w0 >> 16, w1 & 0xFFFFu};
+#pragma unroll
+        for (int d = 0; d < 3; ++d)
+            p[d] = __fadd_rn(__fmul_rn(__fmul_rn((float)q[d], 1.0f / 65535.0f), P.aext[d]), P.amin[d]);
+        const int ox = (int)(signed char)((w1 >> 16) & 0xFFu), oy = (int)(signed char)(w1 >> 24);
+        if (ox == -128 && oy == -128) { n[0] = n[1] = n[2] = 0.0f; }
+        else oct_decode((float)ox * (1.0f / 127.0f), (float)oy * (1.0f / 127.0f), n);
+    }
 }
 
 }  // namespace niv

@@ -27,7 +27,10 @@ __device__ __forceinline__ uint32_t pack_relu_half2(float lo, float hi) {
 // changes its schedule for the worse (0.193 instead of 0.189 ms, profiles/r01_v2.md); the per-texel-parameter
 // variants are capped too (two parameters at width 64 would take 140 registers)
 // NC: the coarsest NC levels are read from their cell-block copies, one 32- / 64-byte load per level
-template <int WIDTH, int L, int NB, int F, bool RAWDIR, bool OUT128, int NPT, bool IMG, int NC>
+// PACKED: the caller's buffers are in one of the compact G-buffer / output formats (P.gbuf_fmt, P.out_fmt: a uniform
+// run-time switch per tile); false = fp32 x 3 in and out with no trace of the switch in the code (it cost the headline
+// kernel 1.5 %: its level loop sits at the register cap and every live value more changes the schedule)
+template <int WIDTH, int L, int NB, int F, bool RAWDIR, bool OUT128, int NPT, bool IMG, int NC, bool PACKED>
 __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_fused_kernel(
                                                                const __grid_constant__ KParams P,
                                                                const float* __restrict__ pos,
@@ -149,8 +152,7 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
         bool ok;
         const size_t i0 = texel_of(blockIdx.x, txy, ok);
         if (ok) {
-            load3(pos, i0, pn);
-            load3(nrm, i0, nn);
+            load_texel_raw(PACKED ? P.gbuf_fmt : 0u, pos, nrm, i0, pn, nn);
 #pragma unroll
             for (int q = 0; q < NPT; ++q) tn[q] = __ldg(P.tparam + i0 * NPT + q);
         }
@@ -159,7 +161,8 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
     while (tile < n_tiles) {
         bool valid;
         const size_t i = texel_of(tile, txy, valid);
-        const float p[3] = {pn[0], pn[1], pn[2]}, nv[3] = {nn[0], nn[1], nn[2]};
+        float p[3] = {pn[0], pn[1], pn[2]}, nv[3] = {nn[0], nn[1], nn[2]};
+        if constexpr (PACKED) decode_texel(P, pn, nn, p, nv);     // the raw words of a compact format -> fp32 position, normal
         float tv[NPT > 0 ? NPT : 1];
 #pragma unroll
         for (int q = 0; q < NPT; ++q) tv[q] = tn[q];
@@ -177,8 +180,7 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
 #pragma unroll
             for (int d = 0; d < 3; ++d) { pn[d] = 0.f; nn[d] = 0.f; }
             if (ok) {
-                load3(pos, inext, pn);
-                load3(nrm, inext, nn);
+                load_texel_raw(PACKED ? P.gbuf_fmt : 0u, pos, nrm, inext, pn, nn);
 #pragma unroll
                 for (int q = 0; q < NPT; ++q) tn[q] = __ldg(P.tparam + inext * NPT + q);
             }
@@ -326,7 +328,10 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
                     float* so = reinterpret_cast<float*>(smem + P.misc_off + 64) + warp * 96;
                     const size_t w0 = ((size_t)tile * kTile + warp * 32u) * 3;        // first float of the warp
                     const bool vec = (w0 + 96 <= 3 * n) && ((reinterpret_cast<uintptr_t>(out) & 15u) == 0);
-                    if (vec) {
+                    if (PACKED && P.out_fmt == NIV_OUTFMT_F16X4) {      // 8 bytes per texel: a warp's stores are 256 contiguous bytes
+                        if (valid)
+                            reinterpret_cast<uint2*>(out)[i] = make_uint2(pack_half2(y[0], y[1]), pack_half2(y[2], 0.0f));
+                    } else if (vec) {
                         so[lane * 3] = y[0];
                         so[lane * 3 + 1] = y[1];
                         so[lane * 3 + 2] = y[2];
@@ -346,9 +351,13 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
                         if (P.out_act == NIV_OUT_SIGMOID) v = __fdividef(1.0f, 1.0f + __expf(-v));
                         y[c] = masked ? 0.0f : v;
                     }
-                    out[3 * i] = y[0];
-                    out[3 * i + 1] = y[1];
-                    out[3 * i + 2] = y[2];
+                    if (PACKED && P.out_fmt == NIV_OUTFMT_F16X4) {      // (r, g, b, 0) as four fp16: one 8-byte store
+                        reinterpret_cast<uint2*>(out)[i] = make_uint2(pack_half2(y[0], y[1]), pack_half2(y[2], 0.0f));
+                    } else {
+                        out[3 * i] = y[0];
+                        out[3 * i + 1] = y[1];
+                        out[3 * i + 2] = y[2];
+                    }
                 }
             }
         }

@@ -352,3 +352,59 @@ def make_probe_grid(dims: Tuple[int, int, int], seed: int, scale: float = 1.0) -
 def probe_grid_dims_for_spacing(aabb_min, aabb_max, spacing: float) -> Tuple[int, int, int]:
     """Probes on a regular lattice over the box, faces included, about `spacing` apart."""
     return tuple(int(max(2, round((float(hi) - float(lo)) / spacing) + 1)) for lo, hi in zip(aabb_min, aabb_max))
+
+
+# ----------------------------------------------------------------------------
+# Compact G-buffer layouts (include/niv.h NIV_GBUF_*; DESIGN.md 3.4).  This is the PRODUCER side -- what a renderer would
+# write -- so it lives with the input generators; the decode (the method's side) exists twice, in oracle/ and in csrc/.
+GBUF_F32X3, GBUF_F32X4, GBUF_P32_OCT16, GBUF_P16_OCT8 = 0, 1, 2, 3
+OUTFMT_F32X3, OUTFMT_F16X4 = 0, 1
+
+
+def _oct_encode(nrm: np.ndarray) -> np.ndarray:
+    """unit vectors [n][3] -> octahedral coordinates [n][2] in [-1, 1] (float64)"""
+    n = nrm.astype(np.float64)
+    s = np.abs(n).sum(axis=1, keepdims=True)
+    s[s == 0] = 1.0
+    n = n / s
+    x, y, z = n[:, 0], n[:, 1], n[:, 2]
+    neg = z < 0
+    fx = np.where(neg, (1.0 - np.abs(y)) * np.where(x >= 0, 1.0, -1.0), x)
+    fy = np.where(neg, (1.0 - np.abs(x)) * np.where(y >= 0, 1.0, -1.0), y)
+    return np.stack([fx, fy], axis=1)
+
+
+def pack_gbuffer(fmt: int, pos: np.ndarray, nrm: np.ndarray, aabb=None):
+    """-> (a, b): the arrays the *_packed entry points take (b is None for the single-array formats).  Background texels
+    (nrm == 0) get the reserved normal code; positions of format 3 are quantised to unorm16 of `aabb` (clipped)."""
+    pos = np.ascontiguousarray(pos, dtype=np.float32)
+    nrm = np.ascontiguousarray(nrm, dtype=np.float32)
+    n = pos.shape[0]
+    if fmt == GBUF_F32X3:
+        return pos, nrm
+    if fmt == GBUF_F32X4:
+        a = np.zeros((n, 4), dtype=np.float32)
+        b = np.zeros((n, 4), dtype=np.float32)
+        a[:, :3], b[:, :3] = pos, nrm
+        a[:, 3], b[:, 3] = 1.0, 0.0
+        return a, b
+    bg = np.all(nrm == 0, axis=1)
+    o = _oct_encode(nrm)
+    if fmt == GBUF_P32_OCT16:
+        q = np.clip(np.rint(o * 32767.0), -32767, 32767).astype(np.int16)
+        q[bg] = -32768
+        rec = np.zeros((n, 4), dtype=np.uint32)
+        rec[:, :3] = pos.view(np.uint32)
+        rec[:, 3] = q[:, 0].view(np.uint16).astype(np.uint32) | (q[:, 1].view(np.uint16).astype(np.uint32) << 16)
+        return rec, None
+    if fmt == GBUF_P16_OCT8:
+        lo, hi = np.asarray(aabb[0], dtype=np.float64), np.asarray(aabb[1], dtype=np.float64)
+        u = np.clip((pos.astype(np.float64) - lo) / (hi - lo), 0.0, 1.0)
+        qp = np.rint(u * 65535.0).astype(np.uint16)
+        q = np.clip(np.rint(o * 127.0), -127, 127).astype(np.int8)
+        q[bg] = -128
+        rec = np.zeros((n, 8), dtype=np.uint8)
+        rec[:, :6] = qp.view(np.uint8).reshape(n, 6)
+        rec[:, 6:] = q.view(np.uint8)
+        return rec, None
+    raise ValueError("unknown G-buffer format")

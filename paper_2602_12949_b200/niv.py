@@ -25,8 +25,14 @@ NIV_OUT_SIGMOID = 1
 NIV_CENSUS_COUNTS = 49      # niv_probe_sectors: [0,16) sectors, [16,32) lines, [32] active texels, [33,49) touched
 
 # every symbol include/niv.h declares (tests check that the library exports all of them)
+NIV_GBUF_F32X3, NIV_GBUF_F32X4, NIV_GBUF_P32_OCT16, NIV_GBUF_P16_OCT8 = 0, 1, 2, 3
+NIV_OUTFMT_F32X3, NIV_OUTFMT_F16X4 = 0, 1
+_GBUF_BYTES = {0: (12, 12), 1: (16, 16), 2: (16, 0), 3: (8, 0)}      # bytes per texel of gbuf_a, gbuf_b
+_OUT_BYTES = {0: 12, 1: 8}
+
 EXPORTS = ("niv_create", "niv_get_info", "niv_load_params", "niv_infer", "niv_infer_image", "niv_infer_texel_params",
            "niv_infer_host", "niv_probe_sectors_image",
+           "niv_infer_packed", "niv_infer_image_packed", "niv_infer_host_packed", "niv_decode_gbuffer",
            "niv_encode",
            "niv_debug_encode", "niv_compose", "niv_destroy", "niv_error_string", "niv_last_cuda_error", "niv_probe_gather",
            "niv_probe_sectors",
@@ -92,6 +98,10 @@ def lib():
         L.niv_infer_image.argtypes = [vp, vp, vp, C.POINTER(C.c_float), vp, C.c_uint32, C.c_uint32, vp]
         L.niv_probe_sectors_image.argtypes = [vp, vp, vp, C.c_uint32, C.c_uint32, vp, vp]
         L.niv_encode.argtypes = [vp, vp, vp, C.POINTER(C.c_float), vp, sz, vp]
+        L.niv_infer_packed.argtypes = [vp, C.c_int, vp, vp, C.POINTER(C.c_float), C.c_int, vp, sz, vp]
+        L.niv_infer_image_packed.argtypes = [vp, C.c_int, vp, vp, C.POINTER(C.c_float), C.c_int, vp, C.c_uint32, C.c_uint32, vp]
+        L.niv_infer_host_packed.argtypes = [vp, C.c_int, vp, vp, C.POINTER(C.c_float), C.c_int, vp, sz, vp]
+        L.niv_decode_gbuffer.argtypes = [vp, C.c_int, vp, vp, vp, vp, sz, vp]
         L.niv_debug_encode.argtypes = [vp, vp, vp, C.POINTER(C.c_float), sz, vp, vp, vp, vp, vp]
         L.niv_compose.argtypes = [vp, C.c_uint32, C.c_uint32, vp, vp, vp, vp, C.c_uint32, C.c_uint32, vp]
         L.niv_destroy.argtypes = [vp]
@@ -268,6 +278,69 @@ class NivModel:
         if rc != NIV_OK:
             raise NivError(rc, "niv_infer_host")
         return out
+
+    # ---- compact G-buffer formats / fp16 output (include/niv.h: *_packed).  Buffers are taken by byte size: any dtype.
+    @staticmethod
+    def _raw(t, name, nbytes, cuda):
+        """pointer of a contiguous buffer (CUDA tensor, or host numpy array / CPU tensor) holding exactly nbytes"""
+        import numpy as np
+        if t is None:
+            if nbytes:
+                raise TypeError("%s is required for this format" % name)
+            return None
+        if isinstance(t, np.ndarray):
+            if cuda or not t.flags.c_contiguous:
+                raise TypeError("%s must be a contiguous %s buffer" % (name, "CUDA" if cuda else "host"))
+            have, ptr = t.nbytes, t.ctypes.data
+        else:
+            import torch
+            if not isinstance(t, torch.Tensor) or t.is_cuda != cuda or not t.is_contiguous():
+                raise TypeError("%s must be a contiguous %s buffer" % (name, "CUDA" if cuda else "host"))
+            have, ptr = t.numel() * t.element_size(), t.data_ptr()
+        if nbytes and have != nbytes:
+            raise ValueError("%s holds %d bytes, the call needs %d" % (name, have, nbytes))
+        return ptr
+
+    def _packed_args(self, gbuf_format, a, b, out_format, out, n, cuda):
+        ab, bb = _GBUF_BYTES[int(gbuf_format)]
+        return (self._raw(a, "gbuf_a", ab * n, cuda), self._raw(b, "gbuf_b", bb * n, cuda) if bb else None,
+                self._raw(out, "out", _OUT_BYTES[int(out_format)] * n, cuda))
+
+    def infer_packed(self, gbuf_format, a, b, out, n, out_format=NIV_OUTFMT_F32X3, param=None, stream=None):
+        pa, pb, po = self._packed_args(gbuf_format, a, b, out_format, out, n, True)
+        rc = lib().niv_infer_packed(self._h, int(gbuf_format), pa, pb, _params(param, self.spec.n_params),
+                                    int(out_format), po, n, _stream_ptr(stream))
+        if rc != NIV_OK:
+            raise NivError(rc, "niv_infer_packed")
+        return out
+
+    def infer_image_packed(self, gbuf_format, a, b, out, width, height, out_format=NIV_OUTFMT_F32X3, param=None, stream=None):
+        n = int(width) * int(height)
+        pa, pb, po = self._packed_args(gbuf_format, a, b, out_format, out, n, True)
+        rc = lib().niv_infer_image_packed(self._h, int(gbuf_format), pa, pb, _params(param, self.spec.n_params),
+                                          int(out_format), po, int(width), int(height), _stream_ptr(stream))
+        if rc != NIV_OK:
+            raise NivError(rc, "niv_infer_image_packed")
+        return out
+
+    def infer_host_packed(self, gbuf_format, a, b, out, n, out_format=NIV_OUTFMT_F32X3, param=None, stream=None):
+        pa, pb, po = self._packed_args(gbuf_format, a, b, out_format, out, n, False)
+        rc = lib().niv_infer_host_packed(self._h, int(gbuf_format), pa, pb, _params(param, self.spec.n_params),
+                                         int(out_format), po, n, _stream_ptr(stream))
+        if rc != NIV_OK:
+            raise NivError(rc, "niv_infer_host_packed")
+        return out
+
+    def decode_gbuffer(self, gbuf_format, a, b, pos, nrm, n, stream=None):
+        """pos, nrm: device [n][3] fp32 outputs = what the fused kernels decode from the compact G-buffer."""
+        import torch
+        ab, bb = _GBUF_BYTES[int(gbuf_format)]
+        rc = lib().niv_decode_gbuffer(self._h, int(gbuf_format), self._raw(a, "gbuf_a", ab * n, True),
+                                      self._raw(b, "gbuf_b", bb * n, True) if bb else None,
+                                      _dev(pos, torch.float32, "pos", 3), _dev(nrm, torch.float32, "nrm", 3), n,
+                                      _stream_ptr(stream))
+        if rc != NIV_OK:
+            raise NivError(rc, "niv_decode_gbuffer")
 
     def encode(self, pos, nrm, features, param=None, stream=None):
         """features: device [n][in_dim] fp16."""
