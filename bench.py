@@ -54,8 +54,9 @@ PAPER_TABLE1_MS = {(0, 16): 0.19, (0, 32): 0.20, (0, 64): 0.25, (2, 64): 0.31, (
 PAPER_TABLE1_HALF_MS = {(0, 16): 0.029, (0, 32): 0.031, (0, 64): 0.069, (2, 64): 0.088, (4, 64): 0.18, (6, 64): 0.26, (8, 64): 0.37}
 
 
-def make_workload(name: str, frame: int):
-    """-> spec, table, wblob, bblob, pos, nrm, param, description"""
+def make_workload(name: str, frame: int, with_params: bool = True):
+    """-> spec, table, wblob, bblob, pos, nrm, param, description  (with_params False: table and blobs are None -- a rank
+    that receives the parameters by broadcast does not generate them)"""
     paper_levels, paper_width = PAPER_LEVELS, PAPER_WIDTH
     if name == "param":
         spec, param = I.spec_param(), [0.625]
@@ -64,8 +65,8 @@ def make_workload(name: str, frame: int):
         param = None
     else:
         spec, param = I.spec_fullhd(), None
-    table = I.make_table(spec, 0)
-    w, b = I.make_mlp(spec, 0)
+    table = I.make_table(spec, 0) if with_params else None
+    w, b = I.make_mlp(spec, 0) if with_params else (None, None)
     if name == "incoherent":
         pos = I.positions_uniform(N_TEXELS, (spec.aabb_min, spec.aabb_max), frame)
         nrm = I.normals_uniform(N_TEXELS, frame)
@@ -81,7 +82,8 @@ def make_workload(name: str, frame: int):
                     "the configs[1] G-buffer, %.1f%% background texels"
                     % (paper_width, paper_levels or "-", "F=4, scale sqrt 2, T=2^17" if paper_levels else
                        "eight-band positional encoding", 100 * masked))
-    return spec, table, I.pack_weights(w), I.pack_biases(b), pos, nrm, param, desc, masked
+    return (spec, table, I.pack_weights(w) if with_params else None, I.pack_biases(b) if with_params else None, pos, nrm,
+            param, desc, masked)
 
 
 def load_peaks():
@@ -269,11 +271,34 @@ def run_ours(args):
         dist.barrier()
     niv.lib()
 
-    # each rank owns one full frame per step (weak scaling: texels shard, the model is replicated)
-    spec, table, wb, bb, pos, nrm, param, desc, masked = make_workload(args.workload, D.frame_of_rank(rank, world)[0])
+    # weak scaling: each rank owns one full frame per step; strong scaling: the ranks share ONE frame, each a block of
+    # rows.  The model is replicated: rank 0 builds the parameters, one broadcast per blob hands them out.
+    strong = args.scaling == "strong" and world > 1
+    frame = 0 if strong else D.frame_of_rank(rank, world)[0]
+    spec, table, wb, bb, pos, nrm, param, desc, masked = make_workload(args.workload, frame, with_params=(rank == 0))
+    img_w, img_h = W_PX, H_PX
+    n_job = pos.shape[0] * (1 if strong else world)                 # texels all ranks process per step
+    if strong:
+        if args.workload == "incoherent":
+            lo, hi = D.texel_range_of_rank(pos.shape[0], rank, world)
+        else:
+            r0, r1 = D.row_range_of_rank(H_PX, rank, world)
+            lo, hi, img_h = r0 * W_PX, r1 * W_PX, r1 - r0
+        pos, nrm = np.ascontiguousarray(pos[lo:hi]), np.ascontiguousarray(nrm[lo:hi])
+        masked = float(np.mean(np.all(nrm == 0, axis=1)))
     n = pos.shape[0]
     model = niv.NivModel(spec, local)
-    model.load_params(table, wb, bb)
+    if world > 1:
+        wl = sum(a * b_ for a, b_ in zip([spec.in_dim] + [spec.hidden_width] * spec.n_hidden_layers,
+                                         [spec.hidden_width] * spec.n_hidden_layers + [3]))
+        bl = spec.hidden_width * spec.n_hidden_layers + 3
+        shapes = [((spec.n_levels * spec.table_size * spec.n_features,), torch.float16), ((wl,), torch.float16),
+                  ((bl,), torch.float32)]
+        t_table, t_w, t_b = D.broadcast_params([table, wb, bb] if rank == 0 else None, shapes, torch.device("cuda", local))
+        model.load_params(t_table, t_w, t_b)
+        del t_table, t_w, t_b
+    else:
+        model.load_params(table, wb, bb)
     info = model.info
 
     d_pos = [torch.from_numpy(pos).cuda() for _ in range(RING)]
@@ -295,7 +320,7 @@ def run_ours(args):
         if d_tp is not None:
             model.infer_texel_params(d_pos[k], d_nrm[k], d_tp, d_out[k])
         elif image:
-            model.infer_image(d_pos[k], d_nrm[k], d_out[k], W_PX, H_PX, param=param)
+            model.infer_image(d_pos[k], d_nrm[k], d_out[k], img_w, img_h, param=param)
         else:
             model.infer(d_pos[k], d_nrm[k], d_out[k], param=param)
 
@@ -334,7 +359,7 @@ def run_ours(args):
     clk = clocks.stop() if clocks else None
     total_ms = D.reduce_max(total_ms, "cuda")
     ms_step = total_ms / args.steps
-    value = D.whole_job_gqps(n, world, ms_step)
+    value = n_job / (ms_step * 1e-3) / 1e9               # whole job: all ranks' texels over the slowest rank's time
 
     # ---- end to end: pinned host buffers through niv_infer_host ------------------------------------
     e2e_steps = max(3, min(args.steps, 20))
@@ -350,7 +375,7 @@ def run_ours(args):
     torch.cuda.synchronize()
     e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
     e2e_ms = D.reduce_max(e2e_ms, "cuda")
-    e2e_value = D.whole_job_gqps(n, world, e2e_ms)
+    e2e_value = n_job / (e2e_ms * 1e-3) / 1e9
     checksum = float(h_out[0].sum())
 
     # ---- the same end-to-end call on the compact G-buffer formats / fp16 output: fewer bytes per
@@ -371,7 +396,7 @@ def run_ours(args):
                 model.infer_host_packed(gf, ha[s % 2], None, ho[s % 2], n, out_format=of, param=param)
             torch.cuda.synchronize()
             ms = D.reduce_max((time.perf_counter() - t0) * 1e3 / e2e_steps, "cuda")
-            e2e_compact.append({"formats": name, "gbuf_format": gf, "out_format": of, "value": D.whole_job_gqps(n, world, ms),
+            e2e_compact.append({"formats": name, "gbuf_format": gf, "out_format": of, "value": n_job / (ms * 1e-3) / 1e9,
                                 "unit": UNIT, "ms_per_step": ms, "h2d_bytes_per_step": int(a.nbytes), "d2h_bytes_per_step": 8 * n,
                                 "api": "niv_infer_host_packed (pinned host buffers, zero copy)"})
             del ha, ho
@@ -385,7 +410,7 @@ def run_ours(args):
     peaks = load_peaks()
     counts = torch.zeros(niv.NIV_CENSUS_COUNTS, dtype=torch.int64, device="cuda")
     if image:
-        model.probe_sectors_image(d_pos[0], d_nrm[0], W_PX, H_PX, counts)      # the census of the warps that ran
+        model.probe_sectors_image(d_pos[0], d_nrm[0], img_w, img_h, counts)    # the census of the warps that ran
     else:
         model.probe_sectors(d_pos[0], d_nrm[0], counts)
     torch.cuda.synchronize()
@@ -456,7 +481,7 @@ def run_ours(args):
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong" if strong else "weak",
         # BASELINE.md holds a paper number only for the paper's own model: 1.35 ms per full-HD frame on an RTX 4090
         # = 1.536 Gqueries/s -- another machine's, context not target
         "vs_baseline": (value / (N_TEXELS / ((PAPER_TABLE1_HALF_MS if args.half else PAPER_TABLE1_MS)[(PAPER_LEVELS, PAPER_WIDTH)]
@@ -464,8 +489,9 @@ def run_ours(args):
         if (args.workload == "paper" and world == 1 and (PAPER_LEVELS, PAPER_WIDTH) in PAPER_TABLE1_MS) else None,
         "dtype": "f16 operands / f32 accumulate (index path: f32 + u32)", "data": "synthetic",
         "config": {"workload": args.workload, "description": desc, "model": _model_str(spec),
-                   "texels_per_gpu_per_step": n, "masked_fraction": masked, "parallelism": "dp%d (replicated model, "
-                   "texels sharded, no data-path collective)" % world,
+                   "texels_per_gpu_per_step": n, "masked_fraction": masked, "parallelism": "dp%d (model replicated by one "
+                   "broadcast per blob, %s, no data-path collective)" % (world, "row blocks of ONE frame per rank" if strong
+                                                                         else "one frame per rank"),
                    "l2": "inputs/outputs rotate over %d distinct buffer sets (%.0f MB > 126 MB L2) so G-buffer reads "
                          "come from HBM; the %.0f MiB table stays L2-resident by design" %
                          (RING, RING * 36 * n / 1e6, info.table_bytes / 2 ** 20),
@@ -737,12 +763,72 @@ def run_compose(args):
                                            "frac": nbytes / ms / 1e6 / peaks["hbm_gbs"], "peak_source": peaks["source"]}}), flush=True)
 
 
+def run_dry(args):
+    """--dry: the multi-rank plumbing of run_ours WITHOUT a GPU (gloo): self-launch, one broadcast per parameter blob from
+    rank 0, the weak / strong split, max-over-ranks timing, one JSON line from rank 0.  The "step" is a checksum of the
+    rank's slice and of the received parameters (no kernel, no oracle): for the world-size-2 CPU test of the launcher."""
+    import torch
+    import torch.distributed as dist
+    rank, world, local = D.env_rank_world()
+    if world > 1:
+        dist.init_process_group("gloo")
+    spec = I.spec_tiny()
+    strong = args.scaling == "strong" and world > 1
+    w_px, h_px = 64, 64
+    g = I.make_gbuffer(w_px, h_px, 0, frame=0 if strong else D.frame_of_rank(rank, world)[0])
+    pos, nrm = g["pos"], g["nrm"]
+    n_job = pos.shape[0] * (1 if strong else world)
+    if strong:
+        r0, r1 = D.row_range_of_rank(h_px, rank, world)
+        pos, nrm = pos[r0 * w_px:r1 * w_px], nrm[r0 * w_px:r1 * w_px]
+    table = wb = bb = None
+    if rank == 0:
+        table = I.make_table(spec, 0)
+        w, b = I.make_mlp(spec, 0)
+        wb, bb = I.pack_weights(w), I.pack_biases(b)
+    wl = spec.in_dim * spec.hidden_width + 3 * spec.hidden_width
+    shapes = [((spec.n_levels * spec.table_size * spec.n_features,), torch.float16), ((wl,), torch.float16),
+              ((spec.hidden_width + 3,), torch.float32)]
+    t_table, t_w, t_b = D.broadcast_params([table, wb, bb] if rank == 0 else None, shapes, "cpu")
+    check = float(t_table.double().sum() + t_w.double().sum() + t_b.double().sum())
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        local_sum = float(np.abs(pos).sum() + np.abs(nrm).sum())
+    ms = (time.perf_counter() - t0) * 1e3 / max(args.steps, 1) + 1e-6
+    ms_max = D.reduce_max(ms)
+    checks = [None] * world
+    if world > 1:
+        dist.all_gather_object(checks, (check, pos.shape[0], local_sum))
+    else:
+        checks = [(check, pos.shape[0], local_sum)]
+    if rank == 0:
+        print(json.dumps({"dry": True, "metric": METRIC, "value": n_job / (ms_max * 1e-3) / 1e9, "unit": UNIT, "n_gpus": world,
+                          "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_max, "higher_is_better": True,
+                          "scaling": "strong" if strong else "weak", "texels_per_rank": [c[1] for c in checks],
+                          "param_checksums": [c[0] for c in checks], "texels_per_step": n_job}))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def self_launch(args):
+    """python bench.py --gpus N (N > 1) outside torchrun: start N ranks of this script on this node, one per GPU."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = D.launcher_command(args.gpus, port, os.path.abspath(__file__), sys.argv[1:])
+    raise SystemExit(subprocess.run(cmd).returncode)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=None)
     ap.add_argument("--warmup", type=int, default=None)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: one frame per rank (weak) or the row blocks of ONE frame (strong, SURVEY 8(e))")
+    ap.add_argument("--dry", action="store_true", help="multi-rank plumbing only, on the CPU over gloo (for the launcher test)")
     ap.add_argument("--workload", default="fullhd", choices=["fullhd", "incoherent", "param", "paper", "probes"])
     ap.add_argument("--probe-spacing", type=float, default=0.16, help="workload probes: probe spacing in metres (0.16 m = "
                     "the 5.4 MB budget of PAPER.md:462 in the 10 x 4 x 10 m room)")
@@ -760,6 +846,13 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle wall time for cpu_baseline")
     ap.add_argument("--ref-sample", type=int, default=131072, help="texels per step of the reference arm")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:           # not under torchrun: start the ranks ourselves
+        self_launch(args)
+    if args.dry:
+        args.steps = 3 if args.steps is None else args.steps
+        args.warmup = 0 if args.warmup is None else args.warmup
+        run_dry(args)
+        return
     global PAPER_LEVELS, PAPER_WIDTH
     PAPER_LEVELS, PAPER_WIDTH = args.paper_levels, args.paper_width
     if args.sweep:

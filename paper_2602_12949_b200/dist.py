@@ -1,6 +1,7 @@
-"""Host-side multi-GPU plumbing of the benchmark: the path shards by texels with the model
-replicated and NO data-path collective, so all that is distributed is (a) which frame a rank owns and (b) the
-max-over-ranks of the device time.  torch.distributed only (nccl on GPUs, gloo in the CPU tests)."""
+"""Host-side multi-GPU plumbing of the benchmark: the path shards by texels with the
+model replicated and NO data-path collective, so all that is distributed is (a) the parameter blob, broadcast once from
+rank 0, (b) which frame -- or which rows of the one frame -- a rank owns and (c) the max-over-ranks of the device time.
+torch.distributed only (nccl on GPUs, gloo in the CPU tests)."""
 from __future__ import annotations
 
 import os
@@ -45,3 +46,39 @@ def reduce_max(value: float, device=None) -> float:
 def whole_job_gqps(texels_per_rank: int, world: int, ms_per_step_max: float) -> float:
     """Aggregate throughput of all ranks in Gqueries/s from the max-over-ranks step time."""
     return world * texels_per_rank / (ms_per_step_max * 1e-3) / 1e9
+
+
+def row_range_of_rank(height: int, rank: int, world: int, rows_per_tile: int = 4) -> tuple:
+    """Strong-scaling split of ONE image for niv_infer_image: contiguous blocks of whole 4-row tile rows (SURVEY 8(e):
+    "contiguous row-blocks of the frame per GPU")."""
+    tiles = (height + rows_per_tile - 1) // rows_per_tile
+    lo = (tiles * rank) // world * rows_per_tile
+    hi = min(height, (tiles * (rank + 1)) // world * rows_per_tile)
+    return lo, hi
+
+
+def broadcast_params(arrays, shapes_dtypes, device, src: int = 0):
+    """The model is replicated: rank `src` holds the parameter blobs as numpy arrays (`arrays`: a list, None elsewhere),
+    every rank gets them as tensors on `device` through ONE broadcast per blob ("ncclBroadcast of the
+    parameter blob once").  shapes_dtypes: [(shape, torch dtype)] -- known to every rank from the model spec."""
+    import torch
+    import torch.distributed as dist
+    out = []
+    world = dist.get_world_size() if (dist.is_available() and dist.is_initialized()) else 1
+    rank = dist.get_rank() if world > 1 else src
+    for k, (shape, dtype) in enumerate(shapes_dtypes):
+        if rank == src:
+            t = torch.from_numpy(arrays[k]).reshape(shape).to(device=device, dtype=dtype)
+        else:
+            t = torch.empty(shape, dtype=dtype, device=device)
+        if world > 1:
+            dist.broadcast(t, src=src)
+        out.append(t)
+    return out
+
+
+def launcher_command(n_ranks: int, port: int, script: str, argv: list) -> list:
+    """`python bench.py --gpus N` outside torchrun starts its own ranks: one process per GPU on this node."""
+    import sys
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(n_ranks),
+            "--master-addr", "127.0.0.1", "--master-port", str(port), script] + list(argv)

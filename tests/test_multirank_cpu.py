@@ -68,3 +68,35 @@ def test_single_process_defaults(monkeypatch):
     assert D.reduce_max(1.5) == 1.5
     with pytest.raises(ValueError):
         D.frame_of_rank(2, 2)
+
+
+def test_bench_launches_its_own_ranks_and_broadcasts_the_parameters():
+    """`python bench.py --gpus 2` outside torchrun starts two ranks itself (torch.distributed.run, 127.0.0.1); --dry runs
+    the plumbing of the GPU arm over gloo: parameters built on rank 0 only and broadcast, weak / strong split, max over
+    ranks, ONE JSON line."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    for scaling, per_rank, total in (("weak", [4096, 4096], 8192), ("strong", [2048, 2048], 4096)):
+        res = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--dry", "--scaling", scaling],
+                             capture_output=True, text=True, env=env, timeout=600)
+        assert res.returncode == 0, res.stderr[-3000:]
+        lines = [l for l in res.stdout.splitlines() if l.startswith("{")]
+        assert len(lines) == 1, res.stdout
+        d = json.loads(lines[0])
+        assert d["dry"] is True and d["n_gpus"] == 2 and d["scaling"] == scaling
+        assert d["texels_per_rank"] == per_rank and d["texels_per_step"] == total
+        assert d["param_checksums"][0] == d["param_checksums"][1] != 0.0            # rank 1 got rank 0's parameters
+        assert d["value"] > 0
+
+
+def test_row_split_covers_the_image():
+    for h in (1, 3, 4, 5, 540, 1080, 2160, 4099):
+        for world in (1, 2, 3, 8):
+            spans = [D.row_range_of_rank(h, r, world) for r in range(world)]
+            assert spans[0][0] == 0 and spans[-1][1] == h
+            for a, b in zip(spans, spans[1:]):
+                assert a[1] == b[0] and a[0] <= a[1]
+            assert all(s[0] % 4 == 0 for s in spans)
