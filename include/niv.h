@@ -210,6 +210,14 @@ int niv_infer_image_packed(niv_model *m, int gbuf_format, const void *gbuf_a, co
                            int out_format, void *out, uint32_t width, uint32_t height, void *stream);
 int niv_infer_host_packed(niv_model *m, int gbuf_format, const void *gbuf_a, const void *gbuf_b, const float *param,
                           int out_format, void *out, size_t n, void *stream);
+/* Debug: niv_infer, and besides `out` every texel's layer-1 A row as the FUSED kernel built it (the 32-bit words the
+ * tensor core reads: L*F/2 words of fp16 latent pairs -- 24 words of positional encoding for the grid-less models --
+ * then the direction (8 words SH-16, or (x, y | z, 0)), zero-padded to a multiple of 8 words = row_words).  arow is
+ * device, [n][row_words] uint32; rows of background texels hold zeros.  row_words other than that -> NIV_ERR_INVALID_ARG.
+ * For feature-level parity of the fused path (cell-block levels, packed-fp16 blend) in every model family. */
+int niv_debug_arow(niv_model *m, const float *pos, const float *nrm, const float *param, float *out,
+                   uint32_t *arow, uint32_t row_words, size_t n, void *stream);
+
 /* The fp32 position and normal ([n][3] each, device) the fused kernels decode from a compact G-buffer (device). */
 int niv_decode_gbuffer(niv_model *m, int gbuf_format, const void *gbuf_a, const void *gbuf_b, float *pos, float *nrm,
                        size_t n, void *stream);

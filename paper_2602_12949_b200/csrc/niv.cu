@@ -448,11 +448,9 @@ static fused_fn pick_levels_f4(uint32_t L) {        // the paper's own family: F
 // PK: the variant that reads the compact G-buffer formats / writes fp16 (linear tiles; the grid models of both families)
 template <bool O, bool C, bool PK = false>
 static fused_fn pick_fused(uint32_t W, uint32_t L, uint32_t F) {
-    if (L == 0) {                                   // grid-less: positional encoding, no gathers
-        if (PK) return nullptr;
-        return W == 16 ? fused_inst<16, 0, 2, true, O, 0, false, false>() : W == 32 ? fused_inst<32, 0, 2, true, O, 0, false, false>()
-             : W == 64 ? fused_inst<64, 0, 2, true, O, 0, false, false>() : nullptr;
-    }
+    if (L == 0)                                     // grid-less: positional encoding, no gathers
+        return W == 16 ? fused_inst<16, 0, 2, true, O, 0, false, false, PK>() : W == 32 ? fused_inst<32, 0, 2, true, O, 0, false, false, PK>()
+             : W == 64 ? fused_inst<64, 0, 2, true, O, 0, false, false, PK>() : nullptr;
     if (F == 4) return W == 32 ? pick_levels_f4<32, O, C, PK>(L) : W == 64 ? pick_levels_f4<64, O, C, PK>(L) : nullptr;
     return W == 32 ? pick_levels_f2<32, O, 0, false, C, PK>(L) : W == 64 ? pick_levels_f2<64, O, 0, false, C, PK>(L) : nullptr;
 }
@@ -1067,6 +1065,28 @@ extern "C" int niv_infer_packed(niv_model* m, int gbuf_format, const void* gbuf_
     if (rc != NIV_OK) return rc;
     set_formats(m, P, gbuf_format, out_format);
     return launch_fused(m, P, (const float*)gbuf_a, (const float*)gbuf_b, (float*)out, n, (cudaStream_t)stream);
+}
+
+// Debug: niv_infer through the PACKED kernel variant (fp32 x 3 in and out) which also writes every texel's layer-1 A
+// row -- the packed fp16 words the tensor core reads: latents, direction, zero padding -- for feature-level parity of
+// the FUSED path (cell-block levels, packed-fp16 blend) in every model family.
+extern "C" int niv_debug_arow(niv_model* m, const float* pos, const float* nrm, const float* param, float* out,
+                              uint32_t* arow, uint32_t row_words, size_t n, void* stream)
+{
+    int rc = check_call(m, pos, nrm, out, n);
+    if (rc != NIV_OK) return rc > 0 ? NIV_OK : rc;
+    if (!arow || !m->fused_pk.fn) return arow ? NIV_ERR_UNSUPPORTED : NIV_ERR_INVALID_ARG;
+    const uint32_t hw = m->cfg.n_levels ? m->cfg.n_levels * m->cfg.n_features / 2 : 24u;
+    const uint32_t need = (hw + (m->cfg.sh_degree ? 8u : 2u) + 7u) / 8u * 8u;
+    if (row_words != need) return NIV_ERR_INVALID_ARG;
+    KParams P;
+    rc = fill_params(m, param, P);
+    if (rc != NIV_OK) return rc;
+    set_formats(m, P, NIV_GBUF_F32X3, NIV_OUTFMT_F32X3);
+    P.dump_a = arow;
+    P.dump_words = row_words;
+    draw_tile_counter(m, (cudaStream_t)stream, P);
+    return launch_one(m, m->fused_pk, (cudaStream_t)stream, m->pdl, P, pos, nrm, out, n, (uint32_t)((n + kTile - 1) / kTile));
 }
 
 extern "C" int niv_infer(niv_model* m, const float* pos, const float* nrm, const float* param,

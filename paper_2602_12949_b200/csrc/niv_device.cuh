@@ -65,6 +65,8 @@ struct KParams {
     uint32_t misc_off;          // byte offset of folded bias / barriers
     const uint32_t* wmma;       // weights in the layout of the mma.sync A/B kernel (niv_fused_mma.cuh), else NULL
     const float* tparam;        // per-texel scene parameters [n][n_params] (niv_infer_texel_params), else NULL
+    uint32_t* dump_a;           // niv_debug_arow (PACKED kernels): every texel's layer-1 A row, [n][dump_words] x 32 bit
+    uint32_t dump_words;
     uint32_t gbuf_fmt;          // NIV_GBUF_*: how the caller's G-buffer texels are stored (load_texel_raw / decode_texel)
     uint32_t out_fmt;           // NIV_OUTFMT_*: fp32 x 3 or fp16 x 4 per texel
     float    aext[3];           // fl32(max - min): the scale of the unorm16 position format

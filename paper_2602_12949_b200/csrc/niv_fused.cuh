@@ -229,6 +229,12 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
 #pragma unroll
             for (int q = 0; q < NPT; ++q) param_encode8_packed(tv[q], a + AW + 8 * q);
         }
+        if constexpr (PACKED) {                       // niv_debug_arow: the row as the tensor core will read it
+            if (P.dump_a && valid) {
+#pragma unroll
+                for (int k = 0; k < AWT; ++k) P.dump_a[i * P.dump_words + k] = a[k];
+            }
+        }
         prefetch_next();
         __syncwarp();
         if constexpr (AW == 8) tmem_st_x8(lane_taddr + A_COL, a);

@@ -32,7 +32,7 @@ _OUT_BYTES = {0: 12, 1: 8}
 
 EXPORTS = ("niv_create", "niv_get_info", "niv_load_params", "niv_infer", "niv_infer_image", "niv_infer_texel_params",
            "niv_infer_host", "niv_probe_sectors_image",
-           "niv_infer_packed", "niv_infer_image_packed", "niv_infer_host_packed", "niv_decode_gbuffer",
+           "niv_infer_packed", "niv_infer_image_packed", "niv_infer_host_packed", "niv_decode_gbuffer", "niv_debug_arow",
            "niv_encode",
            "niv_debug_encode", "niv_compose", "niv_destroy", "niv_error_string", "niv_last_cuda_error", "niv_probe_gather",
            "niv_probe_sectors",
@@ -102,6 +102,7 @@ def lib():
         L.niv_infer_image_packed.argtypes = [vp, C.c_int, vp, vp, C.POINTER(C.c_float), C.c_int, vp, C.c_uint32, C.c_uint32, vp]
         L.niv_infer_host_packed.argtypes = [vp, C.c_int, vp, vp, C.POINTER(C.c_float), C.c_int, vp, sz, vp]
         L.niv_decode_gbuffer.argtypes = [vp, C.c_int, vp, vp, vp, vp, sz, vp]
+        L.niv_debug_arow.argtypes = [vp, vp, vp, C.POINTER(C.c_float), vp, vp, C.c_uint32, sz, vp]
         L.niv_debug_encode.argtypes = [vp, vp, vp, C.POINTER(C.c_float), sz, vp, vp, vp, vp, vp]
         L.niv_compose.argtypes = [vp, C.c_uint32, C.c_uint32, vp, vp, vp, vp, C.c_uint32, C.c_uint32, vp]
         L.niv_destroy.argtypes = [vp]
@@ -330,6 +331,22 @@ class NivModel:
         if rc != NIV_OK:
             raise NivError(rc, "niv_infer_host_packed")
         return out
+
+    def arow_words(self) -> int:
+        """32-bit words of one layer-1 A row of the fused kernel (include/niv.h niv_debug_arow)."""
+        hw = self.spec.n_levels * self.spec.n_features // 2 if self.spec.n_levels else 24
+        return (hw + (8 if self.spec.sh_degree else 2) + 7) // 8 * 8
+
+    def debug_arow(self, pos, nrm, out, arow, param=None, stream=None):
+        """niv_infer + the fused kernel's layer-1 A rows: arow device int32 [n][arow_words()]."""
+        import torch
+        n = pos.shape[0]
+        _same_rows(n, nrm=nrm, out=out, arow=arow)
+        rc = lib().niv_debug_arow(self._h, _dev(pos, torch.float32, "pos", 3), _dev(nrm, torch.float32, "nrm", 3),
+                                  _params(param, self.spec.n_params), _dev(out, torch.float32, "out", 3),
+                                  _dev(arow, torch.int32, "arow", self.arow_words()), self.arow_words(), n, _stream_ptr(stream))
+        if rc != NIV_OK:
+            raise NivError(rc, "niv_debug_arow")
 
     def decode_gbuffer(self, gbuf_format, a, b, pos, nrm, n, stream=None):
         """pos, nrm: device [n][3] fp32 outputs = what the fused kernels decode from the compact G-buffer."""
