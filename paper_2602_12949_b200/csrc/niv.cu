@@ -654,7 +654,7 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
         m->fused.smem = P.misc_off + 64;
         rc = m->fused.fn ? setup_kernel(m, m->fused, 128, "fused_w128") : NIV_ERR_UNSUPPORTED;
     } else {
-        const int tmem_cols = 128;                       // D | A | ones in one allocation
+        const int tmem_cols = W == 16 ? 64 : 128;        // D | A | ones in one allocation (niv_fused.cuh TMEM_COLS)
         m->fused.fn = use_cells ? pick_fused<false, true>(W, cfg->n_levels, cfg->n_features)
                                 : pick_fused<false, false>(W, cfg->n_levels, cfg->n_features);
         m->fused.smem = smem_dev;

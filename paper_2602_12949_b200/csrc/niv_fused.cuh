@@ -39,7 +39,9 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
 {
     static_assert(WIDTH <= 64, "A-in-TMEM kernel: D + A + ones must fit 128 columns");
     static_assert(NC <= L, "cell-block levels are the leading levels");
-    constexpr uint32_t TMEM_COLS = 128, A_COL = 64, ONES_COL = NPT == 2 ? 104 : 96;
+    // width 16 (the paper's smallest grid-less model): D 16 | A 32 | ones 8 fit 64 columns -> eight CTAs per SM
+    constexpr uint32_t TMEM_COLS = WIDTH == 16 ? 64 : 128, A_COL = WIDTH == 16 ? 16 : 64,
+                       ONES_COL = WIDTH == 16 ? 48 : NPT == 2 ? 104 : 96;
     constexpr int NG = L / NB;
     constexpr int HW = L ? L * F / 2 : 24;            // 32-bit words of hash latents in one A row (L = 0: the
                                                       // 3 x 8 (sin, cos) pairs of the positional encoding)
