@@ -678,6 +678,89 @@ def run_probes(args):
     grid.close()
 
 
+def run_probe_patterns(args):
+    """The gather micro-benchmark in all its access patterns (include/niv.h niv_probe_gather) on an L1-resident, a
+    borderline and an L2-resident buffer: clocks per warp-wide load instruction.  A table for profiles/, not the
+    contract line."""
+    import torch
+
+    from paper_2602_12949_b200 import build as B
+    from paper_2602_12949_b200 import niv
+
+    B.build()
+    niv.lib()
+    torch.cuda.set_device(0)
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    mhz = 1965.0
+    sink = torch.zeros(4, dtype=torch.int32, device="cuda")
+    for kb in (32, 64, 8192):
+        buf = torch.zeros(kb * 256, dtype=torch.int32, device="cuda")
+        for pat in range(10):
+            n_ctas, lpl = sms * 8, 256
+            for _ in range(3):
+                niv.probe_gather(buf, pat, n_ctas, lpl, 1, sink)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for r in range(10):
+                niv.probe_gather(buf, pat, n_ctas, lpl, 100 + r, sink)
+            e1.record()
+            torch.cuda.synchronize()
+            dt = e0.elapsed_time(e1) * 1e-3 / 10
+            loads = n_ctas * 256 * lpl
+            per_clk = loads / 32 / dt / sms / (mhz * 1e6)
+            print(json.dumps({"buffer_KB": kb, "pattern": pat, "gloads_per_s": loads / dt / 1e9,
+                              "clocks_per_warp_load_at_1965MHz": 1.0 / per_clk}), flush=True)
+
+
+def run_encode(args):
+    """north_star (2): the stand-alone encoding kernel (niv_encode: rows a1..a9, fp16 feature rows to HBM) on the
+    configs[1] frame: ms, the gather census GB/s and its fraction of the measured random-sector rate, HBM GB/s (24 B in,
+    2 * in_dim B out per texel).  One JSON line (not the contract line); ncu counters: profiles/r02_encode.md."""
+    import torch
+
+    from paper_2602_12949_b200 import build as B
+    from paper_2602_12949_b200 import niv
+
+    B.build()
+    niv.lib()
+    torch.cuda.set_device(0)
+    spec, table, wb, bb, pos, nrm, param, desc, masked = make_workload("fullhd", 0)
+    n = pos.shape[0]
+    model = niv.NivModel(spec, 0)
+    model.load_params(table, wb, bb)
+    ring = 4
+    d_pos = [torch.from_numpy(pos).cuda() for _ in range(ring)]
+    d_nrm = [torch.from_numpy(nrm).cuda() for _ in range(ring)]
+    d_f = [torch.empty((n, spec.in_dim), dtype=torch.float16, device="cuda") for _ in range(ring)]
+    steps = args.steps or 100
+    for k in range(5):
+        model.encode(d_pos[k % ring], d_nrm[k % ring], d_f[k % ring])
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for k in range(steps):
+        model.encode(d_pos[k % ring], d_nrm[k % ring], d_f[k % ring])
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    counts = torch.zeros(niv.NIV_CENSUS_COUNTS, dtype=torch.int64, device="cuda")
+    model.probe_sectors(d_pos[0], d_nrm[0], counts)
+    torch.cuda.synchronize()
+    c = counts.cpu().numpy()
+    sectors = int(c[:spec.n_levels].sum())
+    gpeak, _ = measure_gather_peak(torch, niv, model.info.table_bytes, model.info.num_sms)
+    peaks = load_peaks()
+    hbm_bytes = (24 + 2 * spec.in_dim) * n
+    print(json.dumps({"op": "niv_encode", "workload": "fullhd", "ms": ms, "gqueries_per_s": n / ms / 1e6,
+                      "gather": {"sectors": sectors, "achieved_gbs": sectors * 32 / ms / 1e6,
+                                 "peak_gbs": gpeak["random_sector"]["sector_gbs"],
+                                 "frac": sectors * 32 / ms / 1e6 / gpeak["random_sector"]["sector_gbs"]},
+                      "hbm": {"bytes": hbm_bytes, "achieved_gbs": hbm_bytes / ms / 1e6, "peak_gbs": peaks["hbm_gbs"],
+                              "frac": hbm_bytes / ms / 1e6 / peaks["hbm_gbs"]},
+                      "cell_levels": int(model.info.cell_levels)}))
+    model.close()
+
+
 def run_sweep(args):
     """BASELINE.json configs[4]: table size x MLP width at full HD, and resolution x frames per call.  One JSON line
     per case on stdout (NOT the contract line: a table for profiles/)."""
@@ -873,6 +956,8 @@ def main():
     ap.add_argument("--texel-params", action="store_true",
                     help="--workload param only: time niv_infer_texel_params (one scene parameter value per texel, SURVEY 8 f3)")
     ap.add_argument("--half", action="store_true", help="quarter pixel count: a 960x540 G-buffer (PAPER.md:405, Table 1 'half')")
+    ap.add_argument("--encode", action="store_true", help="time the stand-alone encoding kernel (north_star (2))")
+    ap.add_argument("--probe-patterns", action="store_true", help="niv_probe_gather in all patterns x three buffer sizes")
     ap.add_argument("--sweep", action="store_true", help="BASELINE.json configs[4]: table-size / width / resolution sweep")
     ap.add_argument("--cpu-budget", type=float, default=12.0, help="seconds of oracle wall time for cpu_baseline")
     ap.add_argument("--ref-sample", type=int, default=131072, help="texels per step of the reference arm")
@@ -886,6 +971,12 @@ def main():
         return
     global PAPER_LEVELS, PAPER_WIDTH
     PAPER_LEVELS, PAPER_WIDTH = args.paper_levels, args.paper_width
+    if args.probe_patterns:
+        run_probe_patterns(args)
+        return
+    if args.encode:
+        run_encode(args)
+        return
     if args.sweep:
         run_sweep(args)
         return

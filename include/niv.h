@@ -266,6 +266,8 @@ int niv_last_cuda_error(void);
  *   5  one whole random 32-byte sector per lane, one 256-bit load
  *   6  two 4-byte loads (two instructions) from one random sector per lane
  *   7  as 0 with L1::no_allocate
+ *   8  as 0 through the texture path (tex1Dfetch on a linear texture object made for the call)
+ *   9  as 0, alternating between the LSU path and the texture path
  * buf is device memory of `buf_bytes` (power of two, 32-byte aligned); sink is device, >= 4 bytes.  Asynchronous. */
 int niv_probe_gather(const void *buf, size_t buf_bytes, int pattern, uint32_t n_ctas, uint32_t loads_per_lane,
                      uint32_t seed, void *sink, void *stream);

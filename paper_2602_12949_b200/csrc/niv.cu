@@ -38,6 +38,8 @@ namespace niv {
 // =====================================================================================================
 // stand-alone encode (fp16 features to global) and debug dump
 // =====================================================================================================
+// NC: levels 0 .. NC-1 from their cell-block copies (as the fused kernel); groups of four levels, at most four groups
+template <int NC>
 __global__ void __launch_bounds__(128) niv_encode_kernel(const __grid_constant__ KParams P,
                                                          const float* __restrict__ pos,
                                                          const float* __restrict__ nrm,
@@ -57,7 +59,9 @@ __global__ void __launch_bounds__(128) niv_encode_kernel(const __grid_constant__
     float u[3];
     normalise(P, p, u);
     const uint32_t n_groups = P.L >> 2;
-    for (uint32_t g = 0; g < n_groups; ++g) row[g] = encode_group4(P, (int)(g * 4), u);
+#pragma unroll
+    for (int g = 0; g < kMaxLevels / 4; ++g)
+        if ((uint32_t)g < n_groups) row[g] = encode_group4<NC>(P, g * 4, u);
     float sh[16];
     sh16(nv, sh);
     row[n_groups] = make_uint4(pack_half2(sh[0], sh[1]), pack_half2(sh[2], sh[3]),
@@ -1264,7 +1268,11 @@ extern "C" int niv_encode(niv_model* m, const float* pos, const float* nrm, cons
     int rc = fill_params(m, param, P);
     if (rc != NIV_OK) return rc;
     const unsigned grid = (unsigned)((n + 127) / 128);
-    niv_encode_kernel<<<grid, 128, 0, (cudaStream_t)stream>>>(P, pos, nrm, (uint4*)features_fp16, n);
+    switch (m->info.cell_levels) {                     // (F = 2: four or five cell-block levels, or none)
+        case 5:  niv_encode_kernel<5><<<grid, 128, 0, (cudaStream_t)stream>>>(P, pos, nrm, (uint4*)features_fp16, n); break;
+        case 4:  niv_encode_kernel<4><<<grid, 128, 0, (cudaStream_t)stream>>>(P, pos, nrm, (uint4*)features_fp16, n); break;
+        default: niv_encode_kernel<0><<<grid, 128, 0, (cudaStream_t)stream>>>(P, pos, nrm, (uint4*)features_fp16, n); break;
+    }
     NIV_CUDA(cudaGetLastError());
     return NIV_OK;
 }

@@ -277,9 +277,10 @@ __device__ __forceinline__ void batch_blend(const Batch<NB, F>& b, uint32_t* f) 
 }
 
 // One group of 4 levels (8 latents = one 16-byte fp16 chunk of the A operand), gathers issued together (F = 2).
+template <int NC = 0>
 __device__ __forceinline__ uint4 encode_group4(const KParams& P, int l0, const float u[3]) {
     Batch<4, 2> b;
-    batch_issue<4, 2>(P, l0, u, b);
+    batch_issue<4, 2, NC>(P, l0, u, b);
     uint32_t f[4];
     batch_blend<4, 2>(b, f);
     return make_uint4(f[0], f[1], f[2], f[3]);
