@@ -60,7 +60,8 @@ enum {
     NIV_ERR_UNSUPPORTED = -2,   /* a valid configuration this build has no kernel for             */
     NIV_ERR_NOT_LOADED  = -3,   /* niv_infer before niv_load_params                               */
     NIV_ERR_CUDA        = -4,   /* a CUDA runtime call failed (niv_last_cuda_error has the code)  */
-    NIV_ERR_ALLOC       = -5    /* host or device allocation failed                               */
+    NIV_ERR_ALLOC       = -5,   /* host or device allocation failed                               */
+    NIV_ERR_TOO_LARGE   = -6    /* niv_infer_host_static: n > NIV_STATIC_MAX_TEXELS               */
 };
 
 /* G-buffer and output formats of the *_packed entry points (readings in DESIGN.md 3.4, 3.5) */
@@ -190,6 +191,20 @@ int niv_infer_texel_params(niv_model *m, const float *pos, const float *nrm, con
  * concurrent callers on the same model.  Errors as niv_infer, plus NIV_ERR_ALLOC. */
 int niv_infer_host(niv_model *m, const float *pos, const float *nrm, const float *param,
                    float *out, size_t n, void *stream);
+
+/* niv_infer_host for callers that cannot allocate (code under CUDA graph capture set-up, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same fused kernel, staged through ONE static device array instead of the
+ * cudaMalloc'ed staging buffers and internal streams of niv_infer_host's staged path.  The call makes no cudaMalloc /
+ * cudaFree and creates no stream or event: it clears its tile counters, copies pos and nrm in, launches the kernel,
+ * copies out back -- all on `stream` -- and synchronises `stream`.
+ *   pos, nrm, out  HOST, [n][3] fp32 packed (pageable or pinned);  param  HOST, as niv_infer
+ *   n <= NIV_STATIC_MAX_TEXELS (262,144 = a 512 x 512 tile), else NIV_ERR_TOO_LARGE; larger frames: several calls
+ * The array (9.4 MB) is held by every GPU that loads the library until the process exits and is SHARED by every call on
+ * that device, whatever the model or stream: calls that overlap on the GPU race -- serialise them.  Results equal
+ * niv_infer_host's.  Other errors as niv_infer (NIV_ERR_UNSUPPORTED with NIV_MMA_SYNC=1). */
+#define NIV_STATIC_MAX_TEXELS 262144
+int niv_infer_host_static(niv_model *m, const float *pos, const float *nrm, const float *param,
+                          float *out, size_t n, void *stream);
 
 /* ---- compact G-buffer formats and fp16 output -------------------------------------------------
  * The paper only says "position and normal buffers"; engines keep G-buffers in many layouts, and on the

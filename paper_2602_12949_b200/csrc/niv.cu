@@ -1227,6 +1227,71 @@ extern "C" int niv_infer_host(niv_model* m, const float* pos, const float* nrm, 
     return niv_infer_host_packed(m, NIV_GBUF_F32X3, pos, nrm, param, NIV_OUTFMT_F32X3, out, n, stream);
 }
 
+// ---- niv_infer_host_static: the host-buffer call for callers that must not allocate ---------------------------------
+// The staged path of niv_infer_host keeps its staging buffers in cudaMalloc'ed memory that it grows on demand (and it
+// creates two streams on first use).  This variant runs the same fused kernel on staging buffers that live in ONE
+// file-scope device array of a fixed, modest size, so the call allocates nothing: no cudaMalloc / cudaFree, no stream
+// or event creation, only cudaMemsetAsync, cudaMemcpyAsync, one kernel launch and a stream synchronisation on the
+// caller's stream.  Every GPU that loads the library holds the array (9.4 MB) until the process exits.
+//   layout: [0, 256)  the launch's tile-counter triple (tile, done, complete) -- must start at zero: cleared per call
+//           then pos | nrm | out staging, 12 bytes x NIV_STATIC_MAX_TEXELS each
+// The array is shared by every call of the process on that device (all models, all streams) and keeps the last call's
+// contents: two calls that overlap on the GPU race.
+constexpr size_t kStaticStage = (size_t)12 * NIV_STATIC_MAX_TEXELS;
+static __device__ __align__(256) uint8_t g_static_scratch[256 + 3 * kStaticStage];
+
+// In host code `g_static_scratch` is a host-side stand-in, not a device address: the address the kernel and the copies
+// need comes from cudaGetSymbolAddress, asked once per device with that device current.
+static std::mutex g_static_mu;
+static uint8_t* g_static_ptr[64] = {};
+static int static_scratch_address(int device, uint8_t** out)
+{
+    if (device < 0 || device >= 64) return NIV_ERR_INVALID_ARG;
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_ptr[device]) {
+        NIV_CUDA(cudaSetDevice(device));
+        void* p = nullptr;
+        NIV_CUDA(cudaGetSymbolAddress(&p, g_static_scratch));
+        if (!p) return NIV_ERR_CUDA;
+        g_static_ptr[device] = static_cast<uint8_t*>(p);
+    }
+    *out = g_static_ptr[device];
+    return NIV_OK;
+}
+
+extern "C" int niv_infer_host_static(niv_model* m, const float* pos, const float* nrm, const float* param,
+                                     float* out, size_t n, void* stream)
+{
+    int rc = check_call(m, pos, nrm, out, n);
+    if (rc != NIV_OK) return rc > 0 ? NIV_OK : rc;
+    if (n > (size_t)NIV_STATIC_MAX_TEXELS) return NIV_ERR_TOO_LARGE;
+    if (m->mma_kernel || !m->fused.fn) return NIV_ERR_UNSUPPORTED;
+    KParams P;
+    rc = fill_params(m, param, P);
+    if (rc != NIV_OK) return rc;
+    set_formats(m, P, NIV_GBUF_F32X3, NIV_OUTFMT_F32X3);
+    uint8_t* scratch = nullptr;
+    rc = static_scratch_address(m->cfg.device, &scratch);
+    if (rc != NIV_OK) return rc;
+    NIV_CUDA(cudaSetDevice(m->cfg.device));
+    cudaStream_t st = (cudaStream_t)stream;
+    float* d_pos = reinterpret_cast<float*>(scratch + 256);
+    float* d_nrm = reinterpret_cast<float*>(scratch + 256 + kStaticStage);
+    float* d_out = reinterpret_cast<float*>(scratch + 256 + 2 * kStaticStage);
+    NIV_CUDA(cudaMemsetAsync(scratch, 0, 256, st));                   // the tile counters must start at zero
+    NIV_CUDA(cudaMemcpyAsync(d_pos, pos, n * 12, cudaMemcpyHostToDevice, st));
+    NIV_CUDA(cudaMemcpyAsync(d_nrm, nrm, n * 12, cudaMemcpyHostToDevice, st));
+    P.tile_ctr = reinterpret_cast<uint32_t*>(scratch);               // dynamic tile scheduling on the static counters
+    P.slot_done = nullptr;
+    P.slot_gen = 1;
+    // no programmatic serialisation, no launch overlap: the launch is strictly ordered between its copies
+    rc = launch_one(m, m->fused, st, false, P, d_pos, d_nrm, d_out, n, (uint32_t)((n + kTile - 1) / kTile));
+    if (rc != NIV_OK) return rc;
+    NIV_CUDA(cudaMemcpyAsync(out, d_out, n * 12, cudaMemcpyDeviceToHost, st));
+    NIV_CUDA(cudaStreamSynchronize(st));
+    return NIV_OK;
+}
+
 // The decoded fp32 position and normal of every texel of a compact G-buffer (what the fused kernels work on): for tests
 // (bit-exact positions against the CPU decode) and for callers that want the fp32 buffers.
 __global__ void __launch_bounds__(256) niv_decode_kernel(const __grid_constant__ KParams P, const float* __restrict__ a,
@@ -1486,6 +1551,7 @@ extern "C" const char* niv_error_string(int code)
         case NIV_ERR_NOT_LOADED: return "parameters not loaded";
         case NIV_ERR_CUDA: return "CUDA runtime error (see niv_last_cuda_error)";
         case NIV_ERR_ALLOC: return "allocation failed";
+        case NIV_ERR_TOO_LARGE: return "more texels than the static scratch holds (NIV_STATIC_MAX_TEXELS)";
         default: return "unknown error code";
     }
 }

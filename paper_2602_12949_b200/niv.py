@@ -20,6 +20,8 @@ NIV_ERR_UNSUPPORTED = -2
 NIV_ERR_NOT_LOADED = -3
 NIV_ERR_CUDA = -4
 NIV_ERR_ALLOC = -5
+NIV_ERR_TOO_LARGE = -6
+NIV_STATIC_MAX_TEXELS = 262144        # niv_infer_host_static
 NIV_OUT_LINEAR = 0
 NIV_OUT_SIGMOID = 1
 NIV_CENSUS_COUNTS = 49      # niv_probe_sectors: [0,16) sectors, [16,32) lines, [32] active texels, [33,49) touched
@@ -32,6 +34,7 @@ _OUT_BYTES = {0: 12, 1: 8}
 
 EXPORTS = ("niv_create", "niv_get_info", "niv_load_params", "niv_infer", "niv_infer_image", "niv_infer_texel_params",
            "niv_infer_host", "niv_probe_sectors_image",
+           "niv_infer_host_static",
            "niv_infer_packed", "niv_infer_image_packed", "niv_infer_host_packed", "niv_decode_gbuffer", "niv_debug_arow",
            "niv_encode",
            "niv_debug_encode", "niv_compose", "niv_destroy", "niv_error_string", "niv_last_cuda_error", "niv_probe_gather",
@@ -94,6 +97,7 @@ def lib():
         L.niv_load_params.argtypes = [vp, vp, sz, vp, sz, vp, sz, C.c_int, vp]
         L.niv_infer.argtypes = [vp, vp, vp, C.POINTER(C.c_float), vp, sz, vp]
         L.niv_infer_host.argtypes = [vp, vp, vp, C.POINTER(C.c_float), vp, sz, vp]
+        L.niv_infer_host_static.argtypes = [vp, vp, vp, C.POINTER(C.c_float), vp, sz, vp]
         L.niv_infer_texel_params.argtypes = [vp, vp, vp, vp, vp, sz, vp]
         L.niv_infer_image.argtypes = [vp, vp, vp, C.POINTER(C.c_float), vp, C.c_uint32, C.c_uint32, vp]
         L.niv_probe_sectors_image.argtypes = [vp, vp, vp, C.c_uint32, C.c_uint32, vp, vp]
@@ -358,6 +362,18 @@ class NivModel:
                                       _stream_ptr(stream))
         if rc != NIV_OK:
             raise NivError(rc, "niv_decode_gbuffer")
+
+    def infer_host_static(self, pos, nrm, out, param=None, stream=None):
+        """infer_host without any allocation: staged through the library's static device array; at most
+        NIV_STATIC_MAX_TEXELS texels per call (include/niv.h niv_infer_host_static)."""
+        n = pos.shape[0]
+        _same_rows(n, nrm=nrm, out=out)
+        rc = lib().niv_infer_host_static(self._h, _host_ptr(pos, "pos"), _host_ptr(nrm, "nrm"),
+                                         _params(param, self.spec.n_params), _host_ptr(out, "out"), n,
+                                         _stream_ptr(stream))
+        if rc != NIV_OK:
+            raise NivError(rc, "niv_infer_host_static")
+        return out
 
     def encode(self, pos, nrm, features, param=None, stream=None):
         """features: device [n][in_dim] fp16."""
