@@ -267,3 +267,21 @@ def quantise_f16x4(e) -> np.ndarray:
     if lib().niv_oracle_quantise_f16x4(_p(e), C.c_size_t(e.shape[0]), _p(out)):
         raise ValueError("niv_oracle_quantise_f16x4 failed")
     return out
+
+
+def compose_jb(E, pos_half, nrm_half, pos, nrm, albedo, sigma, power, direct=None, emission=None) -> np.ndarray:
+    """Deferred compose with joint-bilateral upsampling of half-resolution E (niv_oracle_ext.c niv_oracle_compose_jb).
+    E, pos_half, nrm_half [eh][ew][3]; pos, nrm, albedo (, direct, emission) [h][w][3] with (h, w) = (2 eh, 2 ew) -> fp64."""
+    E, pos_half, nrm_half = (_chk(a, np.float32, "half") for a in (E, pos_half, nrm_half))
+    pos, nrm, albedo = (_chk(a, np.float32, "full") for a in (pos, nrm, albedo))
+    direct = None if direct is None else _chk(direct, np.float32, "direct")
+    emission = None if emission is None else _chk(emission, np.float32, "emission")
+    h, w = albedo.shape[:2]
+    eh, ew = E.shape[:2]
+    out = np.zeros((h, w, 3), dtype=np.float64)
+    rc = lib().niv_oracle_compose_jb(_p(E), _p(pos_half), _p(nrm_half), C.c_uint32(ew), C.c_uint32(eh), _p(pos), _p(nrm),
+                                     _p(albedo), _p(direct), _p(emission), C.c_double(sigma), C.c_double(power), _p(out),
+                                     C.c_uint32(w), C.c_uint32(h))
+    if rc:
+        raise ValueError("niv_oracle_compose_jb failed (E must be at exactly half the resolution; sigma > 0, power >= 0)")
+    return out

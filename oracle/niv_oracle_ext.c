@@ -249,3 +249,61 @@ int niv_oracle_quantise_f16x4(const float *e, size_t n, uint16_t *out)
     }
     return 0;
 }
+
+/* =====================================================================================================
+ * Deferred compose with JOINT-BILATERAL upsampling of half-resolution irradiance.
+ * half-resolution rendering "introduces aliasing artifacts which could be partly resolved by using
+ * industry practice upsampling methods" (joint bilateral upsampling); SPEC.md:490 leaves it "a flagged extension".
+ * The paper gives no formula; the reading is the classic one with the full-resolution G-buffer as guide:
+ *   J1 footprint   the four half-res texels q of the bilinear upsample of niv_oracle_compose (full-res pixel x at
+ *                  half-res coordinate x/2 - 1/4, neighbours clamped to the edge) with its bilinear weights b_q
+ *   J2 range       g_q = exp(-|x_p - x_q|^2 / (2 sigma^2)) * max(0, n_p . n_q)^k     (world positions, normals as given)
+ *   J3 floor       w_q = b_q (g_q + 1e-6): a pixel none of whose neighbours resembles it falls back, continuously, to
+ *                  the plain bilinear blend (the floor of the paper's probe interpolation, reused)
+ *   J4 blend       E_p = sum_q w_q E_q / sum_q w_q;      J5 compose  L = albedo / pi * E_p + direct + emission  (Eq. 2)
+ * A clamped neighbour that coincides with another one simply appears twice (as in the bilinear blend).  fp64.
+ * ===================================================================================================== */
+int niv_oracle_compose_jb(const float *E, const float *pos_half, const float *nrm_half, uint32_t ew, uint32_t eh,
+                          const float *pos, const float *nrm, const float *albedo, const float *direct,
+                          const float *emission, double sigma, double power, double *out, uint32_t w, uint32_t h)
+{
+    const double PI = 3.14159265358979323846;
+    if (!E || !pos_half || !nrm_half || !pos || !nrm || !albedo || !out || w == 0 || h == 0) return -1;
+    if (2 * ew != w || 2 * eh != h || !(sigma > 0.0) || !(power >= 0.0)) return -1;
+    for (uint32_t y = 0; y < h; ++y)
+        for (uint32_t x = 0; x < w; ++x) {
+            const size_t p = (size_t)y * w + x;
+            const double fx = 0.5 * (double)x - 0.25, fy = 0.5 * (double)y - 0.25;
+            const double x0f = floor(fx), y0f = floor(fy);
+            const double tx = fx - x0f, ty = fy - y0f;
+            long xs[2] = {(long)x0f, (long)x0f + 1}, ys[2] = {(long)y0f, (long)y0f + 1};
+            for (int k = 0; k < 2; ++k) {
+                if (xs[k] < 0) xs[k] = 0;
+                if (ys[k] < 0) ys[k] = 0;
+                if (xs[k] > (long)ew - 1) xs[k] = (long)ew - 1;
+                if (ys[k] > (long)eh - 1) ys[k] = (long)eh - 1;
+            }
+            double acc[3] = {0.0, 0.0, 0.0}, wsum = 0.0;
+            for (int j = 0; j < 4; ++j) {                                              /* J1 */
+                const size_t q = (size_t)ys[j >> 1] * ew + (size_t)xs[j & 1];
+                const double b = ((j & 1) ? tx : 1.0 - tx) * ((j >> 1) ? ty : 1.0 - ty);
+                double d2 = 0.0, dot = 0.0;
+                for (int d = 0; d < 3; ++d) {
+                    const double dv = (double)pos[3 * p + d] - (double)pos_half[3 * q + d];
+                    d2 += dv * dv;
+                    dot += (double)nrm[3 * p + d] * (double)nrm_half[3 * q + d];
+                }
+                const double g = exp(-d2 / (2.0 * sigma * sigma)) * pow(dot > 0.0 ? dot : 0.0, power);   /* J2 */
+                const double wq = b * (g + 1e-6);                                                       /* J3 */
+                wsum += wq;
+                for (int c = 0; c < 3; ++c) acc[c] += wq * (double)E[3 * q + c];
+            }
+            for (int c = 0; c < 3; ++c) {                                              /* J4, J5 */
+                double v = (double)albedo[3 * p + c] / PI * (acc[c] / wsum);
+                if (direct) v += (double)direct[3 * p + c];
+                if (emission) v += (double)emission[3 * p + c];
+                out[3 * p + c] = v;
+            }
+        }
+    return 0;
+}
