@@ -874,6 +874,36 @@ def run_compose(args):
                               "ms": ms, "algorithmic_bytes": nbytes,
                               "roofline": {"bound": "hbm", "achieved": nbytes / ms / 1e6, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                                            "frac": nbytes / ms / 1e6 / peaks["hbm_gbs"], "peak_source": peaks["source"]}}), flush=True)
+        # joint-bilateral upsample (niv_compose_jb): + the full-resolution position and normal (24 B per pixel) and the
+        # half-resolution guides (6 B per pixel)
+        eh, ew = h // 2, w // 2
+        gf, gh = I.make_gbuffer(w, h, 0), I.make_gbuffer(ew, eh, 0)
+        c = lambda a, sh: torch.from_numpy(np.ascontiguousarray(a.reshape(sh))).cuda()
+        sets = [[c(gf["pos"], (h, w, 3)), c(gf["nrm"], (h, w, 3)), torch.rand((h, w, 3), device="cuda"),
+                 torch.rand((h, w, 3), device="cuda"), torch.rand((h, w, 3), device="cuda"), torch.empty((h, w, 3), device="cuda")]
+                for _ in range(ring)]
+        e_h, p_h, n_h = torch.rand((eh, ew, 3), device="cuda"), c(gh["pos"], (eh, ew, 3)), c(gh["nrm"], (eh, ew, 3))
+
+        def jb(k):
+            p, n_, a, d, le, o = sets[k % ring]
+            niv.compose_jb(e_h, p_h, n_h, p, n_, a, o, 0.15, 8.0, d, le)
+        for k in range(5):
+            jb(k)
+        steps = args.steps or 100
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for k in range(steps):
+            jb(k)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / steps
+        nbytes = (72 + 9) * h * w
+        print(json.dumps({"op": "niv_compose_jb", "E_resolution": "%dx%d" % (ew, eh), "frame": "%dx%d" % (w, h), "ms": ms,
+                          "algorithmic_bytes": nbytes,
+                          "roofline": {"bound": "hbm", "achieved": nbytes / ms / 1e6, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                                       "frac": nbytes / ms / 1e6 / peaks["hbm_gbs"], "peak_source": peaks["source"]}}), flush=True)
+        del sets
 
 
 def run_dry(args):

@@ -263,6 +263,19 @@ int niv_debug_encode(niv_model *m, const float *pos, const float *nrm, const flo
 int niv_compose(const float *E, uint32_t ew, uint32_t eh, const float *albedo, const float *direct,
                 const float *emission, float *out, uint32_t w, uint32_t h, void *stream);
 
+/* The same compose with JOINT-BILATERAL upsampling of half-resolution irradiance: the "industry practice upsampling
+ * methods" PAPER.md:406 names against the aliasing of half-resolution rendering ("a flagged extension").
+ * The paper gives no formula; the reading (steps J1-J5): the four half-res texels q of niv_compose's
+ * bilinear footprint, weight  b_q * (exp(-|x_p - x_q|^2 / (2 sigma^2)) * max(0, n_p . n_q)^power + 1e-6),  renormalised;
+ * the full-resolution G-buffer is the guide.
+ *   E, pos_half, nrm_half  device, [eh][ew][3] fp32: niv_infer's output on the half-size G-buffer, and that G-buffer
+ *   pos, nrm, albedo       device, [h][w][3] fp32 (the full-size G-buffer); direct, emission as niv_compose
+ *   sigma > 0 (world units), power >= 0;  (w, h) == (2 ew, 2 eh) exactly, else NIV_ERR_INVALID_ARG
+ * Asynchronous on `stream`, allocation-free; needs no model. */
+int niv_compose_jb(const float *E, const float *pos_half, const float *nrm_half, uint32_t ew, uint32_t eh,
+                   const float *pos, const float *nrm, const float *albedo, const float *direct, const float *emission,
+                   float sigma, float power, float *out, uint32_t w, uint32_t h, void *stream);
+
 int niv_destroy(niv_model *m);
 
 const char *niv_error_string(int code);

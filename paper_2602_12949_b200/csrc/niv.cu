@@ -1416,6 +1416,26 @@ extern "C" int niv_compose(const float* E, uint32_t ew, uint32_t eh, const float
     return NIV_OK;
 }
 
+extern "C" int niv_compose_jb(const float* E, const float* pos_half, const float* nrm_half, uint32_t ew, uint32_t eh,
+                              const float* pos, const float* nrm, const float* albedo, const float* direct,
+                              const float* emission, float sigma, float power, float* out, uint32_t w, uint32_t h,
+                              void* stream)
+{
+    if (!E || !pos_half || !nrm_half || !pos || !nrm || !albedo || !out) return NIV_ERR_INVALID_ARG;
+    if (!(sigma > 0.0f) || !std::isfinite(sigma) || !(power >= 0.0f) || !std::isfinite(power)) return NIV_ERR_INVALID_ARG;
+    if (w == 0 || h == 0) return NIV_OK;
+    if (2ull * ew != w || 2ull * eh != h) return NIV_ERR_INVALID_ARG;
+    int dev = 0, sms = 0;
+    NIV_CUDA(cudaGetDevice(&dev));
+    NIV_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const size_t n = (size_t)w * h;
+    const unsigned grid = (unsigned)std::min<size_t>((n + 255) / 256, (size_t)sms * 8);
+    niv_compose_jb_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(E, pos_half, nrm_half, ew, eh, pos, nrm, albedo, direct,
+                                                                  emission, 1.0f / (2.0f * sigma * sigma), power, out, w, h);
+    NIV_CUDA(cudaGetLastError());
+    return NIV_OK;
+}
+
 // =====================================================================================================
 // the probe-grid baseline
 // =====================================================================================================

@@ -128,4 +128,60 @@ __global__ void __launch_bounds__(256) niv_compose_scalar_kernel(const float* __
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------------
+// niv_compose_jb: the compose with JOINT-BILATERAL upsampling of half-resolution E ("industry practice
+// upsampling methods"; steps J1..J5 of DESIGN.md 3.7): the four half-res texels of the bilinear footprint, each weighted
+// by its bilinear weight x (exp(-|x_p - x_q|^2 / 2 sigma^2) max(0, n_p . n_q)^k + 1e-6), renormalised.
+// One thread per full-resolution pixel (grid-stride): 72 B of full-resolution streams per pixel (position, normal, albedo,
+// direct, emission in, radiance out) + the half-resolution E, position and normal (9 x 4 B per texel, each texel used by
+// ~9 pixels: L1 / L2).  inv2s2 = 1 / (2 sigma^2).
+__global__ void __launch_bounds__(256) niv_compose_jb_kernel(const float* __restrict__ E, const float* __restrict__ pos_h,
+                                                             const float* __restrict__ nrm_h, uint32_t ew, uint32_t eh,
+                                                             const float* __restrict__ pos, const float* __restrict__ nrm,
+                                                             const float* __restrict__ albedo,
+                                                             const float* __restrict__ direct,
+                                                             const float* __restrict__ emission, float inv2s2, float power,
+                                                             float* __restrict__ out, uint32_t w, uint32_t h)
+{
+    const size_t n = (size_t)w * h;
+    const float inv_pi = 0.318309886183790671538f;
+    for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < n; p += (size_t)gridDim.x * blockDim.x) {
+        const uint32_t y = (uint32_t)(p / w), x = (uint32_t)(p - (size_t)y * w);
+        const int k = (int)(x >> 1), j = (int)(y >> 1);
+        int xs[2], ys[2];
+        float tx, ty;                                                       // J1: the bilinear footprint of pixel (x, y)
+        if (x & 1u) { xs[0] = k; xs[1] = min(k + 1, (int)ew - 1); tx = 0.25f; } else { xs[0] = max(k - 1, 0); xs[1] = k; tx = 0.75f; }
+        if (y & 1u) { ys[0] = j; ys[1] = min(j + 1, (int)eh - 1); ty = 0.25f; } else { ys[0] = max(j - 1, 0); ys[1] = j; ty = 0.75f; }
+        float xp[3], np_[3];
+#pragma unroll
+        for (int d = 0; d < 3; ++d) { xp[d] = __ldcs(pos + 3 * p + d); np_[d] = __ldcs(nrm + 3 * p + d); }
+        float acc[3] = {0.f, 0.f, 0.f}, wsum = 0.f;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const size_t t = ((size_t)ys[q >> 1] * ew + (size_t)xs[q & 1]) * 3;
+            const float b = ((q & 1) ? tx : 1.0f - tx) * ((q >> 1) ? ty : 1.0f - ty);
+            float d2 = 0.f, dot = 0.f;
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                const float dv = xp[d] - __ldg(pos_h + t + d);
+                d2 = fmaf(dv, dv, d2);
+                dot = fmaf(np_[d], __ldg(nrm_h + t + d), dot);
+            }
+            const float g = expf(-d2 * inv2s2) * powf(fmaxf(dot, 0.0f), power);          // J2 (powf(0, 0) = 1, as pow)
+            const float wq = b * (g + 1e-6f);                                            // J3
+            wsum += wq;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) acc[c] = fmaf(wq, __ldg(E + t + c), acc[c]);
+        }
+        const float inv = 1.0f / wsum;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {                                                    // J4, J5
+            float v = __ldcs(albedo + 3 * p + c) * inv_pi * (acc[c] * inv);
+            if (direct) v += __ldcs(direct + 3 * p + c);
+            if (emission) v += __ldcs(emission + 3 * p + c);
+            __stcs(out + 3 * p + c, v);
+        }
+    }
+}
+
 }  // namespace niv

@@ -37,7 +37,7 @@ EXPORTS = ("niv_create", "niv_get_info", "niv_load_params", "niv_infer", "niv_in
            "niv_infer_host_static",
            "niv_infer_packed", "niv_infer_image_packed", "niv_infer_host_packed", "niv_decode_gbuffer", "niv_debug_arow",
            "niv_encode",
-           "niv_debug_encode", "niv_compose", "niv_destroy", "niv_error_string", "niv_last_cuda_error", "niv_probe_gather",
+           "niv_debug_encode", "niv_compose", "niv_compose_jb", "niv_destroy", "niv_error_string", "niv_last_cuda_error", "niv_probe_gather",
            "niv_probe_sectors",
            "niv_probes_create", "niv_probes_load", "niv_probes_query", "niv_probes_census", "niv_probes_destroy")
 
@@ -109,6 +109,8 @@ def lib():
         L.niv_debug_arow.argtypes = [vp, vp, vp, C.POINTER(C.c_float), vp, vp, C.c_uint32, sz, vp]
         L.niv_debug_encode.argtypes = [vp, vp, vp, C.POINTER(C.c_float), sz, vp, vp, vp, vp, vp]
         L.niv_compose.argtypes = [vp, C.c_uint32, C.c_uint32, vp, vp, vp, vp, C.c_uint32, C.c_uint32, vp]
+        L.niv_compose_jb.argtypes = [vp, vp, vp, C.c_uint32, C.c_uint32, vp, vp, vp, vp, vp, C.c_float, C.c_float, vp,
+                                     C.c_uint32, C.c_uint32, vp]
         L.niv_destroy.argtypes = [vp]
         L.niv_error_string.argtypes = [C.c_int]
         L.niv_error_string.restype = C.c_char_p
@@ -447,6 +449,29 @@ def probe_gather(buf, pattern: int, n_ctas: int, loads_per_lane: int, seed: int,
                                 loads_per_lane, seed, sink.data_ptr(), _stream_ptr(stream))
     if rc != NIV_OK:
         raise NivError(rc, "niv_probe_gather")
+
+
+def compose_jb(E, pos_half, nrm_half, pos, nrm, albedo, out, sigma, power, direct=None, emission=None, stream=None):
+    """niv_compose_jb (include/niv.h): the compose with joint-bilateral upsampling of half-resolution E; CUDA fp32 tensors,
+    E / pos_half / nrm_half [eh][ew][3], the rest [2 eh][2 ew][3].  Asynchronous."""
+    import torch
+    h, w = albedo.shape[:2]
+    eh, ew = E.shape[:2]
+    for name, t, shape in (("E", E, (eh, ew, 3)), ("pos_half", pos_half, (eh, ew, 3)), ("nrm_half", nrm_half, (eh, ew, 3)),
+                           ("pos", pos, (h, w, 3)), ("nrm", nrm, (h, w, 3)), ("albedo", albedo, (h, w, 3)),
+                           ("out", out, (h, w, 3)), ("direct", direct, (h, w, 3)), ("emission", emission, (h, w, 3))):
+        if t is None:
+            continue
+        if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous() \
+                or tuple(t.shape) != shape:
+            raise TypeError("%s must be a contiguous CUDA float32 tensor of shape %s" % (name, (shape,)))
+    rc = lib().niv_compose_jb(E.data_ptr(), pos_half.data_ptr(), nrm_half.data_ptr(), ew, eh, pos.data_ptr(), nrm.data_ptr(),
+                              albedo.data_ptr(), None if direct is None else direct.data_ptr(),
+                              None if emission is None else emission.data_ptr(), float(sigma), float(power),
+                              out.data_ptr(), w, h, _stream_ptr(stream))
+    if rc != NIV_OK:
+        raise NivError(rc, "niv_compose_jb")
+    return out
 
 
 def compose(E, albedo, out, direct=None, emission=None, stream=None):

@@ -805,6 +805,44 @@ def test_compose_matches_oracle(torch_cuda, niv, oracle, w, h, half):
     assert np.abs(g[:h].astype(np.float64) - oracle.compose(E, alb)).max() <= 4 * 2.0 ** -23 * 4.0
 
 
+@pytest.mark.parametrize("w,h,sigma,power", [(64, 36, 0.25, 8.0), (30, 14, 0.1, 2.0), (2, 2, 1.0, 0.0), (1920, 1080, 0.15, 16.0),
+                                             (202, 66, 0.05, 32.0)])
+def test_compose_joint_bilateral_matches_oracle(torch_cuda, niv, oracle, w, h, sigma, power):
+    """niv_compose_jb against the fp64 oracle on the seeded scene's G-buffers at full and half resolution (object
+    silhouettes, background texels with zero normals, image borders).  fp32 exp / pow and one normalisation: 5e-5 abs on
+    radiance of order one."""
+    torch = torch_cuda
+    ew, eh = w // 2, h // 2
+    rng = np.random.default_rng(w * 7 + h)
+    if w >= 16:
+        gf, gh = I.make_gbuffer(w, h, 2), I.make_gbuffer(ew, eh, 2)
+    else:                                              # (too small for the scene generator's background quota)
+        gf = {"pos": I.positions_uniform(w * h, I.ROOM_AABB, 1), "nrm": I.normals_uniform(w * h, 1)}
+        gh = {"pos": I.positions_uniform(ew * eh, I.ROOM_AABB, 2), "nrm": I.normals_uniform(ew * eh, 2)}
+    E = rng.uniform(0, 3, (eh, ew, 3)).astype(np.float32)
+    alb = rng.uniform(0, 1, (h, w, 3)).astype(np.float32)
+    D = rng.uniform(0, 2, (h, w, 3)).astype(np.float32)
+    Le = rng.uniform(0, 1, (h, w, 3)).astype(np.float32)
+    pos_f, nrm_f = gf["pos"].reshape(h, w, 3), gf["nrm"].reshape(h, w, 3)
+    pos_h, nrm_h = gh["pos"].reshape(eh, ew, 3), gh["nrm"].reshape(eh, ew, 3)
+    want = oracle.compose_jb(E, pos_h, nrm_h, pos_f, nrm_f, alb, sigma, power, D, Le)
+    c = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    guard = torch.full((h + 1, w, 3), 7.0, dtype=torch.float32, device="cuda")        # writes must stop at h rows
+    niv.compose_jb(c(E), c(pos_h), c(nrm_h), c(pos_f), c(nrm_f), c(alb), guard[:h], sigma, power, c(D), c(Le))
+    torch.cuda.synchronize()
+    g = guard.cpu().numpy()
+    assert np.all(g[h] == 7.0) and np.all(np.isfinite(g))
+    assert np.abs(g[:h].astype(np.float64) - want).max() <= 5e-5
+    if w >= 64:                                                                        # it is not the bilinear blend
+        assert np.abs(want - oracle.compose(E, alb, D, Le)).max() > 1e-2
+    L = niv.lib()
+    z = guard.data_ptr()
+    assert L.niv_compose_jb(z, z, z, ew, eh, z, z, z, None, None, 0.0, 1.0, z, w, h, None) == niv.NIV_ERR_INVALID_ARG
+    assert L.niv_compose_jb(z, z, z, ew, eh, z, z, z, None, None, 0.1, -1.0, z, w, h, None) == niv.NIV_ERR_INVALID_ARG
+    assert L.niv_compose_jb(z, z, z, w, h, z, z, z, None, None, 0.1, 1.0, z, w, h, None) == niv.NIV_ERR_INVALID_ARG
+    assert L.niv_compose_jb(z, None, z, ew, eh, z, z, z, None, None, 0.1, 1.0, z, w, h, None) == niv.NIV_ERR_INVALID_ARG
+
+
 def test_compose_rejects_other_ratios(torch_cuda, niv):
     torch = torch_cuda
     a = torch.zeros((8, 8, 3), dtype=torch.float32, device="cuda")
