@@ -82,7 +82,7 @@ enum { NIV_OUT_LINEAR = 0,      /* the paper: no activation on the final layer (
 typedef struct {
     uint32_t struct_size;         /* = sizeof(niv_config)                                           */
     uint32_t api_version;         /* = NIV_API_VERSION                                              */
-    uint32_t n_levels;            /* L: 4, 8, 12 or 16 (F = 2);  2, 4, 6 or 8 (F = 4);  0 = no grid: the
+    uint32_t n_levels;            /* L: 1..16 (F = 2);  1..8 (F = 4);  0 = no grid: the
                                      position is encoded with n_frequencies sin/cos bands */
     uint32_t n_features;          /* F: fp16 latents per table entry: 2 (BASELINE.json) or 4 (paper) */
     uint32_t log2_table_size;     /* T = 2^k entries PER LEVEL, 4 <= k <= 24                        */
@@ -117,15 +117,17 @@ typedef struct {
     uint32_t texel_params;                 /* 1: niv_infer_texel_params is available for this model */
     uint32_t cell_levels;                  /* levels 0 .. cell_levels-1 are also held as cell blocks (8 corner
                                               entries per cell, one 32- / 64-byte load per texel and level) */
-    uint32_t reserved0;
+    uint32_t kernel_levels;                /* levels the fused kernels run: n_levels rounded up to a whole gather batch
+                                              (the extra ones are dummy levels over zeros); niv_debug_arow rows have
+                                              kernel_levels * F / 2 latent words */
     uint64_t cell_bytes;                   /* device bytes of those copies (budget: NIV_CELL_MB at niv_create) */
 } niv_info;
 
 /* Validate `cfg` completely and allocate device storage for the parameters (uninitialised).
  * Errors: NULL / wrong struct_size / api_version / degenerate AABB / zero resolution -> NIV_ERR_INVALID_ARG;
  * a shape this build has no kernel for -> NIV_ERR_UNSUPPORTED.  Two model families have kernels: BASELINE.json's
- * (F = 2, sh_degree 4, L in {4,8,12,16}, width 32/64/128) and the paper's own (F = 4, sh_degree 0,
- * L in {2,4,6,8}, width 32/64) plus its grid-less models (L = 0, sh_degree 0, width 16/32/64, no table: table_fp16
+ * (F = 2, sh_degree 4, L = 1..16, width 32/64/128) and the paper's own (F = 4, sh_degree 0,
+ * L = 1..8, width 32/64; "the number of levels varies between 2 and 8") plus its grid-less models (L = 0, sh_degree 0, width 16/32/64, no table: table_fp16
  * may be NULL with table_bytes 0); all with n_hidden_layers 1..3, n_params 0..2, n_frequencies 8.
  * Shape errors are raised here, never at inference. */
 int niv_create(const niv_config *cfg, niv_model **out);

@@ -332,6 +332,8 @@ struct niv_model {
     niv_info info;
     KParams kp;
     uint32_t* d_table = nullptr;
+    uint32_t kernel_levels = 0;                    // levels the fused kernels run (n_levels rounded up to whole batches)
+    uint32_t k_shift = 0;                          // (kernel_levels - n_levels) * F: where the direction columns of W1 move to
     uint32_t* d_cells = nullptr;                   // cell-block copies of the coarse levels (KParams::lv[].cells)
     uint64_t cell_off[kMaxLevels] = {};            //   byte offset of a level's blocks in d_cells
     uint8_t* d_wpack = nullptr;
@@ -528,10 +530,15 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
         if (cfg->sh_degree != 0 || cfg->n_frequencies != 8) return NIV_ERR_UNSUPPORTED;
         if (cfg->hidden_width != 16 && cfg->hidden_width != 32 && cfg->hidden_width != 64) return NIV_ERR_UNSUPPORTED;
     } else if (cfg->n_features == 2) {
-        if (cfg->sh_degree != 4 || cfg->n_levels % 4 != 0) return NIV_ERR_UNSUPPORTED;
+        if (cfg->sh_degree != 4) return NIV_ERR_UNSUPPORTED;
     } else if (cfg->n_features == 4) {
-        if (cfg->sh_degree != 0 || cfg->n_levels % 2 != 0 || cfg->n_levels > 8 || cfg->hidden_width > 64) return NIV_ERR_UNSUPPORTED;
+        if (cfg->sh_degree != 0 || cfg->n_levels > 8 || cfg->hidden_width > 64) return NIV_ERR_UNSUPPORTED;
     } else return NIV_ERR_UNSUPPORTED;
+    // Any number of levels: the kernels are compiled for whole gather batches (multiples of 4 levels for F = 2, of 2 for
+    // F = 4); a model with fewer levels runs the next larger kernel with DUMMY levels that read a block of zeros and meet
+    // zero weight columns (their latent columns of W1 are zero in the packed blob), so they add exactly 0 to every sum.
+    const uint32_t lev_step = cfg->n_features == 4 ? 2u : 4u;
+    const uint32_t Lk = cfg->n_levels ? round_up(cfg->n_levels, lev_step) : 0u;
     if (cfg->n_params > 2 || (cfg->n_params && cfg->n_frequencies != 8)) return NIV_ERR_UNSUPPORTED;
     if (cfg->n_hidden_layers > 3) return NIV_ERR_UNSUPPORTED;
     if (cfg->hidden_width != 32 && cfg->hidden_width != 64 && cfg->hidden_width != 128 &&
@@ -577,6 +584,19 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
         volatile float inv = 1.0f / ext;
         P.ainv[d] = inv;
     }
+    for (uint32_t l = cfg->n_levels; l < Lk; ++l) {      // dummy levels: one cell, dense, over a block of zeros
+        P.lv[l].Nf = 1.0f;
+        P.lv[l].Nm1 = 0;
+        P.lv[l].cmaxf = 8388608.0f;
+        P.lv[l].R = 2;
+        P.lv[l].R2 = 4;
+        P.lv[l].dense = 1u;
+        P.lv[l].cs = 1;
+        P.lv[l].cs2 = 1;
+    }
+    m->kernel_levels = Lk;
+    m->k_shift = (Lk - cfg->n_levels) * cfg->n_features;
+    I.kernel_levels = Lk;
     P.L = cfg->n_levels;
     P.tmask = (uint32_t)(T - 1);
     P.n_features = cfg->n_features;
@@ -595,7 +615,7 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     if (cfg->n_levels && cfg->hidden_width <= 64 && !want_mma_sync) {
         const char* s_mb = getenv("NIV_CELL_MB");
         const uint64_t budget = (uint64_t)(s_mb ? std::max(0, atoi(s_mb)) : kCellBudgetMB) << 20;
-        const uint32_t want = (uint32_t)cell_levels_of((int)cfg->n_levels, (int)cfg->n_features);
+        const uint32_t want = std::min((uint32_t)cell_levels_of((int)Lk, (int)cfg->n_features), cfg->n_levels);   // the real ones
         uint64_t off = 0;
         use_cells = true;
         for (uint32_t l = 0; l < want; ++l) {
@@ -628,7 +648,7 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
             in = o;
         }
     }
-    layout_blob(m, P, round_up(P.enc_dim, 16), true);        // layer 1 consumes the encoded part only (parameters fold)
+    layout_blob(m, P, round_up(P.enc_dim + m->k_shift, 16), true);   // layer 1 consumes the encoded part only (parameters fold)
 
     // device side
     g_last_cuda_error = 0;
@@ -647,7 +667,7 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
         m->mma_kernel = true;
         rc = setup_kernel(m, m->fused, 0, "fused_mma_sync");
     } else if (W == 128) {                                // two N = 64 halves per hidden layer (niv_fused_w128.cuh)
-        switch (cfg->n_levels) {
+        switch (Lk) {
             case 4:  m->fused.fn = niv_fused_w128_kernel<4, 4>; break;
             case 8:  m->fused.fn = niv_fused_w128_kernel<8, 4>; break;
             case 12: m->fused.fn = niv_fused_w128_kernel<12, 4>; break;
@@ -659,39 +679,39 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
         rc = m->fused.fn ? setup_kernel(m, m->fused, 128, "fused_w128") : NIV_ERR_UNSUPPORTED;
     } else {
         const int tmem_cols = W == 16 ? 64 : 128;        // D | A | ones in one allocation (niv_fused.cuh TMEM_COLS)
-        m->fused.fn = use_cells ? pick_fused<false, true>(W, cfg->n_levels, cfg->n_features)
-                                : pick_fused<false, false>(W, cfg->n_levels, cfg->n_features);
+        m->fused.fn = use_cells ? pick_fused<false, true>(W, Lk, cfg->n_features)
+                                : pick_fused<false, false>(W, Lk, cfg->n_features);
         m->fused.smem = smem_dev;
         rc = m->fused.fn ? setup_kernel(m, m->fused, tmem_cols, "fused") : NIV_ERR_UNSUPPORTED;
         if (rc == NIV_OK) {
-            m->fused_host.fn = pick_fused<true, false>(W, cfg->n_levels, cfg->n_features);   // PCIe-bound: table gathers
+            m->fused_host.fn = pick_fused<true, false>(W, Lk, cfg->n_features);   // PCIe-bound: table gathers
             m->fused_host.smem = smem_host;
             rc = setup_kernel(m, m->fused_host, tmem_cols, "fused_host");
         }
         if (rc == NIV_OK) {
-            m->fused_pk.fn = use_cells ? pick_fused<false, true, true>(W, cfg->n_levels, cfg->n_features)
-                                       : pick_fused<false, false, true>(W, cfg->n_levels, cfg->n_features);
+            m->fused_pk.fn = use_cells ? pick_fused<false, true, true>(W, Lk, cfg->n_features)
+                                       : pick_fused<false, false, true>(W, Lk, cfg->n_features);
             m->fused_pk.smem = smem_dev;
             rc = setup_kernel(m, m->fused_pk, tmem_cols, "fused_packed");
         }
         if (rc == NIV_OK) {
-            m->fused_host_pk.fn = pick_fused<true, false, true>(W, cfg->n_levels, cfg->n_features);
+            m->fused_host_pk.fn = pick_fused<true, false, true>(W, Lk, cfg->n_features);
             m->fused_host_pk.smem = smem_host;
             rc = setup_kernel(m, m->fused_host_pk, tmem_cols, "fused_host_packed");
         }
         if (rc == NIV_OK) {
-            m->fused_img.fn = use_cells ? pick_fused_img<true>(W, cfg->n_levels, cfg->n_features)
-                                        : pick_fused_img<false>(W, cfg->n_levels, cfg->n_features);
+            m->fused_img.fn = use_cells ? pick_fused_img<true>(W, Lk, cfg->n_features)
+                                        : pick_fused_img<false>(W, Lk, cfg->n_features);
             m->fused_img.smem = smem_dev;
             rc = setup_kernel(m, m->fused_img, tmem_cols, "fused_image");
         }
         if (rc == NIV_OK && cfg->n_params) {
-            m->fused_tp.fn = use_cells ? pick_fused_tp<true>(W, cfg->n_levels, cfg->n_features, cfg->sh_degree, cfg->n_params)
-                                       : pick_fused_tp<false>(W, cfg->n_levels, cfg->n_features, cfg->sh_degree, cfg->n_params);
+            m->fused_tp.fn = use_cells ? pick_fused_tp<true>(W, Lk, cfg->n_features, cfg->sh_degree, cfg->n_params)
+                                       : pick_fused_tp<false>(W, Lk, cfg->n_features, cfg->sh_degree, cfg->n_params);
             if (m->fused_tp.fn) {
                 // layout of the per-texel-parameter variant: layer 1 with K = round16(enc_dim) + 16 n_params, no fold blob
                 m->kp_tp = P;
-                layout_blob(m, m->kp_tp, round_up(P.enc_dim, 16) + 16 * cfg->n_params, false);
+                layout_blob(m, m->kp_tp, round_up(P.enc_dim + m->k_shift, 16) + 16 * cfg->n_params, false);
                 m->fused_tp.smem = m->kp_tp.misc_off + 64;
                 rc = setup_kernel(m, m->fused_tp, tmem_cols, "fused_texel_params");
             }
@@ -702,7 +722,8 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     I.smem_bytes = m->fused.smem;
     I.image_tiled = m->fused_img.fn ? 1u : 0u;
     I.texel_params = m->fused_tp.fn ? 1u : 0u;
-    e = cudaMalloc(&m->d_table, I.table_bytes ? I.table_bytes : 16);
+    e = cudaMalloc(&m->d_table, I.table_bytes + 64);          // + a block of zeros for the dummy levels
+    if (e == cudaSuccess) e = cudaMemset(reinterpret_cast<uint8_t*>(m->d_table) + I.table_bytes, 0, 64);
     if (e == cudaSuccess && I.cell_bytes) e = cudaMalloc(&m->d_cells, I.cell_bytes);
     if (e == cudaSuccess) e = cudaMalloc(&m->d_wpack, P.wpack_bytes);
     if (e == cudaSuccess && m->fused_tp.fn) e = cudaMalloc(&m->d_wpack_tp, m->kp_tp.wpack_bytes);
@@ -725,6 +746,11 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     for (uint32_t l = 0; l < cfg->n_levels; ++l) {
         P.lv[l].tb = m->d_table + (size_t)P.lv[l].base * (cfg->n_features / 2);
         if (l < I.cell_levels) P.lv[l].cells = reinterpret_cast<const uint4*>(reinterpret_cast<const uint8_t*>(m->d_cells) + m->cell_off[l]);
+        m->kp_tp.lv[l] = P.lv[l];
+    }
+    for (uint32_t l = cfg->n_levels; l < Lk; ++l) {
+        P.lv[l].tb = reinterpret_cast<const uint32_t*>(reinterpret_cast<const uint8_t*>(m->d_table) + I.table_bytes);
+        P.lv[l].cells = reinterpret_cast<const uint4*>(P.lv[l].tb);
         m->kp_tp.lv[l] = P.lv[l];
     }
     *out = m;
@@ -777,11 +803,15 @@ extern "C" int niv_load_params(niv_model* m, const void* table_fp16, size_t tabl
         const uint32_t o = m->layer_out[k], in = m->layer_in[k];
         const uint32_t kuse = (k == 0) ? P.enc_dim : in;
         uint16_t* dst = reinterpret_cast<uint16_t*>(pack.data() + P.w_off[k]);
+        // (layer 1 of a model with dummy levels: the direction columns sit behind the dummy levels' zero columns)
+        const uint32_t n_lat = m->cfg.n_levels * m->cfg.n_features, shift = (k == 0) ? m->k_shift : 0u;
         for (uint32_t r = 0; r < o; ++r)
-            for (uint32_t c = 0; c < kuse; ++c)
-                dst[(size_t)(c >> 3) * (P.npad[k] * 8) + r * 8 + (c & 7)] = w[wsrc + (size_t)r * in + c];
+            for (uint32_t c = 0; c < kuse; ++c) {
+                const uint32_t ck = (shift && c >= n_lat) ? c + shift : c;
+                dst[(size_t)(ck >> 3) * (P.npad[k] * 8) + r * 8 + (ck & 7)] = w[wsrc + (size_t)r * in + c];
+            }
         if (k == 0 && texel_params) {
-            const uint32_t k0 = round_up(P.enc_dim, 16);
+            const uint32_t k0 = round_up(P.enc_dim + m->k_shift, 16);
             for (uint32_t r = 0; r < o; ++r)
                 for (uint32_t c = 0; c < 16 * P.n_params; ++c)
                     dst[(size_t)((k0 + c) >> 3) * (P.npad[k] * 8) + r * 8 + ((k0 + c) & 7)] = w[wsrc + (size_t)r * in + P.enc_dim + c];
@@ -1080,7 +1110,7 @@ extern "C" int niv_debug_arow(niv_model* m, const float* pos, const float* nrm, 
     int rc = check_call(m, pos, nrm, out, n);
     if (rc != NIV_OK) return rc > 0 ? NIV_OK : rc;
     if (!arow || !m->fused_pk.fn) return arow ? NIV_ERR_UNSUPPORTED : NIV_ERR_INVALID_ARG;
-    const uint32_t hw = m->cfg.n_levels ? m->cfg.n_levels * m->cfg.n_features / 2 : 24u;
+    const uint32_t hw = m->cfg.n_levels ? m->kernel_levels * m->cfg.n_features / 2 : 24u;
     const uint32_t need = (hw + (m->cfg.sh_degree ? 8u : 2u) + 7u) / 8u * 8u;
     if (row_words != need) return NIV_ERR_INVALID_ARG;
     KParams P;
@@ -1328,7 +1358,8 @@ extern "C" int niv_encode(niv_model* m, const float* pos, const float* nrm, cons
     if (!m->loaded) return NIV_ERR_NOT_LOADED;
     if (n == 0) return NIV_OK;
     if (!pos || !nrm || !features_fp16 || ((uintptr_t)features_fp16 & 15)) return NIV_ERR_INVALID_ARG;
-    if (m->cfg.n_features != 2) return NIV_ERR_UNSUPPORTED;      // the stand-alone kernel serves the F = 2 / SH-16 family
+    if (m->cfg.n_features != 2 || m->kernel_levels != m->cfg.n_levels || m->cfg.n_levels == 0)
+        return NIV_ERR_UNSUPPORTED;                              // the stand-alone kernel serves F = 2 / SH-16, L a multiple of 4
     KParams P;
     int rc = fill_params(m, param, P);
     if (rc != NIV_OK) return rc;

@@ -62,7 +62,7 @@ class NivInfo(C.Structure):
         ("table_bytes", C.c_uint64), ("weight_bytes", C.c_uint64), ("bias_bytes", C.c_uint64),
         ("num_sms", C.c_uint32), ("ctas_per_sm", C.c_uint32), ("tile_texels", C.c_uint32),
         ("smem_bytes", C.c_uint32), ("image_tiled", C.c_uint32), ("texel_params", C.c_uint32),
-        ("cell_levels", C.c_uint32), ("reserved0", C.c_uint32), ("cell_bytes", C.c_uint64),
+        ("cell_levels", C.c_uint32), ("kernel_levels", C.c_uint32), ("cell_bytes", C.c_uint64),
     ]
 
 
@@ -340,7 +340,7 @@ class NivModel:
 
     def arow_words(self) -> int:
         """32-bit words of one layer-1 A row of the fused kernel (include/niv.h niv_debug_arow)."""
-        hw = self.spec.n_levels * self.spec.n_features // 2 if self.spec.n_levels else 24
+        hw = self.info.kernel_levels * self.spec.n_features // 2 if self.spec.n_levels else 24
         return (hw + (8 if self.spec.sh_degree else 2) + 7) // 8 * 8
 
     def debug_arow(self, pos, nrm, out, arow, param=None, stream=None):

@@ -58,7 +58,8 @@ def test_argument_validation_happens_before_cuda(L):
         (lambda c: c.aabb_max.__setitem__(0, float("nan")), niv.NIV_ERR_INVALID_ARG),
         (lambda c: setattr(c, "per_level_scale", 0.5), niv.NIV_ERR_INVALID_ARG),
         (lambda c: setattr(c, "base_resolution", 0), niv.NIV_ERR_INVALID_ARG),
-        (lambda c: setattr(c, "n_levels", 6), niv.NIV_ERR_UNSUPPORTED),
+        (lambda c: setattr(c, "n_features", 3), niv.NIV_ERR_UNSUPPORTED),
+        (lambda c: setattr(c, "n_features", 4), niv.NIV_ERR_UNSUPPORTED),    # F = 4 goes with the raw direction (sh_degree 0)
         (lambda c: setattr(c, "hidden_width", 48), niv.NIV_ERR_UNSUPPORTED),
         (lambda c: setattr(c, "n_hidden_layers", 4), niv.NIV_ERR_UNSUPPORTED),
         (lambda c: setattr(c, "sh_degree", 3), niv.NIV_ERR_UNSUPPORTED),

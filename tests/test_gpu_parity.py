@@ -509,6 +509,51 @@ def test_fused_kernel_features_match_the_oracle(torch_cuda, niv, oracle, which):
     m.close()
 
 
+@pytest.mark.parametrize("F,L,width", [(2, 1, 64), (2, 2, 32), (2, 3, 64), (2, 5, 64), (2, 6, 32), (2, 7, 64), (2, 9, 64),
+                                       (2, 10, 128), (2, 13, 64), (2, 15, 32), (4, 1, 64), (4, 3, 64), (4, 5, 32), (4, 7, 64)])
+def test_any_number_of_levels(torch_cuda, niv, oracle, F, L, width):
+    """n_levels 1..16 ("the number of levels varies between 2 and 8").  The kernels run whole
+    gather batches; a model with another level count runs the next larger one with dummy levels over zeros.  Indices
+    bit-exact, irradiance within the bar on a loud table with biases, image tiling and the fused kernel's own feature rows
+    included."""
+    torch = torch_cuda
+    if F == 2:
+        spec = dataclasses.replace(I.spec_fullhd(17, width, 2), n_levels=L)
+    else:
+        spec = I.spec_paper(8, width)
+        spec = dataclasses.replace(spec, n_levels=L, resolutions=spec.resolutions[:L])
+    case = Case(spec, 40 + L, table_amp=1.0 if F == 2 else 0.1, bias_scale=0.1)
+    m = case.gpu_model(niv)
+    step = 4 if F == 2 else 2
+    assert m.info.kernel_levels == (L + step - 1) // step * step and m.info.in_dim == spec.in_dim
+    n = 6007
+    pos, nrm = _queries(spec, n, L)
+    pos[:2000], nrm[:2000] = _queries(spec, 2000, L + 1, coherent=True)
+    _check_debug(torch, oracle, m, case, pos, nrm)
+    got = _gpu_infer(torch, m, pos, nrm)
+    want = oracle.infer(spec, case.table, case.wblob, case.bblob, pos, nrm)
+    scale = 1.0 if spec.out_activation == I.OUT_SIGMOID else max(1.0, float(want.max() - want.min()))
+    _check_irradiance(got, want, nrm, pos, scale)
+    dp, dn = torch.from_numpy(pos).cuda(), torch.from_numpy(nrm).cuda()
+    img = torch.full((n, 3), float("nan"), device="cuda")
+    m.infer_image(dp, dn, img, 6007, 1)
+    if width <= 64:
+        arow = torch.zeros((n, m.arow_words()), dtype=torch.int32, device="cuda")
+        out2 = torch.full((n, 3), float("nan"), device="cuda")
+        m.debug_arow(dp, dn, out2, arow)
+        torch.cuda.synchronize()
+        assert np.array_equal(out2.cpu().numpy(), got)
+        rows = arow.cpu().numpy().view(np.uint16).reshape(n, -1).view(np.float16).astype(np.float64)
+        feats = oracle.encode(spec, case.table, pos, nrm)["features"]
+        act = ~np.all(nrm == 0, axis=1)
+        tmax = float(np.abs(case.table.astype(np.float64)).max())
+        assert np.abs(rows[act, :L * F] - feats[act, :L * F]).max() <= 15 * 2.0 ** -11 * tmax
+        assert np.all(rows[:, L * F:m.info.kernel_levels * F] == 0)                    # the dummy levels' latents
+    torch.cuda.synchronize()
+    assert np.array_equal(img.cpu().numpy(), got)
+    m.close()
+
+
 @pytest.mark.parametrize("n", [300, 70001])
 def test_back_to_back_launches_overlap_safely(torch_cuda, niv, monkeypatch, n):
     """a launch whose buffers are disjoint from those of the launch before it (same stream, this library)
