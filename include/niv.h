@@ -121,6 +121,10 @@ typedef struct {
                                               (the extra ones are dummy levels over zeros); niv_debug_arow rows have
                                               kernel_levels * F / 2 latent words */
     uint64_t cell_bytes;                   /* device bytes of those copies (budget: NIV_CELL_MB at niv_create) */
+    uint64_t table_bytes_compact;          /* bytes of the COMPACT table niv_load_params_compact takes: a dense level with
+                                              exactly (N_l + 1)^3 entries, a hashed one with T (the rule behind
+                                              Table 1's memory column)                                               */
+    uint64_t table_bytes_device;           /* what the model holds on the device: the compact table, levels padded to 32 B */
 } niv_info;
 
 /* Validate `cfg` completely and allocate device storage for the parameters (uninitialised).
@@ -145,6 +149,15 @@ int niv_load_params(niv_model *m, const void *table_fp16, size_t table_bytes,
                     const void *weights_fp16, size_t weight_bytes,
                     const float *biases_f32, size_t bias_bytes,
                     int src_on_device, void *stream);
+
+/* The same with the table in compact form: the levels back to back, a dense level with exactly
+ * (N_l + 1)^3 entries (x fastest), a hashed level with its T entries; table_bytes must equal
+ * niv_info.table_bytes_compact.  Either way the model STORES the compact form (niv_info.table_bytes_device): the paper's
+ * largest model is 5.4 MB, not 8 x T entries. */
+int niv_load_params_compact(niv_model *m, const void *table_fp16, size_t table_bytes,
+                            const void *weights_fp16, size_t weight_bytes,
+                            const float *biases_f32, size_t bias_bytes,
+                            int src_on_device, void *stream);
 
 /* The hot path: one fused kernel, out[i] = E_theta(pos[i], nrm[i][, param]) for i < n.
  *   pos, nrm  device, [n][3] fp32 packed, base address 4-byte aligned; world-space position, unit normal

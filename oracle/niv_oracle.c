@@ -441,3 +441,37 @@ int niv_oracle_compose(const float *E, uint32_t ew, uint32_t eh, const float *al
             }
     return 0;
 }
+
+/* ---- f1: compact table storage.  PAPER.md:303 "latents of the finer levels are stored in a hash table": the coarse
+ * (dense) levels need (N_l + 1)^3 entries only, which is the rule that reproduces Table 1's memory column (
+ * reading #4).  The compact table is the levels back to back, a dense level with exactly (N_l + 1)^3 entries (x fastest,
+ * as in the [L][T] layout), a hashed level with its T entries.  niv_oracle_table_compact copies [L][T] -> compact,
+ * niv_oracle_table_expand the other way (unused entries zero); both return the compact size in ENTRIES, and may be
+ * called with NULL buffers to get it. ---- */
+static long long compact_walk(const niv_oracle_config *cfg, const uint16_t *src, uint16_t *dst, int to_compact)
+{
+    uint32_t N[NIV_ORACLE_MAX_LEVELS], dense[NIV_ORACLE_MAX_LEVELS];
+    if (niv_oracle_level_table(cfg, N, dense)) return -1;
+    const uint64_t T = (uint64_t)1 << cfg->log2_table_size, F = cfg->n_features;
+    uint64_t off = 0;
+    for (uint32_t l = 0; l < cfg->n_levels; ++l) {
+        const uint64_t R = (uint64_t)N[l] + 1, cnt = dense[l] ? R * R * R : T;
+        if (src && dst) {
+            if (to_compact) memcpy(dst + off * F, src + (uint64_t)l * T * F, cnt * F * sizeof(uint16_t));
+            else {
+                memset(dst + (uint64_t)l * T * F, 0, T * F * sizeof(uint16_t));
+                memcpy(dst + (uint64_t)l * T * F, src + off * F, cnt * F * sizeof(uint16_t));
+            }
+        }
+        off += cnt;
+    }
+    return (long long)off;
+}
+long long niv_oracle_table_compact(const niv_oracle_config *cfg, const uint16_t *table, uint16_t *compact)
+{
+    return compact_walk(cfg, table, compact, 1);
+}
+long long niv_oracle_table_expand(const niv_oracle_config *cfg, const uint16_t *compact, uint16_t *table)
+{
+    return compact_walk(cfg, compact, table, 0);
+}

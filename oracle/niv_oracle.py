@@ -285,3 +285,35 @@ def compose_jb(E, pos_half, nrm_half, pos, nrm, albedo, sigma, power, direct=Non
     if rc:
         raise ValueError("niv_oracle_compose_jb failed (E must be at exactly half the resolution; sigma > 0, power >= 0)")
     return out
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# SURVEY 8(f1): compact table storage (dense levels hold (N + 1)^3 entries)
+def compact_entries(spec) -> int:
+    cfg = make_config(spec)
+    lib().niv_oracle_table_compact.restype = C.c_longlong
+    n = lib().niv_oracle_table_compact(C.byref(cfg), None, None)
+    if n < 0:
+        raise ValueError("niv_oracle_table_compact failed")
+    return int(n)
+
+
+def table_compact(spec, table) -> np.ndarray:
+    """[L][T][F] fp16 -> the compact table (flat fp16, compact_entries(spec) * F values)."""
+    cfg = make_config(spec)
+    table = _chk(table, np.float16, "table")
+    out = np.zeros(compact_entries(spec) * spec.n_features, dtype=np.float16)
+    lib().niv_oracle_table_compact.restype = C.c_longlong
+    if lib().niv_oracle_table_compact(C.byref(cfg), _p(table), _p(out)) < 0:
+        raise ValueError("niv_oracle_table_compact failed")
+    return out
+
+
+def table_expand(spec, compact) -> np.ndarray:
+    cfg = make_config(spec)
+    compact = _chk(compact, np.float16, "compact")
+    out = np.zeros((spec.n_levels, spec.table_size, spec.n_features), dtype=np.float16)
+    lib().niv_oracle_table_expand.restype = C.c_longlong
+    if lib().niv_oracle_table_expand(C.byref(cfg), _p(compact), _p(out)) < 0:
+        raise ValueError("niv_oracle_table_expand failed")
+    return out

@@ -332,6 +332,8 @@ struct niv_model {
     niv_info info;
     KParams kp;
     uint32_t* d_table = nullptr;
+    uint64_t lev_entries[kMaxLevels] = {};         // entries a level really has: (N + 1)^3 (dense) or T (hashed)
+    uint64_t dev_table_bytes = 0;                  // device storage: the levels back to back, each padded to 8 entries
     uint32_t kernel_levels = 0;                    // levels the fused kernels run (n_levels rounded up to whole batches)
     uint32_t k_shift = 0;                          // (kernel_levels - n_levels) * F: where the direction columns of W1 move to
     uint32_t* d_cells = nullptr;                   // cell-block copies of the coarse levels (KParams::lv[].cells)
@@ -561,6 +563,7 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
 
     // level table (readings #2, #4)
     const uint64_t T = (uint64_t)1 << cfg->log2_table_size;
+    uint64_t dev_entries = 0;
     for (uint32_t l = 0; l < cfg->n_levels; ++l) {
         uint64_t N;
         if (explicit_res) N = cfg->resolutions[l];
@@ -575,9 +578,16 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
         P.lv[l].cmaxf = (float)(8388608u + (uint32_t)N - 1u);               // exact: < 2^24
         P.lv[l].R = (uint32_t)R;
         P.lv[l].R2 = dense ? (uint32_t)(R * R) : 0u;
-        P.lv[l].base = (uint32_t)(l * T);
+        // compact device storage (Table 1's memory column): a dense level holds its (N + 1)^3
+        // entries only; every level starts at a multiple of 8 entries (32-byte sectors, as in the [L][T] layout)
+        m->lev_entries[l] = dense ? R * R * R : T;
+        P.lv[l].base = (uint32_t)(dev_entries);
+        dev_entries += (m->lev_entries[l] + 7) / 8 * 8;
+        I.table_bytes_compact += m->lev_entries[l] * cfg->n_features * 2;
         P.lv[l].dense = dense ? 1u : 0u;
     }
+    m->dev_table_bytes = dev_entries * cfg->n_features * 2;
+    I.table_bytes_device = m->dev_table_bytes;
     for (int d = 0; d < 3; ++d) {
         P.amin[d] = cfg->aabb_min[d];
         volatile float ext = cfg->aabb_max[d] - cfg->aabb_min[d];
@@ -722,8 +732,8 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     I.smem_bytes = m->fused.smem;
     I.image_tiled = m->fused_img.fn ? 1u : 0u;
     I.texel_params = m->fused_tp.fn ? 1u : 0u;
-    e = cudaMalloc(&m->d_table, I.table_bytes + 64);          // + a block of zeros for the dummy levels
-    if (e == cudaSuccess) e = cudaMemset(reinterpret_cast<uint8_t*>(m->d_table) + I.table_bytes, 0, 64);
+    e = cudaMalloc(&m->d_table, m->dev_table_bytes + 64);     // + a block of zeros for the dummy levels
+    if (e == cudaSuccess) e = cudaMemset(m->d_table, 0, m->dev_table_bytes + 64);
     if (e == cudaSuccess && I.cell_bytes) e = cudaMalloc(&m->d_cells, I.cell_bytes);
     if (e == cudaSuccess) e = cudaMalloc(&m->d_wpack, P.wpack_bytes);
     if (e == cudaSuccess && m->fused_tp.fn) e = cudaMalloc(&m->d_wpack_tp, m->kp_tp.wpack_bytes);
@@ -749,7 +759,7 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
         m->kp_tp.lv[l] = P.lv[l];
     }
     for (uint32_t l = cfg->n_levels; l < Lk; ++l) {
-        P.lv[l].tb = reinterpret_cast<const uint32_t*>(reinterpret_cast<const uint8_t*>(m->d_table) + I.table_bytes);
+        P.lv[l].tb = reinterpret_cast<const uint32_t*>(reinterpret_cast<const uint8_t*>(m->d_table) + m->dev_table_bytes);
         P.lv[l].cells = reinterpret_cast<const uint4*>(P.lv[l].tb);
         m->kp_tp.lv[l] = P.lv[l];
     }
@@ -764,12 +774,14 @@ extern "C" int niv_get_info(const niv_model* m, niv_info* info)
     return NIV_OK;
 }
 
-extern "C" int niv_load_params(niv_model* m, const void* table_fp16, size_t table_bytes,
-                               const void* weights_fp16, size_t weight_bytes,
-                               const float* biases_f32, size_t bias_bytes, int src_on_device, void* stream)
+// compact: the table comes as the levels back to back with exactly lev_entries[l] entries each (niv_load_params_compact)
+static int load_params_impl(niv_model* m, const void* table_fp16, size_t table_bytes, bool compact,
+                            const void* weights_fp16, size_t weight_bytes,
+                            const float* biases_f32, size_t bias_bytes, int src_on_device, void* stream)
 {
     if (!m || (!table_fp16 && m->info.table_bytes) || !weights_fp16) return NIV_ERR_INVALID_ARG;
-    if (table_bytes != m->info.table_bytes || weight_bytes != m->info.weight_bytes) return NIV_ERR_INVALID_ARG;
+    if (table_bytes != (compact ? m->info.table_bytes_compact : m->info.table_bytes) || weight_bytes != m->info.weight_bytes)
+        return NIV_ERR_INVALID_ARG;
     if (biases_f32 ? bias_bytes != m->info.bias_bytes : bias_bytes != 0) return NIV_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     NIV_CUDA(cudaSetDevice(m->cfg.device));
@@ -864,8 +876,17 @@ extern "C" int niv_load_params(niv_model* m, const void* table_fp16, size_t tabl
         NIV_CUDA(cudaMemcpyAsync(m->d_wmma, wm.data(), kMmaWords * 4, cudaMemcpyHostToDevice, st));
         m->kp.wmma = m->d_wmma;
     }
-    if (table_bytes) NIV_CUDA(cudaMemcpyAsync(m->d_table, table_fp16, table_bytes,
-                             src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+    {   // the table, level by level, into the compact device storage (a dense level: its first (N + 1)^3 entries)
+        const size_t eb = (size_t)m->cfg.n_features * 2, T = (size_t)1 << m->cfg.log2_table_size;
+        size_t src_off = 0;
+        for (uint32_t l = 0; l < m->cfg.n_levels; ++l) {
+            const size_t bytes = (size_t)m->lev_entries[l] * eb;
+            NIV_CUDA(cudaMemcpyAsync(reinterpret_cast<uint8_t*>(m->d_table) + (size_t)P.lv[l].base * eb,
+                                     static_cast<const uint8_t*>(table_fp16) + (compact ? src_off : (size_t)l * T * eb), bytes,
+                                     src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+            src_off += bytes;
+        }
+    }
     for (uint32_t l = 0; l < m->info.cell_levels; ++l) {            // cell-block copies of the coarse levels
         const uint32_t n_cells = P.lv[l].cs * P.lv[l].cs2;
         niv_build_cells_kernel<<<(n_cells + 255) / 256, 256, 0, st>>>(
@@ -875,6 +896,22 @@ extern "C" int niv_load_params(niv_model* m, const void* table_fp16, size_t tabl
     NIV_CUDA(cudaStreamSynchronize(st));
     m->loaded = true;
     return NIV_OK;
+}
+
+extern "C" int niv_load_params(niv_model* m, const void* table_fp16, size_t table_bytes,
+                               const void* weights_fp16, size_t weight_bytes,
+                               const float* biases_f32, size_t bias_bytes, int src_on_device, void* stream)
+{
+    return load_params_impl(m, table_fp16, table_bytes, false, weights_fp16, weight_bytes, biases_f32, bias_bytes,
+                            src_on_device, stream);
+}
+
+extern "C" int niv_load_params_compact(niv_model* m, const void* table_fp16, size_t table_bytes,
+                                       const void* weights_fp16, size_t weight_bytes,
+                                       const float* biases_f32, size_t bias_bytes, int src_on_device, void* stream)
+{
+    return load_params_impl(m, table_fp16, table_bytes, true, weights_fp16, weight_bytes, biases_f32, bias_bytes,
+                            src_on_device, stream);
 }
 
 static int fill_params(const niv_model* m, const float* param, KParams& P)

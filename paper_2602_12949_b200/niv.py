@@ -32,7 +32,7 @@ NIV_OUTFMT_F32X3, NIV_OUTFMT_F16X4 = 0, 1
 _GBUF_BYTES = {0: (12, 12), 1: (16, 16), 2: (16, 0), 3: (8, 0)}      # bytes per texel of gbuf_a, gbuf_b
 _OUT_BYTES = {0: 12, 1: 8}
 
-EXPORTS = ("niv_create", "niv_get_info", "niv_load_params", "niv_infer", "niv_infer_image", "niv_infer_texel_params",
+EXPORTS = ("niv_create", "niv_get_info", "niv_load_params", "niv_load_params_compact", "niv_infer", "niv_infer_image", "niv_infer_texel_params",
            "niv_infer_host", "niv_probe_sectors_image",
            "niv_infer_host_static",
            "niv_infer_packed", "niv_infer_image_packed", "niv_infer_host_packed", "niv_decode_gbuffer", "niv_debug_arow",
@@ -63,6 +63,7 @@ class NivInfo(C.Structure):
         ("num_sms", C.c_uint32), ("ctas_per_sm", C.c_uint32), ("tile_texels", C.c_uint32),
         ("smem_bytes", C.c_uint32), ("image_tiled", C.c_uint32), ("texel_params", C.c_uint32),
         ("cell_levels", C.c_uint32), ("kernel_levels", C.c_uint32), ("cell_bytes", C.c_uint64),
+        ("table_bytes_compact", C.c_uint64), ("table_bytes_device", C.c_uint64),
     ]
 
 
@@ -95,6 +96,7 @@ def lib():
         L.niv_create.argtypes = [C.POINTER(NivConfig), C.POINTER(vp)]
         L.niv_get_info.argtypes = [vp, C.POINTER(NivInfo)]
         L.niv_load_params.argtypes = [vp, vp, sz, vp, sz, vp, sz, C.c_int, vp]
+        L.niv_load_params_compact.argtypes = [vp, vp, sz, vp, sz, vp, sz, C.c_int, vp]
         L.niv_infer.argtypes = [vp, vp, vp, C.POINTER(C.c_float), vp, sz, vp]
         L.niv_infer_host.argtypes = [vp, vp, vp, C.POINTER(C.c_float), vp, sz, vp]
         L.niv_infer_host_static.argtypes = [vp, vp, vp, C.POINTER(C.c_float), vp, sz, vp]
@@ -208,7 +210,7 @@ class NivModel:
             raise NivError(rc, "niv_get_info")
 
     # ---- parameters -------------------------------------------------------------------------------
-    def load_params(self, table, weights, biases=None, stream=None):
+    def load_params(self, table, weights, biases=None, stream=None, compact=False):
         """table [L][T][F] fp16, weights flat fp16 blob W1|W2|.., biases flat fp32 blob or None.
         Each is a numpy array (host) or a CUDA tensor (device); all three must live on the same side."""
         import numpy as np
@@ -228,9 +230,10 @@ class NivModel:
             else:
                 biases = np.ascontiguousarray(biases, dtype=np.float32)
                 bp, bb = biases.ctypes.data, biases.nbytes
-        rc = lib().niv_load_params(self._h, tp, tb, wp, wb, bp, bb, int(on_dev), _stream_ptr(stream))
+        fn = lib().niv_load_params_compact if compact else lib().niv_load_params     # compact: the table of
+        rc = fn(self._h, tp, tb, wp, wb, bp, bb, int(on_dev), _stream_ptr(stream))      # niv_info.table_bytes_compact
         if rc != NIV_OK:
-            raise NivError(rc, "niv_load_params")
+            raise NivError(rc, "niv_load_params_compact" if compact else "niv_load_params")
 
     # ---- the hot path -----------------------------------------------------------------------------
     def infer(self, pos, nrm, out, param=None, stream=None):

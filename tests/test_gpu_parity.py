@@ -554,6 +554,39 @@ def test_any_number_of_levels(torch_cuda, niv, oracle, F, L, width):
     m.close()
 
 
+@pytest.mark.parametrize("which", ["fullhd", "tiny", "paper8", "paper3"])
+def test_compact_table_storage(torch_cuda, niv, oracle, which):
+    """the model stores dense levels with (N+1)^3 entries (the paper's 5.4 MB for its largest model) and can be
+    loaded from the compact table; the same bits as the [L][T] load, host and device sources."""
+    torch = torch_cuda
+    spec = {"fullhd": I.spec_fullhd(), "tiny": I.spec_tiny(), "paper8": I.spec_paper(8, 64),
+            "paper3": dataclasses.replace(I.spec_paper(8, 64), n_levels=3, resolutions=I.spec_paper(8, 64).resolutions[:3])}[which]
+    case = Case(spec, 17, table_amp=1.0, bias_scale=0.1)
+    comp = oracle.table_compact(spec, case.table)
+    a = case.gpu_model(niv)
+    assert a.info.table_bytes_compact == comp.nbytes == oracle.compact_entries(spec) * spec.n_features * 2
+    assert comp.nbytes <= a.info.table_bytes_device <= comp.nbytes + 7 * spec.n_features * 2 * spec.n_levels < a.info.table_bytes
+    if which == "paper8":
+        mlp = ((4 * 8 + 3) * 64 + 2 * 64 * 64 + 3 * 64) * 2
+        assert abs((a.info.table_bytes_device + mlp) / 1e6 - 5.4) < 0.05              # PAPER.md:389
+    b = niv.NivModel(spec)
+    b.load_params(comp, case.wblob, case.bblob, compact=True)
+    c = niv.NivModel(spec)
+    c.load_params(torch.from_numpy(comp).cuda(), torch.from_numpy(case.wblob).cuda(), torch.from_numpy(case.bblob).cuda(),
+                  compact=True)
+    n = 30011
+    pos, nrm = _queries(spec, n, 3)
+    pos[:9000], nrm[:9000] = _queries(spec, 9000, 4, coherent=True)
+    ra, rb, rc_ = (_gpu_infer(torch, m, pos, nrm) for m in (a, b, c))
+    assert np.array_equal(ra, rb) and np.array_equal(ra, rc_)
+    _check_debug(torch, oracle, b, case, pos[:4000], nrm[:4000])
+    L = niv.lib()
+    assert L.niv_load_params_compact(b._h, comp.ctypes.data, comp.nbytes - 2, case.wblob.ctypes.data, case.wblob.nbytes,
+                                     case.bblob.ctypes.data, case.bblob.nbytes, 0, None) == niv.NIV_ERR_INVALID_ARG
+    for m in (a, b, c):
+        m.close()
+
+
 @pytest.mark.parametrize("n", [300, 70001])
 def test_back_to_back_launches_overlap_safely(torch_cuda, niv, monkeypatch, n):
     """a launch whose buffers are disjoint from those of the launch before it (same stream, this library)

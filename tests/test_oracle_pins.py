@@ -51,6 +51,32 @@ def test_paper_grid_family_memory_matches_table1(oracle):
         assert abs((grid_bytes + mlp_bytes) / 1e6 - mb) / mb < 0.04
 
 
+def test_compact_table_is_the_paper_memory_and_changes_nothing(oracle):
+    """the compact table (dense levels with (N+1)^3 entries) is what Table 1's memory column counts
+    (PAPER.md:386-389), and a model evaluated on the expanded compact table is the model, bit for bit."""
+    for ln in _golden_lines("paper_table1_memory.txt"):
+        L, mb = int(ln.split()[0]), float(ln.split()[1])
+        spec = I.spec_paper(L, 64)
+        mlp_bytes = ((4 * L + 3) * 64 + 64 * 64 * 2 + 64 * 3) * 2
+        assert abs((oracle.compact_entries(spec) * 4 * 2 + mlp_bytes) / 1e6 - mb) / mb < 0.04
+    spec = I.spec_tiny()                                                   # D D D D H H H H, N = 4 6 9 13 ...
+    assert oracle.compact_entries(spec) == 5 ** 3 + 7 ** 3 + 10 ** 3 + 14 ** 3 + 4 * 4096
+    table = I.make_table(spec, 3, -1.0, 1.0)
+    comp = oracle.table_compact(spec, table)
+    assert comp.size == oracle.compact_entries(spec) * 2
+    back = oracle.table_expand(spec, comp)
+    N, dense = oracle.level_table(spec)
+    for l in range(spec.n_levels):
+        cnt = (int(N[l]) + 1) ** 3 if dense[l] else spec.table_size
+        assert np.array_equal(back[l, :cnt], table.reshape(spec.n_levels, spec.table_size, 2)[l, :cnt])
+        assert np.all(back[l, cnt:] == 0)
+    assert np.array_equal(comp[:5 ** 3 * 2].view(np.uint16), table.reshape(-1)[:5 ** 3 * 2].view(np.uint16))   # level 0 first
+    w, b = I.make_mlp(spec, 3)
+    wb, bb = I.pack_weights(w), I.pack_biases(b)
+    pos, nrm = I.positions_uniform(3000, (spec.aabb_min, spec.aabb_max), 1), I.normals_uniform(3000, 2)
+    assert np.array_equal(oracle.infer(spec, back, wb, bb, pos, nrm), oracle.infer(spec, table, wb, bb, pos, nrm))
+
+
 def test_explicit_resolutions_override(oracle):
     spec = dataclasses.replace(I.spec_tiny(), resolutions=(5, 7, 11, 13, 17, 19, 23, 29))
     N, _ = oracle.level_table(spec)
