@@ -838,6 +838,28 @@ def run_sweep(args):
             one(17, 64, w, h, frames)
 
 
+def graph_ms(launch, steps):
+    """ms per launch of `steps` launches (launch(k), k = 0..steps-1) recorded into ONE CUDA graph and replayed between two
+    events: a 25 us kernel is shorter than one call through the Python binding, so a loop of calls would time the host."""
+    import torch
+
+    side = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(g, stream=side):
+            for k in range(steps):
+                launch(k)
+        g.replay()                                       # warm-up of the instantiated graph
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        side.synchronize()
+        e0.record(side)
+        g.replay()
+        e1.record(side)
+        side.synchronize()
+    return e0.elapsed_time(e1) / steps
+
+
 def run_compose(args):
     """the compose kernel alone (HBM-bound) at full HD, E at full and at half resolution.  One JSON line
     per case: ms, algorithmic GB/s and its fraction of the measured HBM copy bandwidth."""
@@ -860,15 +882,11 @@ def run_compose(args):
                 a, d, le, e, o = bufs[k % ring]
                 niv.compose(e, a, o, d, le)
             steps = args.steps or 100
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            torch.cuda.synchronize()
-            e0.record()
-            for k in range(steps):
+
+            def one(k):
                 a, d, le, e, o = bufs[k % ring]
                 niv.compose(e, a, o, d, le)
-            e1.record()
-            torch.cuda.synchronize()
-            ms = e0.elapsed_time(e1) / steps
+            ms = graph_ms(one, steps)
             nbytes = (48 + (3 if half else 12)) * h * w
             print(json.dumps({"op": "niv_compose", "E_resolution": "%dx%d" % (ew, eh), "frame": "%dx%d" % (w, h),
                               "ms": ms, "algorithmic_bytes": nbytes,
@@ -890,20 +908,85 @@ def run_compose(args):
         for k in range(5):
             jb(k)
         steps = args.steps or 100
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        torch.cuda.synchronize()
-        e0.record()
-        for k in range(steps):
-            jb(k)
-        e1.record()
-        torch.cuda.synchronize()
-        ms = e0.elapsed_time(e1) / steps
+        ms = graph_ms(jb, steps)
         nbytes = (72 + 9) * h * w
         print(json.dumps({"op": "niv_compose_jb", "E_resolution": "%dx%d" % (ew, eh), "frame": "%dx%d" % (w, h), "ms": ms,
                           "algorithmic_bytes": nbytes,
                           "roofline": {"bound": "hbm", "achieved": nbytes / ms / 1e6, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                                        "frac": nbytes / ms / 1e6 / peaks["hbm_gbs"], "peak_source": peaks["source"]}}), flush=True)
         del sets
+
+
+def run_shade(args):
+    """full-resolution shading of the configs[1] frame, two ways -- niv_infer_image then niv_compose (the
+    irradiance goes to HBM and comes back), niv_infer (linear tiles) then niv_compose, and niv_infer_shade (the compose as
+    the inference kernel's epilogue).  One JSON line; ms per frame from `steps` launches between two events, buffers rotating
+    over RING sets."""
+    import torch
+
+    from paper_2602_12949_b200 import build as B
+    from paper_2602_12949_b200 import niv
+
+    B.build()
+    niv.lib()
+    torch.cuda.set_device(0)
+    spec, table, wb, bb, pos, nrm, param, desc, masked = make_workload(args.workload, 0)
+    n = pos.shape[0]
+    model = niv.NivModel(spec, 0)
+    model.load_params(table, wb, bb)
+    ring = 4
+    d_pos = [torch.from_numpy(pos).cuda() for _ in range(ring)]
+    d_nrm = [torch.from_numpy(nrm).cuda() for _ in range(ring)]
+    d_alb, d_dir, d_emi = ([torch.rand((n, 3), device="cuda") for _ in range(ring)] for _ in range(3))
+    d_e = [torch.empty((n, 3), device="cuda") for _ in range(ring)]
+    d_out = [torch.empty((n, 3), device="cuda") for _ in range(ring)]
+    img = lambda t: t.view(H_PX, W_PX, 3)
+
+    def two_pass_image(k):
+        model.infer_image(d_pos[k], d_nrm[k], d_e[k], W_PX, H_PX, param=param)
+        niv.compose(img(d_e[k]), img(d_alb[k]), img(d_out[k]), img(d_dir[k]), img(d_emi[k]))
+
+    def two_pass_linear(k):
+        model.infer(d_pos[k], d_nrm[k], d_e[k], param=param)
+        niv.compose(img(d_e[k]), img(d_alb[k]), img(d_out[k]), img(d_dir[k]), img(d_emi[k]))
+
+    def fused(k):
+        model.infer_shade(d_pos[k], d_nrm[k], d_alb[k], d_out[k], n, direct=d_dir[k], emission=d_emi[k], param=param)
+
+    def fused_image(k):
+        model.infer_shade(d_pos[k], d_nrm[k], d_alb[k], d_out[k], n, direct=d_dir[k], emission=d_emi[k], param=param,
+                          image=(W_PX, H_PX))
+
+    def infer_only(k):
+        model.infer(d_pos[k], d_nrm[k], d_e[k], param=param)
+
+    steps, warm = args.steps or 100, max(3, args.warmup or 5)
+    res = {}
+    for name, fn in (("niv_infer_image + niv_compose", two_pass_image), ("niv_infer + niv_compose", two_pass_linear),
+                     ("niv_infer_shade", fused), ("niv_infer_image_shade", fused_image), ("niv_infer", infer_only)):
+        for k in range(warm):
+            fn(k % ring)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for k in range(steps):
+            fn(k % ring)
+        e1.record()
+        torch.cuda.synchronize()
+        res[name] = e0.elapsed_time(e1) / steps
+    # same bits from both paths (fp32 output)
+    two_pass_linear(0)
+    ref = d_out[0].clone()
+    fused(0)
+    torch.cuda.synchronize()
+    same = bool(torch.equal(ref, d_out[0]))
+    fused_image(0)
+    torch.cuda.synchronize()
+    same = same and bool(torch.equal(ref, d_out[0]))
+    print(json.dumps({"op": "shade", "workload": desc, "frame": "%dx%d" % (W_PX, H_PX), "steps": steps, "ms_per_frame": res,
+                      "fused_equals_two_pass_bitwise": same,
+                      "hbm_bytes_per_texel": {"two_pass": 24 + 12 + 12 + 36 + 12, "fused": 24 + 36 + 12}}), flush=True)
+    model.close()
 
 
 def run_dry(args):
@@ -980,6 +1063,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cold-steps", type=int, default=10, help="launches of the cold-L2 variant (0 = skip)")
     ap.add_argument("--no-compact-e2e", action="store_true", help="skip the end-to-end legs on the compact G-buffer formats")
+    ap.add_argument("--shade", action="store_true", help="SURVEY 8(f2): niv_infer_shade against niv_infer + niv_compose")
     ap.add_argument("--compose", action="store_true", help="SURVEY 8(f2): time the compose kernel (HBM roofline)")
     ap.add_argument("--tiling", default="image", choices=["image", "linear"],
                     help="device path of the G-buffer workloads: niv_infer_image (default) or niv_infer")
@@ -1009,6 +1093,9 @@ def main():
         return
     if args.sweep:
         run_sweep(args)
+        return
+    if args.shade:
+        run_shade(args)
         return
     if args.compose:
         run_compose(args)

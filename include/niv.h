@@ -232,7 +232,8 @@ int niv_infer_host_static(niv_model *m, const float *pos, const float *nrm, cons
  * A texel is decoded to an fp32 position and an fp32 unit normal first -- the position by a pinned fp32 op sequence,
  * so the cells and hash indices are those of niv_infer on the decoded values, bit for bit -- and then takes the path of
  * niv_infer.  Grid models of hidden width <= 64 only (NIV_ERR_UNSUPPORTED for width 128 and for the grid-less models);
- * niv_infer_image_packed runs the linear-tile kernel for every format but fp32 x 3 in and out; unknown formats and
+ * niv_infer_image_packed keeps the 8 x 4-block tiling for models with cell-block levels (linear tiles otherwise: the same
+ * result); unknown formats and
  * misaligned buffers -> NIV_ERR_INVALID_ARG; otherwise as the unpacked entry points. */
 int niv_infer_packed(niv_model *m, int gbuf_format, const void *gbuf_a, const void *gbuf_b, const float *param,
                      int out_format, void *out, size_t n, void *stream);
@@ -277,6 +278,25 @@ int niv_debug_encode(niv_model *m, const float *pos, const float *nrm, const flo
  * Asynchronous on `stream`, allocation-free; needs no model.  Runs on the current CUDA device. */
 int niv_compose(const float *E, uint32_t ew, uint32_t eh, const float *albedo, const float *direct,
                 const float *emission, float *out, uint32_t w, uint32_t h, void *stream);
+
+/* the hot path with that compose as its EPILOGUE, for irradiance inferred at full resolution
+ * ("infers pixel-wise E(x, n) in a single batch", then Eq. 2): one kernel,
+ *   out[i] = albedo[i] / pi * E_theta(pos[i], nrm[i][, param]) + direct[i] + emission[i],
+ * the irradiance never goes to memory (24.9 MB written and read again per full-HD frame by niv_infer + niv_compose).
+ *   gbuf_format, gbuf_a, gbuf_b, param, out_format, out   as niv_infer_packed (NIV_GBUF_F32X3 / NIV_OUTFMT_F32X3: niv_infer's)
+ *   albedo            device, [n][3] fp32;  direct, emission  device, [n][3] fp32, or NULL (zero)
+ * The arithmetic of the epilogue is niv_compose's (fma(albedo * fl32(1/pi), E, direct + emission) in fp32), so on fp32
+ * output the result equals niv_compose of niv_infer's output bit for bit.  Background texels have E = 0: out = direct +
+ * emission.  out must not overlap any input.  Models: hidden width <= 64 (NIV_ERR_UNSUPPORTED for width 128); albedo
+ * NULL -> NIV_ERR_INVALID_ARG; other errors, masking and asynchrony as niv_infer.
+ * niv_infer_image_shade is the same for [height][width] row-major buffers, with niv_infer_image's 8 x 4 pixel blocks per
+ * warp where the model has that kernel (BASELINE.json's family with cell-block levels); the same bits either way. */
+int niv_infer_shade(niv_model *m, int gbuf_format, const void *gbuf_a, const void *gbuf_b, const float *param,
+                    const float *albedo, const float *direct, const float *emission, int out_format, void *out,
+                    size_t n, void *stream);
+int niv_infer_image_shade(niv_model *m, int gbuf_format, const void *gbuf_a, const void *gbuf_b, const float *param,
+                          const float *albedo, const float *direct, const float *emission, int out_format, void *out,
+                          uint32_t width, uint32_t height, void *stream);
 
 /* The same compose with JOINT-BILATERAL upsampling of half-resolution irradiance: the "industry practice upsampling
  * methods" PAPER.md:406 names against the aliasing of half-resolution rendering ("a flagged extension").

@@ -345,6 +345,7 @@ struct niv_model {
     FusedKernel fused_host;                        // niv_infer_host, pinned buffers: 128-bit output stores
     FusedKernel fused_pk, fused_host_pk;           // *_packed entry points: compact G-buffer formats / fp16 output
     FusedKernel fused_img;                         // niv_infer_image: 8 x 4 pixel blocks per warp
+    FusedKernel fused_img_pk;                      //   ... with the compact formats / the shading epilogue (cell-block models)
     FusedKernel fused_tp;                          // niv_infer_texel_params: parameter columns as K-steps of layer 1,
     KParams kp_tp;                                 //   with its own packed weights and shared-memory layout
     uint8_t* d_wpack_tp = nullptr;
@@ -465,10 +466,10 @@ static fused_fn pick_fused(uint32_t W, uint32_t L, uint32_t F) {
 // image tiling (niv_infer_image): BASELINE.json's family (F = 2, 8..16 levels reach cells smaller than a warp's strip).
 // The paper's own family (F = 4, <= 8 levels, finest cell 5.5 cm) measured SLOWER with it (profiles/r01_v2.md): its
 // cells are larger than a 32-pixel strip anyway; it keeps the linear kernel, as do the grid-less models.
-template <bool C>
+template <bool C, bool PK = false>
 static fused_fn pick_fused_img(uint32_t W, uint32_t L, uint32_t F) {
     if (L == 0 || F != 2) return nullptr;
-    return W == 32 ? pick_levels_f2<32, false, 0, true, C>(L) : W == 64 ? pick_levels_f2<64, false, 0, true, C>(L) : nullptr;
+    return W == 32 ? pick_levels_f2<32, false, 0, true, C, PK>(L) : W == 64 ? pick_levels_f2<64, false, 0, true, C, PK>(L) : nullptr;
 }
 // per-texel scene parameters: BASELINE.json's family, 8 or 16 levels, width 32 / 64, 1 or 2 parameters
 template <int W, int NPT, bool C>
@@ -714,6 +715,11 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
                                         : pick_fused_img<false>(W, Lk, cfg->n_features);
             m->fused_img.smem = smem_dev;
             rc = setup_kernel(m, m->fused_img, tmem_cols, "fused_image");
+        }
+        if (rc == NIV_OK && use_cells && m->fused_img.fn) {
+            m->fused_img_pk.fn = pick_fused_img<true, true>(W, Lk, cfg->n_features);
+            m->fused_img_pk.smem = smem_dev;
+            rc = setup_kernel(m, m->fused_img_pk, tmem_cols, "fused_image_packed");
         }
         if (rc == NIV_OK && cfg->n_params) {
             m->fused_tp.fn = use_cells ? pick_fused_tp<true>(W, Lk, cfg->n_features, cfg->sh_degree, cfg->n_params)
@@ -968,9 +974,10 @@ static void draw_tile_counter(niv_model* m, cudaStream_t st, KParams& P)
 //     griddepcontrol.wait only if n-1, n-2 and n-3 all have such a word (launches recorded into a CUDA graph, on the
 //     static-striding fallback or through another kernel have none: the next launches wait in full);
 //   * niv_destroy forgets all history (cudaFree has synchronised the device by then).
+constexpr int kRanges = 7, kOutRange = 6;
 struct LaunchRec {
     bool tracked = false;
-    uintptr_t lo[4] = {0, 0, 0, 0}, hi[4] = {0, 0, 0, 0};    // pos, nrm, tparam (read), out (written)
+    uintptr_t lo[kRanges] = {}, hi[kRanges] = {};             // pos, nrm, tparam, albedo, direct, emission (read), out (written)
     const uint32_t* done = nullptr;
     uint32_t gen = 0;
 };
@@ -982,10 +989,10 @@ static bool ranges_overlap(const LaunchRec& a, int i, const LaunchRec& b, int j)
     return a.lo[i] < b.hi[j] && b.lo[j] < a.hi[i];
 }
 static bool launches_conflict(const LaunchRec& prev, const LaunchRec& cur) {
-    for (int j = 0; j < 4; ++j)
-        if (ranges_overlap(prev, 3, cur, j)) return true;     // cur touches what prev writes
-    for (int i = 0; i < 3; ++i)
-        if (ranges_overlap(prev, i, cur, 3)) return true;     // cur writes what prev reads
+    for (int j = 0; j < kRanges; ++j)
+        if (ranges_overlap(prev, kOutRange, cur, j)) return true;     // cur touches what prev writes
+    for (int i = 0; i < kOutRange; ++i)
+        if (ranges_overlap(prev, i, cur, kOutRange)) return true;     // cur writes what prev reads
     return false;
 }
 static void forget_history() {
@@ -1000,10 +1007,11 @@ static int launch_one(const niv_model* m, const FusedKernel& k, cudaStream_t st,
 {
     LaunchRec cur;
     static const size_t kA[4] = {12, 16, 16, 8}, kB[4] = {12, 16, 0, 0}, kO[2] = {12, 8};   // bytes per texel by format
-    const void* base[4] = {pos, nrm, P.tparam, out};
-    const size_t bytes[4] = {n * kA[P.gbuf_fmt & 3], n * kB[P.gbuf_fmt & 3], P.tparam ? n * 4 * m->cfg.n_params : 0,
-                             n * kO[P.out_fmt & 1]};
-    for (int i = 0; i < 4; ++i) { cur.lo[i] = (uintptr_t)base[i]; cur.hi[i] = cur.lo[i] + bytes[i]; }
+    const void* base[kRanges] = {pos, nrm, P.tparam, P.shade_albedo, P.shade_direct, P.shade_emission, out};
+    const size_t bytes[kRanges] = {n * kA[P.gbuf_fmt & 3], n * kB[P.gbuf_fmt & 3], P.tparam ? n * 4 * m->cfg.n_params : 0,
+                                   P.shade_albedo ? n * 12 : 0, P.shade_direct ? n * 12 : 0, P.shade_emission ? n * 12 : 0,
+                                   n * kO[P.out_fmt & 1]};
+    for (int i = 0; i < kRanges; ++i) { cur.lo[i] = (uintptr_t)base[i]; cur.hi[i] = cur.lo[i] + bytes[i]; }
     cur.tracked = pdl && m->overlap && P.tile_ctr != nullptr;
     cur.done = P.tile_ctr ? P.tile_ctr + 2 : nullptr;
     cur.gen = P.slot_gen;
@@ -1068,7 +1076,7 @@ static int launch_fused(niv_model* m, const KParams& Pin, const float* pos, cons
     const uint32_t n_tiles = (uint32_t)((n + kTile - 1) / kTile);
     const bool tc5 = m->cfg.hidden_width <= 64;          // the kernels with the griddepcontrol pair
     // (the zero-copy host variant is followed by a stream synchronisation: it has nothing to overlap with)
-    const bool packed = P.gbuf_fmt != NIV_GBUF_F32X3 || P.out_fmt != NIV_OUTFMT_F32X3;
+    const bool packed = P.gbuf_fmt != NIV_GBUF_F32X3 || P.out_fmt != NIV_OUTFMT_F32X3 || P.shade_albedo != nullptr;
     const FusedKernel& k = packed ? (host_variant ? m->fused_host_pk : m->fused_pk) : (host_variant ? m->fused_host : m->fused);
     if (!k.fn) return NIV_ERR_UNSUPPORTED;
     return launch_one(m, k, st, m->pdl && tc5 && !host_variant, P, pos, nrm, out, n, n_tiles);
@@ -1138,6 +1146,27 @@ extern "C" int niv_infer_packed(niv_model* m, int gbuf_format, const void* gbuf_
     return launch_fused(m, P, (const float*)gbuf_a, (const float*)gbuf_b, (float*)out, n, (cudaStream_t)stream);
 }
 
+// the deferred compose as the EPILOGUE of the inference kernel (Eq. 2, 403): the irradiance
+// never goes to memory, out = albedo / pi * E + direct + emission in the arithmetic of niv_compose.
+extern "C" int niv_infer_shade(niv_model* m, int gbuf_format, const void* gbuf_a, const void* gbuf_b, const float* param,
+                               const float* albedo, const float* direct, const float* emission, int out_format, void* out,
+                               size_t n, void* stream)
+{
+    FmtInfo f;
+    int rc = check_packed(m, gbuf_format, gbuf_a, gbuf_b, out_format, out, n, f);
+    if (rc != NIV_OK) return rc > 0 ? NIV_OK : rc;
+    if (!albedo) return NIV_ERR_INVALID_ARG;
+    if (m->cfg.hidden_width > 64 || m->mma_kernel || !m->fused_pk.fn) return NIV_ERR_UNSUPPORTED;
+    KParams P;
+    rc = fill_params(m, param, P);
+    if (rc != NIV_OK) return rc;
+    set_formats(m, P, gbuf_format, out_format);
+    P.shade_albedo = albedo;
+    P.shade_direct = direct;
+    P.shade_emission = emission;
+    return launch_fused(m, P, (const float*)gbuf_a, (const float*)gbuf_b, (float*)out, n, (cudaStream_t)stream);
+}
+
 // Debug: niv_infer through the PACKED kernel variant (fp32 x 3 in and out) which also writes every texel's layer-1 A
 // row -- the packed fp16 words the tensor core reads: latents, direction, zero padding -- for feature-level parity of
 // the FUSED path (cell-block levels, packed-fp16 blend) in every model family.
@@ -1166,6 +1195,24 @@ extern "C" int niv_infer(niv_model* m, const float* pos, const float* nrm, const
     return niv_infer_packed(m, NIV_GBUF_F32X3, pos, nrm, param, NIV_OUTFMT_F32X3, out, n, stream);
 }
 
+// an image call: the 8 x 4-block kernel where the model has one for this call (fp32 x 3 in and out: fused_img; compact
+// formats or the shading epilogue: fused_img_pk), else linear tiles -- the same result
+static int launch_image(niv_model* m, KParams& P, const void* gbuf_a, const void* gbuf_b, void* out, uint32_t width,
+                        uint32_t height, cudaStream_t st)
+{
+    const size_t n = (size_t)width * height;
+    const bool packed = P.gbuf_fmt != NIV_GBUF_F32X3 || P.out_fmt != NIV_OUTFMT_F32X3 || P.shade_albedo != nullptr;
+    const FusedKernel& k = packed ? m->fused_img_pk : m->fused_img;
+    if (!k.fn || width > (1u << 20) || height > (1u << 17) || m->image_linear)
+        return launch_fused(m, P, (const float*)gbuf_a, (const float*)gbuf_b, (float*)out, n, st);
+    P.img_w = width;
+    P.img_h = height;
+    P.tiles_x = (width + 31u) / 32u;
+    const uint32_t n_tiles = P.tiles_x * ((height + 3u) / 4u);
+    draw_tile_counter(m, st, P);
+    return launch_one(m, k, st, m->pdl, P, (const float*)gbuf_a, (const float*)gbuf_b, (float*)out, n, n_tiles);
+}
+
 extern "C" int niv_infer_image_packed(niv_model* m, int gbuf_format, const void* gbuf_a, const void* gbuf_b,
                                       const float* param, int out_format, void* out, uint32_t width, uint32_t height,
                                       void* stream)
@@ -1180,16 +1227,28 @@ extern "C" int niv_infer_image_packed(niv_model* m, int gbuf_format, const void*
     set_formats(m, P, gbuf_format, out_format);
     // models without an image-tiled kernel (and images beyond the packed tile coordinates): same result, linear tiles
     // (and the compact formats, whose kernels are linear-tile ones)
-    const bool packed = gbuf_format != NIV_GBUF_F32X3 || out_format != NIV_OUTFMT_F32X3;
-    if (!m->fused_img.fn || width > (1u << 20) || height > (1u << 17) || m->image_linear || packed)
-        return launch_fused(m, P, (const float*)gbuf_a, (const float*)gbuf_b, (float*)out, n, (cudaStream_t)stream);
-    P.img_w = width;
-    P.img_h = height;
-    P.tiles_x = (width + 31u) / 32u;
-    const uint32_t n_tiles = P.tiles_x * ((height + 3u) / 4u);
-    draw_tile_counter(m, (cudaStream_t)stream, P);
-    return launch_one(m, m->fused_img, (cudaStream_t)stream, m->pdl, P, (const float*)gbuf_a, (const float*)gbuf_b,
-                      (float*)out, n, n_tiles);
+    return launch_image(m, P, gbuf_a, gbuf_b, out, width, height, (cudaStream_t)stream);
+}
+
+// niv_infer_shade for a G-buffer that is an image (8 x 4 pixel blocks per warp where the model has that kernel)
+extern "C" int niv_infer_image_shade(niv_model* m, int gbuf_format, const void* gbuf_a, const void* gbuf_b,
+                                     const float* param, const float* albedo, const float* direct, const float* emission,
+                                     int out_format, void* out, uint32_t width, uint32_t height, void* stream)
+{
+    const size_t n = (size_t)width * height;
+    FmtInfo f;
+    int rc = check_packed(m, gbuf_format, gbuf_a, gbuf_b, out_format, out, n, f);
+    if (rc != NIV_OK) return rc > 0 ? NIV_OK : rc;
+    if (!albedo) return NIV_ERR_INVALID_ARG;
+    if (m->cfg.hidden_width > 64 || m->mma_kernel || !m->fused_pk.fn) return NIV_ERR_UNSUPPORTED;
+    KParams P;
+    rc = fill_params(m, param, P);
+    if (rc != NIV_OK) return rc;
+    set_formats(m, P, gbuf_format, out_format);
+    P.shade_albedo = albedo;
+    P.shade_direct = direct;
+    P.shade_emission = emission;
+    return launch_image(m, P, gbuf_a, gbuf_b, out, width, height, (cudaStream_t)stream);
 }
 
 extern "C" int niv_infer_image(niv_model* m, const float* pos, const float* nrm, const float* param,
@@ -1455,6 +1514,34 @@ extern "C" int niv_probe_sectors_image(const niv_model* m, const float* pos, con
     return NIV_OK;
 }
 
+// SM count of the current device, looked up once per device
+static cudaError_t current_device_sms(int* sms)
+{
+    static std::atomic<int> cache[64];
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    int v = (dev >= 0 && dev < 64) ? cache[dev].load(std::memory_order_relaxed) : 0;
+    if (v == 0) {
+        e = cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return e;
+        if (dev >= 0 && dev < 64) cache[dev].store(v, std::memory_order_relaxed);
+    }
+    *sms = v;
+    return cudaSuccess;
+}
+
+// Grid of 256-thread CTAs for a grid-stride loop over `items`: at most 8 CTAs per SM (one resident wave), and every
+// thread the same number of iterations -- with min(ceil(items / 256), 8 * sms) CTAs a full-HD frame (518,400 groups
+// of four pixels over 303,104 threads) gave 71 % of the threads two iterations and the rest one: a tail of 15 %
+static unsigned balanced_grid(size_t items, int sms)
+{
+    const size_t wave = (size_t)sms * 8 * 256;
+    const size_t iters = (items + wave - 1) / wave;
+    const size_t threads = (items + iters - 1) / (iters ? iters : 1);
+    return (unsigned)std::max<size_t>(1, (threads + 255) / 256);
+}
+
 extern "C" int niv_compose(const float* E, uint32_t ew, uint32_t eh, const float* albedo, const float* direct,
                            const float* emission, float* out, uint32_t w, uint32_t h, void* stream)
 {
@@ -1464,20 +1551,19 @@ extern "C" int niv_compose(const float* E, uint32_t ew, uint32_t eh, const float
     if (ew == w && eh == h) half = 0;
     else if (2ull * ew == w && 2ull * eh == h) half = 1;
     else return NIV_ERR_INVALID_ARG;
-    int dev = 0, sms = 0;
-    NIV_CUDA(cudaGetDevice(&dev));
-    NIV_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    int sms = 0;
+    NIV_CUDA(current_device_sms(&sms));
     cudaStream_t st = (cudaStream_t)stream;
     const uintptr_t align = (uintptr_t)albedo | (uintptr_t)out | (uintptr_t)(direct ? direct : albedo) |
                             (uintptr_t)(emission ? emission : albedo) | (half ? 0 : (uintptr_t)E);
     const size_t n = (size_t)w * h;
     if ((w & 3u) == 0 && (align & 15u) == 0) {
         const size_t groups = n / 4;
-        const unsigned grid = (unsigned)std::min<size_t>((groups + 255) / 256, (size_t)sms * 8);   // 8 x 256 threads per SM
+        const unsigned grid = balanced_grid(groups, sms);
         if (half) niv_compose_kernel<true><<<grid, 256, 0, st>>>(E, ew, eh, albedo, direct, emission, out, w, h);
         else niv_compose_kernel<false><<<grid, 256, 0, st>>>(E, ew, eh, albedo, direct, emission, out, w, h);
     } else {
-        const unsigned grid = (unsigned)std::min<size_t>((n + 255) / 256, (size_t)sms * 8);
+        const unsigned grid = balanced_grid(n, sms);
         niv_compose_scalar_kernel<<<grid, 256, 0, st>>>(E, ew, eh, albedo, direct, emission, out, w, h, half);
     }
     NIV_CUDA(cudaGetLastError());
@@ -1493,11 +1579,10 @@ extern "C" int niv_compose_jb(const float* E, const float* pos_half, const float
     if (!(sigma > 0.0f) || !std::isfinite(sigma) || !(power >= 0.0f) || !std::isfinite(power)) return NIV_ERR_INVALID_ARG;
     if (w == 0 || h == 0) return NIV_OK;
     if (2ull * ew != w || 2ull * eh != h) return NIV_ERR_INVALID_ARG;
-    int dev = 0, sms = 0;
-    NIV_CUDA(cudaGetDevice(&dev));
-    NIV_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    int sms = 0;
+    NIV_CUDA(current_device_sms(&sms));
     const size_t n = (size_t)w * h;
-    const unsigned grid = (unsigned)std::min<size_t>((n + 255) / 256, (size_t)sms * 8);
+    const unsigned grid = balanced_grid(n, sms);
     niv_compose_jb_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(E, pos_half, nrm_half, ew, eh, pos, nrm, albedo, direct,
                                                                   emission, 1.0f / (2.0f * sigma * sigma), power, out, w, h);
     NIV_CUDA(cudaGetLastError());

@@ -72,6 +72,11 @@ struct KParams {
     float    aext[3];           // fl32(max - min): the scale of the unorm16 position format
     uint32_t img_w, img_h;      // niv_infer_image: the buffers are a row-major img_h x img_w image ...
     uint32_t tiles_x;           // ... cut into 32 x 4 pixel tiles, tiles_x = ceil(img_w / 32) per tile row (else 0)
+    // niv_infer_shade (PACKED kernels): the deferred compose as the epilogue, out = albedo / pi * E + direct + emission
+    // (Eq. 2, 403); [n][3] fp32 each, shade_albedo NULL = plain inference, the other two may be NULL (zero)
+    const float* shade_albedo;
+    const float* shade_direct;
+    const float* shade_emission;
 };
 
 // ---------------------------------------------------------------- O0: background / non-finite mask

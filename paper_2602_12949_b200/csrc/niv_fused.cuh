@@ -17,6 +17,8 @@
 
 namespace niv {
 
+constexpr float kInvPi = 0.318309886183790671538f;
+
 __device__ __forceinline__ uint32_t pack_relu_half2(float lo, float hi) {
     uint32_t d;
     asm("cvt.rn.relu.f16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
@@ -238,6 +240,18 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
             }
         }
         prefetch_next();
+        // niv_infer_shade: this texel's albedo and direct + emission, requested here so that they arrive under the layers
+        float sh_a[3] = {0.f, 0.f, 0.f}, sh_v[3] = {0.f, 0.f, 0.f};
+        if constexpr (PACKED) {
+            if (P.shade_albedo && valid) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    sh_a[c] = __ldcs(P.shade_albedo + 3 * i + c);
+                    if (P.shade_direct) sh_v[c] = __ldcs(P.shade_direct + 3 * i + c);
+                    if (P.shade_emission) sh_v[c] += __ldcs(P.shade_emission + 3 * i + c);
+                }
+            }
+        }
         __syncwarp();
         if constexpr (AW == 8) tmem_st_x8(lane_taddr + A_COL, a);
         else tmem_st_x16(lane_taddr + A_COL, a);
@@ -331,6 +345,7 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
                         float v = __uint_as_float(r[c]);
                         if (P.out_act == NIV_OUT_SIGMOID) v = __fdividef(1.0f, 1.0f + __expf(-v));
                         y[c] = masked ? 0.0f : v;
+                        if (PACKED && P.shade_albedo) y[c] = fmaf(sh_a[c] * kInvPi, y[c], sh_v[c]);
                     }
                     const uint32_t lane = tid & 31u;
                     float* so = reinterpret_cast<float*>(smem + P.misc_off + 64) + warp * 96;
@@ -358,6 +373,7 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
                         float v = __uint_as_float(r[c]);
                         if (P.out_act == NIV_OUT_SIGMOID) v = __fdividef(1.0f, 1.0f + __expf(-v));
                         y[c] = masked ? 0.0f : v;
+                        if (PACKED && P.shade_albedo) y[c] = fmaf(sh_a[c] * kInvPi, y[c], sh_v[c]);   // Eq. 2, as niv_compose
                     }
                     if (PACKED && P.out_fmt == NIV_OUTFMT_F16X4) {      // (r, g, b, 0) as four fp16: one 8-byte store
                         reinterpret_cast<uint2*>(out)[i] = make_uint2(pack_half2(y[0], y[1]), pack_half2(y[2], 0.0f));

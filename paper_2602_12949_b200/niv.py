@@ -36,6 +36,7 @@ EXPORTS = ("niv_create", "niv_get_info", "niv_load_params", "niv_load_params_com
            "niv_infer_host", "niv_probe_sectors_image",
            "niv_infer_host_static",
            "niv_infer_packed", "niv_infer_image_packed", "niv_infer_host_packed", "niv_decode_gbuffer", "niv_debug_arow",
+           "niv_infer_shade", "niv_infer_image_shade",
            "niv_encode",
            "niv_debug_encode", "niv_compose", "niv_compose_jb", "niv_destroy", "niv_error_string", "niv_last_cuda_error", "niv_probe_gather",
            "niv_probe_sectors",
@@ -105,6 +106,9 @@ def lib():
         L.niv_probe_sectors_image.argtypes = [vp, vp, vp, C.c_uint32, C.c_uint32, vp, vp]
         L.niv_encode.argtypes = [vp, vp, vp, C.POINTER(C.c_float), vp, sz, vp]
         L.niv_infer_packed.argtypes = [vp, C.c_int, vp, vp, C.POINTER(C.c_float), C.c_int, vp, sz, vp]
+        L.niv_infer_shade.argtypes = [vp, C.c_int, vp, vp, C.POINTER(C.c_float), vp, vp, vp, C.c_int, vp, sz, vp]
+        L.niv_infer_image_shade.argtypes = [vp, C.c_int, vp, vp, C.POINTER(C.c_float), vp, vp, vp, C.c_int, vp,
+                                            C.c_uint32, C.c_uint32, vp]
         L.niv_infer_image_packed.argtypes = [vp, C.c_int, vp, vp, C.POINTER(C.c_float), C.c_int, vp, C.c_uint32, C.c_uint32, vp]
         L.niv_infer_host_packed.argtypes = [vp, C.c_int, vp, vp, C.POINTER(C.c_float), C.c_int, vp, sz, vp]
         L.niv_decode_gbuffer.argtypes = [vp, C.c_int, vp, vp, vp, vp, sz, vp]
@@ -322,6 +326,29 @@ class NivModel:
                                     int(out_format), po, n, _stream_ptr(stream))
         if rc != NIV_OK:
             raise NivError(rc, "niv_infer_packed")
+        return out
+
+    def infer_shade(self, a, b, albedo, out, n, direct=None, emission=None, gbuf_format=NIV_GBUF_F32X3,
+                    out_format=NIV_OUTFMT_F32X3, param=None, stream=None, image=None):
+        """niv_infer_shade (include/niv.h): out = albedo / pi * E + direct + emission in the inference kernel's epilogue;
+        a, b, out as infer_packed, albedo / direct / emission CUDA float32 [n][3] (the last two optional).
+        image = (width, height): niv_infer_image_shade on row-major buffers of width * height == n texels."""
+        pa, pb, po = self._packed_args(gbuf_format, a, b, out_format, out, n, True)
+        import torch
+        sh = [None if t is None else _dev(t, torch.float32, name, 3) for name, t in
+              (("albedo", albedo), ("direct", direct), ("emission", emission))]
+        _same_rows(n, **{k: v for k, v in (("albedo", albedo), ("direct", direct), ("emission", emission)) if v is not None})
+        if image is not None:
+            w, h = int(image[0]), int(image[1])
+            if w * h != n:
+                raise ValueError("image is %d x %d, the buffers hold %d texels" % (w, h, n))
+            rc = lib().niv_infer_image_shade(self._h, int(gbuf_format), pa, pb, _params(param, self.spec.n_params),
+                                             sh[0], sh[1], sh[2], int(out_format), po, w, h, _stream_ptr(stream))
+        else:
+            rc = lib().niv_infer_shade(self._h, int(gbuf_format), pa, pb, _params(param, self.spec.n_params),
+                                       sh[0], sh[1], sh[2], int(out_format), po, n, _stream_ptr(stream))
+        if rc != NIV_OK:
+            raise NivError(rc, "niv_infer_shade")
         return out
 
     def infer_image_packed(self, gbuf_format, a, b, out, width, height, out_format=NIV_OUTFMT_F32X3, param=None, stream=None):
