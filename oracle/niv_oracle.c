@@ -56,6 +56,7 @@ typedef struct {
     uint32_t n_hidden_layers;
     uint32_t hidden_width;
     uint32_t out_activation;    /* 0 linear, 1 sigmoid */
+    uint32_t dir_frequencies;   /* sh_degree 0 only: bands of frequency encoding appended to the raw direction (0 = none) */
 } niv_oracle_config;
 
 /* ---- fp16 -> fp64, exact, subnormals included (no flush to zero) ---- */
@@ -223,14 +224,23 @@ void niv_oracle_param_encode(double t, uint32_t n_frequencies, double *out)
  * sh_degree 0 -> the direction itself, (x, y, z) as given: the paper's own model feeds "the input
  * position and direction" to the network and needs no basis functions (
  * SPEC.md:306 "raw 3-vector"). ---- */
+/* With dir_frequencies = B > 0 the raw direction is followed by its frequency encoding ("directionEncoding:
+ * raw 3-vector (plus optional frequency)", "The paper does not specify ... whether the direction vector is
+ * frequency-encoded"; freq_encode of SPEC.md:211-214 on scalars in [-1, 1], axis after axis):
+ *   [n_x, n_y, n_z | s(n_x) | s(n_y) | s(n_z)],  s(p) = [sin(2^0 pi p), cos(2^0 pi p), ..., sin(2^(B-1) pi p), cos(2^(B-1) pi p)]
+ * = 3 + 6 B values (reading 3.8). */
 static uint32_t dir_dim_of(const niv_oracle_config *cfg)
 {
-    return cfg->sh_degree == 0 ? 3u : cfg->sh_degree * cfg->sh_degree;
+    return cfg->sh_degree == 0 ? 3u + 6u * cfg->dir_frequencies : cfg->sh_degree * cfg->sh_degree;
 }
 
 static void dir_encode(const niv_oracle_config *cfg, const double n[3], double *out)
 {
-    if (cfg->sh_degree == 0) { out[0] = n[0]; out[1] = n[1]; out[2] = n[2]; }
+    if (cfg->sh_degree == 0) {
+        out[0] = n[0]; out[1] = n[1]; out[2] = n[2];
+        for (int d = 0; d < 3; ++d)
+            niv_oracle_param_encode(n[d], cfg->dir_frequencies, out + 3 + 2 * cfg->dir_frequencies * d);
+    }
     else niv_oracle_sh16(n, out);
 }
 
@@ -286,6 +296,7 @@ static int check_cfg(const niv_oracle_config *cfg)
     if (cfg->n_features == 0 || cfg->n_features > 16) return -1;
     if (cfg->log2_table_size == 0 || cfg->log2_table_size > 30) return -1;
     if (cfg->sh_degree != 4 && cfg->sh_degree != 0) return -1;
+    if (cfg->dir_frequencies > 16 || (cfg->sh_degree != 0 && cfg->dir_frequencies != 0)) return -1;
     if (in_dim_of(cfg) > NIV_ORACLE_MAX_DIM || cfg->hidden_width > NIV_ORACLE_MAX_DIM) return -1;
     return 0;
 }

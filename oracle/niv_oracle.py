@@ -26,6 +26,7 @@ class OracleConfig(C.Structure):
         ("aabb_min", C.c_float * 3), ("aabb_max", C.c_float * 3),
         ("sh_degree", C.c_uint32), ("n_params", C.c_uint32), ("n_frequencies", C.c_uint32),
         ("n_hidden_layers", C.c_uint32), ("hidden_width", C.c_uint32), ("out_activation", C.c_uint32),
+        ("dir_frequencies", C.c_uint32),
     ]
 
 
@@ -75,6 +76,7 @@ def make_config(spec) -> OracleConfig:
     cfg.n_hidden_layers = spec.n_hidden_layers
     cfg.hidden_width = spec.hidden_width
     cfg.out_activation = spec.out_activation
+    cfg.dir_frequencies = getattr(spec, "dir_frequencies", 0)
     return cfg
 
 

@@ -82,6 +82,7 @@ class ModelSpec:
     n_frequencies: int = 8        # sin/cos bands per parameter
     sh_degree: int = 4            # 4 => 16 SH coefficients (BASELINE.json); 0 => the raw direction, 3 values (paper)
     resolutions: Optional[Tuple[int, ...]] = None   # explicit N_l override
+    dir_frequencies: int = 0      # sh_degree 0 only: sin/cos bands per axis appended to the raw direction
 
     @property
     def table_size(self) -> int:
@@ -89,7 +90,7 @@ class ModelSpec:
 
     @property
     def dir_dim(self) -> int:
-        return 3 if self.sh_degree == 0 else self.sh_degree ** 2
+        return 3 + 6 * self.dir_frequencies if self.sh_degree == 0 else self.sh_degree ** 2
 
     @property
     def pos_dim(self) -> int:
@@ -136,6 +137,14 @@ def spec_paper(n_levels: int = 8, width: int = 64) -> ModelSpec:
     Resolutions are passed explicitly so that no pow() rounding decides an integer."""
     return ModelSpec(n_levels, 4, 17, 16, 2.0 ** 0.5, *ROOM_AABB, hidden_width=width, n_hidden_layers=3,
                      out_activation=OUT_LINEAR, sh_degree=0, resolutions=PAPER_RESOLUTIONS[:n_levels])
+
+
+def spec_paper_dirfreq(n_levels: int = 8, width: int = 64, bands: int = 4) -> ModelSpec:
+    """The paper's family with the direction frequency-encoded on top of the raw vector ("raw 3-vector (plus
+    optional frequency)"): 3 + 6 * bands direction inputs."""
+    return ModelSpec(n_levels, 4, 17, 16, 2.0 ** 0.5, *ROOM_AABB, hidden_width=width, n_hidden_layers=3,
+                     out_activation=OUT_LINEAR, sh_degree=0, resolutions=PAPER_RESOLUTIONS[:n_levels],
+                     dir_frequencies=bands)
 
 
 def spec_paper_pe(width: int = 64) -> ModelSpec:

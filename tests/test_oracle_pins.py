@@ -419,6 +419,58 @@ def test_paper_gridless_models_brute_force_4x4(oracle):
     np.testing.assert_allclose(out64, h, rtol=0, atol=1e-11)
 
 
+def test_direction_frequency_encoding(oracle):
+    """SPEC.md:198 "directionEncoding: raw 3-vector (plus optional frequency)" with freq_encode of SPEC.md:211-219 per
+    axis (reading 3.8): [n | s(n_x) | s(n_y) | s(n_z)], s(p) = (sin, cos)(2^k pi p), k < B.  Pins: the SPEC
+    examples on the direction path (n_d = 0 -> (0, 1) pairs; n_d = 0.5 -> first band (1, 0); n_d = -0.5 -> (-1, 0): the
+    input range is [-1, 1], sin is odd), numpy for the whole feature block, B = 0 reduces to the raw model bit for bit,
+    one-hot first-layer weights read single features out through the MLP, and the whole path against a numpy chain."""
+    B = 4
+    spec = I.spec_paper_dirfreq(2, 32, B)
+    raw = I.spec_paper(2, 32)
+    assert spec.dir_dim == 3 + 6 * B and spec.in_dim == raw.in_dim + 6 * B == 8 + 27
+    table = I.make_table(spec, 3, -1.0, 1.0)
+    pos = I.positions_uniform(40, (spec.aabb_min, spec.aabb_max), 2)
+    nrm = I.normals_uniform(40, 2)
+    nrm[0] = (0.0, 0.5, -0.5)                      # not unit: the encoding is defined on the values as given
+    nrm[1] = (1.0, 0.0, 0.0)
+    enc = oracle.encode(spec, table, pos, nrm)["features"]
+    enc_raw = oracle.encode(raw, table, pos, nrm)["features"]
+    assert np.array_equal(enc[:, :11], enc_raw)                     # latents and the raw vector are untouched
+    d0 = enc[0, 11:]
+    np.testing.assert_allclose(d0[0:2 * B], np.tile([0.0, 1.0], B), atol=1e-15)              # n_x = 0
+    np.testing.assert_allclose(d0[2 * B:2 * B + 2], [1.0, 0.0], atol=1e-15)                  # n_y = 0.5, band 0
+    np.testing.assert_allclose(d0[4 * B:4 * B + 2], [-1.0, 0.0], atol=1e-15)                 # n_z = -0.5, band 0
+    np.testing.assert_allclose(enc[1, 11:13], [0.0, -1.0], atol=2e-16)                       # n_x = 1: (sin pi, cos pi)
+    k = 2.0 ** np.arange(B)
+    want = np.empty((40, 6 * B))
+    n64 = nrm.astype(np.float64)
+    for d in range(3):
+        want[:, 2 * B * d:2 * B * (d + 1):2] = np.sin(np.pi * n64[:, d:d + 1] * k)
+        want[:, 2 * B * d + 1:2 * B * (d + 1):2] = np.cos(np.pi * n64[:, d:d + 1] * k)
+    np.testing.assert_allclose(enc[:, 11:], want, atol=1e-12)
+    # dir_frequencies = 0 is the raw model
+    zero = dataclasses.replace(spec, dir_frequencies=0)
+    assert zero.in_dim == raw.in_dim and np.array_equal(oracle.encode(zero, table, pos, nrm)["features"], enc_raw)
+    # through the MLP: a one-layer-deep probe of single input columns (hidden unit j = +feature c, unit j+1 = -feature c)
+    one = dataclasses.replace(spec, n_hidden_layers=1)
+    for c in (8, 10, 11, 12, 11 + 2 * B, 11 + 6 * B - 1):
+        w1 = np.zeros((32, one.in_dim), np.float16)
+        w1[0, c], w1[1, c] = 1.0, -1.0
+        w2 = np.zeros((3, 32), np.float16)
+        w2[0, 0], w2[0, 1] = 1.0, -1.0                               # relu(f) - relu(-f) = f
+        out32, out64 = oracle.infer(one, table, I.pack_weights([w1, w2]), None, pos, nrm, want_f64=True)
+        np.testing.assert_allclose(out64[:, 0], enc[:, c], atol=1e-15)
+    weights, biases = I.make_mlp(spec, 4, bias_scale=0.1)
+    h = enc.copy()
+    for j, (w, b) in enumerate(zip(weights, biases)):
+        h = h @ w.astype(np.float64).T + b.astype(np.float64)
+        if j + 1 < len(weights):
+            h = np.maximum(h, 0.0)
+    out32, out64 = oracle.infer(spec, table, I.pack_weights(weights), I.pack_biases(biases), pos, nrm, want_f64=True)
+    np.testing.assert_allclose(out64, h, rtol=0, atol=1e-11)
+
+
 # ------------------------------------------------------------------ SH-16
 def _sh16_scipy(n):
     """Real orthonormal SH, bands 0..3, index l(l+1)+m, no Condon-Shortley sign, from scipy's complex Y_l^m."""
