@@ -49,6 +49,7 @@ def _env_int(name, default):
 
 
 PAPER_LEVELS, PAPER_WIDTH = 8, 64        # --paper-levels / --paper-width (workload "paper")
+PAPER_DIR_BANDS = 0                      # --paper-dir-bands: frequency bands on the direction, 0 or 4
 # PAPER.md:383-389 (Table 1, RTX 4090, full HD): ms per frame by (grid levels, width)
 PAPER_TABLE1_MS = {(0, 16): 0.19, (0, 32): 0.20, (0, 64): 0.25, (2, 64): 0.31, (4, 64): 0.67, (6, 64): 1.06, (8, 64): 1.35}
 PAPER_TABLE1_HALF_MS = {(0, 16): 0.029, (0, 32): 0.031, (0, 64): 0.069, (2, 64): 0.088, (4, 64): 0.18, (6, 64): 0.26, (8, 64): 0.37}
@@ -62,6 +63,8 @@ def make_workload(name: str, frame: int, with_params: bool = True):
         spec, param = I.spec_param(), [0.625]
     elif name == "paper":
         spec = I.spec_paper(paper_levels, paper_width) if paper_levels else I.spec_paper_pe(paper_width)
+        if PAPER_DIR_BANDS:
+            spec = I.spec_paper_dirfreq(paper_levels, paper_width, PAPER_DIR_BANDS)
         param = None
     else:
         spec, param = I.spec_fullhd(), None
@@ -82,6 +85,8 @@ def make_workload(name: str, frame: int, with_params: bool = True):
                     "the configs[1] G-buffer, %.1f%% background texels"
                     % (paper_width, paper_levels or "-", "F=4, scale sqrt 2, T=2^17" if paper_levels else
                        "eight-band positional encoding", 100 * masked))
+            if PAPER_DIR_BANDS:
+                desc += "; direction = raw vector + %d frequency bands per axis" % PAPER_DIR_BANDS
     return (spec, table, I.pack_weights(w) if with_params else None, I.pack_biases(b) if with_params else None, pos, nrm,
             param, desc, masked)
 
@@ -514,7 +519,7 @@ def run_ours(args):
         # = 1.536 Gqueries/s -- another machine's, context not target
         "vs_baseline": (value / (N_TEXELS / ((PAPER_TABLE1_HALF_MS if args.half else PAPER_TABLE1_MS)[(PAPER_LEVELS, PAPER_WIDTH)]
                                              * 1e-3) / 1e9))
-        if (args.workload == "paper" and world == 1 and (PAPER_LEVELS, PAPER_WIDTH) in PAPER_TABLE1_MS) else None,
+        if (args.workload == "paper" and world == 1 and (PAPER_LEVELS, PAPER_WIDTH) in PAPER_TABLE1_MS and not PAPER_DIR_BANDS) else None,
         "dtype": "f16 operands / f32 accumulate (index path: f32 + u32)", "data": "synthetic",
         "config": {"workload": args.workload, "description": desc, "model": _model_str(spec),
                    "texels_per_gpu_per_step": n, "masked_fraction": masked, "parallelism": "dp%d (model replicated by one "
@@ -1060,6 +1065,8 @@ def main():
                     "the 5.4 MB budget of PAPER.md:462 in the 10 x 4 x 10 m room)")
     ap.add_argument("--paper-levels", type=int, default=8, choices=[0, 2, 4, 6, 8], help="workload paper: grid levels (0 = none)")
     ap.add_argument("--paper-width", type=int, default=64, choices=[16, 32, 64])
+    ap.add_argument("--paper-dir-bands", type=int, default=0, choices=[0, 4],
+                    help="workload paper: frequency bands per axis on top of the raw direction (grid models, width 64)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cold-steps", type=int, default=10, help="launches of the cold-L2 variant (0 = skip)")
     ap.add_argument("--no-compact-e2e", action="store_true", help="skip the end-to-end legs on the compact G-buffer formats")
@@ -1083,8 +1090,8 @@ def main():
         args.warmup = 0 if args.warmup is None else args.warmup
         run_dry(args)
         return
-    global PAPER_LEVELS, PAPER_WIDTH
-    PAPER_LEVELS, PAPER_WIDTH = args.paper_levels, args.paper_width
+    global PAPER_LEVELS, PAPER_WIDTH, PAPER_DIR_BANDS
+    PAPER_LEVELS, PAPER_WIDTH, PAPER_DIR_BANDS = args.paper_levels, args.paper_width, args.paper_dir_bands
     if args.probe_patterns:
         run_probe_patterns(args)
         return

@@ -98,12 +98,15 @@ typedef struct {
     uint32_t hidden_width;        /* 32, 64 or 128 (F = 4: 32 or 64)                                */
     uint32_t out_activation;      /* NIV_OUT_*                                                      */
     int32_t  device;              /* CUDA device ordinal                                            */
+    uint32_t dir_frequencies;     /* sh_degree 0 only: sin/cos bands of frequency encoding per axis appended to the raw
+                                     direction ("raw 3-vector (plus optional frequency)", 211-214; DESIGN.md
+                                     3.8): 3 + 6 * dir_frequencies direction inputs.  0 (the paper's default) or 4      */
 } niv_config;
 
 /* What niv_create derived from the configuration (for tests, benchmarks and roofline arithmetic). */
 typedef struct {
     uint32_t struct_size;
-    uint32_t in_dim;                       /* L*F + (16 | 3) + 2*n_frequencies*n_params             */
+    uint32_t in_dim;                       /* L*F + (16 | 3 + 6*dir_frequencies) + 2*n_frequencies*n_params */
     uint32_t resolution[NIV_MAX_LEVELS];   /* N_l                                                   */
     uint32_t is_dense[NIV_MAX_LEVELS];     /* 1: dense index, 0: spatial hash (reading #4)          */
     uint64_t table_bytes;                  /* L * T * F * 2                                         */
@@ -131,7 +134,7 @@ typedef struct {
  * Errors: NULL / wrong struct_size / api_version / degenerate AABB / zero resolution -> NIV_ERR_INVALID_ARG;
  * a shape this build has no kernel for -> NIV_ERR_UNSUPPORTED.  Two model families have kernels: BASELINE.json's
  * (F = 2, sh_degree 4, L = 1..16, width 32/64/128) and the paper's own (F = 4, sh_degree 0,
- * L = 1..8, width 32/64; "the number of levels varies between 2 and 8") plus its grid-less models (L = 0, sh_degree 0, width 16/32/64, no table: table_fp16
+ * L = 1..8, width 32/64; "the number of levels varies between 2 and 8"; with dir_frequencies = 4: width 64) plus its grid-less models (L = 0, sh_degree 0, width 16/32/64, no table: table_fp16
  * may be NULL with table_bytes 0); all with n_hidden_layers 1..3, n_params 0..2, n_frequencies 8.
  * Shape errors are raised here, never at inference. */
 int niv_create(const niv_config *cfg, niv_model **out);
@@ -243,7 +246,8 @@ int niv_infer_host_packed(niv_model *m, int gbuf_format, const void *gbuf_a, con
                           int out_format, void *out, size_t n, void *stream);
 /* Debug: niv_infer, and besides `out` every texel's layer-1 A row as the FUSED kernel built it (the 32-bit words the
  * tensor core reads: L*F/2 words of fp16 latent pairs -- 24 words of positional encoding for the grid-less models --
- * then the direction (8 words SH-16, or (x, y | z, 0)), zero-padded to a multiple of 8 words = row_words).  arow is
+ * then the direction (8 words SH-16, or (x, y | z, 0), or with dir_frequencies the 3 + 6 B values in consecutive
+ * pairs), zero-padded to a multiple of 8 words = row_words).  arow is
  * device, [n][row_words] uint32; rows of background texels hold zeros.  row_words other than that -> NIV_ERR_INVALID_ARG.
  * For feature-level parity of the fused path (cell-block levels, packed-fp16 blend) in every model family. */
 int niv_debug_arow(niv_model *m, const float *pos, const float *nrm, const float *param, float *out,

@@ -133,8 +133,15 @@ __global__ void __launch_bounds__(128) niv_debug_kernel(const __grid_constant__ 
         const uint32_t o = L ? P.n_features * L : 48u;
         uint32_t dd;
         if (P.raw_dir) {
-            dd = 3;
+            dd = 3 + 6 * P.dir_freq;
             for (int k = 0; k < 3; ++k) feat[i * P.in_dim + o + k] = masked ? 0.f : nv[k];
+            for (uint32_t d = 0; d < 3; ++d)         // accurate per-band sincospi (the fused path doubles angles)
+                for (uint32_t k = 0; k < P.dir_freq; ++k) {
+                    float sn, cs;
+                    sincospif(nv[d] * (float)(1u << k), &sn, &cs);
+                    feat[i * P.in_dim + o + 3 + 2 * (P.dir_freq * d + k)] = masked ? 0.f : sn;
+                    feat[i * P.in_dim + o + 3 + 2 * (P.dir_freq * d + k) + 1] = masked ? 0.f : cs;
+                }
         } else {
             dd = 16;
             float sh[16];
@@ -427,12 +434,12 @@ static int setup_kernel(niv_model* m, FusedKernel& k, int tmem_cols, const char*
 // levels; a sixth would take 57 MB); the paper's family (F = 4, 64-byte blocks) four (its 8-level model: 0.1093 ms
 // without, 0.0998 with four, 0.119 with five) -- profiles/r02_cells.md
 constexpr int cell_levels_of(int L, int F) { return F == 4 ? (L < 4 ? L : 4) : (L < 5 ? L : 5); }
-template <int W, int L, int F, bool RAWDIR, bool O, int NPT, bool IMG, bool C, bool PK = false>
+template <int W, int L, int F, bool RAWDIR, bool O, int NPT, bool IMG, bool C, bool PK = false, int DB = 0>
 static fused_fn fused_inst() {
     // levels per gather batch (two batches in flight): BASELINE.json's family four = 32 gathers; the paper's family
     // (8-byte entries) two = 32 registers
     constexpr int NB = L == 0 ? 1 : F == 4 ? 2 : 4;
-    return niv_fused_kernel<W, L, NB, F, RAWDIR, O, NPT, IMG, C ? cell_levels_of(L, F) : 0, PK>;
+    return niv_fused_kernel<W, L, NB, F, RAWDIR, O, NPT, IMG, C ? cell_levels_of(L, F) : 0, PK, DB>;
 }
 template <int W, bool O, int NPT, bool IMG, bool C, bool PK = false>
 static fused_fn pick_levels_f2(uint32_t L) {        // BASELINE.json's family: F = 2, SH-16
@@ -444,19 +451,23 @@ static fused_fn pick_levels_f2(uint32_t L) {        // BASELINE.json's family: F
         default: return nullptr;
     }
 }
-template <int W, bool O, bool C, bool PK = false>
+template <int W, bool O, bool C, bool PK = false, int DB = 0>
 static fused_fn pick_levels_f4(uint32_t L) {        // the paper's own family: F = 4, raw direction
     switch (L) {
-        case 2: return fused_inst<W, 2, 4, true, O, 0, false, C, PK>();
-        case 4: return fused_inst<W, 4, 4, true, O, 0, false, C, PK>();
-        case 6: return fused_inst<W, 6, 4, true, O, 0, false, C, PK>();
-        case 8: return fused_inst<W, 8, 4, true, O, 0, false, C, PK>();
+        case 2: return fused_inst<W, 2, 4, true, O, 0, false, C, PK, DB>();
+        case 4: return fused_inst<W, 4, 4, true, O, 0, false, C, PK, DB>();
+        case 6: return fused_inst<W, 6, 4, true, O, 0, false, C, PK, DB>();
+        case 8: return fused_inst<W, 8, 4, true, O, 0, false, C, PK, DB>();
         default: return nullptr;
     }
 }
 // PK: the variant that reads the compact G-buffer formats / writes fp16 (linear tiles; the grid models of both families)
 template <bool O, bool C, bool PK = false>
-static fused_fn pick_fused(uint32_t W, uint32_t L, uint32_t F) {
+static fused_fn pick_fused(uint32_t W, uint32_t L, uint32_t F, uint32_t dir_freq = 0) {
+    if (dir_freq) {                                 // frequency-encoded direction: the paper's family at width 64, device buffers
+        if constexpr (!O) return (F == 4 && W == 64 && dir_freq == 4) ? pick_levels_f4<64, false, C, PK, 4>(L) : nullptr;
+        else return nullptr;                        // (host buffers take niv_infer_host's staged path)
+    }
     if (L == 0)                                     // grid-less: positional encoding, no gathers
         return W == 16 ? fused_inst<16, 0, 2, true, O, 0, false, false, PK>() : W == 32 ? fused_inst<32, 0, 2, true, O, 0, false, false, PK>()
              : W == 64 ? fused_inst<64, 0, 2, true, O, 0, false, false, PK>() : nullptr;
@@ -537,6 +548,10 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     } else if (cfg->n_features == 4) {
         if (cfg->sh_degree != 0 || cfg->n_levels > 8 || cfg->hidden_width > 64) return NIV_ERR_UNSUPPORTED;
     } else return NIV_ERR_UNSUPPORTED;
+    // frequency-encoded direction: on top of the raw vector only; kernels for 4 bands, the paper's grid family, width 64
+    if (cfg->dir_frequencies && cfg->sh_degree != 0) return NIV_ERR_INVALID_ARG;
+    if (cfg->dir_frequencies && (cfg->dir_frequencies != 4 || cfg->n_levels == 0 || cfg->n_features != 4 || cfg->hidden_width != 64))
+        return NIV_ERR_UNSUPPORTED;
     // Any number of levels: the kernels are compiled for whole gather batches (multiples of 4 levels for F = 2, of 2 for
     // F = 4); a model with fewer levels runs the next larger kernel with DUMMY levels that read a block of zeros and meet
     // zero weight columns (their latent columns of W1 are zero in the packed blob), so they add exactly 0 to every sum.
@@ -612,7 +627,8 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     P.tmask = (uint32_t)(T - 1);
     P.n_features = cfg->n_features;
     P.raw_dir = cfg->sh_degree == 0 ? 1u : 0u;
-    P.enc_dim = (cfg->n_levels ? cfg->n_levels * cfg->n_features : 6u * cfg->n_frequencies) + (P.raw_dir ? 3u : 16u);
+    P.dir_freq = cfg->dir_frequencies;
+    P.enc_dim = (cfg->n_levels ? cfg->n_levels * cfg->n_features : 6u * cfg->n_frequencies) + (P.raw_dir ? 3u + 6u * P.dir_freq : 16u);
     P.in_dim = P.enc_dim + 2 * cfg->n_frequencies * cfg->n_params;
     P.n_params = cfg->n_params;
     P.n_layers = cfg->n_hidden_layers + 1;
@@ -690,23 +706,23 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
         rc = m->fused.fn ? setup_kernel(m, m->fused, 128, "fused_w128") : NIV_ERR_UNSUPPORTED;
     } else {
         const int tmem_cols = W == 16 ? 64 : 128;        // D | A | ones in one allocation (niv_fused.cuh TMEM_COLS)
-        m->fused.fn = use_cells ? pick_fused<false, true>(W, Lk, cfg->n_features)
-                                : pick_fused<false, false>(W, Lk, cfg->n_features);
+        m->fused.fn = use_cells ? pick_fused<false, true>(W, Lk, cfg->n_features, cfg->dir_frequencies)
+                                : pick_fused<false, false>(W, Lk, cfg->n_features, cfg->dir_frequencies);
         m->fused.smem = smem_dev;
         rc = m->fused.fn ? setup_kernel(m, m->fused, tmem_cols, "fused") : NIV_ERR_UNSUPPORTED;
         if (rc == NIV_OK) {
-            m->fused_host.fn = pick_fused<true, false>(W, Lk, cfg->n_features);   // PCIe-bound: table gathers
+            m->fused_host.fn = pick_fused<true, false>(W, Lk, cfg->n_features, cfg->dir_frequencies);   // PCIe-bound: table gathers
             m->fused_host.smem = smem_host;
             rc = setup_kernel(m, m->fused_host, tmem_cols, "fused_host");
         }
         if (rc == NIV_OK) {
-            m->fused_pk.fn = use_cells ? pick_fused<false, true, true>(W, Lk, cfg->n_features)
-                                       : pick_fused<false, false, true>(W, Lk, cfg->n_features);
+            m->fused_pk.fn = use_cells ? pick_fused<false, true, true>(W, Lk, cfg->n_features, cfg->dir_frequencies)
+                                       : pick_fused<false, false, true>(W, Lk, cfg->n_features, cfg->dir_frequencies);
             m->fused_pk.smem = smem_dev;
             rc = setup_kernel(m, m->fused_pk, tmem_cols, "fused_packed");
         }
         if (rc == NIV_OK) {
-            m->fused_host_pk.fn = pick_fused<true, false, true>(W, Lk, cfg->n_features);
+            m->fused_host_pk.fn = pick_fused<true, false, true>(W, Lk, cfg->n_features, cfg->dir_frequencies);
             m->fused_host_pk.smem = smem_host;
             rc = setup_kernel(m, m->fused_host_pk, tmem_cols, "fused_host_packed");
         }
@@ -1177,7 +1193,7 @@ extern "C" int niv_debug_arow(niv_model* m, const float* pos, const float* nrm, 
     if (rc != NIV_OK) return rc > 0 ? NIV_OK : rc;
     if (!arow || !m->fused_pk.fn) return arow ? NIV_ERR_UNSUPPORTED : NIV_ERR_INVALID_ARG;
     const uint32_t hw = m->cfg.n_levels ? m->kernel_levels * m->cfg.n_features / 2 : 24u;
-    const uint32_t need = (hw + (m->cfg.sh_degree ? 8u : 2u) + 7u) / 8u * 8u;
+    const uint32_t need = (hw + (m->cfg.sh_degree ? 8u : (3u + 6u * m->cfg.dir_frequencies + 1u) / 2u) + 7u) / 8u * 8u;
     if (row_words != need) return NIV_ERR_INVALID_ARG;
     KParams P;
     rc = fill_params(m, param, P);

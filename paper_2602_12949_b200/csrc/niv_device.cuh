@@ -74,6 +74,7 @@ struct KParams {
     uint32_t tiles_x;           // ... cut into 32 x 4 pixel tiles, tiles_x = ceil(img_w / 32) per tile row (else 0)
     // niv_infer_shade (PACKED kernels): the deferred compose as the epilogue, out = albedo / pi * E + direct + emission
     // (Eq. 2, 403); [n][3] fp32 each, shade_albedo NULL = plain inference, the other two may be NULL (zero)
+    uint32_t dir_freq;          // raw_dir only: bands of frequency encoding appended to the direction (0 or 4)
     const float* shade_albedo;
     const float* shade_direct;
     const float* shade_emission;
@@ -327,6 +328,25 @@ __device__ __forceinline__ void posenc8_packed(float uu, uint32_t o[8]) {
         s = s2;
         c = c2;
         o[k] = pack_half2(s, c);
+    }
+}
+
+// frequency encoding of one direction component v in [-1, 1], B bands, as floats (sin, cos per band): one sincospi and
+// B - 1 angle doublings (error <= 2^(B-1) * 6e-8, far below the fp16 rounding of the A operand)
+template <int B>
+__device__ __forceinline__ void dirfreq(float v, float* o) {
+    float s, c;
+    sincospif(v, &s, &c);
+    o[0] = s;
+    o[1] = c;
+#pragma unroll
+    for (int k = 1; k < B; ++k) {
+        const float s2 = 2.0f * s * c;
+        const float c2 = fmaf(-2.0f * s, s, 1.0f);
+        s = s2;
+        c = c2;
+        o[2 * k] = s;
+        o[2 * k + 1] = c;
     }
 }
 

@@ -32,7 +32,9 @@ __device__ __forceinline__ uint32_t pack_relu_half2(float lo, float hi) {
 // PACKED: the caller's buffers are in one of the compact G-buffer / output formats (P.gbuf_fmt, P.out_fmt: a uniform
 // run-time switch per tile); false = fp32 x 3 in and out with no trace of the switch in the code (it cost the headline
 // kernel 1.5 %: its level loop sits at the register cap and every live value more changes the schedule)
-template <int WIDTH, int L, int NB, int F, bool RAWDIR, bool OUT128, int NPT, bool IMG, int NC, bool PACKED>
+// DIRB (RAWDIR only): bands of frequency encoding appended to the raw direction: the row holds
+// the 3 + 6 DIRB direction values in consecutive fp16 pairs, the column order of W1
+template <int WIDTH, int L, int NB, int F, bool RAWDIR, bool OUT128, int NPT, bool IMG, int NC, bool PACKED, int DIRB = 0>
 __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_fused_kernel(
                                                                const __grid_constant__ KParams P,
                                                                const float* __restrict__ pos,
@@ -47,7 +49,8 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
     constexpr int NG = L / NB;
     constexpr int HW = L ? L * F / 2 : 24;            // 32-bit words of hash latents in one A row (L = 0: the
                                                       // 3 x 8 (sin, cos) pairs of the positional encoding)
-    constexpr int DW = RAWDIR ? 2 : 8;                // ... of the direction input: (x, y | z, 0) or SH-16
+    static_assert(DIRB == 0 || RAWDIR, "frequency bands ride on the raw direction");
+    constexpr int DW = RAWDIR ? (3 + 6 * DIRB + 1) / 2 : 8;   // ... of the direction input: (x, y | z, 0) [+ bands] or SH-16
     constexpr int AW = (HW + DW + 7) / 8 * 8;         // ... of the position + direction part of a layer-1 A row
     constexpr int AWT = AW + 8 * NPT;                 // ... of the whole row (K1 = 2 * AWT)
     static_assert(AWT <= 40 && A_COL + AWT <= ONES_COL, "layer-1 A row must end before the ones chunk");
@@ -200,7 +203,15 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
             float u[3];
             normalise(P, p, u);
             auto encode_direction = [&]() {
-                if (RAWDIR) {                         // the paper's model: the direction itself
+                if constexpr (RAWDIR && DIRB > 0) {   // ... followed by its frequency encoding, axis after axis
+                    float dv[2 * DW];
+                    dv[0] = nv[0]; dv[1] = nv[1]; dv[2] = nv[2];
+                    dv[2 * DW - 1] = 0.0f;
+#pragma unroll
+                    for (int d = 0; d < 3; ++d) dirfreq<DIRB>(nv[d], dv + 3 + 2 * DIRB * d);
+#pragma unroll
+                    for (int k = 0; k < DW; ++k) a[HW + k] = pack_half2(dv[2 * k], dv[2 * k + 1]);
+                } else if (RAWDIR) {                  // the paper's model: the direction itself
                     a[HW] = pack_half2(nv[0], nv[1]);
                     a[HW + 1] = pack_half2(nv[2], 0.0f);
                 } else {

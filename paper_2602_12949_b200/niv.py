@@ -52,7 +52,7 @@ class NivConfig(C.Structure):
         ("aabb_min", C.c_float * 3), ("aabb_max", C.c_float * 3),
         ("sh_degree", C.c_uint32), ("n_params", C.c_uint32), ("n_frequencies", C.c_uint32),
         ("n_hidden_layers", C.c_uint32), ("hidden_width", C.c_uint32), ("out_activation", C.c_uint32),
-        ("device", C.c_int32),
+        ("device", C.c_int32), ("dir_frequencies", C.c_uint32),
     ]
 
 
@@ -158,6 +158,7 @@ def make_config(spec, device: int = 0) -> NivConfig:
     cfg.n_hidden_layers = spec.n_hidden_layers
     cfg.hidden_width = spec.hidden_width
     cfg.out_activation = spec.out_activation
+    cfg.dir_frequencies = getattr(spec, "dir_frequencies", 0)
     cfg.device = device
     return cfg
 
@@ -371,7 +372,7 @@ class NivModel:
     def arow_words(self) -> int:
         """32-bit words of one layer-1 A row of the fused kernel (include/niv.h niv_debug_arow)."""
         hw = self.info.kernel_levels * self.spec.n_features // 2 if self.spec.n_levels else 24
-        return (hw + (8 if self.spec.sh_degree else 2) + 7) // 8 * 8
+        return (hw + (8 if self.spec.sh_degree else (3 + 6 * getattr(self.spec, "dir_frequencies", 0) + 1) // 2) + 7) // 8 * 8
 
     def debug_arow(self, pos, nrm, out, arow, param=None, stream=None):
         """niv_infer + the fused kernel's layer-1 A rows: arow device int32 [n][arow_words()]."""

@@ -368,6 +368,39 @@ def test_paper_family_parity(torch_cuda, niv, oracle, L, width):
     m.close()
 
 
+@pytest.mark.parametrize("L", [8, 4, 2, 3])
+def test_paper_family_frequency_encoded_direction(torch_cuda, niv, oracle, L):
+    """SURVEY 8(f1) "raw or frequency-encoded direction": four bands per axis behind
+    the raw vector, 27 direction inputs; L = 3 runs the 4-level kernel with a dummy level (the direction columns move)."""
+    spec = I.spec_paper_dirfreq(L, 64, 4)
+    case = Case(spec, 300 + L, table_amp=0.1, bias_scale=0.05)
+    pos, nrm = _queries(spec, 148 * 128 + 45, 23, coherent=(L == 8))
+    nrm[3] = 0.0
+    nrm[4] = (1.0, 0.0, 0.0)
+    nrm[5] = (0.0, -1.0, 0.0)
+    m = case.gpu_model(niv)
+    assert m.info.in_dim == 4 * L + 27
+    ref = _check_debug(torch_cuda, oracle, m, case, pos, nrm)
+    assert ref["features"].shape[1] == 4 * L + 27
+    got = _gpu_infer(torch_cuda, m, pos, nrm)
+    want = oracle.infer(spec, case.table, case.wblob, case.bblob, pos, nrm)
+    _check_irradiance(got, want, nrm, pos, scale=max(1.0, float(want.max() - want.min())))
+    # the bands matter: the same weights on a model without them would not even load (sizes differ); a sign flip of the
+    # normal changes the result through the sin bands as well as through the raw vector
+    m.close()
+
+
+def test_frequency_encoded_direction_error_codes(torch_cuda, niv):
+    import dataclasses
+    for bad, code in ((dataclasses.replace(I.spec_paper_dirfreq(8, 64, 4), dir_frequencies=3), niv.NIV_ERR_UNSUPPORTED),
+                      (I.spec_paper_dirfreq(8, 32, 4), niv.NIV_ERR_UNSUPPORTED),
+                      (dataclasses.replace(I.spec_paper_pe(64), dir_frequencies=4), niv.NIV_ERR_UNSUPPORTED),
+                      (dataclasses.replace(I.spec_fullhd(), dir_frequencies=4), niv.NIV_ERR_INVALID_ARG)):
+        with pytest.raises(niv.NivError) as e:
+            niv.NivModel(bad)
+        assert e.value.code == code
+
+
 def test_paper_family_full_hd_sampled(torch_cuda, niv, oracle):
     torch = torch_cuda
     spec = I.spec_paper(8, 64)
@@ -460,7 +493,8 @@ def test_cell_block_levels_are_exact_copies(torch_cuda, niv, oracle, monkeypatch
     m_off.close()
 
 
-@pytest.mark.parametrize("which", ["fullhd", "tiny", "param", "paper8", "paper6_w32", "paper2", "gridless16", "gridless64"])
+@pytest.mark.parametrize("which", ["fullhd", "tiny", "param", "paper8", "paper6_w32", "paper2", "gridless16", "gridless64",
+                                   "paper8_dirfreq", "paper2_dirfreq"])
 def test_fused_kernel_features_match_the_oracle(torch_cuda, niv, oracle, which):
     """Feature-level parity of the FUSED path ("the parity tolerance cannot see encoding bugs on its own"): the
     layer-1 A row the fused kernel hands to the tensor core (niv_debug_arow) against the oracle's features, on a loud
@@ -470,7 +504,8 @@ def test_fused_kernel_features_match_the_oracle(torch_cuda, niv, oracle, which):
     torch = torch_cuda
     spec = {"fullhd": I.spec_fullhd(), "tiny": I.spec_tiny(), "param": I.spec_param(), "paper8": I.spec_paper(8, 64),
             "paper6_w32": I.spec_paper(6, 32), "paper2": I.spec_paper(2, 64), "gridless16": I.spec_paper_pe(16),
-            "gridless64": I.spec_paper_pe(64)}[which]
+            "gridless64": I.spec_paper_pe(64), "paper8_dirfreq": I.spec_paper_dirfreq(8, 64, 4),
+            "paper2_dirfreq": I.spec_paper_dirfreq(2, 64, 4)}[which]
     case = Case(spec, 31, table_amp=1.0, bias_scale=0.1)
     n = 9001
     pos, nrm = _queries(spec, n, 12, coherent=False)
@@ -495,7 +530,7 @@ def test_fused_kernel_features_match_the_oracle(torch_cuda, niv, oracle, which):
     assert masked[11] and np.all(got[masked] == 0)
     act = ~masked
     n_lat = spec.n_levels * spec.n_features if spec.n_levels else 48
-    n_dir = 3 if spec.sh_degree == 0 else 16
+    n_dir = spec.dir_dim
     tmax = float(np.abs(case.table.astype(np.float64)).max()) if spec.n_levels else 1.0
     lat_err = np.abs(got[act, :n_lat] - want[act, :n_lat])
     if spec.n_levels:
@@ -504,7 +539,8 @@ def test_fused_kernel_features_match_the_oracle(torch_cuda, niv, oracle, which):
     else:                                                           # sin / cos bands: fp16 rounding + angle doubling
         assert lat_err.max() <= 2.0 ** -11 + 2e-5
     d_got, d_want = got[act, n_lat:n_lat + n_dir], want[act, n_lat:n_lat + n_dir]
-    assert np.all(np.abs(d_got - d_want) <= 2.0 ** -11 * np.maximum(np.abs(d_want), 2.0 ** -14) + 1e-7)
+    slack = 2e-6 if spec.dir_frequencies else 1e-7                  # (bands: + the angle-doubling error, 2^3 x 6e-8 and sincospi's)
+    assert np.all(np.abs(d_got - d_want) <= 2.0 ** -11 * np.maximum(np.abs(d_want), 2.0 ** -14) + slack)
     assert np.all(got[:, n_lat + n_dir:] == 0)                      # zero padding up to the K-step
     m.close()
 
