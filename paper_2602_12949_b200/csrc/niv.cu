@@ -401,12 +401,18 @@ static bool env_flag(const char* name, bool dflt) {
 // answers 1 for kernels that allocate tensor memory on driver 580 -- measured, DESIGN.md section 6 -- so it is not used.)
 static int setup_kernel(niv_model* m, FusedKernel& k, int tmem_cols, const char* name) {
     if (!k.fn) return NIV_OK;
-    NIV_CUDA(cudaFuncSetAttribute(k.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.smem));
     cudaFuncAttributes fa;
     NIV_CUDA(cudaFuncGetAttributes(&fa, k.fn));
     cudaDeviceProp prop;
     NIV_CUDA(cudaGetDeviceProperties(&prop, m->cfg.device));
     const int regs_per_cta = ((fa.numRegs + 7) / 8 * 8) * kTile;
+    // 96 columns = two allocations per CTA (64, then 32): eight CTAs holding 64 each and waiting for 32 would wait for
+    // ever, so such a kernel must never have eight CTAs on an SM (launches overlap: the grid size alone does not say).
+    // Today's kernels take >= 72 registers (seven CTAs); should one drop to <= 64, its shared memory is padded to an
+    // eighth of the SM's so that seven fit at most.
+    if (tmem_cols == 96 && prop.regsPerMultiprocessor / regs_per_cta >= 8)
+        k.smem = std::max<uint32_t>(k.smem, (uint32_t)prop.sharedMemPerMultiprocessor / 8 + 128);
+    NIV_CUDA(cudaFuncSetAttribute(k.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k.smem));
     const int smem_per_cta = (int)round_up(k.smem + (uint32_t)fa.sharedSizeBytes + (uint32_t)prop.reservedSharedMemPerBlock, 128);
     int blocks = prop.regsPerMultiprocessor / regs_per_cta;
     blocks = std::min(blocks, (int)prop.sharedMemPerMultiprocessor / smem_per_cta);
@@ -433,13 +439,17 @@ static int setup_kernel(niv_model* m, FusedKernel& k, int tmem_cols, const char*
 // how many: BASELINE.json's family (F = 2) five (0.1673 -> 0.1613 / 0.1585 / 0.1567 ms per full-HD frame with 3 / 4 / 5
 // levels; a sixth would take 57 MB); the paper's family (F = 4, 64-byte blocks) four (its 8-level model: 0.1093 ms
 // without, 0.0998 with four, 0.119 with five) -- profiles/r02_cells.md
+// the bias K-step's ones tile in shared memory instead of tensor memory (niv_fused.cuh OS): the paper's family and its
+// grid-less models at width 32 / 64, whose 56..106 registers allow five to eight CTAs per SM once a tile takes 96 / 64
+// tensor-memory columns instead of 128; BASELINE.json's family sits at the register cap with four CTAs either way
+constexpr bool ones_in_smem(uint32_t W, uint32_t L, uint32_t F) { return (F == 4 || L == 0) && (W == 32 || W == 64); }
 constexpr int cell_levels_of(int L, int F) { return F == 4 ? (L < 4 ? L : 4) : (L < 5 ? L : 5); }
 template <int W, int L, int F, bool RAWDIR, bool O, int NPT, bool IMG, bool C, bool PK = false, int DB = 0>
 static fused_fn fused_inst() {
     // levels per gather batch (two batches in flight): BASELINE.json's family four = 32 gathers; the paper's family
     // (8-byte entries) two = 32 registers
     constexpr int NB = L == 0 ? 1 : F == 4 ? 2 : 4;
-    return niv_fused_kernel<W, L, NB, F, RAWDIR, O, NPT, IMG, C ? cell_levels_of(L, F) : 0, PK, DB>;
+    return niv_fused_kernel<W, L, NB, F, RAWDIR, O, NPT, IMG, C ? cell_levels_of(L, F) : 0, PK, DB, ones_in_smem(W, L, F)>;
 }
 template <int W, bool O, int NPT, bool IMG, bool C, bool PK = false>
 static fused_fn pick_levels_f2(uint32_t L) {        // BASELINE.json's family: F = 2, SH-16
@@ -686,6 +696,8 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     if (e != cudaSuccess) { g_last_cuda_error = (int)e; (void)cudaGetLastError(); delete m; return NIV_ERR_CUDA; }
     if (prop.major != 10) { delete m; return NIV_ERR_UNSUPPORTED; }           // sm_100a only; no fallback
     I.num_sms = (uint32_t)prop.multiProcessorCount;
+    const bool os = ones_in_smem(W, cfg->n_levels, cfg->n_features) && !want_mma_sync;
+    if (os) P.misc_off = P.ones_off + 2 * kTile * 16;    // weights | ones tile (4 KB, SS-form bias K-step) | barriers
     const uint32_t smem_dev = P.misc_off + 64, smem_host = smem_dev + 4 * 384;  // host variant: + output staging
     if (want_mma_sync && W == 64 && cfg->n_levels == 16 && cfg->n_features == 2 && cfg->n_hidden_layers == 2 &&
         cfg->n_params == 0) {
@@ -705,7 +717,8 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
         m->fused.smem = P.misc_off + 64;
         rc = m->fused.fn ? setup_kernel(m, m->fused, 128, "fused_w128") : NIV_ERR_UNSUPPORTED;
     } else {
-        const int tmem_cols = W == 16 ? 64 : 128;        // D | A | ones in one allocation (niv_fused.cuh TMEM_COLS)
+        // D | A | ones in one allocation (niv_fused.cuh TMEM_COLS); ones in shared memory: D 64 + A 32, or D 32 | A 32
+        const int tmem_cols = os ? (W == 64 ? 96 : 64) : W == 16 ? 64 : 128;
         m->fused.fn = use_cells ? pick_fused<false, true>(W, Lk, cfg->n_features, cfg->dir_frequencies)
                                 : pick_fused<false, false>(W, Lk, cfg->n_features, cfg->dir_frequencies);
         m->fused.smem = smem_dev;

@@ -34,7 +34,13 @@ __device__ __forceinline__ uint32_t pack_relu_half2(float lo, float hi) {
 // kernel 1.5 %: its level loop sits at the register cap and every live value more changes the schedule)
 // DIRB (RAWDIR only): bands of frequency encoding appended to the raw direction: the row holds
 // the 3 + 6 DIRB direction values in consecutive fp16 pairs, the column order of W1
-template <int WIDTH, int L, int NB, int F, bool RAWDIR, bool OUT128, int NPT, bool IMG, int NC, bool PACKED, int DIRB = 0>
+// OS (ones in shared memory): the (1, 1, 0, ...) A operand of the bias K-step is a 4 KB shared-memory tile read by an
+// SS-form MMA (as in niv_fused_w128.cuh) instead of 8 tensor-memory columns, so a tile needs D + A columns only:
+//   width 64: D [0, 64) and A [0, 32) in TWO allocations (64 + 32 = 96 columns: five CTAs per SM instead of four)
+//   width 32: D [0, 32) | A [32, 64) in one allocation of 64 (eight CTAs per SM)
+// For the kernels whose registers allow that many CTAs: the paper's family (F = 4) and its grid-less models.
+template <int WIDTH, int L, int NB, int F, bool RAWDIR, bool OUT128, int NPT, bool IMG, int NC, bool PACKED, int DIRB = 0,
+          bool OS = false>
 __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_fused_kernel(
                                                                const __grid_constant__ KParams P,
                                                                const float* __restrict__ pos,
@@ -44,8 +50,10 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
     static_assert(WIDTH <= 64, "A-in-TMEM kernel: D + A + ones must fit 128 columns");
     static_assert(NC <= L, "cell-block levels are the leading levels");
     // width 16 (the paper's smallest grid-less model): D 16 | A 32 | ones 8 fit 64 columns -> eight CTAs per SM
-    constexpr uint32_t TMEM_COLS = WIDTH == 16 ? 64 : 128, A_COL = WIDTH == 16 ? 16 : 64,
-                       ONES_COL = WIDTH == 16 ? 48 : NPT == 2 ? 104 : 96;
+    static_assert(!OS || ((WIDTH == 32 || WIDTH == 64) && NPT == 0), "ones in shared memory: width 32 / 64, no per-texel parameters");
+    constexpr bool OS64 = OS && WIDTH == 64;          // A in a second allocation of 32 columns
+    constexpr uint32_t TMEM_COLS = (OS || WIDTH == 16) ? 64 : 128, A_COL = OS64 ? 0 : OS ? 32 : WIDTH == 16 ? 16 : 64,
+                       ONES_COL = OS ? A_COL + 32 : WIDTH == 16 ? 48 : NPT == 2 ? 104 : 96;
     constexpr int NG = L / NB;
     constexpr int HW = L ? L * F / 2 : 24;            // 32-bit words of hash latents in one A row (L = 0: the
                                                       // 3 x 8 (sin, cos) pairs of the positional encoding)
@@ -53,13 +61,15 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
     constexpr int DW = RAWDIR ? (3 + 6 * DIRB + 1) / 2 : 8;   // ... of the direction input: (x, y | z, 0) [+ bands] or SH-16
     constexpr int AW = (HW + DW + 7) / 8 * 8;         // ... of the position + direction part of a layer-1 A row
     constexpr int AWT = AW + 8 * NPT;                 // ... of the whole row (K1 = 2 * AWT)
-    static_assert(AWT <= 40 && A_COL + AWT <= ONES_COL, "layer-1 A row must end before the ones chunk");
+    static_assert(AWT <= 40 && A_COL + AWT <= ONES_COL, "layer-1 A row must end before the ones chunk (OS: fit the A columns)");
     extern __shared__ __align__(1024) uint8_t smem[];
     uint8_t* sW = smem;
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + P.misc_off);
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2);
     uint32_t* s_tile = tmem_slot + 1;                 // [2]: the tile after next, handed from thread 0 to the CTA
     uint32_t* s_txy = s_tile + 2;                     // [2]: IMG: its (tile column | tile row << 16)
+    uint32_t* tmem_slot2 = s_txy + 2;                 // OS64: the A allocation
+    uint8_t* sOnes = smem + P.ones_off;               // OS: [2][128 rows][16 B], K columns 0..7 | 8..15 of the ones tile
 
     const uint32_t tid = threadIdx.x;
     const uint32_t warp = tid >> 5;
@@ -72,7 +82,19 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
         mbar_init(bar_mma, 1);
         mbar_fence_init();
     }
-    if (warp == 0) tmem_alloc(smem_u32(tmem_slot), TMEM_COLS);
+    if (warp == 0) {
+        if constexpr (OS64) {
+            tmem_alloc_keep(smem_u32(tmem_slot), 64);
+            tmem_alloc_keep(smem_u32(tmem_slot2), 32);
+            tmem_relinquish();
+        } else {
+            tmem_alloc(smem_u32(tmem_slot), TMEM_COLS);
+        }
+    }
+    if constexpr (OS) {                               // the bias K-step's A operand: (1, 1, 0, ..., 0) in every row
+        *reinterpret_cast<uint4*>(sOnes + tid * 16) = make_uint4(0x3C003C00u, 0u, 0u, 0u);
+        *reinterpret_cast<uint4*>(sOnes + 2048 + tid * 16) = make_uint4(0u, 0u, 0u, 0u);
+    }
     // dynamic tile scheduling: tile blockIdx.x is static, every further tile comes from a global counter, so a CTA
     // that drew cheap (background) tiles or a fast SM simply draws more of them and the grid drains together
     auto next_tile = [&](uint32_t after) -> uint32_t {
@@ -88,14 +110,18 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
     tc_fence_after_sync();
     const uint32_t tmem = *tmem_slot;
     const uint32_t lane_taddr = tmem + ((warp * 32u) << 16);
+    uint32_t tmem_a = tmem + A_COL;                   // first column of the A operand
+    if constexpr (OS64) tmem_a = *tmem_slot2;
+    const uint32_t lane_a = tmem_a + ((warp * 32u) << 16);
     if (tid == 0) {
         mbar_arrive_expect_tx(bar_w, P.wpack_bytes);
         bulk_g2s(sW_u32, P.wpack, P.wpack_bytes, bar_w);
     }
-    {   // the bias K-step's A operand: (1, 1, 0, ..., 0) in every row, written once
+    if constexpr (!OS) {   // the bias K-step's A operand: (1, 1, 0, ..., 0) in every row, written once
         uint32_t ones[8] = {0x3C003C00u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
         tmem_st_x8(lane_taddr + ONES_COL, ones);
     }
+    const uint64_t desc_ones = make_smem_desc(smem_u32(sOnes), 2048u, 128u);
     mbar_wait(bar_w, 0);
 
     // ---- a8: fold the per-call parameter encoding into layer 1's bias K-row (hi, lo) in shared memory
@@ -264,12 +290,12 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
             }
         }
         __syncwarp();
-        if constexpr (AW == 8) tmem_st_x8(lane_taddr + A_COL, a);
-        else tmem_st_x16(lane_taddr + A_COL, a);
-        if constexpr (AW == 24) tmem_st_x8(lane_taddr + A_COL + 16, a + 16);
-        if constexpr (AW == 32) tmem_st_x16(lane_taddr + A_COL + 16, a + 16);
-        if constexpr (NPT >= 1) tmem_st_x8(lane_taddr + A_COL + AW, a + AW);
-        if constexpr (NPT == 2) tmem_st_x8(lane_taddr + A_COL + AW + 8, a + AW + 8);
+        if constexpr (AW == 8) tmem_st_x8(lane_a, a);
+        else tmem_st_x16(lane_a, a);
+        if constexpr (AW == 24) tmem_st_x8(lane_a + 16, a + 16);
+        if constexpr (AW == 32) tmem_st_x16(lane_a + 16, a + 16);
+        if constexpr (NPT >= 1) tmem_st_x8(lane_a + AW, a + AW);
+        if constexpr (NPT == 2) tmem_st_x8(lane_a + AW + 8, a + AW + 8);
         tmem_st_wait();
         if (tid == 0) {
             s_tile[(it + 1) & 1] = tnn_mine;
@@ -296,8 +322,11 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
                 const uint32_t lo = desc_lo0[layer], step = 2u * N;
 #pragma unroll
                 for (uint32_t ks = 0; ks < ksteps_ct; ++ks)
-                    umma_f16_ts2(tmem, tmem + A_COL + ks * 8u, lo + ks * step, 0x4008u, idesc, ks > 0 ? 1u : 0u);
-                umma_f16_ts2(tmem, tmem + ONES_COL, lo + ksteps_ct * step, 0x4008u, idesc, 1u);        // + bias
+                    umma_f16_ts2(tmem, tmem_a + ks * 8u, lo + ks * step, 0x4008u, idesc, ks > 0 ? 1u : 0u);
+                if constexpr (OS)                                                                       // + bias
+                    umma_f16_ss(tmem, desc_ones, ((uint64_t)0x4008u << 32) | (uint64_t)(lo + ksteps_ct * step), idesc, 1u);
+                else
+                    umma_f16_ts2(tmem, tmem + ONES_COL, lo + ksteps_ct * step, 0x4008u, idesc, 1u);
                 umma_commit(bar_mma);
             }
             mbar_wait(bar_mma, phase);
@@ -317,8 +346,8 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
                         pk[h] = pack_relu_half2(__uint_as_float(r0[2 * h]), __uint_as_float(r0[2 * h + 1]));
                         pk[16 + h] = pack_relu_half2(__uint_as_float(r1[2 * h]), __uint_as_float(r1[2 * h + 1]));
                     }
-                    tmem_st_x16(lane_taddr + A_COL, pk);
-                    tmem_st_x16(lane_taddr + A_COL + 16, pk + 16);
+                    tmem_st_x16(lane_a, pk);
+                    tmem_st_x16(lane_a + 16, pk + 16);
                 } else if constexpr (WIDTH == 32) {
                     uint32_t r[32];
                     tmem_ld_x32(lane_taddr, r);
@@ -327,7 +356,7 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
 #pragma unroll
                     for (int h = 0; h < 16; ++h)
                         pk[h] = pack_relu_half2(__uint_as_float(r[2 * h]), __uint_as_float(r[2 * h + 1]));
-                    tmem_st_x16(lane_taddr + A_COL, pk);
+                    tmem_st_x16(lane_a, pk);
                 } else {                              // width 16
                     uint32_t r[16];
                     tmem_ld_x16(lane_taddr, r);
@@ -336,7 +365,7 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
 #pragma unroll
                     for (int h = 0; h < 8; ++h)
                         pk[h] = pack_relu_half2(__uint_as_float(r[2 * h]), __uint_as_float(r[2 * h + 1]));
-                    tmem_st_x8(lane_taddr + A_COL, pk);
+                    tmem_st_x8(lane_a, pk);
                 }
                 tmem_st_wait();
                 tc_fence_before_sync();
@@ -403,7 +432,10 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
     }
 
     __syncthreads();
-    if (warp == 0) tmem_dealloc(tmem, TMEM_COLS);
+    if (warp == 0) {
+        tmem_dealloc(tmem, TMEM_COLS);
+        if constexpr (OS64) tmem_dealloc(tmem_a, 32);
+    }
     if (tid == 0 && P.tile_ctr) {   // the last CTA to finish leaves the (tile, done) counter pair zero and reports the slot free
         __threadfence();
         if (atomicAdd(P.tile_ctr + 1, 1u) == gridDim.x - 1) {

@@ -64,7 +64,12 @@ __device__ __forceinline__ void tmem_alloc(uint32_t dst_smem, uint32_t ncols) { 
                  : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
 }
-// one block of 32 columns; the permit is given up once, after the CTA's last allocation (tmem_relinquish)
+// several allocations per CTA: the permit is given up once, after the CTA's last allocation (tmem_relinquish)
+__device__ __forceinline__ void tmem_alloc_keep(uint32_t dst_smem, uint32_t ncols) { // one full warp
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst_smem), "r"(ncols)
+                 : "memory");
+}
+// one block of 32 columns
 __device__ __forceinline__ void tmem_alloc32(uint32_t dst_smem) {                 // one full warp
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 32;" ::"r"(dst_smem) : "memory");
 }
