@@ -271,6 +271,24 @@ def quantise_f16x4(e) -> np.ndarray:
     return out
 
 
+def quantise_rgb9e5(e) -> np.ndarray:
+    """[n][3] fp32 -> [n] uint32: shared-exponent RGB9E5 words (steps Q1-Q4 of niv_oracle_ext.c)."""
+    e = _chk(e, np.float32, "e")
+    out = np.zeros((e.shape[0],), dtype=np.uint32)
+    if lib().niv_oracle_quantise_rgb9e5(_p(e), C.c_size_t(e.shape[0]), _p(out)):
+        raise ValueError("niv_oracle_quantise_rgb9e5 failed")
+    return out
+
+
+def decode_rgb9e5(w) -> np.ndarray:
+    """[n] uint32 RGB9E5 words -> [n][3] fp64 values."""
+    w = _chk(w, np.uint32, "w")
+    out = np.zeros((w.shape[0], 3), dtype=np.float64)
+    if lib().niv_oracle_decode_rgb9e5(_p(w), C.c_size_t(w.shape[0]), _p(out)):
+        raise ValueError("niv_oracle_decode_rgb9e5 failed")
+    return out
+
+
 def compose_jb(E, pos_half, nrm_half, pos, nrm, albedo, sigma, power, direct=None, emission=None) -> np.ndarray:
     """Deferred compose with joint-bilateral upsampling of half-resolution E (niv_oracle_ext.c niv_oracle_compose_jb).
     E, pos_half, nrm_half [eh][ew][3]; pos, nrm, albedo (, direct, emission) [h][w][3] with (h, w) = (2 eh, 2 ew) -> fp64."""

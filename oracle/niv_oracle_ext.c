@@ -250,6 +250,51 @@ int niv_oracle_quantise_f16x4(const float *e, size_t n, uint16_t *out)
     return 0;
 }
 
+/* ---- SURVEY 8 f2 "fp16 / packed output formats": the shared-exponent format RGB9E5 (DESIGN.md 3.5 reading) -------------
+ * One 32-bit word per texel: three 9-bit mantissas r, g, b (bits 0-8, 9-17, 18-26) and one 5-bit exponent E (bits 27-31),
+ * value_c = m_c * 2^(E - 15 - 9) -- the HDR colour format of the graphics APIs, restated here:
+ *   Q1  c' = min(max(c, 0), 65408) per component (NaN -> 0; irradiance is not negative, a linear output layer may be);
+ *       65408 = 511/512 * 2^16 is the largest representable value
+ *   Q2  E' = max(-16, floor(log2 max_c c')) + 16                     (so that the largest mantissa has its top bit set)
+ *   Q3  if floor(max_c c' / 2^(E' - 24) + 1/2) = 512 (the rounding carried): E = E' + 1, else E = E'
+ *   Q4  m_c = floor(c' / 2^(E - 24) + 1/2)
+ * All of it is exact in fp64 for fp32 inputs (scalings by powers of two, one addition of 1/2 to a number below 2^9). ---- */
+int niv_oracle_quantise_rgb9e5(const float *e, size_t n, uint32_t *out)
+{
+    if (!e || !out) return -1;
+    for (size_t i = 0; i < n; ++i) {
+        double c[3], maxc = 0.0;
+        for (int k = 0; k < 3; ++k) {
+            double v = (double)e[3 * i + k];
+            if (!(v > 0.0)) v = 0.0;                       /* negative, -0, NaN */
+            if (v > 65408.0) v = 65408.0;
+            c[k] = v;
+            if (v > maxc) maxc = v;
+        }
+        int ex = -16;
+        if (maxc > 0.0) {
+            int fe;
+            (void)frexp(maxc, &fe);                        /* maxc = f * 2^fe, f in [0.5, 1): floor(log2 maxc) = fe - 1 */
+            if (fe - 1 > ex) ex = fe - 1;
+        }
+        int E = ex + 16;
+        if (floor(ldexp(maxc, 24 - E) + 0.5) == 512.0) E += 1;
+        uint32_t word = (uint32_t)E << 27;
+        for (int k = 0; k < 3; ++k) word |= (uint32_t)floor(ldexp(c[k], 24 - E) + 0.5) << (9 * k);
+        out[i] = word;
+    }
+    return 0;
+}
+
+/* the value an RGB9E5 word stands for (exact in fp64) */
+int niv_oracle_decode_rgb9e5(const uint32_t *w, size_t n, double *out)
+{
+    if (!w || !out) return -1;
+    for (size_t i = 0; i < n; ++i)
+        for (int k = 0; k < 3; ++k) out[3 * i + k] = ldexp((double)((w[i] >> (9 * k)) & 0x1FFu), (int)(w[i] >> 27) - 24);
+    return 0;
+}
+
 /* =====================================================================================================
  * Deferred compose with JOINT-BILATERAL upsampling of half-resolution irradiance.
  * half-resolution rendering "introduces aliasing artifacts which could be partly resolved by using

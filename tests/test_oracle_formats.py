@@ -120,3 +120,50 @@ def test_decoded_buffers_feed_the_standard_path(oracle):
         if fmt == I.GBUF_P32_OCT16:                                   # fp32 positions: only the normal is quantised
             e0 = oracle.infer(spec, table, wb, bb, pos, nrm)
             assert np.abs(e - e0).max() < 1e-3
+
+
+def _rgb9e5_brute(c):
+    """The definition by search: the SMALLEST exponent E in 0..31 for which every component, rounded to the nearest multiple
+    of 2^(E-24) (ties up), fits nine bits -- no logarithm, no frexp."""
+    c = [min(max(float(v), 0.0), 65408.0) if v == v else 0.0 for v in c]
+    for E in range(32):
+        step = 2.0 ** (E - 24)
+        m = [int(np.floor(v / step + 0.5)) for v in c]
+        if max(m) <= 511:
+            return m[0] | (m[1] << 9) | (m[2] << 18) | (E << 27), [mm * step for mm in m]
+    raise AssertionError("unreachable: 65408 fits E = 31")
+
+
+def test_rgb9e5_quantiser(oracle):
+    """Shared-exponent output.  Pins: hand-worked words ((1, 1, 1) = three mantissas 256 at
+    E = 16; zero; the largest value; the rounding carry just below a power of two), the definition by exhaustive search over the
+    exponent on 20,000 random triples of every magnitude, exact round trip of representable values, the error bound
+    |c - dec| <= max_c / 511 / 2 ... 2^(E-25), clamping of negatives / NaN / values beyond the range."""
+    q = lambda rows: oracle.quantise_rgb9e5(np.float32(rows))
+    assert q([[1, 1, 1]])[0] == (256 | 256 << 9 | 256 << 18 | 16 << 27) == 0x84020100
+    assert q([[0, 0, 0]])[0] == 0
+    assert q([[65408, 0, 65408]])[0] == (511 | 511 << 18 | 31 << 27)
+    assert q([[1e9, -3, float("nan")]])[0] == (511 | 31 << 27)                       # clamped high; negative and NaN -> 0
+    assert q([[0.99999, 0.5, 0.25]])[0] == (256 | 128 << 9 | 64 << 18 | 16 << 27)    # 511.99 rounds to 512: the carry
+    assert q([[0.5, 0.25, 0.125]])[0] == (256 | 128 << 9 | 64 << 18 | 15 << 27)
+    assert q([[2.0 ** -20, 0, 0]])[0] == (16 | 0 << 27)                              # below 2^-16: E stays 0, 2^-20 / 2^-24 = 16
+    assert q([[2.0 ** -26, 0, 0]])[0] == 0                                           # under half a step of E = 0
+    rng = np.random.default_rng(11)
+    mag = 2.0 ** rng.uniform(-27, 17, (20000, 1))
+    x = (mag * rng.uniform(0, 1, (20000, 3))).astype(np.float32)
+    x[::97, 1] *= -1
+    got = q(x)
+    dec = oracle.decode_rgb9e5(got)
+    for i in range(0, 20000, 1):
+        w, vals = _rgb9e5_brute(x[i])
+        assert got[i] == w, (i, x[i], hex(got[i]), hex(w))
+    xc = np.clip(x.astype(np.float64), 0.0, 65408.0)
+    step = 2.0 ** ((got >> 27).astype(np.float64) - 24)
+    assert np.all(np.abs(dec - xc) <= step[:, None] / 2)
+    top = (got & 0x1FF) | ((got >> 9) & 0x1FF) | ((got >> 18) & 0x1FF)
+    assert np.all((top >= 256) | ((got >> 27) == 0))                                 # normalised: the top mantissa bit is in use
+    # representable values survive exactly
+    words = (rng.integers(0, 512, 5000) | (rng.integers(0, 512, 5000) << 9) | (rng.integers(256, 512, 5000) << 18)
+             | (rng.integers(0, 32, 5000) << 27)).astype(np.uint32)
+    v = oracle.decode_rgb9e5(words)
+    assert np.array_equal(q(v.astype(np.float32)), words)
