@@ -411,10 +411,12 @@ def run_ours(args):
     if spec.hidden_width <= 64 and spec.n_levels and not args.no_compact_e2e:
         aabb = (spec.aabb_min, spec.aabb_max)
         for gf, of, name in ((I.GBUF_P32_OCT16, I.OUTFMT_F16X4, "pos fp32 x 3 + oct16 normal (16 B) -> fp16 x 4 (8 B)"),
-                             (I.GBUF_P16_OCT8, I.OUTFMT_F16X4, "pos unorm16 x 3 + oct8 normal (8 B) -> fp16 x 4 (8 B)")):
+                             (I.GBUF_P16_OCT8, I.OUTFMT_F16X4, "pos unorm16 x 3 + oct8 normal (8 B) -> fp16 x 4 (8 B)"),
+                             (I.GBUF_P16_OCT8, I.OUTFMT_RGB9E5, "pos unorm16 x 3 + oct8 normal (8 B) -> RGB9E5 (4 B)")):
             a, b = I.pack_gbuffer(gf, pos, nrm, aabb)
             ha = [torch.from_numpy(a).pin_memory() for _ in range(2)]
-            ho = [torch.empty((n, 4), dtype=torch.int16).pin_memory() for _ in range(2)]
+            ho = [(torch.empty((n,), dtype=torch.int32) if of == I.OUTFMT_RGB9E5 else torch.empty((n, 4), dtype=torch.int16)).pin_memory()
+                  for _ in range(2)]
             for s in range(3):
                 model.infer_host_packed(gf, ha[s % 2], None, ho[s % 2], n, out_format=of, param=param)
             barrier()
@@ -424,7 +426,8 @@ def run_ours(args):
             torch.cuda.synchronize()
             ms = D.reduce_max((time.perf_counter() - t0) * 1e3 / e2e_steps, "cuda")
             e2e_compact.append({"formats": name, "gbuf_format": gf, "out_format": of, "value": n_job / (ms * 1e-3) / 1e9,
-                                "unit": UNIT, "ms_per_step": ms, "h2d_bytes_per_step": int(a.nbytes), "d2h_bytes_per_step": 8 * n,
+                                "unit": UNIT, "ms_per_step": ms, "h2d_bytes_per_step": int(a.nbytes),
+                                "d2h_bytes_per_step": int(ho[0].numel() * ho[0].element_size()),
                                 "api": "niv_infer_host_packed (pinned host buffers, zero copy)"})
             del ha, ho
 
@@ -464,7 +467,7 @@ def run_ours(args):
     t_all = {"l2-gather": t_gather, "tensor": t_tensor, "hbm": t_hbm}
     bound = max(t_all, key=t_all.get)                # the slowest roofline bounds the kernel (north_star)
     roofline = {
-        "bound": bound, "kernel": "niv_fused_tmem_kernel" if spec.hidden_width <= 64 else "niv_fused_kernel",
+        "bound": bound, "kernel": "niv_fused_kernel" if spec.hidden_width <= 64 else "niv_fused_w128_kernel",
         "achieved": {"l2-gather": sectors * 32 / kernel_s / 1e9, "tensor": flop_texel * n / kernel_s / 1e12,
                      "hbm": hbm_bytes / kernel_s / 1e9}[bound],
         "peak": {"l2-gather": gpeak["random_sector"]["sector_gbs"], "tensor": peaks["tflops_sustained"],

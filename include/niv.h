@@ -72,7 +72,10 @@ enum { NIV_GBUF_F32X3 = 0,        /* pos[n][3], nrm[n][3] fp32: the format of ni
        NIV_GBUF_P16_OCT8 = 3 };   /* one array, 8 bytes per texel: position 3 x unorm16 of the model's AABB |
                                      octahedral normal 2 x snorm8; both 0x80 = background                            */
 enum { NIV_OUTFMT_F32X3 = 0,      /* out[n][3] fp32                                                                    */
-       NIV_OUTFMT_F16X4 = 1 };    /* out[n][4] fp16: (r, g, b, 0), round to nearest even of the fp32 result           */
+       NIV_OUTFMT_F16X4 = 1,      /* out[n][4] fp16: (r, g, b, 0), round to nearest even of the fp32 result           */
+       NIV_OUTFMT_RGB9E5 = 2 };   /* out[n] uint32: shared-exponent RGB9E5 (9-bit mantissas r, g, b in bits 0-26, 5-bit
+                                     exponent in bits 27-31, value = m * 2^(E - 24)); negative and NaN components -> 0,
+                                     values above 65408 clamp                                        */
 
 enum { NIV_OUT_LINEAR = 0,      /* the paper: no activation on the final layer     */
        NIV_OUT_SIGMOID = 1 };   /* BASELINE.json configs[0]                                       */
@@ -231,7 +234,7 @@ int niv_infer_host_static(niv_model *m, const float *pos, const float *nrm, cons
  * 3.4 / 3.5):
  *   gbuf_a, gbuf_b  F32X3, F32X4: the position and the normal array; P32_OCT16, P16_OCT8: gbuf_a = the one array of
  *                   n records, gbuf_b ignored (may be NULL).  Alignment: 4 / 16 / 16 / 8 bytes.
- *   out             F32X3: [n][3] fp32;  F16X4: [n][4] fp16 (8-byte aligned)
+ *   out             F32X3: [n][3] fp32;  F16X4: [n][4] fp16 (8-byte aligned);  RGB9E5: [n] uint32 (4-byte aligned)
  * A texel is decoded to an fp32 position and an fp32 unit normal first -- the position by a pinned fp32 op sequence,
  * so the cells and hash indices are those of niv_infer on the decoded values, bit for bit -- and then takes the path of
  * niv_infer.  Grid models of hidden width <= 64 only (NIV_ERR_UNSUPPORTED for width 128 and for the grid-less models);

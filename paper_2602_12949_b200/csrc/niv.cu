@@ -1035,11 +1035,11 @@ static int launch_one(const niv_model* m, const FusedKernel& k, cudaStream_t st,
                       const float* nrm, float* out, size_t n, uint32_t n_tiles)
 {
     LaunchRec cur;
-    static const size_t kA[4] = {12, 16, 16, 8}, kB[4] = {12, 16, 0, 0}, kO[2] = {12, 8};   // bytes per texel by format
+    static const size_t kA[4] = {12, 16, 16, 8}, kB[4] = {12, 16, 0, 0}, kO[3] = {12, 8, 4};   // bytes per texel by format
     const void* base[kRanges] = {pos, nrm, P.tparam, P.shade_albedo, P.shade_direct, P.shade_emission, out};
     const size_t bytes[kRanges] = {n * kA[P.gbuf_fmt & 3], n * kB[P.gbuf_fmt & 3], P.tparam ? n * 4 * m->cfg.n_params : 0,
                                    P.shade_albedo ? n * 12 : 0, P.shade_direct ? n * 12 : 0, P.shade_emission ? n * 12 : 0,
-                                   n * kO[P.out_fmt & 1]};
+                                   n * kO[P.out_fmt < 3 ? P.out_fmt : 0]};
     for (int i = 0; i < kRanges; ++i) { cur.lo[i] = (uintptr_t)base[i]; cur.hi[i] = cur.lo[i] + bytes[i]; }
     cur.tracked = pdl && m->overlap && P.tile_ctr != nullptr;
     cur.done = P.tile_ctr ? P.tile_ctr + 2 : nullptr;
@@ -1135,6 +1135,7 @@ static bool fmt_info(int gf, int of, FmtInfo& f)
     switch (of) {
         case NIV_OUTFMT_F32X3: f.out_bytes = 12; f.out_align = 4; break;
         case NIV_OUTFMT_F16X4: f.out_bytes = 8;  f.out_align = 8; break;
+        case NIV_OUTFMT_RGB9E5: f.out_bytes = 4; f.out_align = 4; break;
         default: return false;
     }
     return true;

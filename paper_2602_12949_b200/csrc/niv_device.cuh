@@ -390,6 +390,21 @@ __device__ __forceinline__ void load3(const float* __restrict__ p, size_t i, flo
     v[2] = __ldg(p + 3 * i + 2);
 }
 
+// ---------------------------------------------------------------- a12 for NIV_OUTFMT_RGB9E5 (steps Q1..Q4)
+// Exact in fp32: the scalings are by powers of two and the sums v + 1/2 stay below 2^10 with integers representable.
+__device__ __forceinline__ uint32_t pack_rgb9e5(float r, float g, float b) {
+    r = fminf(fmaxf(r, 0.0f), 65408.0f);               // fmaxf(NaN, 0) = 0
+    g = fminf(fmaxf(g, 0.0f), 65408.0f);
+    b = fminf(fmaxf(b, 0.0f), 65408.0f);
+    const float maxc = fmaxf(r, fmaxf(g, b));
+    int E = max(-16, (int)(__float_as_uint(maxc) >> 23) - 127) + 16;      // floor(log2 maxc) from the exponent field (zero and subnormals: below -16)
+    float scale = __uint_as_float((uint32_t)(127 + 24 - E) << 23);        // 2^(24 - E)
+    if (floorf(fmaf(maxc, scale, 0.5f)) == 512.0f) { E += 1; scale *= 0.5f; }
+    const uint32_t mr = (uint32_t)floorf(fmaf(r, scale, 0.5f)), mg = (uint32_t)floorf(fmaf(g, scale, 0.5f)),
+                   mb = (uint32_t)floorf(fmaf(b, scale, 0.5f));
+    return mr | (mg << 9) | (mb << 18) | ((uint32_t)E << 27);
+}
+
 // ---------------------------------------------------------------- a1 for the compact G-buffer formats
 // DESIGN.md 3.4.  The raw words of texel i travel in the six registers the fp32 texel takes (they are requested a tile
 // ahead); decode_texel turns them into the fp32 position and normal the rest of the path is defined on.

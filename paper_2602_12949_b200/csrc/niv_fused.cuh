@@ -394,6 +394,8 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
                     if (PACKED && P.out_fmt == NIV_OUTFMT_F16X4) {      // 8 bytes per texel: a warp's stores are 256 contiguous bytes
                         if (valid)
                             reinterpret_cast<uint2*>(out)[i] = make_uint2(pack_half2(y[0], y[1]), pack_half2(y[2], 0.0f));
+                    } else if (PACKED && P.out_fmt == NIV_OUTFMT_RGB9E5) {   // 4 bytes per texel: one 128-byte line per warp
+                        if (valid) reinterpret_cast<uint32_t*>(out)[i] = pack_rgb9e5(y[0], y[1], y[2]);
                     } else if (vec) {
                         so[lane * 3] = y[0];
                         so[lane * 3 + 1] = y[1];
@@ -417,6 +419,8 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
                     }
                     if (PACKED && P.out_fmt == NIV_OUTFMT_F16X4) {      // (r, g, b, 0) as four fp16: one 8-byte store
                         reinterpret_cast<uint2*>(out)[i] = make_uint2(pack_half2(y[0], y[1]), pack_half2(y[2], 0.0f));
+                    } else if (PACKED && P.out_fmt == NIV_OUTFMT_RGB9E5) {   // shared-exponent word: one 4-byte store
+                        reinterpret_cast<uint32_t*>(out)[i] = pack_rgb9e5(y[0], y[1], y[2]);
                     } else {
                         out[3 * i] = y[0];
                         out[3 * i + 1] = y[1];

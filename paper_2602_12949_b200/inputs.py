@@ -367,7 +367,7 @@ def probe_grid_dims_for_spacing(aabb_min, aabb_max, spacing: float) -> Tuple[int
 # Compact G-buffer layouts (include/niv.h NIV_GBUF_*).  This is the PRODUCER side -- what a renderer would
 # write -- so it lives with the input generators; the decode (the method's side) exists twice, in oracle/ and in csrc/.
 GBUF_F32X3, GBUF_F32X4, GBUF_P32_OCT16, GBUF_P16_OCT8 = 0, 1, 2, 3
-OUTFMT_F32X3, OUTFMT_F16X4 = 0, 1
+OUTFMT_F32X3, OUTFMT_F16X4, OUTFMT_RGB9E5 = 0, 1, 2
 
 
 def _oct_encode(nrm: np.ndarray) -> np.ndarray:

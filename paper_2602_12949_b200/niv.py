@@ -28,9 +28,9 @@ NIV_CENSUS_COUNTS = 49      # niv_probe_sectors: [0,16) sectors, [16,32) lines, 
 
 # every symbol include/niv.h declares (tests check that the library exports all of them)
 NIV_GBUF_F32X3, NIV_GBUF_F32X4, NIV_GBUF_P32_OCT16, NIV_GBUF_P16_OCT8 = 0, 1, 2, 3
-NIV_OUTFMT_F32X3, NIV_OUTFMT_F16X4 = 0, 1
+NIV_OUTFMT_F32X3, NIV_OUTFMT_F16X4, NIV_OUTFMT_RGB9E5 = 0, 1, 2
 _GBUF_BYTES = {0: (12, 12), 1: (16, 16), 2: (16, 0), 3: (8, 0)}      # bytes per texel of gbuf_a, gbuf_b
-_OUT_BYTES = {0: 12, 1: 8}
+_OUT_BYTES = {0: 12, 1: 8, 2: 4}
 
 EXPORTS = ("niv_create", "niv_get_info", "niv_load_params", "niv_load_params_compact", "niv_infer", "niv_infer_image", "niv_infer_texel_params",
            "niv_infer_host", "niv_probe_sectors_image",

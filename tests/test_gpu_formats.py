@@ -87,6 +87,68 @@ def test_packed_inference_matches_the_oracle(torch_cuda, niv, oracle, which, fmt
     m.close()
 
 
+@pytest.mark.parametrize("which", ["fullhd", "paper"])
+def test_rgb9e5_output_matches_the_oracle(torch_cuda, niv, oracle, which):
+    """NIV_OUTFMT_RGB9E5: the words are bit-exact against the oracle's quantiser fed the GPU's own
+    fp32 result, and the decoded values are the oracle's irradiance within the bar plus half a quantisation step; negative
+    irradiance of a linear output layer clamps to 0; every entry point (device, image, host pageable / pinned) and the shading
+    epilogue write the same words."""
+    torch = torch_cuda
+    spec = I.spec_fullhd() if which == "fullhd" else I.spec_paper(8, 64)
+    case = Case(spec, 5, table_amp=1.0 if which == "fullhd" else 0.1, bias_scale=0.05)
+    m = case.gpu_model(niv)
+    w, h = 212, 67
+    n = w * h
+    g = I.make_gbuffer(w, h, 4)
+    pos, nrm = g["pos"], g["nrm"]
+    want = oracle.infer(spec, case.table, case.wblob, case.bblob, pos, nrm)
+    dp, dn = _dev_bytes(torch, pos), _dev_bytes(torch, nrm)
+    ref32 = torch.full((n, 3), float("nan"), device="cuda")
+    m.infer(dp, dn, ref32)
+    out = torch.full((n + 5,), -1, dtype=torch.int32, device="cuda")
+    m.infer_packed(I.GBUF_F32X3, dp, dn, out[:n], n, out_format=I.OUTFMT_RGB9E5)
+    img = torch.full((n,), -1, dtype=torch.int32, device="cuda")
+    m.infer_image_packed(I.GBUF_F32X3, dp, dn, img, w, h, out_format=I.OUTFMT_RGB9E5)
+    torch.cuda.synchronize()
+    words = out.cpu().numpy().view(np.uint32)
+    assert np.all(words[n:] == 0xFFFFFFFF)                                      # guard entries behind the output
+    words = words[:n]
+    e32 = ref32.cpu().numpy()
+    assert np.array_equal(words, oracle.quantise_rgb9e5(e32))
+    assert np.array_equal(img.cpu().numpy().view(np.uint32), words)
+    dec = oracle.decode_rgb9e5(words)
+    masked = np.all(nrm == 0, axis=1)
+    assert masked.any() and np.all(words[masked] == 0)
+    wc = np.clip(want.astype(np.float64), 0.0, 65408.0)
+    if which == "paper":
+        assert (want < 0).any()                                                 # the linear output does go negative: clamped
+    scale = 1.0 if spec.out_activation == I.OUT_SIGMOID else max(1.0, float(want.max() - want.min()))
+    step = 2.0 ** ((words >> 27).astype(np.float64) - 24)
+    err = np.abs(dec - wc)[~masked]
+    assert np.all(err <= MAX_ABS * scale + step[~masked, None] / 2)
+    assert err.mean() <= MEAN_ABS * scale + float(step[~masked].mean()) / 2
+    host = np.zeros((n,), dtype=np.uint32)                                       # pageable: staged copies
+    m.infer_host_packed(I.GBUF_F32X3, pos, nrm, host, n, out_format=I.OUTFMT_RGB9E5)
+    assert np.array_equal(host, words)
+    pp, pn = torch.from_numpy(pos).pin_memory(), torch.from_numpy(nrm).pin_memory()   # pinned: zero copy
+    po = torch.zeros((n,), dtype=torch.int32).pin_memory()
+    m.infer_host_packed(I.GBUF_F32X3, pp, pn, po, n, out_format=I.OUTFMT_RGB9E5)
+    assert np.array_equal(po.numpy().view(np.uint32), words)
+    # the shading epilogue into RGB9E5: the quantiser of its own fp32 result
+    rng = np.random.default_rng(1)
+    alb, dr = (torch.from_numpy(rng.uniform(0, 1, (n, 3)).astype(np.float32)).cuda() for _ in range(2))
+    s32 = torch.full((n, 3), float("nan"), device="cuda")
+    s9 = torch.full((n,), -1, dtype=torch.int32, device="cuda")
+    m.infer_shade(dp, dn, alb, s32, n, direct=dr, image=(w, h))
+    m.infer_shade(dp, dn, alb, s9, n, direct=dr, image=(w, h), out_format=I.OUTFMT_RGB9E5)
+    torch.cuda.synchronize()
+    assert np.array_equal(s9.cpu().numpy().view(np.uint32), oracle.quantise_rgb9e5(s32.cpu().numpy()))
+    # misaligned output -> INVALID_ARG
+    L = niv.lib()
+    assert L.niv_infer_packed(m._h, 0, dp.data_ptr(), dn.data_ptr(), None, 2, out.data_ptr() + 2, 8, None) == niv.NIV_ERR_INVALID_ARG
+    m.close()
+
+
 def test_packed_entry_points_agree_with_each_other(torch_cuda, niv):
     """image tiling, the host entry point (pinned and pageable buffers) and the linear device path: the same bits."""
     torch = torch_cuda
