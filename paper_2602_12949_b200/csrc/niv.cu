@@ -324,7 +324,7 @@ __global__ void __launch_bounds__(128) niv_sector_census_kernel(const __grid_con
 // =====================================================================================================
 using namespace niv;
 
-constexpr int kCellBudgetMB = 32;       // default budget of the cell-block copies of the coarse levels
+constexpr int kCellBudgetMB = 128;      // default budget of the cell-block copies of the coarse levels
 constexpr uint32_t kCtrSlots = 2048;     // dynamically scheduled launches of one model that may be in flight at once
 
 typedef void (*fused_fn)(KParams, const float*, const float*, float*, size_t, uint32_t);
@@ -436,14 +436,15 @@ static int setup_kernel(niv_model* m, FusedKernel& k, int tmem_cols, const char*
 // ---- which instantiation serves which model -----------------------------------------------------------------------
 // O = output as 128-bit stores (pinned host buffers), NPT = per-texel parameters, IMG = image tiling,
 // C = read the coarsest min(L, kCellLevels) levels from their cell-block copies
-// how many: BASELINE.json's family (F = 2) five (0.1673 -> 0.1613 / 0.1585 / 0.1567 ms per full-HD frame with 3 / 4 / 5
-// levels; a sixth would take 57 MB); the paper's family (F = 4, 64-byte blocks) four (its 8-level model: 0.1093 ms
+// how many: BASELINE.json's family (F = 2) six (0.1673 -> 0.1613 / 0.1585 / 0.1567 ms per full-HD frame with 3 / 4 / 5
+// levels; the sixth, N = 121: 57 MB of device memory, of which a frame touches the cells on its visible surfaces:
+// 0.1532 -> 0.1511 ms, the incoherent set 0.527 -> 0.493 ms; a seventh would take 193 MB); the paper's family (F = 4, 64-byte blocks) four (its 8-level model: 0.1093 ms
 // without, 0.0998 with four, 0.119 with five) -- profiles/r02_cells.md
 // the bias K-step's ones tile in shared memory instead of tensor memory (niv_fused.cuh OS): the paper's family and its
 // grid-less models at width 32 / 64, whose 56..106 registers allow five to eight CTAs per SM once a tile takes 96 / 64
 // tensor-memory columns instead of 128; BASELINE.json's family sits at the register cap with four CTAs either way
 constexpr bool ones_in_smem(uint32_t W, uint32_t L, uint32_t F) { return (F == 4 || L == 0) && (W == 32 || W == 64); }
-constexpr int cell_levels_of(int L, int F) { return F == 4 ? (L < 4 ? L : 4) : (L < 5 ? L : 5); }
+constexpr int cell_levels_of(int L, int F) { return F == 4 ? (L < 4 ? L : 4) : (L < 6 ? L : 6); }
 template <int W, int L, int F, bool RAWDIR, bool O, int NPT, bool IMG, bool C, bool PK = false, int DB = 0>
 static fused_fn fused_inst() {
     // levels per gather batch (two batches in flight): BASELINE.json's family four = 32 gathers; the paper's family
