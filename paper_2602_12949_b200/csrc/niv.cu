@@ -1046,6 +1046,7 @@ static int launch_one(const niv_model* m, const FusedKernel& k, cudaStream_t st,
     cur.done = P.tile_ctr ? P.tile_ctr + 2 : nullptr;
     cur.gen = P.slot_gen;
     P.grid_wait = 1;
+    P.early_read = 0;
     P.wait_a = P.wait_b = nullptr;
     P.gen_a = P.gen_b = 0;
 
@@ -1058,6 +1059,15 @@ static int launch_one(const niv_model* m, const FusedKernel& k, cudaStream_t st,
         if (a && a->tracked) { P.wait_a = a->done; P.gen_a = a->gen; }
         if (b && b->tracked && P.wait_a) { P.wait_b = b->done; P.gen_b = b->gen; }
         if (h.r[0].tracked && h.r[1].tracked && h.r[2].tracked && !launches_conflict(h.r[0], cur)) P.grid_wait = 0;
+        // A CTA of launch n starts only after every CTA of n-1 has passed ITS waits (griddepcontrol.launch_dependents comes
+        // after them in the kernel), i.e. with n-3 and everything older complete; n-1 writes nothing this launch reads
+        // (grid_wait = 0); if n-2 does not either, the first texel can be requested at the very top of the kernel, before
+        // this launch's own polls (which still precede everything else it does with a caller's buffer)
+        if (P.grid_wait == 0) {
+            bool raw = false;
+            for (int j = 0; j < kOutRange; ++j) raw |= ranges_overlap(h.r[1], kOutRange, cur, j);
+            P.early_read = raw ? 0u : 1u;
+        }
     }
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));

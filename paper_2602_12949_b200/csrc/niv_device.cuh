@@ -49,6 +49,8 @@ struct KParams {
     // disjoint buffers, so this one may run beside its last tiles.  wait_a / wait_b: completion words of the two
     // launches before that one, polled until they reach gen_a / gen_b (NULL: nothing to poll)
     uint32_t grid_wait;
+    uint32_t early_read;        // 1: none of this launch's INPUT buffers is written by the two launches that may still be running
+                                // (grid_wait = 0 and no overlap with their outputs): the first texel may be requested at once
     uint32_t gen_a, gen_b;
     const uint32_t* wait_a;
     const uint32_t* wait_b;

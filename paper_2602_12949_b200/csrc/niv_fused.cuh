@@ -82,6 +82,31 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
         mbar_init(bar_mma, 1);
         mbar_fence_init();
     }
+    // G-buffer texel of the first tile.  Requested here, ahead of everything, when the host found that no launch that
+    // may still be running writes this launch's inputs (P.early_read); otherwise after the waits below.  Inside the loop
+    // the NEXT tile's texel is requested a tile ahead, so its HBM latency hides under a whole tile of work (a1 prefetch)
+    float pn[3] = {0.f, 0.f, 0.f}, nn[3] = {0.f, 0.f, 0.f};
+    float tn[NPT > 0 ? NPT : 1] = {0.f};              // per-texel scene parameters, prefetched like the G-buffer
+    // texel of thread tid in tile t: 128 consecutive texels per tile, or (IMG) a 32 x 4 pixel tile of the image
+    //   (txy: the tile's packed image coordinates, which thread 0 works out with the tile index; unused otherwise)
+    auto texel_of = [&](uint32_t t, uint32_t txy, bool& ok) -> size_t {
+        if constexpr (IMG) return image_texel_xy(P, txy, tid, ok);
+        const size_t idx = (size_t)t * kTile + tid;
+        ok = idx < n;
+        return idx;
+    };
+    uint32_t txy = 0, txy_next = 0;
+    if constexpr (IMG) txy = image_tile_xy(P, blockIdx.x);
+    auto load_first_texel = [&]() {
+        bool ok;
+        const size_t i0 = texel_of(blockIdx.x, txy, ok);
+        if (ok) {
+            load_texel_raw(PACKED ? P.gbuf_fmt : 0u, pos, nrm, i0, pn, nn);
+#pragma unroll
+            for (int q = 0; q < NPT; ++q) tn[q] = __ldg(P.tparam + i0 * NPT + q);
+        }
+    };
+    if (P.early_read) load_first_texel();
     if (warp == 0) {
         if constexpr (OS64) {
             tmem_alloc_keep(smem_u32(tmem_slot), 64);
@@ -122,6 +147,37 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
         tmem_st_x8(lane_taddr + ONES_COL, ones);
     }
     const uint64_t desc_ones = make_smem_desc(smem_u32(sOnes), 2048u, 128u);
+    // shared-memory descriptor (low half) of every layer's B operand at K-step 0: (address >> 4) | (N * 16 >> 4) << 16,
+    // the high half is the constant 0x4008 = SBO 128 B >> 4 | descriptor version 1 << 14 (niv_tc.cuh make_smem_desc)
+    constexpr uint32_t K1 = 2 * AWT;
+    const uint32_t n_layers = P.n_layers;
+    uint32_t desc_lo0[kMaxLayers];
+#pragma unroll
+    for (int l = 0; l < kMaxLayers; ++l) {
+        const uint32_t N = (l + 1 == (int)n_layers) ? 16u : (uint32_t)WIDTH;
+        desc_lo0[l] = (((sW_u32 + P.w_off[l]) & 0x3FFFFu) >> 4) | (N << 16);
+    }
+    uint32_t phase = 0;
+    // Programmatic dependent launch (launch_fused sets the stream-serialisation attribute): everything above touches
+    // only the model's own memory, so this launch's CTAs may take the place of the previous launch's as those drain,
+    // with TMEM allocated and weights staged; from here on the caller's buffers are read and written, which needs the
+    // previous kernel of the stream complete.  The next launch may start filling in behind this one right away.
+    if (P.grid_wait) pdl_wait();
+    if (P.wait_a) {                    // launches two and three back: complete before this one touches a buffer
+        if (tid == 0) {                // (both words requested before either is looked at)
+            uint32_t va = ld_acquire_gpu(P.wait_a), vb = P.wait_b ? ld_acquire_gpu(P.wait_b) : P.gen_b;
+            while ((int32_t)(va - P.gen_a) < 0) { __nanosleep(64); va = ld_acquire_gpu(P.wait_a); }
+            while ((int32_t)(vb - P.gen_b) < 0) { __nanosleep(64); vb = ld_acquire_gpu(P.wait_b); }
+        }
+        __syncthreads();
+    }
+    // only now may the NEXT launch's CTAs be scheduled: when one of them starts, every CTA of this launch has passed the
+    // waits above, so the launches two and more before THIS one are complete -- which is what lets the next launch
+    // request its first texel at once (P.early_read: the host has checked this launch and the one before it)
+    pdl_launch_dependents();
+    if constexpr (IMG) txy_next = s_txy[0];
+    if (!P.early_read) load_first_texel();
+    // the weights are waited for only now: their copy (issued in the prologue) and the first texel's trip from HBM overlap
     mbar_wait(bar_w, 0);
 
     // ---- a8: fold the per-call parameter encoding into layer 1's bias K-row (hi, lo) in shared memory
@@ -142,54 +198,6 @@ __global__ void __launch_bounds__(kTile, (WIDTH == 32 || NPT >= 1) ? 4 : 0) niv_
     }
     fence_proxy_async_smem();          // the bias row is read by the tensor core through the async proxy
 
-    // shared-memory descriptor (low half) of every layer's B operand at K-step 0: (address >> 4) | (N * 16 >> 4) << 16,
-    // the high half is the constant 0x4008 = SBO 128 B >> 4 | descriptor version 1 << 14 (niv_tc.cuh make_smem_desc)
-    constexpr uint32_t K1 = 2 * AWT;
-    const uint32_t n_layers = P.n_layers;
-    uint32_t desc_lo0[kMaxLayers];
-#pragma unroll
-    for (int l = 0; l < kMaxLayers; ++l) {
-        const uint32_t N = (l + 1 == (int)n_layers) ? 16u : (uint32_t)WIDTH;
-        desc_lo0[l] = (((sW_u32 + P.w_off[l]) & 0x3FFFFu) >> 4) | (N << 16);
-    }
-    uint32_t phase = 0;
-    // Programmatic dependent launch (launch_fused sets the stream-serialisation attribute): everything above touches
-    // only the model's own memory, so this launch's CTAs may take the place of the previous launch's as those drain,
-    // with TMEM allocated and weights staged; from here on the caller's buffers are read and written, which needs the
-    // previous kernel of the stream complete.  The next launch may start filling in behind this one right away.
-    pdl_launch_dependents();
-    if (P.grid_wait) pdl_wait();
-    if (P.wait_a) {                    // launches two and three back: complete before this one touches a buffer
-        if (tid == 0) {
-            while ((int32_t)(ld_acquire_gpu(P.wait_a) - P.gen_a) < 0) __nanosleep(64);
-            if (P.wait_b)
-                while ((int32_t)(ld_acquire_gpu(P.wait_b) - P.gen_b) < 0) __nanosleep(64);
-        }
-        __syncthreads();
-    }
-    // G-buffer texel of the first tile; inside the loop the NEXT tile's texel is requested before the current
-    // one is encoded, so its HBM latency hides under a whole tile of work (a1 prefetch)
-    float pn[3] = {0.f, 0.f, 0.f}, nn[3] = {0.f, 0.f, 0.f};
-    float tn[NPT > 0 ? NPT : 1] = {0.f};              // per-texel scene parameters, prefetched like the G-buffer
-    // texel of thread tid in tile t: 128 consecutive texels per tile, or (IMG) a 32 x 4 pixel tile of the image
-    //   (txy: the tile's packed image coordinates, which thread 0 works out with the tile index; unused otherwise)
-    auto texel_of = [&](uint32_t t, uint32_t txy, bool& ok) -> size_t {
-        if constexpr (IMG) return image_texel_xy(P, txy, tid, ok);
-        const size_t idx = (size_t)t * kTile + tid;
-        ok = idx < n;
-        return idx;
-    };
-    uint32_t txy = 0, txy_next = 0;
-    if constexpr (IMG) { txy = image_tile_xy(P, blockIdx.x); txy_next = s_txy[0]; }
-    {
-        bool ok;
-        const size_t i0 = texel_of(blockIdx.x, txy, ok);
-        if (ok) {
-            load_texel_raw(PACKED ? P.gbuf_fmt : 0u, pos, nrm, i0, pn, nn);
-#pragma unroll
-            for (int q = 0; q < NPT; ++q) tn[q] = __ldg(P.tparam + i0 * NPT + q);
-        }
-    }
     uint32_t tile = blockIdx.x, tnext = s_tile[0], it = 0;
     while (tile < n_tiles) {
         bool valid;
