@@ -30,7 +30,10 @@
  *     library and none of its buffers overlaps a buffer of this launch in a way that matters (nothing this launch
  *     touches is written by it, nothing this launch writes is read by it) -- the two then run beside each other for
  *     the previous launch's last tiles, and the launches two and three back are known complete (completion words
- *     polled on the device) before this one touches a buffer.  The result is that of serial execution in every case
+ *     polled on the device) before this one touches a buffer -- with one exception: when neither the previous launch nor
+ *     the one before it writes any INPUT of this launch (host-side range check), each thread requests its first texel
+ *     before those polls; a CTA of a launch starts only after every CTA of the launch before it has passed its own
+ *     polls, so all older launches are complete by then.  The result is that of serial execution in every case
  *     (tests: back-to-back calls on aliased buffers); NIV_OVERLAP=0 turns it off;
  *   - environment knobs, all read ONCE at niv_create and never on the call path: NIV_PDL=0 (no programmatic stream
  *     serialisation), NIV_OVERLAP=0 (every launch waits for the previous kernel of its stream), NIV_CELL_MB=<n> (budget of
