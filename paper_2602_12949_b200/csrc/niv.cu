@@ -324,7 +324,7 @@ __global__ void __launch_bounds__(128) niv_sector_census_kernel(const __grid_con
 // =====================================================================================================
 using namespace niv;
 
-constexpr int kCellBudgetMB = 128;      // default budget of the cell-block copies of the coarse levels
+constexpr int kCellBudgetMB = 320;      // default budget of the cell-block copies of the coarse levels
 constexpr uint32_t kCtrSlots = 2048;     // dynamically scheduled launches of one model that may be in flight at once
 
 typedef void (*fused_fn)(KParams, const float*, const float*, float*, size_t, uint32_t);
@@ -436,23 +436,27 @@ static int setup_kernel(niv_model* m, FusedKernel& k, int tmem_cols, const char*
 // ---- which instantiation serves which model -----------------------------------------------------------------------
 // O = output as 128-bit stores (pinned host buffers), NPT = per-texel parameters, IMG = image tiling,
 // C = read the coarsest min(L, kCellLevels) levels from their cell-block copies
-// how many: BASELINE.json's family (F = 2) six (0.1673 -> 0.1613 / 0.1585 / 0.1567 ms per full-HD frame with 3 / 4 / 5
-// levels; the sixth, N = 121: 57 MB of device memory, of which a frame touches the cells on its visible surfaces:
-// 0.1532 -> 0.1511 ms, the incoherent set 0.527 -> 0.493 ms; a seventh would take 193 MB); the paper's family (F = 4, 64-byte blocks) four (its 8-level model: 0.1093 ms
+// how many: BASELINE.json's family (F = 2) seven (0.1673 -> 0.1613 / 0.1585 / 0.1567 ms per full-HD frame with 3 / 4 / 5
+// levels; the sixth, N = 121, 57 MB: 0.1532 -> 0.1511 ms; the seventh, N = 182, 193 MB: 0.1508 -> 0.1459 ms -- a frame
+// touches only the cells on its visible surfaces, a few MB; the incoherent set 0.527 -> 0.493 -> 0.477 ms), or five when
+// the budget or a level's cell count (< 2^24) does not allow seven (tiers 2 and 1 of `C`); the paper's family (F = 4, 64-byte blocks) four (its 8-level model: 0.1093 ms
 // without, 0.0998 with four, 0.119 with five) -- profiles/r02_cells.md
 // the bias K-step's ones tile in shared memory instead of tensor memory (niv_fused.cuh OS): the paper's family and its
 // grid-less models at width 32 / 64, whose 56..106 registers allow five to eight CTAs per SM once a tile takes 96 / 64
 // tensor-memory columns instead of 128; BASELINE.json's family sits at the register cap with four CTAs either way
 constexpr bool ones_in_smem(uint32_t W, uint32_t L, uint32_t F) { return (F == 4 || L == 0) && (W == 32 || W == 64); }
-constexpr int cell_levels_of(int L, int F) { return F == 4 ? (L < 4 ? L : 4) : (L < 6 ? L : 6); }
-template <int W, int L, int F, bool RAWDIR, bool O, int NPT, bool IMG, bool C, bool PK = false, int DB = 0>
+// tier C: 0 = none; 1 = the first five levels (F = 2) / four (F = 4); 2 = seven levels (F = 2: N = 16 .. 182, 274 MB of copies)
+constexpr int cell_levels_of(int L, int F, int C = 2) {
+    return C == 0 ? 0 : F == 4 ? (L < 4 ? L : 4) : C == 1 ? (L < 5 ? L : 5) : (L < 7 ? L : 7);
+}
+template <int W, int L, int F, bool RAWDIR, bool O, int NPT, bool IMG, int C, bool PK = false, int DB = 0>
 static fused_fn fused_inst() {
     // levels per gather batch (two batches in flight): BASELINE.json's family four = 32 gathers; the paper's family
     // (8-byte entries) two = 32 registers
     constexpr int NB = L == 0 ? 1 : F == 4 ? 2 : 4;
-    return niv_fused_kernel<W, L, NB, F, RAWDIR, O, NPT, IMG, C ? cell_levels_of(L, F) : 0, PK, DB, ones_in_smem(W, L, F)>;
+    return niv_fused_kernel<W, L, NB, F, RAWDIR, O, NPT, IMG, cell_levels_of(L, F, C), PK, DB, ones_in_smem(W, L, F)>;
 }
-template <int W, bool O, int NPT, bool IMG, bool C, bool PK = false>
+template <int W, bool O, int NPT, bool IMG, int C, bool PK = false>
 static fused_fn pick_levels_f2(uint32_t L) {        // BASELINE.json's family: F = 2, SH-16
     switch (L) {
         case 4:  return fused_inst<W, 4, 2, false, O, NPT, IMG, C, PK>();
@@ -462,7 +466,7 @@ static fused_fn pick_levels_f2(uint32_t L) {        // BASELINE.json's family: F
         default: return nullptr;
     }
 }
-template <int W, bool O, bool C, bool PK = false, int DB = 0>
+template <int W, bool O, int C, bool PK = false, int DB = 0>
 static fused_fn pick_levels_f4(uint32_t L) {        // the paper's own family: F = 4, raw direction
     switch (L) {
         case 2: return fused_inst<W, 2, 4, true, O, 0, false, C, PK, DB>();
@@ -473,32 +477,32 @@ static fused_fn pick_levels_f4(uint32_t L) {        // the paper's own family: F
     }
 }
 // PK: the variant that reads the compact G-buffer formats / writes fp16 (linear tiles; the grid models of both families)
-template <bool O, bool C, bool PK = false>
+template <bool O, int C, bool PK = false>
 static fused_fn pick_fused(uint32_t W, uint32_t L, uint32_t F, uint32_t dir_freq = 0) {
     if (dir_freq) {                                 // frequency-encoded direction: the paper's family at width 64, device buffers
-        if constexpr (!O) return (F == 4 && W == 64 && dir_freq == 4) ? pick_levels_f4<64, false, C, PK, 4>(L) : nullptr;
+        if constexpr (!O) return (F == 4 && W == 64 && dir_freq == 4) ? pick_levels_f4<64, false, (C > 1 ? 1 : C), PK, 4>(L) : nullptr;
         else return nullptr;                        // (host buffers take niv_infer_host's staged path)
     }
     if (L == 0)                                     // grid-less: positional encoding, no gathers
-        return W == 16 ? fused_inst<16, 0, 2, true, O, 0, false, false, PK>() : W == 32 ? fused_inst<32, 0, 2, true, O, 0, false, false, PK>()
-             : W == 64 ? fused_inst<64, 0, 2, true, O, 0, false, false, PK>() : nullptr;
-    if (F == 4) return W == 32 ? pick_levels_f4<32, O, C, PK>(L) : W == 64 ? pick_levels_f4<64, O, C, PK>(L) : nullptr;
+        return W == 16 ? fused_inst<16, 0, 2, true, O, 0, false, 0, PK>() : W == 32 ? fused_inst<32, 0, 2, true, O, 0, false, 0, PK>()
+             : W == 64 ? fused_inst<64, 0, 2, true, O, 0, false, 0, PK>() : nullptr;
+    if (F == 4) return W == 32 ? pick_levels_f4<32, O, (C > 1 ? 1 : C), PK>(L) : W == 64 ? pick_levels_f4<64, O, (C > 1 ? 1 : C), PK>(L) : nullptr;
     return W == 32 ? pick_levels_f2<32, O, 0, false, C, PK>(L) : W == 64 ? pick_levels_f2<64, O, 0, false, C, PK>(L) : nullptr;
 }
 // image tiling (niv_infer_image): BASELINE.json's family (F = 2, 8..16 levels reach cells smaller than a warp's strip).
 // The paper's own family (F = 4, <= 8 levels, finest cell 5.5 cm) measured SLOWER with it (profiles/r01_v2.md): its
 // cells are larger than a 32-pixel strip anyway; it keeps the linear kernel, as do the grid-less models.
-template <bool C, bool PK = false>
+template <int C, bool PK = false>
 static fused_fn pick_fused_img(uint32_t W, uint32_t L, uint32_t F) {
     if (L == 0 || F != 2) return nullptr;
     return W == 32 ? pick_levels_f2<32, false, 0, true, C, PK>(L) : W == 64 ? pick_levels_f2<64, false, 0, true, C, PK>(L) : nullptr;
 }
 // per-texel scene parameters: BASELINE.json's family, 8 or 16 levels, width 32 / 64, 1 or 2 parameters
-template <int W, int NPT, bool C>
+template <int W, int NPT, int C>
 static fused_fn pick_tp_levels(uint32_t L) {
     return L == 8 ? fused_inst<W, 8, 2, false, false, NPT, false, C>() : L == 16 ? fused_inst<W, 16, 2, false, false, NPT, false, C>() : nullptr;
 }
-template <bool C>
+template <int C>
 static fused_fn pick_fused_tp(uint32_t W, uint32_t L, uint32_t F, uint32_t sh_degree, uint32_t n_params) {
     if (F != 2 || sh_degree != 4) return nullptr;
     if (n_params == 1) return W == 32 ? pick_tp_levels<32, 1, C>(L) : W == 64 ? pick_tp_levels<64, 1, C>(L) : nullptr;
@@ -649,28 +653,31 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     // cell-block copies of the coarsest min(L, kCellLevels) levels, if their N^3 blocks of 8 entries fit
     // the budget (NIV_CELL_MB, read once here; 0 = none): the kernels that read them are compiled for exactly that
     // many levels, so it is all of them or none.  (width 128 and the mma.sync A/B kernel gather from the table)
-    bool use_cells = false;
+    int cell_tier = 0;                             // 0 none, 1 five (four) levels, 2 seven: the highest that fits
     if (cfg->n_levels && cfg->hidden_width <= 64 && !want_mma_sync) {
         const char* s_mb = getenv("NIV_CELL_MB");
         const uint64_t budget = (uint64_t)(s_mb ? std::max(0, atoi(s_mb)) : kCellBudgetMB) << 20;
-        const uint32_t want = std::min((uint32_t)cell_levels_of((int)Lk, (int)cfg->n_features), cfg->n_levels);   // the real ones
-        uint64_t off = 0;
-        use_cells = true;
-        for (uint32_t l = 0; l < want; ++l) {
-            const uint64_t N = I.resolution[l], bytes = N * N * N * 8 * cfg->n_features * 2;
-            if (N * N * N >= (1u << 24) || off + bytes > budget) { use_cells = false; break; }
-            m->cell_off[l] = off;
-            off += bytes;
-        }
-        if (use_cells) {
+        for (int tier = cfg->n_features == 4 ? 1 : 2; tier >= 1 && cell_tier == 0; --tier) {
+            const uint32_t want = std::min((uint32_t)cell_levels_of((int)Lk, (int)cfg->n_features, tier), cfg->n_levels);   // the real ones
+            uint64_t off = 0;
+            bool fits = true;
+            for (uint32_t l = 0; l < want && fits; ++l) {
+                const uint64_t N = I.resolution[l], bytes = N * N * N * 8 * cfg->n_features * 2;
+                if (N * N * N >= (1u << 24) || off + bytes > budget) fits = false;
+                m->cell_off[l] = off;
+                off += bytes;
+            }
+            if (!fits) continue;
             for (uint32_t l = 0; l < want; ++l) {
                 P.lv[l].cs = I.resolution[l];
                 P.lv[l].cs2 = I.resolution[l] * I.resolution[l];
             }
             I.cell_levels = want;
             I.cell_bytes = off;
+            cell_tier = tier;
         }
     }
+    const bool use_cells = cell_tier != 0;
     I.tile_texels = kTile;
 
     // layer shapes and the packed weight blob layout
@@ -720,40 +727,45 @@ extern "C" int niv_create(const niv_config* cfg, niv_model** out)
     } else {
         // D | A | ones in one allocation (niv_fused.cuh TMEM_COLS); ones in shared memory: D 64 + A 32, or D 32 | A 32
         const int tmem_cols = os ? (W == 64 ? 96 : 64) : W == 16 ? 64 : 128;
-        m->fused.fn = use_cells ? pick_fused<false, true>(W, Lk, cfg->n_features, cfg->dir_frequencies)
-                                : pick_fused<false, false>(W, Lk, cfg->n_features, cfg->dir_frequencies);
+        m->fused.fn = cell_tier == 2 ? pick_fused<false, 2>(W, Lk, cfg->n_features, cfg->dir_frequencies)
+                    : cell_tier == 1 ? pick_fused<false, 1>(W, Lk, cfg->n_features, cfg->dir_frequencies)
+                                     : pick_fused<false, 0>(W, Lk, cfg->n_features, cfg->dir_frequencies);
         m->fused.smem = smem_dev;
         rc = m->fused.fn ? setup_kernel(m, m->fused, tmem_cols, "fused") : NIV_ERR_UNSUPPORTED;
         if (rc == NIV_OK) {
-            m->fused_host.fn = pick_fused<true, false>(W, Lk, cfg->n_features, cfg->dir_frequencies);   // PCIe-bound: table gathers
+            m->fused_host.fn = pick_fused<true, 0>(W, Lk, cfg->n_features, cfg->dir_frequencies);   // PCIe-bound: table gathers
             m->fused_host.smem = smem_host;
             rc = setup_kernel(m, m->fused_host, tmem_cols, "fused_host");
         }
         if (rc == NIV_OK) {
-            m->fused_pk.fn = use_cells ? pick_fused<false, true, true>(W, Lk, cfg->n_features, cfg->dir_frequencies)
-                                       : pick_fused<false, false, true>(W, Lk, cfg->n_features, cfg->dir_frequencies);
+            m->fused_pk.fn = cell_tier == 2 ? pick_fused<false, 2, true>(W, Lk, cfg->n_features, cfg->dir_frequencies)
+                           : cell_tier == 1 ? pick_fused<false, 1, true>(W, Lk, cfg->n_features, cfg->dir_frequencies)
+                                            : pick_fused<false, 0, true>(W, Lk, cfg->n_features, cfg->dir_frequencies);
             m->fused_pk.smem = smem_dev;
             rc = setup_kernel(m, m->fused_pk, tmem_cols, "fused_packed");
         }
         if (rc == NIV_OK) {
-            m->fused_host_pk.fn = pick_fused<true, false, true>(W, Lk, cfg->n_features, cfg->dir_frequencies);
+            m->fused_host_pk.fn = pick_fused<true, 0, true>(W, Lk, cfg->n_features, cfg->dir_frequencies);
             m->fused_host_pk.smem = smem_host;
             rc = setup_kernel(m, m->fused_host_pk, tmem_cols, "fused_host_packed");
         }
         if (rc == NIV_OK) {
-            m->fused_img.fn = use_cells ? pick_fused_img<true>(W, Lk, cfg->n_features)
-                                        : pick_fused_img<false>(W, Lk, cfg->n_features);
+            m->fused_img.fn = cell_tier == 2 ? pick_fused_img<2>(W, Lk, cfg->n_features)
+                            : cell_tier == 1 ? pick_fused_img<1>(W, Lk, cfg->n_features)
+                                             : pick_fused_img<0>(W, Lk, cfg->n_features);
             m->fused_img.smem = smem_dev;
             rc = setup_kernel(m, m->fused_img, tmem_cols, "fused_image");
         }
         if (rc == NIV_OK && use_cells && m->fused_img.fn) {
-            m->fused_img_pk.fn = pick_fused_img<true, true>(W, Lk, cfg->n_features);
+            m->fused_img_pk.fn = cell_tier == 2 ? pick_fused_img<2, true>(W, Lk, cfg->n_features)
+                                                : pick_fused_img<1, true>(W, Lk, cfg->n_features);
             m->fused_img_pk.smem = smem_dev;
             rc = setup_kernel(m, m->fused_img_pk, tmem_cols, "fused_image_packed");
         }
         if (rc == NIV_OK && cfg->n_params) {
-            m->fused_tp.fn = use_cells ? pick_fused_tp<true>(W, Lk, cfg->n_features, cfg->sh_degree, cfg->n_params)
-                                       : pick_fused_tp<false>(W, Lk, cfg->n_features, cfg->sh_degree, cfg->n_params);
+            m->fused_tp.fn = cell_tier == 2 ? pick_fused_tp<2>(W, Lk, cfg->n_features, cfg->sh_degree, cfg->n_params)
+                           : cell_tier == 1 ? pick_fused_tp<1>(W, Lk, cfg->n_features, cfg->sh_degree, cfg->n_params)
+                                            : pick_fused_tp<0>(W, Lk, cfg->n_features, cfg->sh_degree, cfg->n_params);
             if (m->fused_tp.fn) {
                 // layout of the per-texel-parameter variant: layer 1 with K = round16(enc_dim) + 16 n_params, no fold blob
                 m->kp_tp = P;

@@ -136,8 +136,8 @@ def test_fused_kernels_keep_the_descriptor_uniform(L):
         #  is not the failure this guards against: that one re-creates the descriptor in front of EVERY gather)
         assert v["recreated"] <= max(16, v["ldg"] // 6), (k, v)
     # the headline kernels (BASELINE.json configs[1]: width 64, 16 levels, F = 2; device path, linear and image tiling,
-    # six cell-block levels) keep everything in registers
-    head = [k for k in fused if re.search(r"ILi64ELi16ELi4ELi2ELb0ELb0ELi0ELb[01]ELi6ELb0ELi0ELb0EEE", k)]
+    # seven cell-block levels) keep everything in registers
+    head = [k for k in fused if re.search(r"ILi64ELi16ELi4ELi2ELb0ELb0ELi0ELb[01]ELi7ELb0ELi0ELb0EEE", k)]
     assert len(head) == 2
     for k in head:
         assert fused[k]["local"] == 0, (k, fused[k])

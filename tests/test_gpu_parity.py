@@ -479,7 +479,7 @@ def test_cell_block_levels_are_exact_copies(torch_cuda, niv, oracle, monkeypatch
     pos[8] = np.asarray(spec.aabb_min, dtype=np.float32)
     param = [0.3] if spec.n_params else None
     m_on = case.gpu_model(niv)
-    want_levels = min(spec.n_levels, 4 if spec.n_features == 4 else 6)
+    want_levels = min(spec.n_levels, 4 if spec.n_features == 4 else 7)
     assert m_on.info.cell_levels == want_levels and m_on.info.cell_bytes > 0
     monkeypatch.setenv("NIV_CELL_MB", "0")
     m_off = case.gpu_model(niv)
@@ -502,6 +502,17 @@ def test_cell_block_levels_are_exact_copies(torch_cuda, niv, oracle, monkeypatch
         m_off.infer_image(dp, dn, ob, w, h)
         torch.cuda.synchronize()
         assert torch.equal(oa, ob)
+        # a budget that holds five levels (23.5 MB) but not seven (274 MB): the second tier of kernels, the same bits
+        monkeypatch.setenv("NIV_CELL_MB", "100")
+        m_five = case.gpu_model(niv)
+        monkeypatch.delenv("NIV_CELL_MB")
+        assert m_five.info.cell_levels == 5 and 0 < m_five.info.cell_bytes < m_on.info.cell_bytes
+        assert np.array_equal(_gpu_infer(torch, m_five, pos, nrm, param), a)
+        oc = torch.full((w * h, 3), float("nan"), device="cuda")
+        m_five.infer_image(dp, dn, oc, w, h)
+        torch.cuda.synchronize()
+        assert torch.equal(oa, oc)
+        m_five.close()
     if which == "param_tp":                                        # ... and so has the per-texel-parameter kernel
         dp, dn = torch.from_numpy(pos).cuda(), torch.from_numpy(nrm).cuda()
         tp = torch.from_numpy(I.uniform01(77, 3, n).astype(np.float32).reshape(n, 1)).cuda()
