@@ -490,6 +490,9 @@ def run_ours(args):
                     "note": "what the kernel's own layout reads: levels held as cell blocks cost one sector per "
                             "distinct cell instead of the 8 corners' sectors"},
         "gather_rate_ggathers_per_s": 8 * L * n_active / kernel_s / 1e9,
+        "frac_note": ("frac is the ALGORITHMIC census (sectors of the [L][T] table the frame needs) over the probe's random-sector "
+                      "rate; on levels held as cell blocks one sector serves the 8 corners the census counts up to 8 sectors for, so "
+                      "on scattered queries it can exceed 1 -- `touched` is the same ratio for what is really read"),
         "probe": gpeak,
         "t_roofline_us": {"l2_gather": t_gather * 1e6, "tensor": t_tensor * 1e6, "hbm": t_hbm * 1e6},
         "tensor": {"achieved": flop_texel * n / kernel_s / 1e12, "peak": peaks["tflops_sustained"],
