@@ -439,15 +439,16 @@ static int setup_kernel(niv_model* m, FusedKernel& k, int tmem_cols, const char*
 // how many: BASELINE.json's family (F = 2) seven (0.1673 -> 0.1613 / 0.1585 / 0.1567 ms per full-HD frame with 3 / 4 / 5
 // levels; the sixth, N = 121, 57 MB: 0.1532 -> 0.1511 ms; the seventh, N = 182, 193 MB: 0.1508 -> 0.1459 ms -- a frame
 // touches only the cells on its visible surfaces, a few MB; the incoherent set 0.527 -> 0.493 -> 0.477 ms), or five when
-// the budget or a level's cell count (< 2^24) does not allow seven (tiers 2 and 1 of `C`); the paper's family (F = 4, 64-byte blocks) four (its 8-level model: 0.1093 ms
-// without, 0.0998 with four, 0.119 with five) -- profiles/r02_cells.md
+// the budget or a level's cell count (< 2^24) does not allow seven (tiers 2 and 1 of `C`); the paper's family (F = 4, 64-byte blocks) six (N = 16 .. 90,
+// 68 MB; its 8-level model: 0.0932 ms with four, 0.0802 with six, 0.0881 with seven -- a kernel whose time also moves by
+// several per cent with its place in the module) -- profiles/r02_cells.md
 // the bias K-step's ones tile in shared memory instead of tensor memory (niv_fused.cuh OS): the paper's family and its
 // grid-less models at width 32 / 64, whose 56..106 registers allow five to eight CTAs per SM once a tile takes 96 / 64
 // tensor-memory columns instead of 128; BASELINE.json's family sits at the register cap with four CTAs either way
 constexpr bool ones_in_smem(uint32_t W, uint32_t L, uint32_t F) { return (F == 4 || L == 0) && (W == 32 || W == 64); }
-// tier C: 0 = none; 1 = the first five levels (F = 2) / four (F = 4); 2 = seven levels (F = 2: N = 16 .. 182, 274 MB of copies)
+// tier C: 0 = none; 1 = the first five levels (F = 2) / six (F = 4); 2 = seven levels (F = 2: N = 16 .. 182, 274 MB of copies)
 constexpr int cell_levels_of(int L, int F, int C = 2) {
-    return C == 0 ? 0 : F == 4 ? (L < 4 ? L : 4) : C == 1 ? (L < 5 ? L : 5) : (L < 7 ? L : 7);
+    return C == 0 ? 0 : F == 4 ? (L < 6 ? L : 6) : C == 1 ? (L < 5 ? L : 5) : (L < 7 ? L : 7);
 }
 template <int W, int L, int F, bool RAWDIR, bool O, int NPT, bool IMG, int C, bool PK = false, int DB = 0>
 static fused_fn fused_inst() {

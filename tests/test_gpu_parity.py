@@ -479,7 +479,7 @@ def test_cell_block_levels_are_exact_copies(torch_cuda, niv, oracle, monkeypatch
     pos[8] = np.asarray(spec.aabb_min, dtype=np.float32)
     param = [0.3] if spec.n_params else None
     m_on = case.gpu_model(niv)
-    want_levels = min(spec.n_levels, 4 if spec.n_features == 4 else 7)
+    want_levels = min(spec.n_levels, 6 if spec.n_features == 4 else 7)
     assert m_on.info.cell_levels == want_levels and m_on.info.cell_bytes > 0
     monkeypatch.setenv("NIV_CELL_MB", "0")
     m_off = case.gpu_model(niv)
