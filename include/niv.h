@@ -37,7 +37,7 @@
  *     (tests: back-to-back calls on aliased buffers); NIV_OVERLAP=0 turns it off;
  *   - environment knobs, all read ONCE at niv_create and never on the call path: NIV_PDL=0 (no programmatic stream
  *     serialisation), NIV_OVERLAP=0 (every launch waits for the previous kernel of its stream), NIV_CELL_MB=<n> (budget of
- *     the cell-block copies of the coarse levels in MiB, default 320, 0 = none; seven levels, else five, else none), NIV_IMAGE_LINEAR=1 (niv_infer_image through the linear-tile kernel), NIV_HOST_STAGED=1
+ *     the cell-block copies of the coarse levels in MiB, default 320, 0 = none; F = 2: the seven coarsest levels, else five, else none; F = 4: six, else none), NIV_IMAGE_LINEAR=1 (niv_infer_image through the linear-tile kernel), NIV_HOST_STAGED=1
  *     (niv_infer_host through staging copies even for pinned buffers), NIV_MMA_SYNC=1 (the mma.sync A/B kernel for the
  *     BASELINE.json configs[1] shape), NIV_DEBUG=1 (resource report on stderr);
  *   - there is no CPU fallback: without a CUDA device every entry point that needs one returns NIV_ERR_CUDA.
