@@ -69,10 +69,6 @@ __device__ __forceinline__ void tmem_alloc_keep(uint32_t dst_smem, uint32_t ncol
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst_smem), "r"(ncols)
                  : "memory");
 }
-// one block of 32 columns
-__device__ __forceinline__ void tmem_alloc32(uint32_t dst_smem) {                 // one full warp
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 32;" ::"r"(dst_smem) : "memory");
-}
 __device__ __forceinline__ void tmem_relinquish() {
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
 }
