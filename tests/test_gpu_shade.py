@@ -166,3 +166,40 @@ def test_shade_back_to_back_on_rotating_and_aliased_buffers(torch_cuda, niv):
 
     assert torch.equal(chain(False), chain(True))
     m.close()
+
+
+def test_shade_full_hd_frame(torch_cuda, niv, oracle):
+    """BASELINE.json configs[1] at full size through the launch `bench.py --shade` times (niv_infer_image_shade): every texel
+    bit-equal to niv_infer_image + niv_compose, 100,000 sampled texels against the oracle's infer + compose, RGB9E5 words of
+    the whole frame against the oracle's quantiser."""
+    torch = torch_cuda
+    spec = I.spec_fullhd()
+    case = Case(spec, 0)
+    m = case.gpu_model(niv)
+    w, h = 1920, 1080
+    n = w * h
+    g = I.make_gbuffer(w, h, 0)
+    pos, nrm = g["pos"], g["nrm"]
+    rng = np.random.default_rng(5)
+    albedo = rng.uniform(0, 1, (n, 3)).astype(np.float32)
+    direct = rng.uniform(0, 2, (n, 3)).astype(np.float32)
+    dp, dn, da, dd = (_dev_bytes(torch, x) for x in (pos, nrm, albedo, direct))
+    out = torch.full((n, 3), float("nan"), device="cuda")
+    m.infer_shade(dp, dn, da, out, n, direct=dd, image=(w, h))
+    e = torch.full((n, 3), float("nan"), device="cuda")
+    m.infer_image(dp, dn, e, w, h)
+    two = torch.full((h, w, 3), float("nan"), device="cuda")
+    niv.compose(e.view(h, w, 3), da.view(h, w, 3), two, dd.view(h, w, 3))
+    words = torch.full((n,), -1, dtype=torch.int32, device="cuda")
+    m.infer_shade(dp, dn, da, words, n, direct=dd, image=(w, h), out_format=I.OUTFMT_RGB9E5)
+    torch.cuda.synchronize()
+    assert torch.equal(out, two.view(n, 3))
+    got = out.cpu().numpy()
+    assert np.array_equal(words.cpu().numpy().view(np.uint32), oracle.quantise_rgb9e5(got))
+    sel = np.unique((I.random_u64(91, 1, 100000) % np.uint64(n)).astype(np.int64))
+    eo = oracle.infer(spec, case.table, case.wblob, case.bblob, pos[sel], nrm[sel])
+    k = sel.shape[0]
+    want = oracle.compose(eo.reshape(1, k, 3), albedo[sel].reshape(1, k, 3), direct[sel].reshape(1, k, 3)).reshape(k, 3)
+    err = np.abs(got[sel].astype(np.float64) - want)
+    assert err.max() <= MAX_ABS / np.pi + 1e-6 * float(np.abs(want).max()) and err.mean() <= MEAN_ABS / np.pi + 1e-6
+    m.close()
